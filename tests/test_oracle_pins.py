@@ -1,0 +1,377 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these touches the CUDA path.  The paper prints no worked example of this layer, so the pins are closed
+forms, invariants, special cases that reduce to library routines (numpy fp64 matmul, scipy softmax),
+brute force on tiny inputs, finite differences in fp64 and one self-made hand-checkable example
+(tests/golden/p12_worked_example.txt).
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import tqp_inputs as ti
+
+CFG0 = ti.CONFIGS[0]
+
+
+def widen(x):
+    return ti.bf16_bits_to_f32(x) if x.dtype == np.uint16 else x.astype(np.float32)
+
+
+def f64_inputs(inp):
+    """All real tensors of the layer widened exactly to float64 (for finite differences)."""
+    out = dict(inp)
+    for key, v in inp.items():
+        if isinstance(v, np.ndarray) and v.dtype in (np.uint16, np.float16, np.float32):
+            out[key] = widen(v).astype(np.float64)
+    return out
+
+
+@pytest.fixture(scope="module")
+def inp0():
+    return ti.make_inputs(CFG0)
+
+
+# ---------------------------------------------------------------- P1: dequant closed form
+def test_p1_dequant_is_scale_times_codebook_entry(inp0):
+    e = 3
+    idx = inp0["idx_gate"][e]              # [F][d/8]
+    W = oracle.dequant(idx, inp0["scale_gate"][e], inp0["codebook"], np.float32)   # [d][F]
+    cb = inp0["codebook"].astype(np.float32)
+    sc = inp0["scale_gate"][e].astype(np.float32)
+    F, nvec = idx.shape
+    rng = np.random.default_rng(1)
+    for _ in range(500):
+        o = int(rng.integers(F)); i = int(rng.integers(nvec * 8))
+        # product of two fp16 values is exact in fp32 -> must be bit-identical
+        assert W[i, o] == np.float32(sc[o]) * np.float32(cb[idx[o, i // 8], i % 8])
+    # a transposed / mis-strided read would break this: rows of W for a fixed o follow the codes of row o
+    o = 5
+    expect = (cb[idx[o]].reshape(-1) * sc[o]).astype(np.float32)
+    np.testing.assert_array_equal(W[:, o], expect)
+
+
+# ---------------------------------------------------------------- P12: hand-checkable 0/1 worked example
+def _parse_golden():
+    path = os.path.join(os.path.dirname(__file__), "golden", "p12_worked_example.txt")
+    vals = {}
+    for line in open(path):
+        line = line.split("#")[0].strip()
+        if "=" in line:
+            key, v = line.split("=")
+            vals[key.strip()] = np.array([float(t) for t in v.split()])
+    return vals
+
+
+def _p12_inputs():
+    g = _parse_golden()
+    d = F = 8
+    cb = np.zeros((256, 8), np.float16)
+    cb[:8] = np.eye(8, dtype=np.float16)
+    W_r = np.zeros((d, 2), np.float32)
+    W_r[0, 0], W_r[0, 1] = 1.0, -1.0
+    mk = lambda a, b: np.stack([g[a], g[b]]).astype(np.uint8).reshape(2, 8, 1)
+    inp = dict(
+        T=2, d=d, F=F, E=2, k=1, r=1, lora_scale=1.0,
+        X=ti.f32_to_bf16_bits(np.stack([g["x0"], g["x1"]]).astype(np.float32)),
+        dY=ti.f32_to_bf16_bits(np.ones((2, d), np.float32)),
+        W_r=W_r, codebook=cb, logit_bias=None,
+        idx_gate=mk("idx_gate_e0", "idx_gate_e1"), idx_up=mk("idx_up_e0", "idx_up_e1"),
+        idx_down=mk("idx_down_e0", "idx_down_e1"),
+        scale_gate=np.ones((2, F), np.float16), scale_up=np.ones((2, F), np.float16),
+        scale_down=np.ones((2, d), np.float16),
+        A_gate=np.zeros((2, d, 1), np.uint16), B_gate=np.zeros((2, 1, F), np.uint16),
+        A_up=np.zeros((2, d, 1), np.uint16), B_up=np.zeros((2, 1, F), np.uint16),
+        A_down=np.zeros((2, F, 1), np.uint16), B_down=np.zeros((2, 1, d), np.uint16),
+    )
+    return inp, g
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_p12_worked_example(dtype):
+    inp, g = _p12_inputs()
+    out = oracle.layer(inp, dtype=dtype, backward=False)
+    np.testing.assert_array_equal(out["topk_idx"].ravel(), [0, 1])       # x0[0] > 0 -> e0, x1[0] < 0 -> e1
+    np.testing.assert_array_equal(out["topk_w"].ravel(), [1.0, 1.0])
+    np.testing.assert_array_equal(out["perm"], [0, 1])
+    np.testing.assert_array_equal(out["G"], np.stack([g["G0"], g["G1"]]))  # read off by inspection
+    np.testing.assert_array_equal(out["U"], np.stack([g["U0"], g["U1"]]))
+    silu = lambda v: v / (1.0 + math.exp(-v))
+    H = np.array([[silu(a) * b for a, b in zip(g["G0"], g["U0"])],
+                  [silu(a) * b for a, b in zip(g["G1"], g["U1"])]])
+    assert np.all(out["H"][1, :4] == 0.0)
+    idx_down = [g["idx_down_e0"].astype(int), g["idx_down_e1"].astype(int)]
+    Y = np.stack([H[0][idx_down[0]], H[1][idx_down[1]]])
+    tol = 1e-6 if dtype == np.float32 else 1e-14
+    np.testing.assert_allclose(out["H"], H, rtol=tol, atol=tol)
+    np.testing.assert_allclose(out["Y"], Y, rtol=tol, atol=tol)
+
+
+# ---------------------------------------------------------------- P3: brute-force top-k with exact ties
+def test_p3_topk_bruteforce_with_ties():
+    rng = np.random.default_rng(7)
+    T, E, k = 40, 11, 4
+    lg = rng.standard_normal((T, E)).astype(np.float32)
+    lg[:, 7] = lg[:, 2]          # exact ties between experts 2 and 7 on every token
+    lg[5, :] = 0.25              # a fully tied row: expect experts 0..k-1
+    lg[6, 3:9] = lg[6].max() + 1  # six-way tie at the top
+    idx, w = oracle.topk(lg, k)
+    for t in range(T):
+        order = sorted(range(E), key=lambda e: (-float(lg[t, e]), e))[:k]
+        assert list(idx[t]) == order
+    np.testing.assert_array_equal(idx[5], np.arange(k))
+    np.testing.assert_array_equal(idx[6], [3, 4, 5, 6])
+
+
+def test_p3_routing_ties_from_duplicate_router_columns(inp0):
+    W_r = inp0["W_r"].copy()
+    W_r[:, 5] = W_r[:, 1]        # duplicate columns -> identical fp32 logits under the canonical order
+    lg = oracle.logits(inp0["X"], W_r)
+    np.testing.assert_array_equal(lg[:, 5], lg[:, 1])
+    idx, _ = oracle.topk(lg, 2)
+    for t in range(lg.shape[0]):
+        sel = list(idx[t])
+        if 5 in sel:
+            assert 1 in sel and sel.index(1) < sel.index(5)
+
+
+def test_logits_canonical_order_is_sequential_fma(inp0):
+    """R1: acc = fmaf(x_i, w_i, acc), i ascending.  Cross-check with exact rational arithmetic of the same
+    recurrence (fractions) on a few (t, e): each step rounds the exact x*w+acc once to fp32."""
+    from fractions import Fraction
+    X = widen(inp0["X"]); W = inp0["W_r"]
+    lg = oracle.logits(inp0["X"], W)
+    for (t, e) in [(0, 0), (3, 5), (63, 7)]:
+        acc = np.float32(0)
+        for i in range(X.shape[1]):
+            exact = Fraction(float(X[t, i])) * Fraction(float(W[i, e])) + Fraction(float(acc))
+            acc = np.float32(float(exact)) if abs(exact) < 2 ** 100 else acc
+            # float(Fraction) rounds to fp64 first; guard against double rounding by checking it is harmless
+            f64 = float(exact)
+            assert Fraction(f64) == exact or np.float32(np.nextafter(f64, np.inf)) == np.float32(np.nextafter(f64, -np.inf))
+        assert lg[t, e] == acc
+    # and it agrees with a float64 matmul to fp32 accuracy
+    ref = X.astype(np.float64) @ W.astype(np.float64)
+    np.testing.assert_allclose(lg, ref, atol=2e-6)
+
+
+def test_logit_bias_is_added_after_the_sum(inp0):
+    bias = np.linspace(-1, 1, CFG0.E).astype(np.float32)
+    a = oracle.logits(inp0["X"], inp0["W_r"])
+    b = oracle.logits(inp0["X"], inp0["W_r"], bias)
+    np.testing.assert_array_equal(b, a + bias[None, :])
+
+
+# ---------------------------------------------------------------- P6: gate-weight special cases
+def test_p6_softmax_special_cases():
+    from scipy.special import softmax
+    rng = np.random.default_rng(3)
+    lg = rng.standard_normal((17, 6))
+    idx, w = oracle.topk(lg, 6)                        # k = E -> ordinary softmax, reordered
+    full = softmax(lg, axis=1)
+    np.testing.assert_allclose(w, np.take_along_axis(full, idx, 1), rtol=1e-12)
+    idx1, w1 = oracle.topk(lg, 1)                      # k = 1 -> weight exactly 1, the argmax
+    np.testing.assert_array_equal(w1, 1.0)
+    np.testing.assert_array_equal(idx1[:, 0], lg.argmax(1))
+    idx3, w3 = oracle.topk(lg.astype(np.float32), 3)
+    np.testing.assert_allclose(w3.sum(1), 1.0, atol=1e-6)
+    assert (w3 > 0).all() and (np.diff(w3, axis=1) <= 0).all()   # descending logits -> descending weights
+    # softmax over the selected only: equals the full softmax renormalised on the selected set
+    sel = np.take_along_axis(full, idx3, 1)
+    np.testing.assert_allclose(w3, sel / sel.sum(1, keepdims=True), rtol=2e-6)
+
+
+# ---------------------------------------------------------------- P4: permutation invariants
+def test_p4_dispatch_invariants_and_identity(inp0):
+    out = oracle.layer(inp0, backward=False)
+    N, E, k, T = CFG0.N, CFG0.E, CFG0.k, CFG0.T
+    counts, offsets, perm, inv = out["counts"], out["offsets"], out["perm"], out["inv_perm"]
+    assert counts.sum() == N and offsets[0] == 0 and offsets[-1] == N
+    np.testing.assert_array_equal(np.diff(offsets), counts)
+    np.testing.assert_array_equal(counts, np.bincount(out["topk_idx"].ravel(), minlength=E))
+    np.testing.assert_array_equal(inv[perm], np.arange(N))
+    np.testing.assert_array_equal(perm[inv], np.arange(N))
+    flat = out["topk_idx"].ravel()
+    for e in range(E):
+        seg = perm[offsets[e]:offsets[e + 1]]
+        assert (flat[seg] == e).all() and (np.diff(seg) > 0).all()      # stable: ascending a inside an expert
+    # combine(dispatch(X)) with Ye := Xp returns X * sum_j w = X
+    X = widen(inp0["X"]).astype(np.float64)
+    Xp = X[perm // k]
+    Y = oracle.combine(Xp, inv, out["topk_w"].astype(np.float64))
+    np.testing.assert_allclose(Y, X, rtol=1e-6, atol=1e-6)
+    # and dispatch_bwd sums each token's k rows
+    dX = oracle.dispatch_bwd(Xp, inv, T, k)
+    np.testing.assert_allclose(dX, k * X, rtol=1e-12)
+
+
+def test_dispatch_empty_and_single_expert():
+    idx = np.array([[2, 0], [2, 0], [0, 2]], np.int32)       # expert 1 and 3 empty
+    counts, offsets, perm, inv = oracle.dispatch(idx, 4)
+    np.testing.assert_array_equal(counts, [3, 0, 3, 0])
+    np.testing.assert_array_equal(offsets, [0, 3, 3, 6, 6])
+    np.testing.assert_array_equal(perm, [1, 3, 4, 0, 2, 5])
+    np.testing.assert_array_equal(inv, [3, 0, 4, 1, 2, 5])
+
+
+# ---------------------------------------------------------------- P2 / P8: adapter wiring
+def _with(inp, **kw):
+    out = dict(inp); out.update(kw); return out
+
+
+def test_p2_zero_B_reproduces_base(inp0):
+    zero = lambda a: np.zeros_like(a)
+    base = oracle.layer(_with(inp0, lora_scale=0.0), backward=False)["Y"]
+    zb = oracle.layer(_with(inp0, B_gate=zero(inp0["B_gate"]), B_up=zero(inp0["B_up"]), B_down=zero(inp0["B_down"])),
+                      backward=False)["Y"]
+    np.testing.assert_array_equal(zb, base)
+    full = oracle.layer(inp0, backward=False)["Y"]
+    assert np.abs(full - base).max() > 1e-6            # the adapters do contribute otherwise
+
+
+def test_p7_p8_single_expert_is_dense_ffn_and_merge_identity():
+    """E=1, k=1: one dense SwiGLU FFN.  Compare with numpy fp64 matmuls of the MERGED weights
+    W_eff = Wdeq + s*A@B (the paper's consolidation)."""
+    cfg = ti.Config("p7", T=9, d=32, F=48, E=1, k=1, r=4, seed=11, lora_scale=0.5)
+    inp = ti.make_inputs(cfg)
+    # make the adapters large enough to matter
+    rng = np.random.default_rng(0)
+    for key in ("A_gate", "B_gate", "A_up", "B_up", "A_down", "B_down"):
+        inp[key] = ti.f32_to_bf16_bits(rng.standard_normal(inp[key].shape).astype(np.float32) * 0.1)
+    out = oracle.layer(inp, dtype=np.float64, backward=False)
+    X = widen(inp["X"]).astype(np.float64)
+    cb = inp["codebook"].astype(np.float64)
+
+    def merged(idx, scale, A, B):
+        out_dim = idx.shape[0]
+        Wdeq = (cb[idx].reshape(out_dim, -1) * scale.astype(np.float64)[:, None]).T     # [in][out]
+        return Wdeq + cfg.lora_scale * widen(A).astype(np.float64) @ widen(B).astype(np.float64)
+
+    Wg = merged(inp["idx_gate"][0], inp["scale_gate"][0], inp["A_gate"][0], inp["B_gate"][0])
+    Wu = merged(inp["idx_up"][0], inp["scale_up"][0], inp["A_up"][0], inp["B_up"][0])
+    Wd = merged(inp["idx_down"][0], inp["scale_down"][0], inp["A_down"][0], inp["B_down"][0])
+    G = X @ Wg; U = X @ Wu
+    H = G / (1 + np.exp(-G)) * U
+    Y = H @ Wd
+    np.testing.assert_allclose(out["G"], G, rtol=1e-11, atol=1e-13)
+    np.testing.assert_allclose(out["H"], H, rtol=1e-11, atol=1e-13)
+    np.testing.assert_allclose(out["Y"], Y, rtol=1e-11, atol=1e-13)
+    assert np.abs(cfg.lora_scale * (X @ widen(inp["A_gate"][0]).astype(np.float64)) @ widen(inp["B_gate"][0])).max() > 1e-3
+
+
+# ---------------------------------------------------------------- P5: finite differences in fp64 on cfg 0
+def _loss(inp64):
+    out = oracle.layer(inp64, dtype=np.float64, backward=False)
+    return float((out["Y"] * inp64["dY"]).sum()), out
+
+
+def test_p5_finite_differences_cfg0(inp0):
+    inp64 = f64_inputs(inp0)
+    ana = oracle.layer(inp64, dtype=np.float64, backward=True, router_grad=True)
+    lg = ana["logits"]
+    srt = np.sort(lg, axis=1)[:, ::-1]
+    gap = srt[:, CFG0.k - 1] - srt[:, CFG0.k]
+    h = 1e-5
+    # a step h on one W_r entry moves one logit by h*|x| <= ~5e-5; on one X entry by h*|W_r| ~ 1e-6
+    assert gap.min() > 1e-4, "top-k gap too small for finite differences on cfg 0"
+    rng = np.random.default_rng(5)
+    checks = [("X", "dX"), ("W_r", "dW_r"), ("A_gate", "dA_gate"), ("B_gate", "dB_gate"), ("A_up", "dA_up"),
+              ("B_up", "dB_up"), ("A_down", "dA_down"), ("B_down", "dB_down")]
+    for name, gname in checks:
+        base = inp64[name]
+        worst = 0.0
+        for _ in range(12):
+            pos = tuple(int(rng.integers(s)) for s in base.shape)
+            if name.startswith(("A_", "B_")) and ana["counts"][pos[0]] == 0:
+                continue
+            vals = []
+            for sgn in (+1, -1):
+                pert = base.copy(); pert[pos] += sgn * h
+                L, o = _loss(_with(inp64, **{name: pert}))
+                np.testing.assert_array_equal(o["topk_idx"], ana["topk_idx"])    # selection unchanged
+                vals.append(L)
+            fd = (vals[0] - vals[1]) / (2 * h)
+            an = ana[gname][pos]
+            scale = max(abs(an), np.abs(ana[gname]).max() * 1e-3)
+            worst = max(worst, abs(fd - an) / scale)
+        assert worst < 2e-5, (name, worst)
+    # dtopk_w: perturb the gate weights directly through the combine
+    Ye = ana["Ye"]
+    for _ in range(8):
+        t, j = int(rng.integers(CFG0.T)), int(rng.integers(CFG0.k))
+        w = ana["topk_w"].copy(); w[t, j] += h
+        Lp = (oracle.combine(Ye, ana["inv_perm"], w) * inp64["dY"]).sum()
+        w[t, j] -= 2 * h
+        Lm = (oracle.combine(Ye, ana["inv_perm"], w) * inp64["dY"]).sum()
+        np.testing.assert_allclose((Lp - Lm) / (2 * h), ana["dtopk_w"][t, j], rtol=1e-6, atol=1e-8)
+
+
+def test_p5_dx_without_router_term(inp0):
+    """dX_experts is the derivative with the routing weights held constant: check by FD with frozen routing."""
+    inp64 = f64_inputs(inp0)
+    ana = oracle.layer(inp64, dtype=np.float64, backward=True)
+    rng = np.random.default_rng(9)
+    h = 1e-4
+
+    def loss_frozen(X):
+        Ye = oracle.expert_fwd(_with(inp64, X=X), ana["offsets"], ana["perm"], np.float64, save=False)
+        return float((oracle.combine(Ye, ana["inv_perm"], ana["topk_w"]) * inp64["dY"]).sum())
+
+    for _ in range(10):
+        pos = (int(rng.integers(CFG0.T)), int(rng.integers(CFG0.d)))
+        Xp = inp64["X"].copy(); Xp[pos] += h
+        Xm = inp64["X"].copy(); Xm[pos] -= h
+        fd = (loss_frozen(Xp) - loss_frozen(Xm)) / (2 * h)
+        np.testing.assert_allclose(fd, ana["dX_experts"][pos], rtol=2e-6, atol=1e-8)
+
+
+# ---------------------------------------------------------------- P9: linearity in dY, empty experts
+def test_p9_backward_linear_in_dY_and_empty_experts(inp0):
+    inp64 = f64_inputs(inp0)
+    # force experts 6 and 7 empty with a large negative bias
+    bias = np.zeros(CFG0.E); bias[6:] = -100.0
+    inp64 = _with(inp64, logit_bias=bias)
+    a = oracle.layer(inp64, dtype=np.float64, router_grad=True)
+    b = oracle.layer(_with(inp64, dY=-2.5 * inp64["dY"]), dtype=np.float64, router_grad=True)
+    assert a["counts"][6] == 0 and a["counts"][7] == 0
+    for key in ("dX", "dX_experts", "dW_r", "dtopk_w", "dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down"):
+        assert np.isfinite(a[key]).all()
+        np.testing.assert_allclose(b[key], -2.5 * a[key], rtol=1e-10, atol=1e-14)
+    for key in ("dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down"):
+        assert (a[key][6:] == 0).all()
+        assert np.abs(a[key][:6]).max() > 0
+
+
+# ---------------------------------------------------------------- P10: fp32 vs fp64 instantiation
+def test_p10_f32_vs_f64(inp0):
+    a = oracle.layer(inp0, dtype=np.float32, router_grad=True)
+    b = oracle.layer(inp0, dtype=np.float64, router_grad=True)
+    np.testing.assert_array_equal(a["topk_idx"], b["topk_idx"])
+    np.testing.assert_array_equal(a["perm"], b["perm"])
+    for key in ("Y", "dX", "dW_r", "dtopk_w", "dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down", "topk_w"):
+        ref = b[key]
+        err = np.abs(a[key] - ref).max() / np.abs(ref).max()
+        assert err < 2e-5, (key, err)
+
+
+# ---------------------------------------------------------------- P11: shapes fixed by the paper's counts
+def test_p11_parameter_counts_from_the_paper():
+    """rank 16 on each of 3 packs x 460 experts x 20 layers = 'about 2.26B' adapter params;
+    L934: 20 x 460 x 3 x (4096 x 1024) = 'something over 100B'.  This fixes A:[in,r], B:[r,out] PER EXPERT."""
+    d, F, r, E, L = 4096, 1024, 16, 460, 20
+    adapters = 3 * (d * r + r * F) * E * L
+    assert abs(adapters / 1e9 - 2.26) < 0.005
+    assert 20 * 460 * 3 * d * F > 100e9
+    inp = ti.make_inputs(CFG0)
+    assert inp["A_gate"].shape == (CFG0.E, CFG0.d, CFG0.r) and inp["B_gate"].shape == (CFG0.E, CFG0.r, CFG0.F)
+    assert inp["A_down"].shape == (CFG0.E, CFG0.F, CFG0.r) and inp["B_down"].shape == (CFG0.E, CFG0.r, CFG0.d)
+
+
+def test_zipf_bias_recipe():
+    b = ti.zipf_logit_bias(460, 3)
+    p = np.exp(np.sort(b.astype(np.float64))[::-1])
+    np.testing.assert_allclose(p.sum(), 1.0, rtol=1e-5)
+    np.testing.assert_allclose(p[0] / p[1], 2 ** 1.1, rtol=1e-5)
