@@ -1,0 +1,153 @@
+/* tqp.h — C ABI of the B200-native routed-expert layer of the TQP method
+ * ("Reversible Foundations: Training a 120B Sparse MoE through State-Preserving Scaling", arxiv 2606.07404).
+ *
+ * The path (§3.4 L224 router; Table 4 L237-239 top-k routed experts; §5.1 L401 gate/up/down
+ * projections; §9.1 L938 rank-r adapters on each of the three packs, frozen base; §9.2 "reconstruction
+ * looks up the codebook values and rescales by the stored norm"):
+ *
+ *   forward :  tqp_route -> tqp_dispatch -> tqp_expert_fwd -> tqp_combine
+ *   backward:  tqp_combine_bwd -> tqp_expert_bwd -> tqp_dispatch_bwd [-> tqp_route_bwd]
+ *
+ * Notation: T tokens, d = d_model, F = per-expert d_ff, E experts, k = top-k, r = adapter rank,
+ * N = T*k routed rows, a = t*k + j the flat assignment index of token t's j-th choice,
+ * p the row position after the stable sort by expert (perm[p] = a, inv_perm[a] = p).
+ *
+ * Conventions for EVERY entry point below unless a comment says otherwise:
+ *  - All tensor pointers are DEVICE pointers, row-major, contiguous, 16-byte aligned, caller-owned; the
+ *    library never frees or retains them beyond the call, except the tqp_weights pointers and the bound
+ *    workspace, which must stay valid while the ctx uses them.
+ *  - "bf16" / "fp16" tensors are passed as const void* (2 bytes per element).
+ *  - `stream` is a cudaStream_t passed as void*.  Every call only enqueues work on it: no host
+ *    synchronisation, no device->host copy.  Expert counts/offsets are consumed on the device.
+ *  - Return value: TQP_OK or an error code; nothing throws or aborts.  Host-side argument validation runs
+ *    first; CUDA errors map to TQP_ERR_CUDA with the text kept in tqp_last_error(ctx).
+ *  - There is NO CPU fallback: without an sm_100 device the calls return TQP_ERR_ARCH / TQP_ERR_CUDA.
+ *  - Non-finite inputs: undefined results.
+ */
+#ifndef TQP_H_
+#define TQP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tqp_ctx tqp_ctx; /* opaque; owns only host-side state (descriptors, pointers) */
+
+typedef enum {
+    TQP_OK = 0,
+    TQP_ERR_ARG = 1,       /* NULL pointer or value out of range */
+    TQP_ERR_SHAPE = 2,     /* unsupported shape (see tqp_layer_desc) */
+    TQP_ERR_ALIGN = 3,     /* pointer not 16-byte aligned */
+    TQP_ERR_WORKSPACE = 4, /* workspace missing or too small */
+    TQP_ERR_STATE = 5,     /* call order violated (e.g. expert_bwd without a training-mode expert_fwd) */
+    TQP_ERR_ARCH = 6,      /* device is not sm_100 */
+    TQP_ERR_CUDA = 7       /* a CUDA runtime/driver call failed; see tqp_last_error */
+} tqp_status;
+
+/* Shape of one layer.  Constraints: d % 128 == 0, F % 128 == 0, 1 <= k <= min(E, 32), E <= 1024,
+ * r in {8, 16, 32}, vec == 8, codes == 256, T_max * k < 2^31 / 64. */
+typedef struct {
+    int32_t T_max;    /* largest T any call will pass */
+    int32_t d, F, E, k, r;
+    int32_t vec;      /* vector length of the quantiser: 8 (BASELINE.json configs[0]) */
+    int32_t codes;    /* codebook entries: 256 */
+    float lora_scale; /* s in W_eff = deq(W) + s*A*B  (R7; 1.0 in all configs) */
+    int32_t training; /* 1: expert_fwd saves G, U, H in the workspace for expert_bwd */
+} tqp_layer_desc;
+
+/* Frozen quantised base + trained adapters of all E experts.  All DEVICE pointers.
+ * W_eff[in][out] = scale[out] * codebook[idx[out][in/8]][in%8] + lora_scale * (A . B)[in][out]. */
+typedef struct {
+    const uint8_t *idx_gate, *idx_up; /* [E][F][d/8]  row = output channel, codes along the input dim */
+    const uint8_t *idx_down;          /* [E][d][F/8] */
+    const void *scale_gate, *scale_up; /* fp16 [E][F] */
+    const void *scale_down;            /* fp16 [E][d] */
+    const void *codebook;              /* fp16 [256][8], shared by all experts and the three packs */
+    const void *A_gate, *A_up;         /* bf16 [E][d][r] */
+    const void *B_gate, *B_up;         /* bf16 [E][r][F] */
+    const void *A_down;                /* bf16 [E][F][r] */
+    const void *B_down;                /* bf16 [E][r][d] */
+} tqp_weights;
+
+/* --- lifetime ----------------------------------------------------------------------------------------- */
+tqp_status tqp_create(tqp_ctx **out, const tqp_layer_desc *desc); /* validates desc and the device */
+void tqp_destroy(tqp_ctx *ctx);
+/* Bytes of device scratch the ctx needs (saved G/U/H, permuted rows, adapter projections, tile lists). */
+size_t tqp_workspace_bytes(const tqp_layer_desc *desc);
+/* Caller allocates (e.g. torch.empty) and lends the workspace; it is zero-filled on `stream`. */
+tqp_status tqp_bind_workspace(tqp_ctx *ctx, void *dev_ptr, size_t bytes, void *stream);
+/* Records the weight pointers, builds the TMA descriptors over the code indices and converts the codebook
+ * to the bf16 lookup table the GEMM mainloop gathers from.  One-time, untimed; needs a bound workspace. */
+tqp_status tqp_bind_weights(tqp_ctx *ctx, const tqp_weights *w, void *stream);
+/* Options (debug / ablation).  "gemm_impl": 0 = tcgen05 grouped GEMM (default), 1 = CUDA-core scaffold. */
+tqp_status tqp_set_option(tqp_ctx *ctx, const char *name, int value);
+
+/* --- forward ------------------------------------------------------------------------------------------ */
+/* Router (R1-R5).  logits[t][e] = fmaf-chain over i ascending of
+ * float(X[t][i]) * W_r[i][e], then + logit_bias[e] if given; top-k by (-logit, id) (ties -> lower id);
+ * topk_w = softmax over the k selected logits.  X bf16 [T][d]; W_r fp32 [d][E]; logit_bias fp32 [E] or
+ * NULL; topk_idx int32 [T][k]; topk_w fp32 [T][k]; logits_out fp32 [T][E] or NULL. */
+tqp_status tqp_route(tqp_ctx *ctx, int T, const void *X, const float *W_r, const float *logit_bias,
+                     int32_t *topk_idx, float *topk_w, float *logits_out, void *stream);
+/* Stable counting sort of a = t*k+j by expert id ("expert dispatch").  counts int32 [E];
+ * offsets int32 [E+1] (exclusive scan, offsets[E] = N); perm int32 [N]; inv_perm int32 [N].  Also builds
+ * the grouped-GEMM tile list inside the workspace. */
+tqp_status tqp_dispatch(tqp_ctx *ctx, int T, const int32_t *topk_idx, int32_t *counts, int32_t *offsets,
+                        int32_t *perm, int32_t *inv_perm, void *stream);
+/* Routed experts: for row p of expert e, x = X[perm[p]/k]:
+ * g = x.Wg_eff, u = x.Wu_eff, h = silu(g)*u, Ye[p] = h.Wd_eff.  Ye bf16 [N][d].  Must follow tqp_dispatch
+ * with the same T on the same stream (uses its tile list). */
+tqp_status tqp_expert_fwd(tqp_ctx *ctx, int T, const void *X, const int32_t *offsets, const int32_t *perm,
+                          void *Ye, void *stream);
+/* Weighted combine: Y[t] = sum_j topk_w[t][j] * Ye[inv_perm[t*k+j]] (fp32 accumulate, j ascending).
+ * Y bf16 [T][d]. */
+tqp_status tqp_combine(tqp_ctx *ctx, int T, const void *Ye, const int32_t *inv_perm, const float *topk_w,
+                       void *Y, void *stream);
+
+/* --- backward (loss L = sum(Y * dY)) -------------------------------------------------------------------- */
+/* dYe[p] = topk_w[a] * dY[t] (bf16 [N][d]);  dtopk_w[a] = <dY[t], Ye[p]> (fp32 [T][k], NULL to skip). */
+tqp_status tqp_combine_bwd(tqp_ctx *ctx, int T, const void *dY, const void *Ye, const int32_t *inv_perm,
+                           const float *topk_w, void *dYe, float *dtopk_w, void *stream);
+/* Activation gradient through the frozen dequantised weights and weight gradients of the adapters only
+ * (PAPER.md L938).  Needs training=1 and the preceding tqp_expert_fwd of the same T.  dXp bf16 [N][d];
+ * dA_gate/dA_up fp32 [E][d][r]; dB_gate/dB_up fp32 [E][r][F]; dA_down fp32 [E][F][r]; dB_down fp32
+ * [E][r][d]; gradients are overwritten (exactly 0 for experts with no rows). */
+tqp_status tqp_expert_bwd(tqp_ctx *ctx, int T, const void *X, const void *dYe, const int32_t *offsets,
+                          const int32_t *perm, void *dXp, float *dA_gate, float *dB_gate, float *dA_up,
+                          float *dB_up, float *dA_down, float *dB_down, void *stream);
+/* dX[t] = sum_j dXp[inv_perm[t*k+j]] (fp32 accumulate, j ascending); dX bf16 [T][d]. */
+tqp_status tqp_dispatch_bwd(tqp_ctx *ctx, int T, const void *dXp, const int32_t *inv_perm, void *dX,
+                            void *stream);
+/* Router gradient with the selection held constant: dl_j = w_j (dw_j - sum_i w_i dw_i);
+ * dX[t] += sum_j dl_j W_r[:,e_j] (dX bf16 [T][d], read-modify-write); dW_r[:,e] = sum X[t] dl (fp32 [d][E],
+ * overwritten).  Uses the perm/offsets of the preceding tqp_dispatch for a deterministic reduction. */
+tqp_status tqp_route_bwd(tqp_ctx *ctx, int T, const void *X, const float *W_r, const int32_t *topk_idx,
+                         const float *topk_w, const float *dtopk_w, const int32_t *offsets,
+                         const int32_t *perm, void *dX, float *dW_r, void *stream);
+
+/* --- whole step through HOST buffers (end-to-end measurement) ------------------------------------------- */
+/* Copies X and dY (bf16 [T][d], pinned HOST memory) to the device, runs the whole forward+backward chain
+ * above on `stream` and copies Y and dX (bf16 [T][d]) back to the HOST buffers.  W_r / logit_bias and the
+ * adapter-gradient outputs are DEVICE pointers as above (dW_r may be NULL to skip tqp_route_bwd).
+ * Synchronises `stream` before returning. */
+tqp_status tqp_step_host(tqp_ctx *ctx, int T, const void *X_host, const void *dY_host, const float *W_r,
+                         const float *logit_bias, void *Y_host, void *dX_host, float *dA_gate,
+                         float *dB_gate, float *dA_up, float *dB_up, float *dA_down, float *dB_down,
+                         float *dW_r, void *stream);
+
+/* --- introspection ------------------------------------------------------------------------------------- */
+/* Device pointers of workspace tensors, for tests: "G","U","H" bf16 [N][F]; "Xp" bf16 [N][d];
+ * "dH","dG","dU" bf16 [N][F]; "num_tiles" int32 [1].  NULL if unknown. */
+void *tqp_debug_buffer(tqp_ctx *ctx, const char *name);
+/* Kernels launched by the last call on this ctx (for bench.py's gpu_launches). */
+int tqp_last_launch_count(const tqp_ctx *ctx);
+const char *tqp_status_string(tqp_status s);
+const char *tqp_last_error(const tqp_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TQP_H_ */

@@ -1,0 +1,241 @@
+"""ctypes binding of include/tqp.h.  Argument marshalling only."""
+from __future__ import annotations
+
+import ctypes
+import os
+import re
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libtqp.so")
+HEADER = os.path.join(HERE, "..", "include", "tqp.h")
+_lib = None
+
+STATUS = {0: "TQP_OK", 1: "TQP_ERR_ARG", 2: "TQP_ERR_SHAPE", 3: "TQP_ERR_ALIGN", 4: "TQP_ERR_WORKSPACE",
+          5: "TQP_ERR_STATE", 6: "TQP_ERR_ARCH", 7: "TQP_ERR_CUDA"}
+
+
+class TqpError(RuntimeError):
+    def __init__(self, code, msg=""):
+        self.code = code
+        super().__init__(f"{STATUS.get(code, code)}: {msg}")
+
+
+class LayerDesc(ctypes.Structure):
+    _fields_ = [("T_max", ctypes.c_int32), ("d", ctypes.c_int32), ("F", ctypes.c_int32), ("E", ctypes.c_int32),
+                ("k", ctypes.c_int32), ("r", ctypes.c_int32), ("vec", ctypes.c_int32), ("codes", ctypes.c_int32),
+                ("lora_scale", ctypes.c_float), ("training", ctypes.c_int32)]
+
+
+_WEIGHT_FIELDS = ["idx_gate", "idx_up", "idx_down", "scale_gate", "scale_up", "scale_down", "codebook",
+                  "A_gate", "A_up", "B_gate", "B_up", "A_down", "B_down"]
+
+
+class Weights(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_void_p) for n in _WEIGHT_FIELDS]
+
+
+def abi_symbols() -> list[str]:
+    """Function names declared in include/tqp.h."""
+    text = open(HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(tqp_[a-z_0-9]+)\s*\(", text)))
+
+
+def load_library() -> ctypes.CDLL:
+    """Loads libtqp.so; raises loudly if it has not been built (no fallback of any kind)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise TqpError(-1, f"{LIB_PATH} is missing: run `python -m paper_2606_07404_b200.build` (needs nvcc)")
+        lib = ctypes.CDLL(LIB_PATH)
+        vp, ci = ctypes.c_void_p, ctypes.c_int
+        lib.tqp_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(LayerDesc)]
+        lib.tqp_destroy.argtypes = [vp]
+        lib.tqp_destroy.restype = None
+        lib.tqp_workspace_bytes.argtypes = [ctypes.POINTER(LayerDesc)]
+        lib.tqp_workspace_bytes.restype = ctypes.c_size_t
+        lib.tqp_bind_workspace.argtypes = [vp, vp, ctypes.c_size_t, vp]
+        lib.tqp_bind_weights.argtypes = [vp, ctypes.POINTER(Weights), vp]
+        lib.tqp_set_option.argtypes = [vp, ctypes.c_char_p, ci]
+        lib.tqp_route.argtypes = [vp, ci] + [vp] * 7
+        lib.tqp_dispatch.argtypes = [vp, ci] + [vp] * 6
+        lib.tqp_expert_fwd.argtypes = [vp, ci] + [vp] * 5
+        lib.tqp_combine.argtypes = [vp, ci] + [vp] * 5
+        lib.tqp_combine_bwd.argtypes = [vp, ci] + [vp] * 7
+        lib.tqp_expert_bwd.argtypes = [vp, ci] + [vp] * 12
+        lib.tqp_dispatch_bwd.argtypes = [vp, ci] + [vp] * 4
+        lib.tqp_route_bwd.argtypes = [vp, ci] + [vp] * 10
+        lib.tqp_step_host.argtypes = [vp, ci] + [vp] * 14
+        lib.tqp_debug_buffer.argtypes = [vp, ctypes.c_char_p]
+        lib.tqp_debug_buffer.restype = vp
+        lib.tqp_last_launch_count.argtypes = [vp]
+        lib.tqp_status_string.argtypes = [ci]
+        lib.tqp_status_string.restype = ctypes.c_char_p
+        lib.tqp_last_error.argtypes = [vp]
+        lib.tqp_last_error.restype = ctypes.c_char_p
+        _lib = lib
+    return _lib
+
+
+def _desc(T_max, d, F, E, k, r, lora_scale=1.0, training=True) -> LayerDesc:
+    return LayerDesc(T_max, d, F, E, k, r, 8, 256, float(lora_scale), 1 if training else 0)
+
+
+def workspace_bytes(T_max, d, F, E, k, r, lora_scale=1.0, training=True) -> int:
+    return int(load_library().tqp_workspace_bytes(ctypes.byref(_desc(T_max, d, F, E, k, r, lora_scale, training))))
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+class TqpLayer:
+    """One routed-expert layer on the current CUDA device.  Methods carry the C names without the tqp_ prefix."""
+
+    def __init__(self, T_max, d, F, E, k, r, lora_scale=1.0, training=True, device="cuda:0"):
+        import torch
+        self.torch = torch
+        self.lib = load_library()
+        if not torch.cuda.is_available():
+            raise TqpError(6, "no CUDA device: the TQP path has no CPU fallback")
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.T_max, self.d, self.F, self.E, self.k, self.r = T_max, d, F, E, k, r
+        self.training = training
+        self.desc = _desc(T_max, d, F, E, k, r, lora_scale, training)
+        self.ctx = ctypes.c_void_p()
+        self._check(self.lib.tqp_create(ctypes.byref(self.ctx), ctypes.byref(self.desc)))
+        nbytes = int(self.lib.tqp_workspace_bytes(ctypes.byref(self.desc)))
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self._check(self.lib.tqp_bind_workspace(self.ctx, _ptr(self.workspace), nbytes, self._stream()))
+        self.weights = None
+
+    def __del__(self):
+        try:
+            if getattr(self, "ctx", None):
+                self.lib.tqp_destroy(self.ctx)
+                self.ctx = None
+        except Exception:
+            pass
+
+    def _stream(self):
+        return ctypes.c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream)
+
+    def _check(self, code):
+        if code != 0:
+            msg = self.lib.tqp_last_error(self.ctx).decode() if self.ctx else ""
+            raise TqpError(code, msg)
+
+    def set_option(self, name: str, value: int):
+        self._check(self.lib.tqp_set_option(self.ctx, name.encode(), int(value)))
+
+    def bind_weights(self, **w):
+        """w: device tensors named as tqp_weights' fields (uint8 codes, fp16 scales/codebook, bf16 adapters)."""
+        self.weights = {n: w[n].contiguous() for n in _WEIGHT_FIELDS}
+        ws = Weights(*[self.weights[n].data_ptr() for n in _WEIGHT_FIELDS])
+        self._check(self.lib.tqp_bind_weights(self.ctx, ctypes.byref(ws), self._stream()))
+
+    # ---- forward ----
+    def route(self, X, W_r, logit_bias=None, want_logits=False):
+        t = self.torch
+        T = X.shape[0]
+        idx = t.empty((T, self.k), dtype=t.int32, device=self.device)
+        w = t.empty((T, self.k), dtype=t.float32, device=self.device)
+        lg = t.empty((T, self.E), dtype=t.float32, device=self.device) if want_logits else None
+        self._check(self.lib.tqp_route(self.ctx, T, _ptr(X), _ptr(W_r), _ptr(logit_bias), _ptr(idx), _ptr(w), _ptr(lg),
+                                       self._stream()))
+        return (idx, w, lg) if want_logits else (idx, w)
+
+    def dispatch(self, topk_idx):
+        t = self.torch
+        T = topk_idx.shape[0]
+        N = T * self.k
+        counts = t.empty(self.E, dtype=t.int32, device=self.device)
+        offsets = t.empty(self.E + 4, dtype=t.int32, device=self.device)[: self.E + 1]
+        perm = t.empty(N, dtype=t.int32, device=self.device)
+        inv = t.empty(N, dtype=t.int32, device=self.device)
+        self._check(self.lib.tqp_dispatch(self.ctx, T, _ptr(topk_idx), _ptr(counts), _ptr(offsets), _ptr(perm), _ptr(inv),
+                                          self._stream()))
+        return counts, offsets, perm, inv
+
+    def expert_fwd(self, X, offsets, perm, out=None):
+        t = self.torch
+        T = X.shape[0]
+        Ye = out if out is not None else t.empty((T * self.k, self.d), dtype=t.bfloat16, device=self.device)
+        self._check(self.lib.tqp_expert_fwd(self.ctx, T, _ptr(X), _ptr(offsets), _ptr(perm), _ptr(Ye), self._stream()))
+        return Ye
+
+    def combine(self, Ye, inv_perm, topk_w, out=None):
+        t = self.torch
+        T = topk_w.shape[0]
+        Y = out if out is not None else t.empty((T, self.d), dtype=t.bfloat16, device=self.device)
+        self._check(self.lib.tqp_combine(self.ctx, T, _ptr(Ye), _ptr(inv_perm), _ptr(topk_w), _ptr(Y), self._stream()))
+        return Y
+
+    # ---- backward ----
+    def combine_bwd(self, dY, Ye, inv_perm, topk_w, want_dw=True, out=None):
+        t = self.torch
+        T = topk_w.shape[0]
+        dYe = out if out is not None else t.empty((T * self.k, self.d), dtype=t.bfloat16, device=self.device)
+        dw = t.empty((T, self.k), dtype=t.float32, device=self.device) if want_dw else None
+        self._check(self.lib.tqp_combine_bwd(self.ctx, T, _ptr(dY), _ptr(Ye), _ptr(inv_perm), _ptr(topk_w), _ptr(dYe),
+                                             _ptr(dw), self._stream()))
+        return dYe, dw
+
+    def alloc_grads(self):
+        t = self.torch
+        E, d, F, r = self.E, self.d, self.F, self.r
+        mk = lambda *s: t.empty(s, dtype=t.float32, device=self.device)
+        return {"dA_gate": mk(E, d, r), "dB_gate": mk(E, r, F), "dA_up": mk(E, d, r), "dB_up": mk(E, r, F),
+                "dA_down": mk(E, F, r), "dB_down": mk(E, r, d)}
+
+    def expert_bwd(self, X, dYe, offsets, perm, grads=None, out=None):
+        t = self.torch
+        T = X.shape[0]
+        g = grads if grads is not None else self.alloc_grads()
+        dXp = out if out is not None else t.empty((T * self.k, self.d), dtype=t.bfloat16, device=self.device)
+        self._check(self.lib.tqp_expert_bwd(self.ctx, T, _ptr(X), _ptr(dYe), _ptr(offsets), _ptr(perm), _ptr(dXp),
+                                            _ptr(g["dA_gate"]), _ptr(g["dB_gate"]), _ptr(g["dA_up"]), _ptr(g["dB_up"]),
+                                            _ptr(g["dA_down"]), _ptr(g["dB_down"]), self._stream()))
+        return dXp, g
+
+    def dispatch_bwd(self, dXp, inv_perm, out=None):
+        t = self.torch
+        T = dXp.shape[0] // self.k
+        dX = out if out is not None else t.empty((T, self.d), dtype=t.bfloat16, device=self.device)
+        self._check(self.lib.tqp_dispatch_bwd(self.ctx, T, _ptr(dXp), _ptr(inv_perm), _ptr(dX), self._stream()))
+        return dX
+
+    def route_bwd(self, X, W_r, topk_idx, topk_w, dtopk_w, offsets, perm, dX):
+        t = self.torch
+        T = X.shape[0]
+        dW_r = t.empty((self.d, self.E), dtype=t.float32, device=self.device)
+        self._check(self.lib.tqp_route_bwd(self.ctx, T, _ptr(X), _ptr(W_r), _ptr(topk_idx), _ptr(topk_w), _ptr(dtopk_w),
+                                           _ptr(offsets), _ptr(perm), _ptr(dX), _ptr(dW_r), self._stream()))
+        return dW_r
+
+    def step_host(self, X_host, dY_host, W_r, logit_bias, Y_host, dX_host, grads, dW_r=None):
+        """Whole forward+backward through HOST (pinned) X/dY/Y/dX buffers; grads / dW_r stay on the device."""
+        T = X_host.shape[0]
+        g = grads
+        self._check(self.lib.tqp_step_host(self.ctx, T, _ptr(X_host), _ptr(dY_host), _ptr(W_r), _ptr(logit_bias),
+                                           _ptr(Y_host), _ptr(dX_host), _ptr(g["dA_gate"]), _ptr(g["dB_gate"]),
+                                           _ptr(g["dA_up"]), _ptr(g["dB_up"]), _ptr(g["dA_down"]), _ptr(g["dB_down"]),
+                                           _ptr(dW_r), self._stream()))
+
+    # ---- introspection ----
+    def last_launch_count(self) -> int:
+        return int(self.lib.tqp_last_launch_count(self.ctx))
+
+    def debug_buffer(self, name, shape, dtype):
+        """A torch view of a workspace tensor (tests only)."""
+        t = self.torch
+        ptr = self.lib.tqp_debug_buffer(self.ctx, name.encode())
+        if not ptr:
+            raise KeyError(name)
+        off = ptr - self.workspace.data_ptr()
+        n = 1
+        for s in shape:
+            n *= s
+        nbytes = n * t.empty((), dtype=dtype).element_size()
+        return self.workspace[off: off + nbytes].view(dtype).view(*shape)

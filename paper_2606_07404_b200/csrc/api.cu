@@ -1,0 +1,412 @@
+// C-ABI entry points (include/tqp.h): argument validation, workspace layout, TMA descriptors, call chains.
+#include <cstring>
+#include <new>
+
+#include "common.cuh"
+
+using namespace tqp;
+
+namespace {
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+bool desc_ok(const tqp_layer_desc *d) {
+    if (!d) return false;
+    if (d->T_max <= 0 || d->d <= 0 || d->F <= 0 || d->E <= 0 || d->k <= 0) return false;
+    if (d->d % 128 || d->F % 128) return false;
+    if (d->k > d->E || d->k > 32 || d->E > 1024) return false;
+    if (!(d->r == 8 || d->r == 16 || d->r == 32)) return false;
+    if (d->vec != 8 || d->codes != 256) return false;
+    if ((long long)d->T_max * d->k >= (1ll << 31) / 64) return false;
+    return true;
+}
+
+Workspace layout(const tqp_layer_desc &d) {
+    Workspace w;
+    const size_t T = d.T_max, N = T * d.k, Np = N + kRowPad, dm = d.d, F = d.F, E = d.E;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 1024); return o; };
+    w.Xp = take(Np * dm * 2);
+    w.G = take(Np * F * 2); w.U = take(Np * F * 2); w.H = take(Np * F * 2);
+    w.dH = take(Np * F * 2); w.dG = take(Np * F * 2); w.dU = take(Np * F * 2);
+    w.XAg = take(Np * kLoraPad * 2); w.XAu = take(Np * kLoraPad * 2); w.HAd = take(Np * kLoraPad * 2);
+    w.Zd = take(Np * kLoraPad * 2); w.Zg = take(Np * kLoraPad * 2); w.Zu = take(Np * kLoraPad * 2);
+    w.logits = take(T * E * 4);
+    w.blk_counts = take(((N + kDispChunk - 1) / kDispChunk + 4) * E * 4);
+    w.tiles = take((E + N / kTileRows + 2) * sizeof(Tile));
+    w.num_tiles = take(16);
+    w.lut = take(256 * 8 * 2);
+    w.WrT = take(E * dm * 4);
+    w.dl = take(N * 4);
+    w.hX = take(T * dm * 2); w.hdY = take(T * dm * 2); w.hY = take(T * dm * 2); w.hdX = take(T * dm * 2);
+    w.topk_idx = take(N * 4); w.topk_w = take(N * 4); w.counts = take(E * 4); w.offsets = take((E + 1) * 4);
+    w.perm = take(N * 4); w.inv_perm = take(N * 4);
+    w.Ye = take(N * dm * 2); w.dYe = take(N * dm * 2); w.dXp = take(N * dm * 2); w.dtopk_w = take(N * 4);
+    w.total = off;
+    return w;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+// 2-D row-major tensor [rows][cols] of `esize`-byte elements, box {box_cols, box_rows}
+tqp_status make_map(tqp_ctx *c, CUtensorMap *m, const void *ptr, CUtensorMapDataType dt, size_t esize, uint64_t rows,
+                    uint64_t cols, uint32_t box_cols, uint32_t box_rows, CUtensorMapSwizzle sw) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) { c->err = "cuTensorMapEncodeTiled not available"; return TQP_ERR_CUDA; }
+    cuuint64_t dims[2] = {cols, rows};
+    cuuint64_t strides[1] = {cols * esize};
+    cuuint32_t box[2] = {box_cols, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(m, dt, 2, const_cast<void *>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, sw,
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { c->err = "cuTensorMapEncodeTiled failed: " + std::to_string((int)r); return TQP_ERR_CUDA; }
+    return TQP_OK;
+}
+
+tqp_status act_map(tqp_ctx *c, CUtensorMap *m, const void *ptr, uint64_t rows, uint64_t K) {
+    return make_map(c, m, ptr, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, rows, K, 64, kTileRows, CU_TENSOR_MAP_SWIZZLE_128B);
+}
+
+tqp_status set_seg(tqp_ctx *c, GemmSeg *s, const bf16 *act, uint64_t act_rows, const uint8_t *idx, const void *scale, int K,
+                   int M, int kmajor) {
+    s->act = act; s->idx = idx; s->scale = (const __half *)scale; s->K = K; s->kmajor = kmajor;
+    tqp_status st = act_map(c, &s->act_map, act, act_rows, K);
+    if (st != TQP_OK) return st;
+    const uint64_t E = c->desc.E;
+    const uint64_t rows = kmajor ? E * M : E * K, bytes = kmajor ? K / 8 : M / 8;
+    return make_map(c, &s->idx_map, idx, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, rows, bytes, 16, 128, CU_TENSOR_MAP_SWIZZLE_NONE);
+}
+
+tqp_status set_lora(tqp_ctx *c, GemmLora *l, const bf16 *lact, uint64_t rows, const void *lw, int mk_layout) {
+    l->lact = lact; l->lw = (const bf16 *)lw; l->mk_layout = mk_layout;
+    return act_map(c, &l->lact_map, lact, rows, kLoraPad);
+}
+
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+#define REQ(ctx, cond, code, msg)              \
+    do {                                       \
+        if (!(cond)) {                         \
+            (ctx)->err = msg;                  \
+            return code;                       \
+        }                                      \
+    } while (0)
+
+#define PTR_OK(ctx, p)                                                     \
+    do {                                                                   \
+        REQ(ctx, (p) != nullptr, TQP_ERR_ARG, #p " is NULL");              \
+        REQ(ctx, aligned16(p), TQP_ERR_ALIGN, #p " is not 16-byte aligned"); \
+    } while (0)
+
+tqp_status common_checks(tqp_ctx *c, int T, bool need_weights) {
+    if (!c) return TQP_ERR_ARG;
+    c->launches = 0;
+    REQ(c, T > 0 && T <= c->desc.T_max, TQP_ERR_ARG, "T out of range (0 < T <= T_max)");
+    REQ(c, c->base != nullptr, TQP_ERR_WORKSPACE, "no workspace bound");
+    if (need_weights) REQ(c, c->have_weights, TQP_ERR_STATE, "tqp_bind_weights has not been called");
+    return TQP_OK;
+}
+
+tqp_status run_gemm(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st) {
+    return c->gemm_impl == 1 ? launch_gemm_scaffold(c, probs, nprob, st) : launch_gemm_tcgen05(c, probs, nprob, st);
+}
+
+}  // namespace
+
+extern "C" {
+
+tqp_status tqp_create(tqp_ctx **out, const tqp_layer_desc *desc) {
+    if (!out) return TQP_ERR_ARG;
+    *out = nullptr;
+    if (!desc) return TQP_ERR_ARG;
+    if (!desc_ok(desc)) return TQP_ERR_SHAPE;
+    int dev = 0, major = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return TQP_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return TQP_ERR_CUDA;
+    if (major != 10) return TQP_ERR_ARCH;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    tqp_ctx *c = new (std::nothrow) tqp_ctx();
+    if (!c) return TQP_ERR_ARG;
+    c->desc = *desc;
+    c->ws = layout(*desc);
+    c->num_sms = sms > 0 ? sms : 148;
+    c->max_tiles = desc->E + (desc->T_max * desc->k) / kTileRows + 1;
+    memset(&c->w, 0, sizeof(c->w));
+    *out = c;
+    return TQP_OK;
+}
+
+void tqp_destroy(tqp_ctx *ctx) { delete ctx; }
+
+size_t tqp_workspace_bytes(const tqp_layer_desc *desc) {
+    if (!desc_ok(desc)) return 0;
+    return layout(*desc).total;
+}
+
+tqp_status tqp_bind_workspace(tqp_ctx *c, void *dev_ptr, size_t bytes, void *stream) {
+    if (!c) return TQP_ERR_ARG;
+    PTR_OK(c, dev_ptr);
+    REQ(c, bytes >= c->ws.total, TQP_ERR_WORKSPACE, "workspace too small");
+    TQP_CUDA_OK(c, cudaMemsetAsync(dev_ptr, 0, c->ws.total, (cudaStream_t)stream));
+    c->base = static_cast<char *>(dev_ptr);
+    c->bound_bytes = bytes;
+    c->have_weights = false;
+    return TQP_OK;
+}
+
+tqp_status tqp_bind_weights(tqp_ctx *c, const tqp_weights *w, void *stream) {
+    if (!c || !w) return TQP_ERR_ARG;
+    REQ(c, c->base != nullptr, TQP_ERR_WORKSPACE, "bind a workspace first");
+    const void *ptrs[] = {w->idx_gate, w->idx_up, w->idx_down, w->scale_gate, w->scale_up, w->scale_down, w->codebook,
+                          w->A_gate, w->A_up, w->B_gate, w->B_up, w->A_down, w->B_down};
+    for (const void *p : ptrs) PTR_OK(c, p);
+    c->w = *w;
+    c->launches = 0;
+    const tqp_layer_desc &D = c->desc;
+    const uint64_t Np = (uint64_t)D.T_max * D.k + kRowPad;
+    tqp_status st = launch_make_lut(c, (const __half *)w->codebook, c->p<bf16>(c->ws.lut), (cudaStream_t)stream);
+    if (st != TQP_OK) return st;
+    bf16 *Xp = c->p<bf16>(c->ws.Xp), *G = c->p<bf16>(c->ws.G), *U = c->p<bf16>(c->ws.U), *H = c->p<bf16>(c->ws.H);
+    bf16 *dH = c->p<bf16>(c->ws.dH), *dG = c->p<bf16>(c->ws.dG), *dU = c->p<bf16>(c->ws.dU);
+    GemmProblem *P;
+#define CK(x) do { st = (x); if (st != TQP_OK) return st; } while (0)
+    P = &c->prob_gate; memset(P, 0, sizeof(*P));
+    P->nseg = 1; P->nlora = 1; P->M = D.F; P->r = D.r; P->out = G;
+    CK(set_seg(c, &P->seg[0], Xp, Np, w->idx_gate, w->scale_gate, D.d, D.F, 1));
+    CK(set_lora(c, &P->lora[0], c->p<bf16>(c->ws.XAg), Np, w->B_gate, 0));
+    P = &c->prob_up; memset(P, 0, sizeof(*P));
+    P->nseg = 1; P->nlora = 1; P->M = D.F; P->r = D.r; P->out = U;
+    CK(set_seg(c, &P->seg[0], Xp, Np, w->idx_up, w->scale_up, D.d, D.F, 1));
+    CK(set_lora(c, &P->lora[0], c->p<bf16>(c->ws.XAu), Np, w->B_up, 0));
+    P = &c->prob_down; memset(P, 0, sizeof(*P));
+    P->nseg = 1; P->nlora = 1; P->M = D.d; P->r = D.r; P->out = nullptr;   // out = Ye, per call
+    CK(set_seg(c, &P->seg[0], H, Np, w->idx_down, w->scale_down, D.F, D.d, 1));
+    CK(set_lora(c, &P->lora[0], c->p<bf16>(c->ws.HAd), Np, w->B_down, 0));
+    P = &c->prob_dh; memset(P, 0, sizeof(*P));
+    P->nseg = 1; P->nlora = 1; P->M = D.F; P->r = D.r; P->out = dH;       // seg[0].act = dYe, per call
+    CK(set_seg(c, &P->seg[0], dH /*placeholder*/, Np, w->idx_down, w->scale_down, D.d, D.F, 0));
+    CK(set_lora(c, &P->lora[0], c->p<bf16>(c->ws.Zd), Np, w->A_down, 1));
+    P = &c->prob_dx; memset(P, 0, sizeof(*P));
+    P->nseg = 2; P->nlora = 2; P->M = D.d; P->r = D.r; P->out = nullptr;   // out = dXp, per call
+    CK(set_seg(c, &P->seg[0], dG, Np, w->idx_gate, w->scale_gate, D.F, D.d, 0));
+    CK(set_seg(c, &P->seg[1], dU, Np, w->idx_up, w->scale_up, D.F, D.d, 0));
+    CK(set_lora(c, &P->lora[0], c->p<bf16>(c->ws.Zg), Np, w->A_gate, 1));
+    CK(set_lora(c, &P->lora[1], c->p<bf16>(c->ws.Zu), Np, w->A_up, 1));
+#undef CK
+    c->have_weights = true;
+    return TQP_OK;
+}
+
+tqp_status tqp_set_option(tqp_ctx *c, const char *name, int value) {
+    if (!c || !name) return TQP_ERR_ARG;
+    if (!strcmp(name, "gemm_impl")) {
+        REQ(c, value == 0 || value == 1, TQP_ERR_ARG, "gemm_impl must be 0 or 1");
+        c->gemm_impl = value;
+        return TQP_OK;
+    }
+    c->err = "unknown option";
+    return TQP_ERR_ARG;
+}
+
+tqp_status tqp_route(tqp_ctx *c, int T, const void *X, const float *W_r, const float *logit_bias, int32_t *topk_idx,
+                     float *topk_w, float *logits_out, void *stream) {
+    tqp_status st = common_checks(c, T, false);
+    if (st != TQP_OK) return st;
+    PTR_OK(c, X); PTR_OK(c, W_r); PTR_OK(c, topk_idx); PTR_OK(c, topk_w);
+    float *lg = logits_out ? logits_out : c->p<float>(c->ws.logits);
+    return launch_route(c, T, (const bf16 *)X, W_r, logit_bias, topk_idx, topk_w, lg, (cudaStream_t)stream);
+}
+
+tqp_status tqp_dispatch(tqp_ctx *c, int T, const int32_t *topk_idx, int32_t *counts, int32_t *offsets, int32_t *perm,
+                        int32_t *inv_perm, void *stream) {
+    tqp_status st = common_checks(c, T, false);
+    if (st != TQP_OK) return st;
+    PTR_OK(c, topk_idx); PTR_OK(c, counts); PTR_OK(c, offsets); PTR_OK(c, perm); PTR_OK(c, inv_perm);
+    c->disp_T = T;
+    c->fwd_T = -1;
+    return launch_dispatch(c, T, topk_idx, counts, offsets, perm, inv_perm, (cudaStream_t)stream);
+}
+
+tqp_status tqp_expert_fwd(tqp_ctx *c, int T, const void *X, const int32_t *offsets, const int32_t *perm, void *Ye,
+                          void *stream) {
+    tqp_status st = common_checks(c, T, true);
+    if (st != TQP_OK) return st;
+    PTR_OK(c, X); PTR_OK(c, offsets); PTR_OK(c, perm); PTR_OK(c, Ye);
+    REQ(c, c->disp_T == T, TQP_ERR_STATE, "tqp_expert_fwd must follow tqp_dispatch with the same T");
+    cudaStream_t s = (cudaStream_t)stream;
+    const tqp_layer_desc &D = c->desc;
+    const int N = T * D.k;
+    const float ls = D.lora_scale;
+    bf16 *Xp = c->p<bf16>(c->ws.Xp), *G = c->p<bf16>(c->ws.G), *U = c->p<bf16>(c->ws.U), *H = c->p<bf16>(c->ws.H);
+#define CK(x) do { st = (x); if (st != TQP_OK) return st; } while (0)
+    CK(launch_gather_rows(c, N, (const bf16 *)X, perm, Xp, s));
+    CK(launch_lora_down(c, Xp, D.d, (const bf16 *)c->w.A_gate, 1, ls, c->p<bf16>(c->ws.XAg), s));
+    CK(launch_lora_down(c, Xp, D.d, (const bf16 *)c->w.A_up, 1, ls, c->p<bf16>(c->ws.XAu), s));
+    GemmProblem pr[2] = {c->prob_gate, c->prob_up};
+    CK(run_gemm(c, pr, 2, s));
+    CK(launch_swiglu_fwd(c, N, G, U, H, s));
+    CK(launch_lora_down(c, H, D.F, (const bf16 *)c->w.A_down, 1, ls, c->p<bf16>(c->ws.HAd), s));
+    GemmProblem pd = c->prob_down;
+    pd.out = (bf16 *)Ye;
+    CK(run_gemm(c, &pd, 1, s));
+#undef CK
+    c->fwd_T = D.training ? T : -1;
+    return TQP_OK;
+}
+
+tqp_status tqp_combine(tqp_ctx *c, int T, const void *Ye, const int32_t *inv_perm, const float *topk_w, void *Y,
+                       void *stream) {
+    tqp_status st = common_checks(c, T, false);
+    if (st != TQP_OK) return st;
+    PTR_OK(c, Ye); PTR_OK(c, inv_perm); PTR_OK(c, topk_w); PTR_OK(c, Y);
+    return launch_combine(c, T, (const bf16 *)Ye, inv_perm, topk_w, (bf16 *)Y, (cudaStream_t)stream);
+}
+
+tqp_status tqp_combine_bwd(tqp_ctx *c, int T, const void *dY, const void *Ye, const int32_t *inv_perm,
+                           const float *topk_w, void *dYe, float *dtopk_w, void *stream) {
+    tqp_status st = common_checks(c, T, false);
+    if (st != TQP_OK) return st;
+    PTR_OK(c, dY); PTR_OK(c, inv_perm); PTR_OK(c, topk_w); PTR_OK(c, dYe);
+    if (dtopk_w) PTR_OK(c, Ye);
+    return launch_combine_bwd(c, T, (const bf16 *)dY, (const bf16 *)Ye, inv_perm, topk_w, (bf16 *)dYe, dtopk_w,
+                              (cudaStream_t)stream);
+}
+
+
+tqp_status tqp_expert_bwd(tqp_ctx *c, int T, const void *X, const void *dYe, const int32_t *offsets, const int32_t *perm,
+                          void *dXp, float *dA_gate, float *dB_gate, float *dA_up, float *dB_up, float *dA_down,
+                          float *dB_down, void *stream) {
+    tqp_status st = common_checks(c, T, true);
+    if (st != TQP_OK) return st;
+    PTR_OK(c, X); PTR_OK(c, dYe); PTR_OK(c, offsets); PTR_OK(c, perm); PTR_OK(c, dXp);
+    PTR_OK(c, dA_gate); PTR_OK(c, dB_gate); PTR_OK(c, dA_up); PTR_OK(c, dB_up); PTR_OK(c, dA_down); PTR_OK(c, dB_down);
+    REQ(c, c->desc.training == 1, TQP_ERR_STATE, "tqp_expert_bwd needs a ctx created with training=1");
+    REQ(c, c->fwd_T == T, TQP_ERR_STATE, "tqp_expert_bwd must follow a training-mode tqp_expert_fwd with the same T");
+    cudaStream_t s = (cudaStream_t)stream;
+    const tqp_layer_desc &D = c->desc;
+    const int N = T * D.k;
+    const float ls = D.lora_scale;
+    const bf16 *dye = (const bf16 *)dYe;
+    bf16 *Xp = c->p<bf16>(c->ws.Xp), *G = c->p<bf16>(c->ws.G), *U = c->p<bf16>(c->ws.U), *H = c->p<bf16>(c->ws.H);
+    bf16 *dH = c->p<bf16>(c->ws.dH), *dG = c->p<bf16>(c->ws.dG), *dU = c->p<bf16>(c->ws.dU);
+    bf16 *Zd = c->p<bf16>(c->ws.Zd), *Zg = c->p<bf16>(c->ws.Zg), *Zu = c->p<bf16>(c->ws.Zu);
+#define CK(x) do { st = (x); if (st != TQP_OK) return st; } while (0)
+    // down projection: dH = dYe . Wd_eff^T,  dB_d = (s h A_d)^T dYe,  dA_d = h^T (s dYe B_d^T)
+    CK(launch_lora_down(c, dye, D.d, (const bf16 *)c->w.B_down, 0, ls, Zd, s));
+    GemmProblem ph = c->prob_dh;
+    ph.seg[0].act = dye;
+    CK(act_map(c, &ph.seg[0].act_map, dye, (uint64_t)N, D.d));
+    CK(run_gemm(c, &ph, 1, s));
+    CK(launch_swiglu_bwd(c, N, dH, G, U, dG, dU, s));
+    CK(launch_lora_wgrad(c, dye, D.d, c->p<bf16>(c->ws.HAd), offsets, 0, dB_down, s));
+    CK(launch_lora_wgrad(c, H, D.F, Zd, offsets, 1, dA_down, s));
+    // gate / up projections: dXp = dG . Wg_eff^T + dU . Wu_eff^T and their adapter gradients
+    CK(launch_lora_down(c, dG, D.F, (const bf16 *)c->w.B_gate, 0, ls, Zg, s));
+    CK(launch_lora_down(c, dU, D.F, (const bf16 *)c->w.B_up, 0, ls, Zu, s));
+    GemmProblem px = c->prob_dx;
+    px.out = (bf16 *)dXp;
+    CK(run_gemm(c, &px, 1, s));
+    CK(launch_lora_wgrad(c, dG, D.F, c->p<bf16>(c->ws.XAg), offsets, 0, dB_gate, s));
+    CK(launch_lora_wgrad(c, dU, D.F, c->p<bf16>(c->ws.XAu), offsets, 0, dB_up, s));
+    CK(launch_lora_wgrad(c, Xp, D.d, Zg, offsets, 1, dA_gate, s));
+    CK(launch_lora_wgrad(c, Xp, D.d, Zu, offsets, 1, dA_up, s));
+#undef CK
+    return TQP_OK;
+}
+
+tqp_status tqp_dispatch_bwd(tqp_ctx *c, int T, const void *dXp, const int32_t *inv_perm, void *dX, void *stream) {
+    tqp_status st = common_checks(c, T, false);
+    if (st != TQP_OK) return st;
+    PTR_OK(c, dXp); PTR_OK(c, inv_perm); PTR_OK(c, dX);
+    return launch_combine(c, T, (const bf16 *)dXp, inv_perm, nullptr, (bf16 *)dX, (cudaStream_t)stream);
+}
+
+tqp_status tqp_route_bwd(tqp_ctx *c, int T, const void *X, const float *W_r, const int32_t *topk_idx,
+                         const float *topk_w, const float *dtopk_w, const int32_t *offsets, const int32_t *perm, void *dX,
+                         float *dW_r, void *stream) {
+    tqp_status st = common_checks(c, T, false);
+    if (st != TQP_OK) return st;
+    PTR_OK(c, X); PTR_OK(c, W_r); PTR_OK(c, topk_idx); PTR_OK(c, topk_w); PTR_OK(c, dtopk_w); PTR_OK(c, offsets);
+    PTR_OK(c, perm); PTR_OK(c, dX); PTR_OK(c, dW_r);
+    return launch_route_bwd(c, T, (const bf16 *)X, W_r, topk_idx, topk_w, dtopk_w, offsets, perm, (bf16 *)dX, dW_r,
+                            (cudaStream_t)stream);
+}
+
+tqp_status tqp_step_host(tqp_ctx *c, int T, const void *X_host, const void *dY_host, const float *W_r,
+                         const float *logit_bias, void *Y_host, void *dX_host, float *dA_gate, float *dB_gate,
+                         float *dA_up, float *dB_up, float *dA_down, float *dB_down, float *dW_r, void *stream) {
+    tqp_status st = common_checks(c, T, true);
+    if (st != TQP_OK) return st;
+    REQ(c, X_host && dY_host && Y_host && dX_host, TQP_ERR_ARG, "host buffer is NULL");
+    cudaStream_t s = (cudaStream_t)stream;
+    const tqp_layer_desc &D = c->desc;
+    const size_t row_bytes = (size_t)T * D.d * 2;
+    bf16 *X = c->p<bf16>(c->ws.hX), *dY = c->p<bf16>(c->ws.hdY), *Y = c->p<bf16>(c->ws.hY), *dX = c->p<bf16>(c->ws.hdX);
+    int32_t *ti = c->p<int32_t>(c->ws.topk_idx), *counts = c->p<int32_t>(c->ws.counts), *offs = c->p<int32_t>(c->ws.offsets);
+    int32_t *perm = c->p<int32_t>(c->ws.perm), *inv = c->p<int32_t>(c->ws.inv_perm);
+    float *tw = c->p<float>(c->ws.topk_w), *dtw = c->p<float>(c->ws.dtopk_w);
+    bf16 *Ye = c->p<bf16>(c->ws.Ye), *dYe = c->p<bf16>(c->ws.dYe), *dXp = c->p<bf16>(c->ws.dXp);
+    int total = 0;
+#define CK(x) do { st = (x); total += c->launches; if (st != TQP_OK) return st; } while (0)
+    TQP_CUDA_OK(c, cudaMemcpyAsync(X, X_host, row_bytes, cudaMemcpyHostToDevice, s));
+    TQP_CUDA_OK(c, cudaMemcpyAsync(dY, dY_host, row_bytes, cudaMemcpyHostToDevice, s));
+    CK(tqp_route(c, T, X, W_r, logit_bias, ti, tw, nullptr, s));
+    CK(tqp_dispatch(c, T, ti, counts, offs, perm, inv, s));
+    CK(tqp_expert_fwd(c, T, X, offs, perm, Ye, s));
+    CK(tqp_combine(c, T, Ye, inv, tw, Y, s));
+    TQP_CUDA_OK(c, cudaMemcpyAsync(Y_host, Y, row_bytes, cudaMemcpyDeviceToHost, s));
+    CK(tqp_combine_bwd(c, T, dY, Ye, inv, tw, dYe, dW_r ? dtw : nullptr, s));
+    CK(tqp_expert_bwd(c, T, X, dYe, offs, perm, dXp, dA_gate, dB_gate, dA_up, dB_up, dA_down, dB_down, s));
+    CK(tqp_dispatch_bwd(c, T, dXp, inv, dX, s));
+    if (dW_r) CK(tqp_route_bwd(c, T, X, W_r, ti, tw, dtw, offs, perm, dX, dW_r, s));
+#undef CK
+    TQP_CUDA_OK(c, cudaMemcpyAsync(dX_host, dX, row_bytes, cudaMemcpyDeviceToHost, s));
+    TQP_CUDA_OK(c, cudaStreamSynchronize(s));
+    c->launches = total;
+    return TQP_OK;
+}
+
+void *tqp_debug_buffer(tqp_ctx *c, const char *name) {
+    if (!c || !name || !c->base) return nullptr;
+    struct { const char *n; size_t off; } tab[] = {
+        {"G", c->ws.G}, {"U", c->ws.U}, {"H", c->ws.H}, {"Xp", c->ws.Xp}, {"dH", c->ws.dH}, {"dG", c->ws.dG},
+        {"dU", c->ws.dU}, {"num_tiles", c->ws.num_tiles}, {"tiles", c->ws.tiles}, {"XAg", c->ws.XAg}, {"Zd", c->ws.Zd},
+        {"logits", c->ws.logits}, {"lut", c->ws.lut}};
+    for (auto &t : tab)
+        if (!strcmp(t.n, name)) return c->base + t.off;
+    return nullptr;
+}
+
+int tqp_last_launch_count(const tqp_ctx *c) { return c ? c->launches : 0; }
+
+const char *tqp_status_string(tqp_status s) {
+    switch (s) {
+        case TQP_OK: return "TQP_OK";
+        case TQP_ERR_ARG: return "TQP_ERR_ARG";
+        case TQP_ERR_SHAPE: return "TQP_ERR_SHAPE";
+        case TQP_ERR_ALIGN: return "TQP_ERR_ALIGN";
+        case TQP_ERR_WORKSPACE: return "TQP_ERR_WORKSPACE";
+        case TQP_ERR_STATE: return "TQP_ERR_STATE";
+        case TQP_ERR_ARCH: return "TQP_ERR_ARCH";
+        case TQP_ERR_CUDA: return "TQP_ERR_CUDA";
+    }
+    return "TQP_ERR_UNKNOWN";
+}
+
+const char *tqp_last_error(const tqp_ctx *c) { return c ? c->err.c_str() : ""; }
+
+}  // extern "C"

@@ -1,0 +1,150 @@
+// Shared declarations of the TQP routed-expert library (sm_100a).  Product code: nothing here is shared
+// with oracle/.
+#pragma once
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "../../include/tqp.h"
+
+namespace tqp {
+
+typedef __nv_bfloat16 bf16;
+
+constexpr int kTileRows = 256;   // max routed rows (UMMA N) of one grouped-GEMM tile
+constexpr int kRowPad = 512;     // rows of slack after N in every [N][*] workspace tensor (TMA boxes / 16-row groups over-read)
+constexpr int kLoraPad = 64;     // adapter projections are stored [N][64] bf16 (one 128-byte swizzle row)
+constexpr int kDispChunk = 256;  // assignments per warp in the dispatch kernels
+
+struct Tile {          // one token tile of the grouped GEMMs: rows [row0, row0+rows) all belong to `expert`
+    int32_t expert, row0, rows, pad;
+};
+
+// One GEMM "problem": out[p][m] = sum_seg sum_k act_seg[p][k] * Wdeq_seg[m][k] + sum_l lact_l[p][q] * lw_l[m][q]
+// (swap-AB on the tensor cores: M = weight output channels, N = routed rows).
+struct GemmSeg {
+    const bf16 *act;        // [N][K] bf16 activations (B operand)
+    const uint8_t *idx;     // codes of all experts
+    const __half *scale;    // per-output-channel scales of all experts
+    int K;                  // contraction length of this segment
+    int kmajor;             // 1: idx[e][M][K/8] (forward), 0: idx[e][K][M/8] (backward, transposed use)
+    CUtensorMap act_map;    // box {64, kTileRows} over act, SWIZZLE_128B
+    CUtensorMap idx_map;    // box {16, 128} over idx viewed as [rows][bytes]
+};
+struct GemmLora {
+    const bf16 *lact;       // [N][kLoraPad] bf16 (already multiplied by lora_scale)
+    const bf16 *lw;         // adapter matrix of all experts
+    int mk_layout;          // 1: lw[e][M][r] (K-major), 0: lw[e][r][M]
+    CUtensorMap lact_map;   // box {64, kTileRows}
+};
+struct GemmProblem {
+    GemmSeg seg[2];
+    GemmLora lora[2];
+    int nseg, nlora;
+    int M;                  // output channels
+    int r;
+    bf16 *out;              // [N][M]
+};
+
+struct GemmArgs {           // passed by value (__grid_constant__) so the tensor maps live in param space
+    GemmProblem p[2];
+    int nprob;
+};
+
+struct Workspace {
+    // sizes
+    size_t total = 0;
+    // offsets (bytes) into the bound buffer
+    size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, lut, WrT, dl,
+        // tqp_step_host staging
+        hX, hdY, hY, hdX, topk_idx, topk_w, counts, offsets, perm, inv_perm, Ye, dYe, dXp, dtopk_w;
+};
+
+}  // namespace tqp
+
+struct tqp_ctx {
+    tqp_layer_desc desc;
+    tqp::Workspace ws;
+    char *base = nullptr;       // bound workspace
+    size_t bound_bytes = 0;
+    tqp_weights w;
+    bool have_weights = false;
+    int gemm_impl = 0;          // 0 tcgen05, 1 scaffold
+    int fwd_T = -1;             // T of the last training-mode expert_fwd (TQP_ERR_STATE check)
+    int disp_T = -1;
+    int launches = 0;
+    int num_sms = 148;
+    int max_tiles = 0;
+    std::string err;
+    // tensor maps over weights / workspace (built in bind_weights)
+    tqp::GemmProblem prob_gate, prob_up, prob_down, prob_dh, prob_dx;
+
+    template <class T> T *p(size_t off) const { return reinterpret_cast<T *>(base + off); }
+};
+
+namespace tqp {
+
+#define TQP_CUDA_OK(ctx, call)                                                          \
+    do {                                                                                \
+        cudaError_t e__ = (call);                                                       \
+        if (e__ != cudaSuccess) {                                                       \
+            (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e__);           \
+            return TQP_ERR_CUDA;                                                        \
+        }                                                                               \
+    } while (0)
+
+#define TQP_LAUNCH_OK(ctx)                                                              \
+    do {                                                                                \
+        (ctx)->launches++;                                                              \
+        cudaError_t e__ = cudaGetLastError();                                           \
+        if (e__ != cudaSuccess) {                                                       \
+            (ctx)->err = std::string(__FILE__) + ":" + std::to_string(__LINE__) + ": " + cudaGetErrorString(e__); \
+            return TQP_ERR_CUDA;                                                        \
+        }                                                                               \
+    } while (0)
+
+// ---- kernels.cu ----------------------------------------------------------------------------------------
+tqp_status launch_route(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const float *bias, int32_t *topk_idx,
+                        float *topk_w, float *logits, cudaStream_t s);
+tqp_status launch_dispatch(tqp_ctx *c, int T, const int32_t *topk_idx, int32_t *counts, int32_t *offsets,
+                           int32_t *perm, int32_t *inv_perm, cudaStream_t s);
+tqp_status launch_gather_rows(tqp_ctx *c, int N, const bf16 *X, const int32_t *perm, bf16 *Xp, cudaStream_t s);
+tqp_status launch_swiglu_fwd(tqp_ctx *c, int N, const bf16 *G, const bf16 *U, bf16 *H, cudaStream_t s);
+tqp_status launch_swiglu_bwd(tqp_ctx *c, int N, const bf16 *dH, const bf16 *G, const bf16 *U, bf16 *dG, bf16 *dU,
+                             cudaStream_t s);
+tqp_status launch_combine(tqp_ctx *c, int T, const bf16 *Ye, const int32_t *inv_perm, const float *topk_w, bf16 *Y,
+                          cudaStream_t s);
+tqp_status launch_combine_bwd(tqp_ctx *c, int T, const bf16 *dY, const bf16 *Ye, const int32_t *inv_perm,
+                              const float *topk_w, bf16 *dYe, float *dtopk_w, cudaStream_t s);
+tqp_status launch_route_bwd(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const int32_t *topk_idx,
+                            const float *topk_w, const float *dtopk_w, const int32_t *offsets, const int32_t *perm,
+                            bf16 *dX, float *dW_r, cudaStream_t s);
+tqp_status launch_make_lut(tqp_ctx *c, const __half *codebook, bf16 *lut, cudaStream_t s);
+
+// ---- lora.cu -------------------------------------------------------------------------------------------
+// out[p][0..r) = s * sum_k in[p][k] * W_e[...]   (W_e [K][r] if w_kr else [r][K]); out is [N][kLoraPad] bf16
+tqp_status launch_lora_down(tqp_ctx *c, const bf16 *in, int K, const bf16 *W, int w_kr, float s, bf16 *out,
+                            cudaStream_t st);
+// grad[e] = sum_{p in e} small[p][q] * big[p][a]; stored [a][q] (out_ar=1: dA) or [q][a] (out_ar=0: dB), fp32
+tqp_status launch_lora_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 *small_, const int32_t *offsets,
+                             int out_ar, float *grad, cudaStream_t st);
+
+// ---- gemm_scaffold.cu / gemm_tcgen05.cu -----------------------------------------------------------------
+tqp_status launch_gemm_scaffold(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);
+tqp_status launch_gemm_tcgen05(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);
+
+// ---- device helpers ------------------------------------------------------------------------------------
+__device__ __forceinline__ float bf16_bits_to_float(uint16_t b) { return __uint_as_float(((uint32_t)b) << 16); }
+__device__ __forceinline__ float2 bf16x2_to_float2(uint32_t v) {
+    return make_float2(__uint_as_float(v << 16), __uint_as_float(v & 0xffff0000u));
+}
+__device__ __forceinline__ uint32_t float2_to_bf16x2(float lo, float hi) {
+    __nv_bfloat162 t = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t *>(&t);
+}
+
+}  // namespace tqp

@@ -1,0 +1,126 @@
+// Dispatch: stable counting sort of the flat assignments a = t*k+j by expert id (histogram / scan / ranked
+// scatter), bit-exact against the oracle, plus the device-side tile list of the grouped GEMMs.
+// PAPER.md L289 ("MoE routing and expert dispatch"), L553 ("grouped MoE expert computation").
+#include "common.cuh"
+
+namespace tqp {
+
+// Phase 1: each warp owns one chunk of kDispChunk consecutive assignments and counts them per expert.
+__global__ void __launch_bounds__(128) dispatch_hist_kernel(const int32_t *__restrict__ topk_idx, int N, int E,
+                                                            int32_t *__restrict__ blk_counts) {
+    extern __shared__ int32_t sm[];
+    const int warp_in_blk = threadIdx.x / 32, lane = threadIdx.x % 32;
+    const int chunk = blockIdx.x * 4 + warp_in_blk;
+    int32_t *cnt = sm + warp_in_blk * E;
+    for (int e = lane; e < E; e += 32) cnt[e] = 0;
+    __syncwarp();
+    const int a0 = chunk * kDispChunk;
+    for (int i = lane; i < kDispChunk; i += 32) {
+        int a = a0 + i;
+        if (a < N) atomicAdd(&cnt[topk_idx[a]], 1);
+    }
+    __syncwarp();
+    if (a0 < N)
+        for (int e = lane; e < E; e += 32) blk_counts[(size_t)chunk * E + e] = cnt[e];
+}
+
+// Phase 2 (one block): per expert exclusive scan over the chunks -> chunk bases; exclusive scan over experts
+// -> offsets; tile list.  blk_counts is overwritten by the absolute base position of (chunk, expert).
+__global__ void __launch_bounds__(1024) dispatch_scan_kernel(int32_t *__restrict__ blk_counts, int nchunks, int N, int E,
+                                                             int32_t *__restrict__ counts, int32_t *__restrict__ offsets,
+                                                             Tile *__restrict__ tiles, int32_t *__restrict__ num_tiles) {
+    __shared__ int32_t s_cnt[1024], s_off[1025], s_tiles[1025];
+    const int e = threadIdx.x;
+    int total = 0;
+    if (e < E) {
+        for (int c = 0; c < nchunks; ++c) {
+            int v = blk_counts[(size_t)c * E + e];
+            blk_counts[(size_t)c * E + e] = total;   // base of this chunk inside the expert's segment
+            total += v;
+        }
+    }
+    s_cnt[e] = (e < E) ? total : 0;
+    __syncthreads();
+    if (e == 0) {
+        int acc = 0, tacc = 0;
+        for (int q = 0; q < E; ++q) {
+            s_off[q] = acc;
+            s_tiles[q] = tacc;
+            acc += s_cnt[q];
+            tacc += (s_cnt[q] + kTileRows - 1) / kTileRows;
+        }
+        s_off[E] = acc;
+        s_tiles[E] = tacc;
+        *num_tiles = tacc;
+    }
+    __syncthreads();
+    if (e < E) {
+        counts[e] = s_cnt[e];
+        offsets[e] = s_off[e];
+        if (e == E - 1) offsets[E] = s_off[E];
+        const int cnt = s_cnt[e], nt = (cnt + kTileRows - 1) / kTileRows;
+        if (nt > 0) {
+            int per = (cnt + nt - 1) / nt;
+            per = (per + 15) & ~15;   // balanced tiles, multiples of 16 rows (UMMA N granularity)
+            for (int i = 0; i < nt; ++i) {
+                Tile t;
+                t.expert = e;
+                t.row0 = s_off[e] + i * per;
+                t.rows = max(0, min(per, cnt - i * per));   // rows == 0: skipped by the consumers
+                t.pad = 0;
+                tiles[s_tiles[e] + i] = t;
+            }
+        }
+        for (int c = 0; c < nchunks; ++c) blk_counts[(size_t)c * E + e] += s_off[e];
+    }
+}
+
+// Phase 3: ranked scatter.  Inside a chunk the 32-wide groups are processed in order; __match_any_sync gives
+// the rank among equal experts inside a group, so rows of one expert stay in ascending a (stable).
+__global__ void __launch_bounds__(128) dispatch_scatter_kernel(const int32_t *__restrict__ topk_idx, int N, int E,
+                                                               const int32_t *__restrict__ blk_base,
+                                                               int32_t *__restrict__ perm, int32_t *__restrict__ inv_perm) {
+    extern __shared__ int32_t sm[];
+    const int warp_in_blk = threadIdx.x / 32, lane = threadIdx.x % 32;
+    const int chunk = blockIdx.x * 4 + warp_in_blk;
+    const int a0 = chunk * kDispChunk;
+    if (a0 >= N) return;
+    int32_t *cur = sm + warp_in_blk * E;
+    for (int e = lane; e < E; e += 32) cur[e] = blk_base[(size_t)chunk * E + e];
+    __syncwarp();
+    for (int i = 0; i < kDispChunk; i += 32) {
+        int a = a0 + i + lane;
+        bool valid = a < N;
+        int e = valid ? topk_idx[a] : -1 - lane;   // invalid lanes get unique keys
+        uint32_t peers = __match_any_sync(0xffffffffu, e);
+        int rank = __popc(peers & ((1u << lane) - 1u));
+        int p = 0;
+        if (valid) p = cur[e] + rank;
+        __syncwarp();
+        if (valid && rank == 0) cur[e] += __popc(peers);   // one leader per expert in this group
+        __syncwarp();
+        if (valid) {
+            perm[p] = a;
+            inv_perm[a] = p;
+        }
+    }
+}
+
+tqp_status launch_dispatch(tqp_ctx *c, int T, const int32_t *topk_idx, int32_t *counts, int32_t *offsets,
+                           int32_t *perm, int32_t *inv_perm, cudaStream_t s) {
+    const int E = c->desc.E, N = T * c->desc.k;
+    const int nchunks = (N + kDispChunk - 1) / kDispChunk;
+    const int nblk = (nchunks + 3) / 4;
+    int32_t *blk = c->p<int32_t>(c->ws.blk_counts);
+    const size_t smem = (size_t)4 * E * sizeof(int32_t);
+    dispatch_hist_kernel<<<nblk, 128, smem, s>>>(topk_idx, N, E, blk);
+    TQP_LAUNCH_OK(c);
+    dispatch_scan_kernel<<<1, 1024, 0, s>>>(blk, nchunks, N, E, counts, offsets, c->p<Tile>(c->ws.tiles),
+                                            c->p<int32_t>(c->ws.num_tiles));
+    TQP_LAUNCH_OK(c);
+    dispatch_scatter_kernel<<<nblk, 128, smem, s>>>(topk_idx, N, E, blk, perm, inv_perm);
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
+
+}  // namespace tqp

@@ -1,0 +1,96 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on seeded inputs.
+Bit-exact for routing/permutation; max-abs <= 2e-2*max|ref| and relative Frobenius <= 1e-2 for floats (north_star)."""
+import numpy as np
+import pytest
+
+import oracle
+import tqp_inputs as ti
+from parity_util import assert_close, assert_routing_exact, errors, run_gpu
+
+pytestmark = pytest.mark.gpu
+
+FWD_KEYS = ("Xp", "G", "U", "H", "Ye", "Y")
+BWD_KEYS = ("dYe", "dXp", "dX_experts", "dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down")
+RG_KEYS = ("dtopk_w", "dW_r", "dX")
+
+
+def oracle_ref(inp, backward, router_grad):
+    ref = oracle.layer(inp, dtype=np.float32, backward=backward, router_grad=router_grad)
+    ref["Xp"] = ti.bf16_bits_to_f32(inp["X"])[ref["perm"] // inp["k"]]
+    return ref
+
+
+def check_all(inp, backward, router_grad, gemm_impl, report=None):
+    ref = oracle_ref(inp, backward, router_grad)
+    gpu = run_gpu(inp, backward=backward, router_grad=router_grad, gemm_impl=gemm_impl)
+    assert_routing_exact(gpu, ref)
+    keys = FWD_KEYS + (BWD_KEYS if backward else ()) + (RG_KEYS if router_grad else ())
+    errs = {}
+    for key in keys:
+        errs[key] = errors(gpu[key], ref[key])
+    if report is not None:
+        report.update(errs)
+    for key in keys:
+        assert_close(key, gpu[key], ref[key])
+    return gpu, ref
+
+
+MID = ti.Config("mid_ragged", T=640, d=256, F=384, E=6, k=3, r=16, seed=21, router_grad=True)
+MID32 = ti.Config("mid_r32", T=300, d=384, F=256, E=5, k=2, r=32, seed=22, router_grad=True)
+
+
+def _skewed(cfg):
+    """Same recipe, plus a logit bias that sends >256 rows to one expert and none to another (several tiles per
+    expert, a ragged tail, an empty expert)."""
+    inp = ti.make_inputs(cfg)
+    bias = np.zeros(cfg.E, np.float32)
+    bias[1] = 2.0
+    bias[cfg.E - 1] = -50.0
+    inp["logit_bias"] = bias
+    return inp
+
+
+@pytest.mark.parametrize("gemm_impl", [1, 0], ids=["scaffold", "tcgen05"])
+def test_cfg0_tiny_full_chain(gemm_impl):
+    cfg = ti.CONFIGS[0]
+    inp = ti.make_inputs(cfg)
+    check_all(inp, backward=True, router_grad=True, gemm_impl=gemm_impl)
+
+
+@pytest.mark.parametrize("gemm_impl", [1, 0], ids=["scaffold", "tcgen05"])
+@pytest.mark.parametrize("cfg", [MID, MID32], ids=lambda c: c.name)
+def test_mid_ragged_multi_tile(cfg, gemm_impl):
+    inp = _skewed(cfg)
+    gpu, ref = check_all(inp, backward=True, router_grad=True, gemm_impl=gemm_impl)
+    assert ref["counts"].max() > 256 and ref["counts"].min() == 0
+    for key in ("dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down"):
+        assert (gpu[key][cfg.E - 1] == 0).all()        # empty expert: exactly zero gradients
+
+
+def test_routing_ties_lower_id_wins():
+    cfg = ti.CONFIGS[0]
+    inp = ti.make_inputs(cfg)
+    inp["W_r"][:, 5] = inp["W_r"][:, 1]      # duplicate router columns -> exact ties
+    inp["W_r"][:, 6] = inp["W_r"][:, 1]
+    ref = oracle_ref(inp, False, False)
+    gpu = run_gpu(inp, backward=False, gemm_impl=1)
+    assert_routing_exact(gpu, ref)
+
+
+def test_error_codes_on_device():
+    import torch
+    import paper_2606_07404_b200 as tq
+    layer = tq.TqpLayer(64, 128, 256, 8, 2, 8)
+    X = torch.zeros(64, 128, dtype=torch.bfloat16, device="cuda")
+    W = torch.zeros(128, 8, device="cuda")
+    idx, w = layer.route(X, W)
+    counts, offsets, perm, inv = layer.dispatch(idx)
+    with pytest.raises(tq.TqpError) as e:
+        layer.expert_fwd(X, offsets, perm)            # no weights bound
+    assert e.value.code == 5
+    with pytest.raises(tq.TqpError) as e:
+        layer.route(X[:0], W)                          # T == 0
+    assert e.value.code == 1
+    with pytest.raises(tq.TqpError) as e:
+        layer.route(torch.zeros(65 * 128 + 1, dtype=torch.bfloat16, device="cuda")[1:].view(65, 128)[:64], W)
+    assert e.value.code == 3                           # misaligned pointer
