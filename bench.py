@@ -1,0 +1,282 @@
+#!/usr/bin/env python
+"""bench.py — expert-layer fwd+bwd throughput of the TQP routed-expert layer on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path (route -> dispatch -> expert_fwd -> combine ->
+combine_bwd -> expert_bwd -> dispatch_bwd [-> route_bwd]) over one synthetic batch of the 120B-shaped config.
+
+    python bench.py --gpus 1 --steps 20 --warmup 5            # our CUDA path (default workload: configs[2])
+    python bench.py --impl reference --steps 3 --warmup 1     # the CPU oracle on a bounded sample (reference arm)
+    torchrun ... bench.py --gpus N ...                        # N independent batches, no collective (weak scaling)
+
+Prints ONE JSON line on rank 0.  Inputs are seeded synthetic tensors (tqp_inputs.py); they are far larger than L2
+(code indices 452 MB + permuted rows 503 MB per step at configs[2]), so no explicit L2 flush is needed.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+import tqp_inputs as ti  # noqa: E402
+
+METRIC = "expert-layer fwd+bwd tokens/s (TQP routed-expert layer, 120B shape)"
+
+
+def flops(cfg, T):
+    """Algorithmic work of one fwd+bwd step; the avoided frozen-weight gradient is not counted."""
+    N = T * cfg.k
+    base = 12.0 * N * cfg.d * cfg.F                      # 3 packs x (fwd + dX) x 2 flop/MAC
+    lora = 18.0 * N * cfg.r * (cfg.d + cfg.F)            # fwd, activation-grad, weight-grad of the adapters
+    router = 2.0 * T * cfg.d * cfg.E
+    gemm = base + 6.0 * N * cfg.r * (cfg.d + cfg.F)      # what the grouped-GEMM kernels themselves execute
+    return dict(total=base + lora + router, base=base, lora=lora, router=router, gemm=gemm)
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(tensor_burst=p["bf16_tflops"], tensor_sustained=p["bf16_tflops_sustained"], hbm=p["hbm_gbs"],
+                    source="measured (MEASURED_PEAKS.json)")
+    return dict(tensor_burst=1590.0, tensor_sustained=1400.0, hbm=6650.0, source="fallback (B200_PROFILING.md)")
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks and throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([c.strip() for c in out.strip().split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        good = [r for r in self.rows if len(r) == 6 and r[0].isdigit()]
+        if not good:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[2 + i] == "Active" for r in good)]
+        return {"sm_mhz": float(np.median([int(r[0]) for r in good])), "sm_max_mhz": float(good[0][1]),
+                "reasons": reasons, "samples": len(good)}
+
+
+def oracle_step(inp, cfg):
+    import oracle
+    return oracle.layer(inp, dtype=np.float32, backward=True, router_grad=cfg.router_grad)
+
+
+def time_oracle(cfg, T_sample, steps, warmup):
+    import oracle
+    oracle.build()
+    inp = ti.make_inputs(cfg, T=T_sample)
+    for _ in range(warmup):
+        oracle_step(inp, cfg)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle_step(inp, cfg)
+    dt = (time.perf_counter() - t0) / max(steps, 1)
+    return dict(value=T_sample / dt, unit="tokens/s", cores=oracle.num_threads(), kind="oracle",
+                sample=f"T={T_sample} of {cfg.T} tokens, all {cfg.E} experts, fwd+bwd, fp32, {steps} step(s) of {dt:.2f} s",
+                seconds_per_step=dt, gflops=flops(cfg, T_sample)["total"] / dt / 1e9)
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    T_s = args.ref_tokens
+    cb = time_oracle(cfg, T_s, args.steps, args.warmup)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": cb["value"], "unit": "tokens/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": cb["seconds_per_step"] * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": cfg.name, "T": cfg.T, "d": cfg.d, "F": cfg.F, "E": cfg.E, "k": cfg.k, "r": cfg.r,
+                   "sample_tokens": T_s},
+        "cpu_baseline": {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")},
+        "e2e": {"value": cb["value"], "unit": "tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, cfg):
+    import torch
+    import paper_2606_07404_b200 as tq
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dev = torch.device(f"cuda:{local}")
+    torch.cuda.set_device(dev)
+
+    # each rank owns an independent batch of the same shape (weak scaling, no data-path collective)
+    import dataclasses
+    rcfg = dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+    inp = ti.make_inputs(rcfg)
+    T, k, d = cfg.T, cfg.k, cfg.d
+    layer = tq.TqpLayer(T, cfg.d, cfg.F, cfg.E, cfg.k, cfg.r, lora_scale=cfg.lora_scale, training=True, device=str(dev))
+    if args.gemm_impl:
+        layer.set_option("gemm_impl", args.gemm_impl)
+
+    def up(a):
+        t = torch.from_numpy(a.view(np.int16)).view(torch.bfloat16) if a.dtype == np.uint16 else torch.from_numpy(a)
+        return t.to(dev)
+
+    wnames = ("idx_gate", "idx_up", "idx_down", "scale_gate", "scale_up", "scale_down", "codebook",
+              "A_gate", "A_up", "B_gate", "B_up", "A_down", "B_down")
+    layer.bind_weights(**{n: up(inp[n]) for n in wnames})
+    X, dY, W_r = up(inp["X"]), up(inp["dY"]), up(inp["W_r"])
+    bias = up(inp["logit_bias"]) if inp["logit_bias"] is not None else None
+    N = T * k
+    bf = torch.bfloat16
+    Ye = torch.empty((N, d), dtype=bf, device=dev); dYe = torch.empty_like(Ye); dXp = torch.empty_like(Ye)
+    Y = torch.empty((T, d), dtype=bf, device=dev); dX = torch.empty_like(Y)
+    grads = layer.alloc_grads()
+    launches = [0]
+
+    def step():
+        n = 0
+        idx, w = layer.route(X, W_r, bias); n += layer.last_launch_count()
+        counts, offsets, perm, inv = layer.dispatch(idx); n += layer.last_launch_count()
+        layer.expert_fwd(X, offsets, perm, out=Ye); n += layer.last_launch_count()
+        layer.combine(Ye, inv, w, out=Y); n += layer.last_launch_count()
+        _, dw = layer.combine_bwd(dY, Ye, inv, w, want_dw=cfg.router_grad, out=dYe); n += layer.last_launch_count()
+        layer.expert_bwd(X, dYe, offsets, perm, grads=grads, out=dXp); n += layer.last_launch_count()
+        layer.dispatch_bwd(dXp, inv, out=dX); n += layer.last_launch_count()
+        if cfg.router_grad:
+            layer.route_bwd(X, W_r, idx, w, dw, offsets, perm, dX); n += layer.last_launch_count()
+        launches[0] = n
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    layer.set_option("time_gemm", 1)
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    sampler.stop_flag = True
+    ms = e0.elapsed_time(e1)
+    gemm_ms, gemm_launches = layer.gemm_time()
+    layer.set_option("time_gemm", 0)
+    if dist is not None:
+        tt = torch.tensor([ms], device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms = float(tt.item())
+    ms_per_step = ms / args.steps
+    value = world * T * args.steps / (ms / 1e3)
+
+    # ---- end to end through the C ABI with HOST buffers (H2D + whole chain + D2H inside the timed region) ----
+    e2e = None
+    if not args.no_e2e:
+        Xh = X.cpu().pin_memory(); dYh = dY.cpu().pin_memory()
+        Yh = torch.empty((T, d), dtype=bf).pin_memory(); dXh = torch.empty((T, d), dtype=bf).pin_memory()
+        dW_r = torch.empty((d, cfg.E), dtype=torch.float32, device=dev) if cfg.router_grad else None
+        for _ in range(min(args.warmup, 3)):
+            layer.step_host(Xh, dYh, W_r, bias, Yh, dXh, grads, dW_r)
+        barrier()
+        e0.record()
+        for _ in range(args.steps):
+            layer.step_host(Xh, dYh, W_r, bias, Yh, dXh, grads, dW_r)
+        e1.record()
+        barrier()
+        ems = e0.elapsed_time(e1)
+        if dist is not None:
+            tt = torch.tensor([ems], device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            ems = float(tt.item())
+        nb = T * d * 2
+        e2e = {"value": world * T * args.steps / (ems / 1e3), "unit": "tokens/s", "h2d_bytes_per_step": 2 * nb,
+               "d2h_bytes_per_step": 2 * nb, "ms_per_step": ems / args.steps}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    fl = flops(cfg, T)
+    pk = peaks()
+    gemm_ms_step = gemm_ms / args.steps
+    gemm_tflops = fl["gemm"] / (gemm_ms_step / 1e3) / 1e12 if gemm_ms_step > 0 else 0.0
+    line = {
+        "metric": METRIC, "value": value, "unit": "tokens/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic",
+        "config": {"workload": cfg.name, "T": T, "d": cfg.d, "F": cfg.F, "E": cfg.E, "k": cfg.k, "r": cfg.r,
+                   "passes": "fwd+bwd" + ("+router_grad" if cfg.router_grad else ""), "routing": "zipf1.1" if cfg.skew else "near-uniform",
+                   "l2": "inputs larger than L2 (452 MB code indices + 503 MB permuted rows per step), no flush",
+                   "gemm_impl": "scaffold" if args.gemm_impl else "tcgen05", "parallelism": f"replicas x{world}, no collective"},
+        "tflops": world * fl["total"] / (ms_per_step / 1e3) / 1e12,
+        "frac_of_bf16_peak": {"measured_burst": fl["total"] / (ms_per_step / 1e3) / 1e12 / pk["tensor_burst"],
+                              "measured_sustained": fl["total"] / (ms_per_step / 1e3) / 1e12 / pk["tensor_sustained"],
+                              "datasheet_2250": fl["total"] / (ms_per_step / 1e3) / 1e12 / 2250.0},
+        "clocks": sampler.summary(),
+        "e2e": e2e,
+        "gpu_launches": launches[0] * args.steps,
+        "roofline": {"kernel": "gemm_tcgen05_kernel (4 launches/step: gate+up, down, dH, dXp)", "bound": "tensor",
+                     "achieved": gemm_tflops, "peak": pk["tensor_sustained"], "unit": "TFLOP/s",
+                     "frac": gemm_tflops / pk["tensor_sustained"], "frac_of_burst": gemm_tflops / pk["tensor_burst"],
+                     "frac_of_datasheet_2250": gemm_tflops / 2250.0, "peak_source": pk["source"] + ", sustained bf16",
+                     "gemm_ms_per_step": gemm_ms_step, "gemm_share_of_step": gemm_ms_step / ms_per_step,
+                     "gemm_launches": gemm_launches, "flops_per_step": fl["gemm"], "traffic": None},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        cb = time_oracle(cfg, args.cpu_tokens, 1, 0)
+        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (2 = 120B shape, fwd+bwd)")
+    ap.add_argument("--gemm-impl", type=int, default=0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-tokens", type=int, default=1024, help="tokens in the bounded cpu_baseline sample")
+    ap.add_argument("--ref-tokens", type=int, default=256, help="tokens per step of the --impl reference arm")
+    args = ap.parse_args()
+    cfg = ti.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

@@ -82,7 +82,8 @@ tqp_status tqp_bind_workspace(tqp_ctx *ctx, void *dev_ptr, size_t bytes, void *s
 /* Records the weight pointers, builds the TMA descriptors over the code indices and converts the codebook
  * to the bf16 lookup table the GEMM mainloop gathers from.  One-time, untimed; needs a bound workspace. */
 tqp_status tqp_bind_weights(tqp_ctx *ctx, const tqp_weights *w, void *stream);
-/* Options (debug / ablation).  "gemm_impl": 0 = tcgen05 grouped GEMM (default), 1 = CUDA-core scaffold. */
+/* Options (debug / ablation).  "gemm_impl": 0 = tcgen05 grouped GEMM (default), 1 = CUDA-core scaffold.
+ * "time_gemm": 0/1, see tqp_gemm_time. */
 tqp_status tqp_set_option(tqp_ctx *ctx, const char *name, int value);
 
 /* --- forward ------------------------------------------------------------------------------------------ */
@@ -142,6 +143,11 @@ tqp_status tqp_step_host(tqp_ctx *ctx, int T, const void *X_host, const void *dY
 /* Device pointers of workspace tensors, for tests: "G","U","H" bf16 [N][F]; "Xp" bf16 [N][d];
  * "dH","dG","dU" bf16 [N][F]; "num_tiles" int32 [1].  NULL if unknown. */
 void *tqp_debug_buffer(tqp_ctx *ctx, const char *name);
+/* Measurement hook (the >= 50 % target applies to the grouped-GEMM kernels' own time).  After
+ * tqp_set_option(ctx, "time_gemm", 1) every grouped-GEMM launch is bracketed by CUDA events on its stream.
+ * tqp_gemm_time waits for the recorded events, returns the summed device time in milliseconds and the number of
+ * GEMM launches since the previous call, and resets the record (at most 4096 launches are kept). */
+tqp_status tqp_gemm_time(tqp_ctx *ctx, float *ms_total, int *launches);
 /* Kernels launched by the last call on this ctx (for bench.py's gpu_launches). */
 int tqp_last_launch_count(const tqp_ctx *ctx);
 const char *tqp_status_string(tqp_status s);

@@ -68,6 +68,7 @@ def load_library() -> ctypes.CDLL:
         lib.tqp_step_host.argtypes = [vp, ci] + [vp] * 14
         lib.tqp_debug_buffer.argtypes = [vp, ctypes.c_char_p]
         lib.tqp_debug_buffer.restype = vp
+        lib.tqp_gemm_time.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_int)]
         lib.tqp_last_launch_count.argtypes = [vp]
         lib.tqp_status_string.argtypes = [ci]
         lib.tqp_status_string.restype = ctypes.c_char_p
@@ -222,6 +223,12 @@ class TqpLayer:
                                            _ptr(Y_host), _ptr(dX_host), _ptr(g["dA_gate"]), _ptr(g["dB_gate"]),
                                            _ptr(g["dA_up"]), _ptr(g["dB_up"]), _ptr(g["dA_down"]), _ptr(g["dB_down"]),
                                            _ptr(dW_r), self._stream()))
+
+    def gemm_time(self):
+        """(summed grouped-GEMM device ms, launches) since the last call; needs set_option('time_gemm', 1)."""
+        ms, n = ctypes.c_float(), ctypes.c_int()
+        self._check(self.lib.tqp_gemm_time(self.ctx, ctypes.byref(ms), ctypes.byref(n)))
+        return float(ms.value), int(n.value)
 
     # ---- introspection ----
     def last_launch_count(self) -> int:

@@ -122,7 +122,14 @@ tqp_status common_checks(tqp_ctx *c, int T, bool need_weights) {
 }
 
 tqp_status run_gemm(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st) {
-    return c->gemm_impl == 1 ? launch_gemm_scaffold(c, probs, nprob, st) : launch_gemm_tcgen05(c, probs, nprob, st);
+    const bool timed = c->time_gemm && c->ev_used + 2 <= (int)c->ev.size();
+    if (timed) TQP_CUDA_OK(c, cudaEventRecord(c->ev[c->ev_used], st));
+    tqp_status r = c->gemm_impl == 1 ? launch_gemm_scaffold(c, probs, nprob, st) : launch_gemm_tcgen05(c, probs, nprob, st);
+    if (timed) {
+        TQP_CUDA_OK(c, cudaEventRecord(c->ev[c->ev_used + 1], st));
+        c->ev_used += 2;
+    }
+    return r;
 }
 
 }  // namespace
@@ -150,7 +157,26 @@ tqp_status tqp_create(tqp_ctx **out, const tqp_layer_desc *desc) {
     return TQP_OK;
 }
 
-void tqp_destroy(tqp_ctx *ctx) { delete ctx; }
+void tqp_destroy(tqp_ctx *ctx) {
+    if (!ctx) return;
+    for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+    delete ctx;
+}
+
+tqp_status tqp_gemm_time(tqp_ctx *c, float *ms_total, int *launches) {
+    if (!c || !ms_total || !launches) return TQP_ERR_ARG;
+    float total = 0.f;
+    for (int i = 0; i + 1 < c->ev_used; i += 2) {
+        TQP_CUDA_OK(c, cudaEventSynchronize(c->ev[i + 1]));
+        float ms = 0.f;
+        TQP_CUDA_OK(c, cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]));
+        total += ms;
+    }
+    *ms_total = total;
+    *launches = c->ev_used / 2;
+    c->ev_used = 0;
+    return TQP_OK;
+}
 
 size_t tqp_workspace_bytes(const tqp_layer_desc *desc) {
     if (!desc_ok(desc)) return 0;
@@ -216,6 +242,15 @@ tqp_status tqp_set_option(tqp_ctx *c, const char *name, int value) {
     if (!strcmp(name, "gemm_impl")) {
         REQ(c, value == 0 || value == 1, TQP_ERR_ARG, "gemm_impl must be 0 or 1");
         c->gemm_impl = value;
+        return TQP_OK;
+    }
+    if (!strcmp(name, "time_gemm")) {
+        c->time_gemm = value ? 1 : 0;
+        if (value && c->ev.empty()) {
+            c->ev.resize(8192);
+            for (auto &e : c->ev) TQP_CUDA_OK(c, cudaEventCreate(&e));
+        }
+        c->ev_used = 0;
         return TQP_OK;
     }
     c->err = "unknown option";

@@ -8,6 +8,7 @@
 #include <stdint.h>
 
 #include <string>
+#include <vector>
 
 #include "../../include/tqp.h"
 
@@ -80,6 +81,9 @@ struct tqp_ctx {
     int num_sms = 148;
     int max_tiles = 0;
     std::string err;
+    int time_gemm = 0;          // bracket GEMM launches with events (tqp_gemm_time)
+    std::vector<cudaEvent_t> ev; // pairs (start, stop)
+    int ev_used = 0;
     // tensor maps over weights / workspace (built in bind_weights)
     tqp::GemmProblem prob_gate, prob_up, prob_down, prob_dh, prob_dx;
 
