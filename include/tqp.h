@@ -82,8 +82,10 @@ tqp_status tqp_bind_workspace(tqp_ctx *ctx, void *dev_ptr, size_t bytes, void *s
 /* Records the weight pointers, builds the TMA descriptors over the code indices and converts the codebook
  * to the bf16 lookup table the GEMM mainloop gathers from.  One-time, untimed; needs a bound workspace. */
 tqp_status tqp_bind_weights(tqp_ctx *ctx, const tqp_weights *w, void *stream);
-/* Options (debug / ablation).  "gemm_impl": 0 = tcgen05 grouped GEMM (default), 1 = CUDA-core scaffold.
- * "time_gemm": 0/1, see tqp_gemm_time. */
+/* Options (debug / ablation).  "gemm_impl": 0 = tcgen05 grouped GEMM on CTA pairs (default), 1 = CUDA-core scaffold,
+ * 2 = tcgen05 grouped GEMM, one CTA per tile.
+ * "time_gemm": 0/1, see tqp_gemm_time.  "ablate": bit mask that disables parts of the dequant producer (results
+ * become wrong; timing experiments only; 0 = off). */
 tqp_status tqp_set_option(tqp_ctx *ctx, const char *name, int value);
 
 /* --- forward ------------------------------------------------------------------------------------------ */
@@ -148,6 +150,9 @@ void *tqp_debug_buffer(tqp_ctx *ctx, const char *name);
  * tqp_gemm_time waits for the recorded events, returns the summed device time in milliseconds and the number of
  * GEMM launches since the previous call, and resets the record (at most 4096 launches are kept). */
 tqp_status tqp_gemm_time(tqp_ctx *ctx, float *ms_total, int *launches);
+/* Same record, per launch: writes up to `cap` per-launch times (ms, launch order) into the HOST array ms_each
+ * and the launch count into *launches; resets the record. */
+tqp_status tqp_gemm_times(tqp_ctx *ctx, float *ms_each, int cap, int *launches);
 /* Kernels launched by the last call on this ctx (for bench.py's gpu_launches). */
 int tqp_last_launch_count(const tqp_ctx *ctx);
 const char *tqp_status_string(tqp_status s);

@@ -69,6 +69,7 @@ def load_library() -> ctypes.CDLL:
         lib.tqp_debug_buffer.argtypes = [vp, ctypes.c_char_p]
         lib.tqp_debug_buffer.restype = vp
         lib.tqp_gemm_time.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_int)]
+        lib.tqp_gemm_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
         lib.tqp_last_launch_count.argtypes = [vp]
         lib.tqp_status_string.argtypes = [ci]
         lib.tqp_status_string.restype = ctypes.c_char_p
@@ -229,6 +230,13 @@ class TqpLayer:
         ms, n = ctypes.c_float(), ctypes.c_int()
         self._check(self.lib.tqp_gemm_time(self.ctx, ctypes.byref(ms), ctypes.byref(n)))
         return float(ms.value), int(n.value)
+
+    def gemm_times(self, cap=4096):
+        """Per-launch grouped-GEMM device times (ms) since the last call."""
+        arr = (ctypes.c_float * cap)()
+        n = ctypes.c_int()
+        self._check(self.lib.tqp_gemm_times(self.ctx, arr, cap, ctypes.byref(n)))
+        return [float(arr[i]) for i in range(min(cap, n.value))]
 
     # ---- introspection ----
     def last_launch_count(self) -> int:

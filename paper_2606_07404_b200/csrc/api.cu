@@ -77,14 +77,16 @@ tqp_status make_map(tqp_ctx *c, CUtensorMap *m, const void *ptr, CUtensorMapData
     return TQP_OK;
 }
 
-tqp_status act_map(tqp_ctx *c, CUtensorMap *m, const void *ptr, uint64_t rows, uint64_t K) {
-    return make_map(c, m, ptr, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, rows, K, 64, kTileRows, CU_TENSOR_MAP_SWIZZLE_128B);
+tqp_status act_map(tqp_ctx *c, CUtensorMap *m, const void *ptr, uint64_t rows, uint64_t K, int box_rows = kTileRows) {
+    return make_map(c, m, ptr, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, rows, K, 64, box_rows, CU_TENSOR_MAP_SWIZZLE_128B);
 }
 
 tqp_status set_seg(tqp_ctx *c, GemmSeg *s, const bf16 *act, uint64_t act_rows, const uint8_t *idx, const void *scale, int K,
                    int M, int kmajor) {
     s->act = act; s->idx = idx; s->scale = (const __half *)scale; s->K = K; s->kmajor = kmajor;
     tqp_status st = act_map(c, &s->act_map, act, act_rows, K);
+    if (st != TQP_OK) return st;
+    st = act_map(c, &s->act_map2, act, act_rows, K, kTileRows / 2);
     if (st != TQP_OK) return st;
     const uint64_t E = c->desc.E;
     const uint64_t rows = kmajor ? E * M : E * K, bytes = kmajor ? K / 8 : M / 8;
@@ -93,6 +95,8 @@ tqp_status set_seg(tqp_ctx *c, GemmSeg *s, const bf16 *act, uint64_t act_rows, c
 
 tqp_status set_lora(tqp_ctx *c, GemmLora *l, const bf16 *lact, uint64_t rows, const void *lw, int mk_layout) {
     l->lact = lact; l->lw = (const bf16 *)lw; l->mk_layout = mk_layout;
+    tqp_status st = act_map(c, &l->lact_map2, lact, rows, kLoraPad, kTileRows / 2);
+    if (st != TQP_OK) return st;
     return act_map(c, &l->lact_map, lact, rows, kLoraPad);
 }
 
@@ -124,7 +128,9 @@ tqp_status common_checks(tqp_ctx *c, int T, bool need_weights) {
 tqp_status run_gemm(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st) {
     const bool timed = c->time_gemm && c->ev_used + 2 <= (int)c->ev.size();
     if (timed) TQP_CUDA_OK(c, cudaEventRecord(c->ev[c->ev_used], st));
-    tqp_status r = c->gemm_impl == 1 ? launch_gemm_scaffold(c, probs, nprob, st) : launch_gemm_tcgen05(c, probs, nprob, st);
+    tqp_status r = c->gemm_impl == 1   ? launch_gemm_scaffold(c, probs, nprob, st)
+                   : c->gemm_impl == 2 ? launch_gemm_tcgen05(c, probs, nprob, st)
+                                       : launch_gemm_tcgen05_2cta(c, probs, nprob, st);
     if (timed) {
         TQP_CUDA_OK(c, cudaEventRecord(c->ev[c->ev_used + 1], st));
         c->ev_used += 2;
@@ -161,6 +167,20 @@ void tqp_destroy(tqp_ctx *ctx) {
     if (!ctx) return;
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     delete ctx;
+}
+
+tqp_status tqp_gemm_times(tqp_ctx *c, float *ms_each, int cap, int *launches) {
+    if (!c || !ms_each || !launches) return TQP_ERR_ARG;
+    int n = 0;
+    for (int i = 0; i + 1 < c->ev_used; i += 2, ++n) {
+        TQP_CUDA_OK(c, cudaEventSynchronize(c->ev[i + 1]));
+        float ms = 0.f;
+        TQP_CUDA_OK(c, cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]));
+        if (n < cap) ms_each[n] = ms;
+    }
+    *launches = n;
+    c->ev_used = 0;
+    return TQP_OK;
 }
 
 tqp_status tqp_gemm_time(tqp_ctx *c, float *ms_total, int *launches) {
@@ -240,8 +260,12 @@ tqp_status tqp_bind_weights(tqp_ctx *c, const tqp_weights *w, void *stream) {
 tqp_status tqp_set_option(tqp_ctx *c, const char *name, int value) {
     if (!c || !name) return TQP_ERR_ARG;
     if (!strcmp(name, "gemm_impl")) {
-        REQ(c, value == 0 || value == 1, TQP_ERR_ARG, "gemm_impl must be 0 or 1");
+        REQ(c, value >= 0 && value <= 2, TQP_ERR_ARG, "gemm_impl must be 0, 1 or 2");
         c->gemm_impl = value;
+        return TQP_OK;
+    }
+    if (!strcmp(name, "ablate")) {
+        c->ablate = value;
         return TQP_OK;
     }
     if (!strcmp(name, "time_gemm")) {
@@ -345,6 +369,7 @@ tqp_status tqp_expert_bwd(tqp_ctx *c, int T, const void *X, const void *dYe, con
     GemmProblem ph = c->prob_dh;
     ph.seg[0].act = dye;
     CK(act_map(c, &ph.seg[0].act_map, dye, (uint64_t)N, D.d));
+    CK(act_map(c, &ph.seg[0].act_map2, dye, (uint64_t)N, D.d, kTileRows / 2));
     CK(run_gemm(c, &ph, 1, s));
     CK(launch_swiglu_bwd(c, N, dH, G, U, dG, dU, s));
     CK(launch_lora_wgrad(c, dye, D.d, c->p<bf16>(c->ws.HAd), offsets, 0, dB_down, s));

@@ -33,7 +33,8 @@ struct GemmSeg {
     const __half *scale;    // per-output-channel scales of all experts
     int K;                  // contraction length of this segment
     int kmajor;             // 1: idx[e][M][K/8] (forward), 0: idx[e][K][M/8] (backward, transposed use)
-    CUtensorMap act_map;    // box {64, kTileRows} over act, SWIZZLE_128B
+    CUtensorMap act_map;    // box {64, kTileRows} over act, SWIZZLE_128B (1-CTA kernel)
+    CUtensorMap act_map2;   // box {64, kTileRows/2}: one CTA's half of the rows (2-CTA kernel)
     CUtensorMap idx_map;    // box {16, 128} over idx viewed as [rows][bytes]
 };
 struct GemmLora {
@@ -41,6 +42,7 @@ struct GemmLora {
     const bf16 *lw;         // adapter matrix of all experts
     int mk_layout;          // 1: lw[e][M][r] (K-major), 0: lw[e][r][M]
     CUtensorMap lact_map;   // box {64, kTileRows}
+    CUtensorMap lact_map2;  // box {64, kTileRows/2}
 };
 struct GemmProblem {
     GemmSeg seg[2];
@@ -74,13 +76,14 @@ struct tqp_ctx {
     size_t bound_bytes = 0;
     tqp_weights w;
     bool have_weights = false;
-    int gemm_impl = 0;          // 0 tcgen05, 1 scaffold
+    int gemm_impl = 0;          // 0 tcgen05 CTA-pair kernel, 1 scaffold, 2 tcgen05 single-CTA kernel
     int fwd_T = -1;             // T of the last training-mode expert_fwd (TQP_ERR_STATE check)
     int disp_T = -1;
     int launches = 0;
     int num_sms = 148;
     int max_tiles = 0;
     std::string err;
+    int ablate = 0;             // timing experiments only (tqp_set_option "ablate")
     int time_gemm = 0;          // bracket GEMM launches with events (tqp_gemm_time)
     std::vector<cudaEvent_t> ev; // pairs (start, stop)
     int ev_used = 0;
@@ -139,7 +142,8 @@ tqp_status launch_lora_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 
 
 // ---- gemm_scaffold.cu / gemm_tcgen05.cu -----------------------------------------------------------------
 tqp_status launch_gemm_scaffold(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);
-tqp_status launch_gemm_tcgen05(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);
+tqp_status launch_gemm_tcgen05(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);       // 1 CTA / tile
+tqp_status launch_gemm_tcgen05_2cta(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);  // CTA pair / tile
 
 // ---- device helpers ------------------------------------------------------------------------------------
 __device__ __forceinline__ float bf16_bits_to_float(uint16_t b) { return __uint_as_float(((uint32_t)b) << 16); }

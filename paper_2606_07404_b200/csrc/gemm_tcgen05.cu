@@ -109,7 +109,7 @@ struct Pipe {   // ring position + phase bit
 // ---- the kernel ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(NTHREADS, 1)
 gemm_tcgen05_kernel(const __grid_constant__ GemmArgs args, const uint4 *__restrict__ lut_g, const Tile *__restrict__ tiles,
-                    const int32_t *__restrict__ num_tiles_p) {
+                    const int32_t *__restrict__ num_tiles_p, int ablate) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     const uint32_t sbase = smem_u32(smem);
@@ -292,11 +292,13 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmArgs args, const uint4 *__restri
 #pragma unroll
                     for (int j = 0; j < 8; ++j) {
                         const uint32_t code = (c01[j >> 2] >> ((j & 3) * 8)) & 0xffu;
-                        uint4 v = lut_s[code * 8 + c];
+                        uint4 v = (ablate & 1) ? make_uint4(code, code, code, code) : lut_s[code * 8 + c];
                         __nv_bfloat162 *pv = reinterpret_cast<__nv_bfloat162 *>(&v);
+                        if (!(ablate & 4)) {
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) pv[q] = __hmul2(pv[q], s2);
-                        *reinterpret_cast<uint4 *>(as + rowoff + ((j ^ sw) << 4)) = v;
+                            for (int q = 0; q < 4; ++q) pv[q] = __hmul2(pv[q], s2);
+                        }
+                        if (!(ablate & 2)) *reinterpret_cast<uint4 *>(as + rowoff + ((j ^ sw) << 4)) = v;
                     }
                     fence_async_smem();
                     __syncwarp();
@@ -383,7 +385,7 @@ tqp_status launch_gemm_tcgen05(tqp_ctx *c, const GemmProblem *probs, int nprob, 
     for (int i = 0; i < nprob; ++i) args.p[i] = probs[i];
     args.nprob = nprob;
     g5::gemm_tcgen05_kernel<<<c->num_sms, g5::NTHREADS, g5::SMEM_BYTES, st>>>(
-        args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles));
+        args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), c->ablate);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }

@@ -1,0 +1,344 @@
+// Grouped dequant GEMM on CTA PAIRS (tcgen05 cta_group::2 + TMEM + TMA), sm_100a — the default GEMM of the layer.
+//
+//   out[p][m] = sum_seg sum_k act_seg[p][k] * W_seg[m][k]  +  sum_l lact_l[p][q] * lw_l[m][q]
+//   W_seg[m][k] = bf16( bf16(codebook[code]) * bf16(scale) )       (look up, rescale by the norm)
+//
+// Same "swap-AB" mapping as gemm_tcgen05.cu (UMMA M = weight output channels, N = routed rows of one expert), but
+// one UMMA instruction spans two SMs: M = 256 (each CTA dequantises and owns 128 output channels), and the routed
+// rows (B operand) are split between the two CTAs' shared memories, so every SM loads, stores and re-reads only
+// half of the activation tile.  That halves the shared-memory traffic of the activation operand, which — next to
+// the codebook gathers — is what bounds this kernel.
+//
+// Warp roles per CTA (480 threads, 1 CTA/SM, persistent over work items, cluster = 2 CTAs):
+//   warp 0  TMA producer of the activation / adapter-projection tiles (signals the LEADER's barrier)
+//   warp 1  MMA issuer (leader CTA only) + TMEM allocation
+//   warp 2  TMA producer of the code-index tiles (deep ring: indices stream from HBM exactly once)
+//   warps 3-10  dequant producers, two groups of four that alternate K-blocks
+//   warps 11-14 epilogue (TMEM -> registers -> bf16 -> global)
+#include "common.cuh"
+#include "tc_ptx.cuh"
+
+namespace tqp {
+namespace g2 {
+using namespace ptx;
+
+constexpr int BM = 128, BK = 64, TN = kTileRows, HN = kTileRows / 2;
+constexpr int NSTAGE = 5, IDXQ = 8;
+constexpr int X_BYTES = HN * 128, A_BYTES = BM * 128, IDX_BYTES = 128 * 16, LUT_BYTES = 256 * 8 * 16;
+constexpr int OFF_X = 0, OFF_A = OFF_X + NSTAGE * X_BYTES, OFF_LUT = OFF_A + NSTAGE * A_BYTES,
+              OFF_IDX = OFF_LUT + LUT_BYTES, OFF_BAR = OFF_IDX + IDXQ * IDX_BYTES;
+constexpr int SMEM_BYTES = OFF_BAR + 512 + 1024;
+constexpr int NTHREADS = 480;
+constexpr int W_DEQ0 = 3, W_EPI0 = 11;
+
+struct Item {
+    Tile t;
+    int prob, m0;
+};
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
+gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__restrict__ lut_g, const Tile *__restrict__ tiles,
+                         const int32_t *__restrict__ num_tiles_p, int ablate) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    const uint32_t sbase = smem_u32(smem);
+    const uint32_t bar0 = sbase + OFF_BAR;
+    auto full_x = [&](int s) { return bar0 + 8u * s; };                              // leader's is used
+    auto full_a = [&](int s) { return bar0 + 8u * (NSTAGE + s); };                   // leader's is used
+    auto empty = [&](int s) { return bar0 + 8u * (2 * NSTAGE + s); };                // local, multicast commit
+    auto idx_full = [&](int s) { return bar0 + 8u * (3 * NSTAGE + s); };             // local
+    auto idx_empty = [&](int s) { return bar0 + 8u * (3 * NSTAGE + IDXQ + s); };     // local
+    auto tmem_full = [&](int s) { return bar0 + 8u * (3 * NSTAGE + 2 * IDXQ + s); }; // local, multicast commit
+    auto tmem_empty = [&](int s) { return bar0 + 8u * (3 * NSTAGE + 2 * IDXQ + 2 + s); };   // leader's is used
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + OFF_BAR + 8 * (3 * NSTAGE + 2 * IDXQ + 4));
+
+    const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+    const uint32_t rank = cluster_ctarank();
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NSTAGE; ++s) { mbar_init(full_x(s), 1); mbar_init(full_a(s), 8); mbar_init(empty(s), 1); }
+        for (int s = 0; s < IDXQ; ++s) { mbar_init(idx_full(s), 1); mbar_init(idx_empty(s), 8); }
+        for (int s = 0; s < 2; ++s) { mbar_init(tmem_full(s), 1); mbar_init(tmem_empty(s), 8); }
+        mbar_init_fence();
+    }
+    if (warp == 1) tmem_alloc<2>(smem_u32(tmem_slot), 512);
+    {   // replicated LUT: entry e, copy c at (e*8 + c) * 16 B  ->  lane c of every quarter-warp hits bank group c
+        uint4 *lut_s = reinterpret_cast<uint4 *>(smem + OFF_LUT);
+        for (int i = threadIdx.x; i < 256 * 8; i += NTHREADS) lut_s[i] = lut_g[i >> 3];
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync();   // both CTAs' barriers are initialised before any remote arrive / TMA completion
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    const int num_tiles = *num_tiles_p;
+    const int nprob = args.nprob;
+    const int MTP = args.p[0].M / (2 * BM);
+    const long long total = (long long)num_tiles * nprob * MTP;
+    const int cid = blockIdx.x >> 1, ncl = gridDim.x >> 1;
+
+    auto get_item = [&](long long item, Item &it) {
+        const int tile_id = (int)(item / (nprob * MTP)), rem = (int)(item % (nprob * MTP));
+        it.t = tiles[tile_id];
+        it.prob = rem / MTP;
+        it.m0 = ((rem % MTP) * 2 + (int)rank) * BM;
+    };
+
+    if (warp == 0) {
+        // =========================== activation TMA producer ===========================
+        if (lane == 0) {
+            Pipe st;
+            for (long long item = cid; item < total; item += ncl) {
+                Item it;
+                get_item(item, it);
+                if (it.t.rows <= 0) continue;
+                const GemmProblem &pb = args.p[it.prob];
+                const int n = max(16, (it.t.rows + 15) & ~15);
+                const int row = it.t.row0 + (int)rank * (n >> 1);
+                for (int sg = 0; sg < pb.nseg; ++sg) {
+                    const GemmSeg &S = pb.seg[sg];
+                    const int nkb = S.K / BK;
+                    for (int kb = 0; kb < nkb; ++kb) {
+                        mbar_wait(empty(st.s), st.ph ^ 1);
+                        if (rank == 0) mbar_expect_tx(full_x(st.s), 2 * X_BYTES);
+                        tma_load_2d_pair(sbase + OFF_X + st.s * X_BYTES, &S.act_map2, kb * BK, row, mapa(full_x(st.s), 0));
+                        st.next(NSTAGE);
+                    }
+                }
+                for (int l = 0; l < pb.nlora; ++l) {
+                    mbar_wait(empty(st.s), st.ph ^ 1);
+                    if (rank == 0) mbar_expect_tx(full_x(st.s), 2 * X_BYTES);
+                    tma_load_2d_pair(sbase + OFF_X + st.s * X_BYTES, &pb.lora[l].lact_map2, 0, row, mapa(full_x(st.s), 0));
+                    st.next(NSTAGE);
+                }
+            }
+        }
+    } else if (warp == 2) {
+        // =========================== code-index TMA producer ===========================
+        if (lane == 0) {
+            Pipe iq;
+            for (long long item = cid; item < total; item += ncl) {
+                Item it;
+                get_item(item, it);
+                if (it.t.rows <= 0) continue;
+                const GemmProblem &pb = args.p[it.prob];
+                for (int sg = 0; sg < pb.nseg; ++sg) {
+                    const GemmSeg &S = pb.seg[sg];
+                    const int npair = S.K / (2 * BK);
+                    for (int kp = 0; kp < npair; ++kp) {
+                        mbar_wait(idx_empty(iq.s), iq.ph ^ 1);
+                        mbar_expect_tx(idx_full(iq.s), IDX_BYTES);
+                        const int c0 = S.kmajor ? kp * 16 : it.m0 / 8;
+                        const int c1 = S.kmajor ? it.t.expert * pb.M + it.m0 : it.t.expert * S.K + kp * 2 * BK;
+                        tma_load_2d(sbase + OFF_IDX + iq.s * IDX_BYTES, &S.idx_map, c0, c1, idx_full(iq.s));
+                        iq.next(IDXQ);
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // =========================== MMA issuer (leader CTA) ===========================
+        if (rank == 0 && lane == 0) {
+            Pipe st;
+            int cnt = 0;
+            for (long long item = cid; item < total; item += ncl) {
+                Item it;
+                get_item(item, it);
+                if (it.t.rows <= 0) continue;
+                const GemmProblem &pb = args.p[it.prob];
+                const int ab = cnt & 1;
+                const uint32_t aph = (cnt >> 1) & 1;
+                ++cnt;
+                const int n = max(16, (it.t.rows + 15) & ~15);
+                mbar_wait<true>(tmem_empty(ab), aph ^ 1);
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + ab * TN;
+                uint32_t accum = 0;
+                for (int sg = 0; sg < pb.nseg; ++sg) {
+                    const GemmSeg &S = pb.seg[sg];
+                    const int nkb = S.K / BK;
+                    const uint32_t idesc = make_idesc(2 * BM, n, S.kmajor ? 0 : 1);
+                    for (int kb = 0; kb < nkb; ++kb) {
+                        mbar_wait<true>(full_x(st.s), st.ph);
+                        mbar_wait<true>(full_a(st.s), st.ph);
+                        tc_fence_after();
+                        const uint32_t xa = sbase + OFF_X + st.s * X_BYTES, aa = sbase + OFF_A + st.s * A_BYTES;
+#pragma unroll
+                        for (int kk = 0; kk < BK / 16; ++kk) {
+                            const uint64_t bd = make_desc(xa + kk * 32, 16, 1024);
+                            const uint64_t ad = S.kmajor ? make_desc(aa + kk * 32, 16, 1024) : make_desc(aa + kk * 4096, 1024, 2048);
+                            umma_bf16<2>(d_tmem, ad, bd, idesc, accum);
+                            accum = 1;
+                        }
+                        umma_commit_pair(empty(st.s), 3);
+                        st.next(NSTAGE);
+                    }
+                }
+                const uint32_t idesc_l = make_idesc(2 * BM, n, 0);
+                const int nmma_l = max(1, pb.r / 16);
+                for (int l = 0; l < pb.nlora; ++l) {
+                    mbar_wait<true>(full_x(st.s), st.ph);
+                    mbar_wait<true>(full_a(st.s), st.ph);
+                    tc_fence_after();
+                    const uint32_t xa = sbase + OFF_X + st.s * X_BYTES, aa = sbase + OFF_A + st.s * A_BYTES;
+                    for (int kk = 0; kk < nmma_l; ++kk) {
+                        umma_bf16<2>(d_tmem, make_desc(aa + kk * 32, 16, 1024), make_desc(xa + kk * 32, 16, 1024), idesc_l, accum);
+                        accum = 1;
+                    }
+                    umma_commit_pair(empty(st.s), 3);
+                    st.next(NSTAGE);
+                }
+                umma_commit_pair(tmem_full(ab), 3);
+            }
+        }
+    } else if (warp >= W_DEQ0 && warp < W_EPI0) {
+        // =========================== dequant producers: 2 groups x 128 threads ===========================
+        const int g = (warp - W_DEQ0) >> 2;
+        const int tid = (threadIdx.x - W_DEQ0 * 32) & 127;
+        const int c = tid & 7;
+        const uint4 *lut_s = reinterpret_cast<const uint4 *>(smem + OFF_LUT);
+        Pipe st, iq;
+        for (long long item = cid; item < total; item += ncl) {
+            Item it;
+            get_item(item, it);
+            if (it.t.rows <= 0) continue;
+            const GemmProblem &pb = args.p[it.prob];
+            const int m0 = it.m0, M = pb.M, e = it.t.expert;
+            for (int sg = 0; sg < pb.nseg; ++sg) {
+                const GemmSeg &S = pb.seg[sg];
+                const int nkb = S.K / BK;
+                const int kmajor = S.kmajor;
+                const int kr = tid & 63, half = tid >> 6;
+                // K-major: one scale per thread row for the whole tile.  MN-major: one per k-row per k-block (prefetched).
+                const __half *scale_p = S.scale + (kmajor ? (size_t)e * M + m0 + tid : (size_t)e * S.K + g * BK + kr);
+                __half sc_next = *scale_p;
+                uint32_t rowoff, sw;
+                if (kmajor) { rowoff = tid * 128; sw = tid & 7; }
+                else { rowoff = ((kr >> 3) * 2 + half) * 1024 + (kr & 7) * 128; sw = kr & 7; }
+                uint2 codes = make_uint2(0, 0);
+                for (int kb = 0; kb < nkb; ++kb) {
+                    if ((kb & 1) == 0) {
+                        mbar_wait(idx_full(iq.s), iq.ph);
+                        const uint8_t *is = smem + OFF_IDX + iq.s * IDX_BYTES;
+                        codes = kmajor ? *reinterpret_cast<const uint2 *>(is + tid * 16 + g * 8)
+                                       : *reinterpret_cast<const uint2 *>(is + (g * 64 + kr) * 16 + half * 8);
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(idx_empty(iq.s));
+                        iq.next(IDXQ);
+                    }
+                    if ((kb & 1) == g) {
+                        const __nv_bfloat162 s2 = __float2bfloat162_rn(__half2float(sc_next));
+                        if (!kmajor && kb + 2 < nkb) sc_next = scale_p[(kb + 2 - g) * BK];
+                        mbar_wait(empty(st.s), st.ph ^ 1);
+                        uint8_t *as = smem + OFF_A + st.s * A_BYTES;
+                        const uint32_t c01[2] = {codes.x, codes.y};
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            const uint32_t code = (c01[j >> 2] >> ((j & 3) * 8)) & 0xffu;
+                            uint4 v = (ablate & 1) ? make_uint4(code, code, code, code) : lut_s[code * 8 + c];
+                            __nv_bfloat162 *pv = reinterpret_cast<__nv_bfloat162 *>(&v);
+                            if (!(ablate & 4)) {
+#pragma unroll
+                                for (int q = 0; q < 4; ++q) pv[q] = __hmul2(pv[q], s2);
+                            }
+                            if (!(ablate & 2)) *reinterpret_cast<uint4 *>(as + rowoff + ((j ^ sw) << 4)) = v;
+                        }
+                        fence_async_smem();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive_cluster(mapa(full_a(st.s), 0));
+                    }
+                    st.next(NSTAGE);
+                }
+            }
+            // adapter K-steps: A tile = lw[m0 + tid][0..r) as a K-major row (chunks beyond r zeroed)
+            const int r = pb.r, nch = 2 * max(1, r / 16);
+            for (int l = 0; l < pb.nlora; ++l) {
+                if ((l & 1) == g) {
+                    const GemmLora &L = pb.lora[l];
+                    uint4 ch[4];
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) ch[j] = make_uint4(0, 0, 0, 0);
+                    if (L.mk_layout) {
+                        const uint4 *src = reinterpret_cast<const uint4 *>(L.lw + ((size_t)e * M + m0 + tid) * r);
+                        for (int j = 0; j < r / 8; ++j) ch[j] = src[j];
+                    } else {
+                        const bf16 *src = L.lw + (size_t)e * r * M + m0 + tid;
+                        uint16_t *h = reinterpret_cast<uint16_t *>(ch);
+                        for (int q = 0; q < r; ++q) h[q] = *reinterpret_cast<const uint16_t *>(src + (size_t)q * M);
+                    }
+                    mbar_wait(empty(st.s), st.ph ^ 1);
+                    uint8_t *as = smem + OFF_A + st.s * A_BYTES;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        if (j < nch) *reinterpret_cast<uint4 *>(as + tid * 128 + ((j ^ (tid & 7)) << 4)) = ch[j];
+                    fence_async_smem();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_cluster(mapa(full_a(st.s), 0));
+                }
+                st.next(NSTAGE);
+            }
+        }
+    } else if (warp >= W_EPI0) {
+        // =========================== epilogue (128 threads) ===========================
+        const int q = warp & 3;             // TMEM lane quadrant this warp may access
+        const int m = q * 32 + lane;        // output channel inside this CTA's 128-row half
+        int cnt = 0;
+        for (long long item = cid; item < total; item += ncl) {
+            Item it;
+            get_item(item, it);
+            if (it.t.rows <= 0) continue;
+            const GemmProblem &pb = args.p[it.prob];
+            const int M = pb.M;
+            const int ab = cnt & 1;
+            const uint32_t aph = (cnt >> 1) & 1;
+            ++cnt;
+            mbar_wait(tmem_full(ab), aph);
+            tc_fence_after();
+            bf16 *outp = pb.out + (size_t)it.t.row0 * M + it.m0 + m;
+            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + ab * TN;
+            for (int c0 = 0; c0 < it.t.rows; c0 += 16) {
+                uint32_t v[16];
+                tmem_ld16(taddr + c0, v);
+                tmem_ld_wait();
+#pragma unroll
+                for (int j = 0; j < 16; ++j)
+                    if (c0 + j < it.t.rows) outp[(size_t)(c0 + j) * M] = __float2bfloat16_rn(__uint_as_float(v[j]));
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(mapa(tmem_empty(ab), 0));
+        }
+    }
+
+    __syncwarp();
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync();   // the peer may still read this CTA's smem / signal its barriers until both are done
+    if (warp == 1) {
+        tc_fence_after();
+        tmem_dealloc<2>(tmem_base, 512);
+    }
+}
+
+}  // namespace g2
+
+tqp_status launch_gemm_tcgen05_2cta(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st) {
+    for (int i = 0; i < nprob; ++i)
+        if (probs[i].M % (2 * g2::BM) != 0) return launch_gemm_tcgen05(c, probs, nprob, st);   // odd number of 128-row tiles
+    static bool attr_set = false;
+    if (!attr_set) {
+        TQP_CUDA_OK(c, cudaFuncSetAttribute(g2::gemm_tcgen05_2cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, g2::SMEM_BYTES));
+        attr_set = true;
+    }
+    GemmArgs args;
+    for (int i = 0; i < nprob; ++i) args.p[i] = probs[i];
+    args.nprob = nprob;
+    const int grid = (c->num_sms / 2) * 2;
+    g2::gemm_tcgen05_2cta_kernel<<<grid, g2::NTHREADS, g2::SMEM_BYTES, st>>>(
+        args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), c->ablate);
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
+
+}  // namespace tqp

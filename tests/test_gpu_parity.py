@@ -50,14 +50,14 @@ def _skewed(cfg):
     return inp
 
 
-@pytest.mark.parametrize("gemm_impl", [1, 0], ids=["scaffold", "tcgen05"])
+@pytest.mark.parametrize("gemm_impl", [1, 2, 0], ids=["scaffold", "tcgen05_1cta", "tcgen05"])
 def test_cfg0_tiny_full_chain(gemm_impl):
     cfg = ti.CONFIGS[0]
     inp = ti.make_inputs(cfg)
     check_all(inp, backward=True, router_grad=True, gemm_impl=gemm_impl)
 
 
-@pytest.mark.parametrize("gemm_impl", [1, 0], ids=["scaffold", "tcgen05"])
+@pytest.mark.parametrize("gemm_impl", [1, 2, 0], ids=["scaffold", "tcgen05_1cta", "tcgen05"])
 @pytest.mark.parametrize("cfg", [MID, MID32], ids=lambda c: c.name)
 def test_mid_ragged_multi_tile(cfg, gemm_impl):
     inp = _skewed(cfg)
