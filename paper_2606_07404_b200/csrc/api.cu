@@ -38,6 +38,7 @@ Workspace layout(const tqp_layer_desc &d) {
     w.lut = take(256 * 8 * 2);
     w.WrT = take(E * dm * 4);
     w.dl = take(N * 4);
+    w.trace = take(16384 * 8);
     w.hX = take(T * dm * 2); w.hdY = take(T * dm * 2); w.hY = take(T * dm * 2); w.hdX = take(T * dm * 2);
     w.topk_idx = take(N * 4); w.topk_w = take(N * 4); w.counts = take(E * 4); w.offsets = take((E + 1) * 4);
     w.perm = take(N * 4); w.inv_perm = take(N * 4);
@@ -264,6 +265,10 @@ tqp_status tqp_set_option(tqp_ctx *c, const char *name, int value) {
         c->gemm_impl = value;
         return TQP_OK;
     }
+    if (!strcmp(name, "trace")) {
+        c->trace = value;
+        return TQP_OK;
+    }
     if (!strcmp(name, "ablate")) {
         c->ablate = value;
         return TQP_OK;
@@ -445,7 +450,7 @@ void *tqp_debug_buffer(tqp_ctx *c, const char *name) {
     struct { const char *n; size_t off; } tab[] = {
         {"G", c->ws.G}, {"U", c->ws.U}, {"H", c->ws.H}, {"Xp", c->ws.Xp}, {"dH", c->ws.dH}, {"dG", c->ws.dG},
         {"dU", c->ws.dU}, {"num_tiles", c->ws.num_tiles}, {"tiles", c->ws.tiles}, {"XAg", c->ws.XAg}, {"Zd", c->ws.Zd},
-        {"logits", c->ws.logits}, {"lut", c->ws.lut}};
+        {"logits", c->ws.logits}, {"lut", c->ws.lut}, {"trace", c->ws.trace}};
     for (auto &t : tab)
         if (!strcmp(t.n, name)) return c->base + t.off;
     return nullptr;

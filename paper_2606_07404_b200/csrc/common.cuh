@@ -64,7 +64,7 @@ struct Workspace {
     // offsets (bytes) into the bound buffer
     size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, lut, WrT, dl,
         // tqp_step_host staging
-        hX, hdY, hY, hdX, topk_idx, topk_w, counts, offsets, perm, inv_perm, Ye, dYe, dXp, dtopk_w;
+        trace, hX, hdY, hY, hdX, topk_idx, topk_w, counts, offsets, perm, inv_perm, Ye, dYe, dXp, dtopk_w;
 };
 
 }  // namespace tqp
@@ -84,6 +84,7 @@ struct tqp_ctx {
     int max_tiles = 0;
     std::string err;
     int ablate = 0;             // timing experiments only (tqp_set_option "ablate")
+    int trace = 0;              // debug: clock64 timeline of one cluster of the CTA-pair GEMM
     int time_gemm = 0;          // bracket GEMM launches with events (tqp_gemm_time)
     std::vector<cudaEvent_t> ev; // pairs (start, stop)
     int ev_used = 0;

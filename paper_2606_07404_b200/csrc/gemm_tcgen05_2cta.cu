@@ -38,13 +38,13 @@ struct Item {
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
 gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__restrict__ lut_g, const Tile *__restrict__ tiles,
-                         const int32_t *__restrict__ num_tiles_p, int ablate) {
+                         const int32_t *__restrict__ num_tiles_p, int ablate, long long *__restrict__ trace) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     const uint32_t sbase = smem_u32(smem);
     const uint32_t bar0 = sbase + OFF_BAR;
-    auto full_x = [&](int s) { return bar0 + 8u * s; };                              // leader's is used
-    auto full_a = [&](int s) { return bar0 + 8u * (NSTAGE + s); };                   // leader's is used
+    // full[s] (the LEADER's is used): 1 arrival + 2 x X_BYTES of TMA from the activation producers, 8 dequant-warp arrivals
+    auto full = [&](int s) { return bar0 + 8u * s; };
     auto empty = [&](int s) { return bar0 + 8u * (2 * NSTAGE + s); };                // local, multicast commit
     auto idx_full = [&](int s) { return bar0 + 8u * (3 * NSTAGE + s); };             // local
     auto idx_empty = [&](int s) { return bar0 + 8u * (3 * NSTAGE + IDXQ + s); };     // local
@@ -54,9 +54,10 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
 
     const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
     const uint32_t rank = cluster_ctarank();
+    const uint32_t full_remote = mapa(full(0), 0), tmem_empty_remote = mapa(tmem_empty(0), 0);   // the leader's barriers
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < NSTAGE; ++s) { mbar_init(full_x(s), 1); mbar_init(full_a(s), 8); mbar_init(empty(s), 1); }
+        for (int s = 0; s < NSTAGE; ++s) { mbar_init(full(s), 9); mbar_init(empty(s), 1); }
         for (int s = 0; s < IDXQ; ++s) { mbar_init(idx_full(s), 1); mbar_init(idx_empty(s), 8); }
         for (int s = 0; s < 2; ++s) { mbar_init(tmem_full(s), 1); mbar_init(tmem_empty(s), 8); }
         mbar_init_fence();
@@ -101,15 +102,16 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                     const int nkb = S.K / BK;
                     for (int kb = 0; kb < nkb; ++kb) {
                         mbar_wait(empty(st.s), st.ph ^ 1);
-                        if (rank == 0) mbar_expect_tx(full_x(st.s), 2 * X_BYTES);
-                        tma_load_2d_pair(sbase + OFF_X + st.s * X_BYTES, &S.act_map2, kb * BK, row, mapa(full_x(st.s), 0));
+                        if (ablate & 8) { if (rank == 0) mbar_arrive(full(st.s)); st.next(NSTAGE); continue; }
+                        if (rank == 0) mbar_expect_tx(full(st.s), 2 * X_BYTES);
+                        tma_load_2d_pair(sbase + OFF_X + st.s * X_BYTES, &S.act_map2, kb * BK, row, full_remote + 8u * st.s);
                         st.next(NSTAGE);
                     }
                 }
                 for (int l = 0; l < pb.nlora; ++l) {
                     mbar_wait(empty(st.s), st.ph ^ 1);
-                    if (rank == 0) mbar_expect_tx(full_x(st.s), 2 * X_BYTES);
-                    tma_load_2d_pair(sbase + OFF_X + st.s * X_BYTES, &pb.lora[l].lact_map2, 0, row, mapa(full_x(st.s), 0));
+                    if (rank == 0) mbar_expect_tx(full(st.s), 2 * X_BYTES);
+                    tma_load_2d_pair(sbase + OFF_X + st.s * X_BYTES, &pb.lora[l].lact_map2, 0, row, full_remote + 8u * st.s);
                     st.next(NSTAGE);
                 }
             }
@@ -128,6 +130,7 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                     const int npair = S.K / (2 * BK);
                     for (int kp = 0; kp < npair; ++kp) {
                         mbar_wait(idx_empty(iq.s), iq.ph ^ 1);
+                        if (ablate & 64) { mbar_arrive(idx_full(iq.s)); iq.next(IDXQ); continue; }
                         mbar_expect_tx(idx_full(iq.s), IDX_BYTES);
                         const int c0 = S.kmajor ? kp * 16 : it.m0 / 8;
                         const int c1 = S.kmajor ? it.t.expert * pb.M + it.m0 : it.t.expert * S.K + kp * 2 * BK;
@@ -141,7 +144,7 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
         // =========================== MMA issuer (leader CTA) ===========================
         if (rank == 0 && lane == 0) {
             Pipe st;
-            int cnt = 0;
+            int cnt = 0, tcount = 0;
             for (long long item = cid; item < total; item += ncl) {
                 Item it;
                 get_item(item, it);
@@ -155,35 +158,41 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + ab * TN;
                 uint32_t accum = 0;
+                const uint32_t hi_k = desc_hi(1024), lo_k = desc_lo_const(16);          // K-major SW128: SBO = 8 rows x 128 B
+                const uint32_t hi_mn = desc_hi(2048), lo_mn = desc_lo_const(1024);      // MN-major SW128 A tile
+                const uint32_t x16 = (sbase + OFF_X) >> 4, a16 = (sbase + OFF_A) >> 4;
                 for (int sg = 0; sg < pb.nseg; ++sg) {
                     const GemmSeg &S = pb.seg[sg];
                     const int nkb = S.K / BK;
-                    const uint32_t idesc = make_idesc(2 * BM, n, S.kmajor ? 0 : 1);
+                    const int kmajor = S.kmajor;
+                    const uint32_t idesc = make_idesc(2 * BM, n, kmajor ? 0 : 1);
+                    const uint32_t a_hi = kmajor ? hi_k : hi_mn, a_lo = kmajor ? lo_k : lo_mn, a_step = kmajor ? 2u : 256u;
                     for (int kb = 0; kb < nkb; ++kb) {
-                        mbar_wait<true>(full_x(st.s), st.ph);
-                        mbar_wait<true>(full_a(st.s), st.ph);
+                        long long tr0 = 0;
+                        if (trace && cid == 0) tr0 = clock64();
+                        mbar_wait<true>(full(st.s), st.ph);
                         tc_fence_after();
-                        const uint32_t xa = sbase + OFF_X + st.s * X_BYTES, aa = sbase + OFF_A + st.s * A_BYTES;
+                        if (trace && cid == 0 && tcount < 2000) { trace[tcount * 4 + 0] = tr0; trace[tcount * 4 + 1] = clock64(); }
+                        const uint32_t xs = x16 + st.s * (X_BYTES >> 4), as = a16 + st.s * (A_BYTES >> 4);
 #pragma unroll
                         for (int kk = 0; kk < BK / 16; ++kk) {
-                            const uint64_t bd = make_desc(xa + kk * 32, 16, 1024);
-                            const uint64_t ad = S.kmajor ? make_desc(aa + kk * 32, 16, 1024) : make_desc(aa + kk * 4096, 1024, 2048);
-                            umma_bf16<2>(d_tmem, ad, bd, idesc, accum);
+                            if (ablate & 32) break;
+                            umma_bf16<2>(d_tmem, desc_from(a_hi, a_lo, as + kk * a_step), desc_from(hi_k, lo_k, xs + kk * 2), idesc, accum);
                             accum = 1;
                         }
                         umma_commit_pair(empty(st.s), 3);
+                        if (trace && cid == 0 && tcount < 2000) { trace[tcount * 4 + 2] = clock64(); trace[tcount * 4 + 3] = kb; ++tcount; }
                         st.next(NSTAGE);
                     }
                 }
                 const uint32_t idesc_l = make_idesc(2 * BM, n, 0);
                 const int nmma_l = max(1, pb.r / 16);
                 for (int l = 0; l < pb.nlora; ++l) {
-                    mbar_wait<true>(full_x(st.s), st.ph);
-                    mbar_wait<true>(full_a(st.s), st.ph);
+                    mbar_wait<true>(full(st.s), st.ph);
                     tc_fence_after();
-                    const uint32_t xa = sbase + OFF_X + st.s * X_BYTES, aa = sbase + OFF_A + st.s * A_BYTES;
+                    const uint32_t xs = x16 + st.s * (X_BYTES >> 4), as = a16 + st.s * (A_BYTES >> 4);
                     for (int kk = 0; kk < nmma_l; ++kk) {
-                        umma_bf16<2>(d_tmem, make_desc(aa + kk * 32, 16, 1024), make_desc(xa + kk * 32, 16, 1024), idesc_l, accum);
+                        umma_bf16<2>(d_tmem, desc_from(hi_k, lo_k, as + kk * 2), desc_from(hi_k, lo_k, xs + kk * 2), idesc_l, accum);
                         accum = 1;
                     }
                     umma_commit_pair(empty(st.s), 3);
@@ -199,6 +208,7 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
         const int c = tid & 7;
         const uint4 *lut_s = reinterpret_cast<const uint4 *>(smem + OFF_LUT);
         Pipe st, iq;
+        int dcount = 0;
         for (long long item = cid; item < total; item += ncl) {
             Item it;
             get_item(item, it);
@@ -230,7 +240,11 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                     if ((kb & 1) == g) {
                         const __nv_bfloat162 s2 = __float2bfloat162_rn(__half2float(sc_next));
                         if (!kmajor && kb + 2 < nkb) sc_next = scale_p[(kb + 2 - g) * BK];
+                        long long tr0 = 0;
+                        const bool tr = trace && cid == 0 && rank == 0 && threadIdx.x == W_DEQ0 * 32 && dcount < 1000;
+                        if (tr) tr0 = clock64();
                         mbar_wait(empty(st.s), st.ph ^ 1);
+                        if (tr) { trace[8000 + dcount * 4] = tr0; trace[8000 + dcount * 4 + 1] = clock64(); }
                         uint8_t *as = smem + OFF_A + st.s * A_BYTES;
                         const uint32_t c01[2] = {codes.x, codes.y};
 #pragma unroll
@@ -244,9 +258,13 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                             }
                             if (!(ablate & 2)) *reinterpret_cast<uint4 *>(as + rowoff + ((j ^ sw) << 4)) = v;
                         }
-                        fence_async_smem();
+                        if (tr) trace[12000 + dcount * 2] = clock64();
+                        if (!(ablate & 128)) fence_async_smem();
+                        if (tr) trace[8000 + dcount * 4 + 2] = clock64();
                         __syncwarp();
-                        if (lane == 0) mbar_arrive_cluster(mapa(full_a(st.s), 0));
+                        if (tr) trace[12000 + dcount * 2 + 1] = clock64();
+                        if (lane == 0) mbar_arrive_cluster(full_remote + 8u * st.s);
+                        if (tr) { trace[8000 + dcount * 4 + 3] = clock64(); ++dcount; }
                     }
                     st.next(NSTAGE);
                 }
@@ -274,7 +292,7 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                         if (j < nch) *reinterpret_cast<uint4 *>(as + tid * 128 + ((j ^ (tid & 7)) << 4)) = ch[j];
                     fence_async_smem();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive_cluster(mapa(full_a(st.s), 0));
+                    if (lane == 0) mbar_arrive_cluster(full_remote + 8u * st.s);
                 }
                 st.next(NSTAGE);
             }
@@ -303,11 +321,11 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                 tmem_ld_wait();
 #pragma unroll
                 for (int j = 0; j < 16; ++j)
-                    if (c0 + j < it.t.rows) outp[(size_t)(c0 + j) * M] = __float2bfloat16_rn(__uint_as_float(v[j]));
+                    if (c0 + j < it.t.rows && !(ablate & 16)) outp[(size_t)(c0 + j) * M] = __float2bfloat16_rn(__uint_as_float(v[j]));
             }
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(mapa(tmem_empty(ab), 0));
+            if (lane == 0) mbar_arrive_cluster(tmem_empty_remote + 8u * ab);
         }
     }
 
@@ -336,7 +354,7 @@ tqp_status launch_gemm_tcgen05_2cta(tqp_ctx *c, const GemmProblem *probs, int np
     args.nprob = nprob;
     const int grid = (c->num_sms / 2) * 2;
     g2::gemm_tcgen05_2cta_kernel<<<grid, g2::NTHREADS, g2::SMEM_BYTES, st>>>(
-        args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), c->ablate);
+        args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), c->ablate, c->trace ? c->p<long long>(c->ws.trace) : nullptr);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }

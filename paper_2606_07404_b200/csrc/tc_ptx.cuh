@@ -32,31 +32,34 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 }
 // arrive on a barrier given by its shared::cluster address (possibly in the peer CTA)
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
 }
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
 template <bool kClusterScope = false>
+__device__ __forceinline__ uint32_t mbar_try(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    if (kClusterScope)
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    else
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    return done;
+}
+template <bool kClusterScope = false>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    uint32_t done = 0;
-    const long long t0 = clock64();
-    while (true) {
-        if (kClusterScope)
-            asm volatile(
-                "{\n\t.reg .pred p;\n\t"
-                "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
-                "selp.u32 %0, 1, 0, p;\n\t}"
-                : "=r"(done) : "r"(bar), "r"(parity) : "memory");
-        else
-            asm volatile(
-                "{\n\t.reg .pred p;\n\t"
-                "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-                "selp.u32 %0, 1, 0, p;\n\t}"
-                : "=r"(done) : "r"(bar), "r"(parity) : "memory");
-        if (done) break;
+    if (mbar_try<kClusterScope>(bar, parity)) return;
+    const long long t0 = clock64();   // slow path only
+    while (!mbar_try<kClusterScope>(bar, parity))
         if (clock64() - t0 > 8000000000ll) __trap();   // a broken pipeline must fault, not hang the GPU
-    }
 }
 
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const void *tmap, int c0, int c1, uint32_t bar) {
@@ -146,6 +149,12 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t addr, uint32_t lbo_bytes,
     d |= (uint64_t)2 << 61;   // layout_type = SWIZZLE_128B
     return d;
 }
+// Hot-loop form: the high word and the LBO half of the low word are loop constants, only the address moves.
+__device__ __forceinline__ uint64_t desc_from(uint32_t hi, uint32_t lo_const, uint32_t addr16) {
+    return ((uint64_t)hi << 32) | (uint64_t)(lo_const | (addr16 & 0x3fff));
+}
+__device__ __forceinline__ uint32_t desc_hi(uint32_t sbo_bytes) { return ((sbo_bytes >> 4) & 0x3fff) | (1u << 14) | (2u << 29); }
+__device__ __forceinline__ uint32_t desc_lo_const(uint32_t lbo_bytes) { return ((lbo_bytes >> 4) & 0x3fff) << 16; }
 // Instruction descriptor (cute::UMMA::InstrDescriptor), kind::f16: D fp32, A/B bf16; a_mn = 1 -> A is MN-major
 __device__ __forceinline__ uint32_t make_idesc(int m, int n, int a_mn) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_mn << 15) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
