@@ -78,6 +78,26 @@ class ClockSampler(threading.Thread):
                 "reasons": reasons, "samples": len(good)}
 
 
+def rank_config(cfg, rank):
+    """Weak scaling: every rank owns an independent batch of the same shape (its own seed); no data-path collective."""
+    import dataclasses
+    return dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+
+
+def max_over_ranks(ms, dist, device):
+    """Device time of the slowest rank (the contract's 'max over ranks')."""
+    if dist is None:
+        return ms
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world, tokens_per_rank, steps, ms):
+    return world * tokens_per_rank * steps / (ms / 1e3)
+
+
 def oracle_step(inp, cfg):
     import oracle
     return oracle.layer(inp, dtype=np.float32, backward=True, router_grad=cfg.router_grad)
@@ -132,9 +152,7 @@ def run_ours(args, cfg):
     torch.cuda.set_device(dev)
 
     # each rank owns an independent batch of the same shape (weak scaling, no data-path collective)
-    import dataclasses
-    rcfg = dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
-    inp = ti.make_inputs(rcfg)
+    inp = ti.make_inputs(rank_config(cfg, rank))
     T, k, d = cfg.T, cfg.k, cfg.d
     layer = tq.TqpLayer(T, cfg.d, cfg.F, cfg.E, cfg.k, cfg.r, lora_scale=cfg.lora_scale, training=True, device=str(dev))
     if args.gemm_impl:
@@ -190,12 +208,9 @@ def run_ours(args, cfg):
     ms = e0.elapsed_time(e1)
     gemm_ms, gemm_launches = layer.gemm_time()
     layer.set_option("time_gemm", 0)
-    if dist is not None:
-        tt = torch.tensor([ms], device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
+    ms = max_over_ranks(ms, dist, dev)
     ms_per_step = ms / args.steps
-    value = world * T * args.steps / (ms / 1e3)
+    value = whole_job_value(world, T, args.steps, ms)
 
     # ---- end to end through the C ABI with HOST buffers (H2D + whole chain + D2H inside the timed region) ----
     e2e = None
@@ -212,12 +227,9 @@ def run_ours(args, cfg):
         e1.record()
         barrier()
         ems = e0.elapsed_time(e1)
-        if dist is not None:
-            tt = torch.tensor([ems], device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            ems = float(tt.item())
+        ems = max_over_ranks(ems, dist, dev)
         nb = T * d * 2
-        e2e = {"value": world * T * args.steps / (ems / 1e3), "unit": "tokens/s", "h2d_bytes_per_step": 2 * nb,
+        e2e = {"value": whole_job_value(world, T, args.steps, ems), "unit": "tokens/s", "h2d_bytes_per_step": 2 * nb,
                "d2h_bytes_per_step": 2 * nb, "ms_per_step": ems / args.steps}
 
     if rank != 0:

@@ -124,12 +124,13 @@ def _weights(inp, dtype):
     return idx, real
 
 
-def expert_fwd(inp, offsets, perm, dtype=np.float32, save=True):
-    """Returns Ye [N,d] (and G, U, H [N,F] when save)."""
+def expert_fwd(inp, offsets, perm, dtype=np.float32, save=True, n_rows=None):
+    """Returns Ye [N,d] (and G, U, H [N,F] when save).  n_rows: number of routed rows actually present
+    (offsets[E]) when the call covers a sample of experts only; default N = T*k."""
     X = _real(inp["X"], dtype)
     T, d = X.shape
     F, E, k, r = inp["F"], inp["E"], inp["k"], inp["r"]
-    N = T * k
+    N = T * k if n_rows is None else n_rows
     idx, real = _weights(inp, dtype)
     Ye = np.empty((N, d), dtype=dtype)
     G = np.empty((N, F), dtype=dtype) if save else None
@@ -162,12 +163,12 @@ def combine_bwd(dY, Ye, inv_perm, topk_w, dtype=np.float32):
     return dYe, dw
 
 
-def expert_bwd(inp, dYe, G, U, H, offsets, perm, dtype=np.float32):
+def expert_bwd(inp, dYe, G, U, H, offsets, perm, dtype=np.float32, n_rows=None):
     """Returns dXp [N,d] and the dict of adapter gradients (fp, overwritten, zero for empty experts)."""
     X = _real(inp["X"], dtype)
     T, d = X.shape
     F, E, k, r = inp["F"], inp["E"], inp["k"], inp["r"]
-    N = T * k
+    N = T * k if n_rows is None else n_rows
     idx, real = _weights(inp, dtype)
     dXp = np.empty((N, d), dtype=dtype)
     g = {
