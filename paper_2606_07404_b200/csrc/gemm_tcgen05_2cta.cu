@@ -206,7 +206,7 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
         const int g = (warp - W_DEQ0) >> 2;
         const int tid = (threadIdx.x - W_DEQ0 * 32) & 127;
         const int c = tid & 7;
-        const uint4 *lut_s = reinterpret_cast<const uint4 *>(smem + OFF_LUT);
+        const uint32_t lut_a = sbase + OFF_LUT + c * 16;
         Pipe st, iq;
         int dcount = 0;
         for (long long item = cid; item < total; item += ncl) {
@@ -230,9 +230,8 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                 for (int kb = 0; kb < nkb; ++kb) {
                     if ((kb & 1) == 0) {
                         mbar_wait(idx_full(iq.s), iq.ph);
-                        const uint8_t *is = smem + OFF_IDX + iq.s * IDX_BYTES;
-                        codes = kmajor ? *reinterpret_cast<const uint2 *>(is + tid * 16 + g * 8)
-                                       : *reinterpret_cast<const uint2 *>(is + (g * 64 + kr) * 16 + half * 8);
+                        const uint32_t is = sbase + OFF_IDX + iq.s * IDX_BYTES;
+                        codes = lds64(kmajor ? is + tid * 16 + g * 8 : is + (g * 64 + kr) * 16 + half * 8);
                         __syncwarp();
                         if (lane == 0) mbar_arrive(idx_empty(iq.s));
                         iq.next(IDXQ);
@@ -245,18 +244,18 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                         if (tr) tr0 = clock64();
                         mbar_wait(empty(st.s), st.ph ^ 1);
                         if (tr) { trace[8000 + dcount * 4] = tr0; trace[8000 + dcount * 4 + 1] = clock64(); }
-                        uint8_t *as = smem + OFF_A + st.s * A_BYTES;
+                        const uint32_t as = sbase + OFF_A + st.s * A_BYTES + rowoff;
                         const uint32_t c01[2] = {codes.x, codes.y};
 #pragma unroll
                         for (int j = 0; j < 8; ++j) {
                             const uint32_t code = (c01[j >> 2] >> ((j & 3) * 8)) & 0xffu;
-                            uint4 v = (ablate & 1) ? make_uint4(code, code, code, code) : lut_s[code * 8 + c];
+                            uint4 v = (ablate & 1) ? make_uint4(code, code, code, code) : lds128(lut_a + code * 128);
                             __nv_bfloat162 *pv = reinterpret_cast<__nv_bfloat162 *>(&v);
                             if (!(ablate & 4)) {
 #pragma unroll
                                 for (int q = 0; q < 4; ++q) pv[q] = __hmul2(pv[q], s2);
                             }
-                            if (!(ablate & 2)) *reinterpret_cast<uint4 *>(as + rowoff + ((j ^ sw) << 4)) = v;
+                            if (!(ablate & 2)) sts128(as + ((j ^ sw) << 4), v);
                         }
                         if (tr) trace[12000 + dcount * 2] = clock64();
                         if (!(ablate & 128)) fence_async_smem();
@@ -286,10 +285,10 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                         for (int q = 0; q < r; ++q) h[q] = *reinterpret_cast<const uint16_t *>(src + (size_t)q * M);
                     }
                     mbar_wait(empty(st.s), st.ph ^ 1);
-                    uint8_t *as = smem + OFF_A + st.s * A_BYTES;
+                    const uint32_t as = sbase + OFF_A + st.s * A_BYTES + tid * 128;
 #pragma unroll
                     for (int j = 0; j < 4; ++j)
-                        if (j < nch) *reinterpret_cast<uint4 *>(as + tid * 128 + ((j ^ (tid & 7)) << 4)) = ch[j];
+                        if (j < nch) sts128(as + ((j ^ (tid & 7)) << 4), ch[j]);
                     fence_async_smem();
                     __syncwarp();
                     if (lane == 0) mbar_arrive_cluster(full_remote + 8u * st.s);
