@@ -24,54 +24,70 @@ __global__ void __launch_bounds__(128) dispatch_hist_kernel(const int32_t *__res
         for (int e = lane; e < E; e += 32) blk_counts[(size_t)chunk * E + e] = cnt[e];
 }
 
-// Phase 2 (one block): per expert exclusive scan over the chunks -> chunk bases; exclusive scan over experts
-// -> offsets; tile list.  blk_counts is overwritten by the absolute base position of (chunk, expert).
-__global__ void __launch_bounds__(1024) dispatch_scan_kernel(int32_t *__restrict__ blk_counts, int nchunks, int N, int E,
-                                                             int32_t *__restrict__ counts, int32_t *__restrict__ offsets,
-                                                             Tile *__restrict__ tiles, int32_t *__restrict__ num_tiles) {
-    __shared__ int32_t s_cnt[1024], s_off[1025], s_tiles[1025];
-    const int e = threadIdx.x;
-    int total = 0;
-    if (e < E) {
-        for (int c = 0; c < nchunks; ++c) {
-            int v = blk_counts[(size_t)c * E + e];
-            blk_counts[(size_t)c * E + e] = total;   // base of this chunk inside the expert's segment
-            total += v;
+// Phase 2a: one warp per expert turns its column of chunk counts into exclusive prefixes (in place) and writes the
+// expert's total.  Phase 2b (one block): exclusive scan over experts -> offsets, and the GEMM tile list.
+__global__ void __launch_bounds__(256) dispatch_scan_chunks_kernel(int32_t *__restrict__ blk_counts, int nchunks, int E,
+                                                                   int32_t *__restrict__ counts) {
+    const int e = (blockIdx.x * blockDim.x + threadIdx.x) / 32, lane = threadIdx.x % 32;
+    if (e >= E) return;
+    int running = 0;
+    for (int c0 = 0; c0 < nchunks; c0 += 32) {
+        const int c = c0 + lane;
+        const int v = (c < nchunks) ? blk_counts[(size_t)c * E + e] : 0;
+        int incl = v;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            int t = __shfl_up_sync(0xffffffffu, incl, off);
+            if (lane >= off) incl += t;
         }
+        if (c < nchunks) blk_counts[(size_t)c * E + e] = running + incl - v;
+        running += __shfl_sync(0xffffffffu, incl, 31);
     }
-    s_cnt[e] = (e < E) ? total : 0;
+    if (lane == 0) counts[e] = running;
+}
+
+__global__ void __launch_bounds__(1024) dispatch_scan_experts_kernel(const int32_t *__restrict__ counts, int E,
+                                                                     int32_t *__restrict__ offsets, Tile *__restrict__ tiles,
+                                                                     int32_t *__restrict__ num_tiles) {
+    __shared__ int32_t w_off[32], w_til[32];
+    const int e = threadIdx.x, lane = e % 32, warp = e / 32;
+    const int cnt = (e < E) ? counts[e] : 0;
+    const int nt = (cnt + kTileRows - 1) / kTileRows;
+    int io = cnt, it = nt;   // inclusive scans inside the warp
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        int a = __shfl_up_sync(0xffffffffu, io, off), b = __shfl_up_sync(0xffffffffu, it, off);
+        if (lane >= off) { io += a; it += b; }
+    }
+    if (lane == 31) { w_off[warp] = io; w_til[warp] = it; }
     __syncthreads();
-    if (e == 0) {
-        int acc = 0, tacc = 0;
-        for (int q = 0; q < E; ++q) {
-            s_off[q] = acc;
-            s_tiles[q] = tacc;
-            acc += s_cnt[q];
-            tacc += (s_cnt[q] + kTileRows - 1) / kTileRows;
+    if (warp == 0) {
+        int a = w_off[lane], b = w_til[lane], ia = a, ib = b;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            int x = __shfl_up_sync(0xffffffffu, ia, off), y = __shfl_up_sync(0xffffffffu, ib, off);
+            if (lane >= off) { ia += x; ib += y; }
         }
-        s_off[E] = acc;
-        s_tiles[E] = tacc;
-        *num_tiles = tacc;
+        w_off[lane] = ia - a;   // exclusive prefix of the warp totals
+        w_til[lane] = ib - b;
     }
     __syncthreads();
+    const int off_e = w_off[warp] + io - cnt, til_e = w_til[warp] + it - nt;
     if (e < E) {
-        counts[e] = s_cnt[e];
-        offsets[e] = s_off[e];
-        if (e == E - 1) offsets[E] = s_off[E];
-        const int cnt = s_cnt[e], nt = (cnt + kTileRows - 1) / kTileRows;
+        offsets[e] = off_e;
+        if (e == E - 1) { offsets[E] = off_e + cnt; *num_tiles = til_e + nt; }
         if (nt > 0) {
             int per = (cnt + nt - 1) / nt;
             per = (per + 15) & ~15;   // balanced tiles, multiples of 16 rows (UMMA N granularity)
             for (int i = 0; i < nt; ++i) {
                 Tile t;
                 t.expert = e;
-                t.row0 = s_off[e] + i * per;
+                t.row0 = off_e + i * per;
                 t.rows = max(0, min(per, cnt - i * per));   // rows == 0: skipped by the consumers
                 t.pad = 0;
-                tiles[s_tiles[e] + i] = t;
+                tiles[til_e + i] = t;
             }
         }
-        for (int c = 0; c < nchunks; ++c) blk_counts[(size_t)c * E + e] += s_off[e];
     }
 }
 
@@ -79,6 +95,7 @@ __global__ void __launch_bounds__(1024) dispatch_scan_kernel(int32_t *__restrict
 // the rank among equal experts inside a group, so rows of one expert stay in ascending a (stable).
 __global__ void __launch_bounds__(128) dispatch_scatter_kernel(const int32_t *__restrict__ topk_idx, int N, int E,
                                                                const int32_t *__restrict__ blk_base,
+                                                               const int32_t *__restrict__ offsets,
                                                                int32_t *__restrict__ perm, int32_t *__restrict__ inv_perm) {
     extern __shared__ int32_t sm[];
     const int warp_in_blk = threadIdx.x / 32, lane = threadIdx.x % 32;
@@ -86,7 +103,7 @@ __global__ void __launch_bounds__(128) dispatch_scatter_kernel(const int32_t *__
     const int a0 = chunk * kDispChunk;
     if (a0 >= N) return;
     int32_t *cur = sm + warp_in_blk * E;
-    for (int e = lane; e < E; e += 32) cur[e] = blk_base[(size_t)chunk * E + e];
+    for (int e = lane; e < E; e += 32) cur[e] = blk_base[(size_t)chunk * E + e] + offsets[e];
     __syncwarp();
     for (int i = 0; i < kDispChunk; i += 32) {
         int a = a0 + i + lane;
@@ -115,10 +132,11 @@ tqp_status launch_dispatch(tqp_ctx *c, int T, const int32_t *topk_idx, int32_t *
     const size_t smem = (size_t)4 * E * sizeof(int32_t);
     dispatch_hist_kernel<<<nblk, 128, smem, s>>>(topk_idx, N, E, blk);
     TQP_LAUNCH_OK(c);
-    dispatch_scan_kernel<<<1, 1024, 0, s>>>(blk, nchunks, N, E, counts, offsets, c->p<Tile>(c->ws.tiles),
-                                            c->p<int32_t>(c->ws.num_tiles));
+    dispatch_scan_chunks_kernel<<<(E + 7) / 8, 256, 0, s>>>(blk, nchunks, E, counts);
     TQP_LAUNCH_OK(c);
-    dispatch_scatter_kernel<<<nblk, 128, smem, s>>>(topk_idx, N, E, blk, perm, inv_perm);
+    dispatch_scan_experts_kernel<<<1, 1024, 0, s>>>(counts, E, offsets, c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles));
+    TQP_LAUNCH_OK(c);
+    dispatch_scatter_kernel<<<nblk, 128, smem, s>>>(topk_idx, N, E, blk, offsets, perm, inv_perm);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }
