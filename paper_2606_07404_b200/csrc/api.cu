@@ -302,6 +302,9 @@ tqp_status tqp_dispatch(tqp_ctx *c, int T, const int32_t *topk_idx, int32_t *cou
     PTR_OK(c, topk_idx); PTR_OK(c, counts); PTR_OK(c, offsets); PTR_OK(c, perm); PTR_OK(c, inv_perm);
     c->disp_T = T;
     c->fwd_T = -1;
+    c->disp_perm = perm;
+    c->disp_inv_perm = inv_perm;
+    c->zd_src = nullptr;
     return launch_dispatch(c, T, topk_idx, counts, offsets, perm, inv_perm, (cudaStream_t)stream);
 }
 
@@ -317,13 +320,20 @@ tqp_status tqp_expert_fwd(tqp_ctx *c, int T, const void *X, const int32_t *offse
     const float ls = D.lora_scale;
     bf16 *Xp = c->p<bf16>(c->ws.Xp), *G = c->p<bf16>(c->ws.G), *U = c->p<bf16>(c->ws.U), *H = c->p<bf16>(c->ws.H);
 #define CK(x) do { st = (x); if (st != TQP_OK) return st; } while (0)
-    CK(launch_gather_rows(c, N, (const bf16 *)X, perm, Xp, s));
-    CK(launch_lora_down(c, Xp, D.d, (const bf16 *)c->w.A_gate, 1, ls, c->p<bf16>(c->ws.XAg), s));
-    CK(launch_lora_down(c, Xp, D.d, (const bf16 *)c->w.A_up, 1, ls, c->p<bf16>(c->ws.XAu), s));
+    const bool fused = D.r == 16 || D.r == 32;   // rank 8 (config 0) keeps the separate CUDA-core kernels
+    if (fused) {   // Xp = gather(X) and both adapter projections x.A_g | x.A_u in one pass over the rows
+        CK(launch_rows_proj(c, (const bf16 *)X, D.d, perm, nullptr, Xp, (const bf16 *)c->w.A_gate, (const bf16 *)c->w.A_up, 1,
+                            ls, c->p<bf16>(c->ws.XAg), c->p<bf16>(c->ws.XAu), s));
+    } else {
+        CK(launch_gather_rows(c, N, (const bf16 *)X, perm, Xp, s));
+        CK(launch_rows_proj(c, Xp, D.d, nullptr, nullptr, nullptr, (const bf16 *)c->w.A_gate, (const bf16 *)c->w.A_up, 1, ls,
+                            c->p<bf16>(c->ws.XAg), c->p<bf16>(c->ws.XAu), s));
+    }
     GemmProblem pr[2] = {c->prob_gate, c->prob_up};
     CK(run_gemm(c, pr, 2, s));
     CK(launch_swiglu_fwd(c, N, G, U, H, s));
-    CK(launch_lora_down(c, H, D.F, (const bf16 *)c->w.A_down, 1, ls, c->p<bf16>(c->ws.HAd), s));
+    CK(launch_rows_proj(c, H, D.F, nullptr, nullptr, nullptr, (const bf16 *)c->w.A_down, nullptr, 1, ls,
+                        c->p<bf16>(c->ws.HAd), nullptr, s));
     GemmProblem pd = c->prob_down;
     pd.out = (bf16 *)Ye;
     CK(run_gemm(c, &pd, 1, s));
@@ -346,6 +356,18 @@ tqp_status tqp_combine_bwd(tqp_ctx *c, int T, const void *dY, const void *Ye, co
     if (st != TQP_OK) return st;
     PTR_OK(c, dY); PTR_OK(c, inv_perm); PTR_OK(c, topk_w); PTR_OK(c, dYe);
     if (dtopk_w) PTR_OK(c, Ye);
+    const tqp_layer_desc &D = c->desc;
+    c->zd_src = nullptr;
+    if ((D.r == 16 || D.r == 32) && D.training && c->have_weights && c->disp_T == T && c->disp_inv_perm == inv_perm) {
+        // Fused: dYe[p] = w[a] dY[t] by sorted position (a = perm[p]) and, from the same rows, Zd = s dYe . B_d^T, the
+        // adapter projection tqp_expert_bwd needs.  dw = <dY, Ye> is a separate reduction when asked for.
+        st = launch_rows_proj(c, (const bf16 *)dY, D.d, c->disp_perm, topk_w, (bf16 *)dYe, (const bf16 *)c->w.B_down, nullptr,
+                              0, D.lora_scale, c->p<bf16>(c->ws.Zd), nullptr, (cudaStream_t)stream);
+        if (st != TQP_OK) return st;
+        c->zd_src = dYe;
+        if (dtopk_w) st = launch_combine_dw(c, T, (const bf16 *)dY, (const bf16 *)Ye, inv_perm, dtopk_w, (cudaStream_t)stream);
+        return st;
+    }
     return launch_combine_bwd(c, T, (const bf16 *)dY, (const bf16 *)Ye, inv_perm, topk_w, (bf16 *)dYe, dtopk_w,
                               (cudaStream_t)stream);
 }
@@ -370,25 +392,26 @@ tqp_status tqp_expert_bwd(tqp_ctx *c, int T, const void *X, const void *dYe, con
     bf16 *Zd = c->p<bf16>(c->ws.Zd), *Zg = c->p<bf16>(c->ws.Zg), *Zu = c->p<bf16>(c->ws.Zu);
 #define CK(x) do { st = (x); if (st != TQP_OK) return st; } while (0)
     // down projection: dH = dYe . Wd_eff^T,  dB_d = (s h A_d)^T dYe,  dA_d = h^T (s dYe B_d^T)
-    CK(launch_lora_down(c, dye, D.d, (const bf16 *)c->w.B_down, 0, ls, Zd, s));
+    if (c->zd_src != dYe)   // not produced by the fused tqp_combine_bwd of this step
+        CK(launch_rows_proj(c, dye, D.d, nullptr, nullptr, nullptr, (const bf16 *)c->w.B_down, nullptr, 0, ls, Zd, nullptr, s));
+    c->zd_src = nullptr;
     GemmProblem ph = c->prob_dh;
     ph.seg[0].act = dye;
     CK(act_map(c, &ph.seg[0].act_map, dye, (uint64_t)N, D.d));
     CK(act_map(c, &ph.seg[0].act_map2, dye, (uint64_t)N, D.d, kTileRows / 2));
     CK(run_gemm(c, &ph, 1, s));
     CK(launch_swiglu_bwd(c, N, dH, G, U, dG, dU, s));
-    CK(launch_lora_wgrad(c, dye, D.d, c->p<bf16>(c->ws.HAd), offsets, 0, dB_down, s));
-    CK(launch_lora_wgrad(c, H, D.F, Zd, offsets, 1, dA_down, s));
+    CK(launch_rows_wgrad(c, dye, D.d, c->p<bf16>(c->ws.HAd), nullptr, offsets, 0, dB_down, nullptr, s));
+    CK(launch_rows_wgrad(c, H, D.F, Zd, nullptr, offsets, 1, dA_down, nullptr, s));
     // gate / up projections: dXp = dG . Wg_eff^T + dU . Wu_eff^T and their adapter gradients
-    CK(launch_lora_down(c, dG, D.F, (const bf16 *)c->w.B_gate, 0, ls, Zg, s));
-    CK(launch_lora_down(c, dU, D.F, (const bf16 *)c->w.B_up, 0, ls, Zu, s));
+    CK(launch_rows_proj(c, dG, D.F, nullptr, nullptr, nullptr, (const bf16 *)c->w.B_gate, nullptr, 0, ls, Zg, nullptr, s));
+    CK(launch_rows_proj(c, dU, D.F, nullptr, nullptr, nullptr, (const bf16 *)c->w.B_up, nullptr, 0, ls, Zu, nullptr, s));
     GemmProblem px = c->prob_dx;
     px.out = (bf16 *)dXp;
     CK(run_gemm(c, &px, 1, s));
-    CK(launch_lora_wgrad(c, dG, D.F, c->p<bf16>(c->ws.XAg), offsets, 0, dB_gate, s));
-    CK(launch_lora_wgrad(c, dU, D.F, c->p<bf16>(c->ws.XAu), offsets, 0, dB_up, s));
-    CK(launch_lora_wgrad(c, Xp, D.d, Zg, offsets, 1, dA_gate, s));
-    CK(launch_lora_wgrad(c, Xp, D.d, Zu, offsets, 1, dA_up, s));
+    CK(launch_rows_wgrad(c, dG, D.F, c->p<bf16>(c->ws.XAg), nullptr, offsets, 0, dB_gate, nullptr, s));
+    CK(launch_rows_wgrad(c, dU, D.F, c->p<bf16>(c->ws.XAu), nullptr, offsets, 0, dB_up, nullptr, s));
+    CK(launch_rows_wgrad(c, Xp, D.d, Zg, Zu, offsets, 1, dA_gate, dA_up, s));   // one pass over Xp for both
 #undef CK
     return TQP_OK;
 }

@@ -79,6 +79,8 @@ struct tqp_ctx {
     int gemm_impl = 0;          // 0 tcgen05 CTA-pair kernel, 1 scaffold, 2 tcgen05 single-CTA kernel
     int fwd_T = -1;             // T of the last training-mode expert_fwd (TQP_ERR_STATE check)
     int disp_T = -1;
+    const int32_t *disp_perm = nullptr, *disp_inv_perm = nullptr;   // arrays written by the last tqp_dispatch
+    const void *zd_src = nullptr;   // dYe tensor whose projection dYe.B_d^T already sits in ws.Zd (fused tqp_combine_bwd)
     int launches = 0;
     int num_sms = 148;
     int max_tiles = 0;
@@ -131,15 +133,18 @@ tqp_status launch_combine_bwd(tqp_ctx *c, int T, const bf16 *dY, const bf16 *Ye,
 tqp_status launch_route_bwd(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const int32_t *topk_idx,
                             const float *topk_w, const float *dtopk_w, const int32_t *offsets, const int32_t *perm,
                             bf16 *dX, float *dW_r, cudaStream_t s);
+tqp_status launch_combine_dw(tqp_ctx *c, int T, const bf16 *dY, const bf16 *Ye, const int32_t *inv_perm, float *dtopk_w,
+                             cudaStream_t s);
 tqp_status launch_make_lut(tqp_ctx *c, const __half *codebook, bf16 *lut, cudaStream_t s);
 
 // ---- lora.cu -------------------------------------------------------------------------------------------
-// out[p][0..r) = s * sum_k in[p][k] * W_e[...]   (W_e [K][r] if w_kr else [r][K]); out is [N][kLoraPad] bf16
-tqp_status launch_lora_down(tqp_ctx *c, const bf16 *in, int K, const bf16 *W, int w_kr, float s, bf16 *out,
-                            cudaStream_t st);
-// grad[e] = sum_{p in e} small[p][q] * big[p][a]; stored [a][q] (out_ar=1: dA) or [q][a] (out_ar=0: dB), fp32
-tqp_status launch_lora_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 *small_, const int32_t *offsets,
-                             int out_ar, float *grad, cudaStream_t st);
+// out_w[p][0..r) = s * row(p) . W_w[e]  for w < (W1 ? 2 : 1); W_e is [K][r] if w_kr else [r][K]; out is [N][kLoraPad] bf16.
+// row(p) = in[p], or with perm: in[perm[p]/k] (* roww[perm[p]] rounded to bf16), also written to through[p][K] if given.
+tqp_status launch_rows_proj(tqp_ctx *c, const bf16 *in, int K, const int32_t *perm, const float *roww, bf16 *through,
+                            const bf16 *W0, const bf16 *W1, int w_kr, float s, bf16 *out0, bf16 *out1, cudaStream_t st);
+// grad_w[e] = sum_{p in e} small_w[p][q] * big[p][a]; stored [a][q] (out_ar=1: dA) or [q][a] (out_ar=0: dB), fp32
+tqp_status launch_rows_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 *small0, const bf16 *small1,
+                             const int32_t *offsets, int out_ar, float *grad0, float *grad1, cudaStream_t st);
 
 // ---- gemm_scaffold.cu / gemm_tcgen05.cu -----------------------------------------------------------------
 tqp_status launch_gemm_scaffold(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);

@@ -135,6 +135,31 @@ __global__ void __launch_bounds__(256) combine_bwd_kernel(const bf16 *__restrict
     }
 }
 
+// dw[a] = <dY[t], Ye[inv_perm[a]]> only (the fused combine-backward writes dYe elsewhere).  One warp per assignment.
+__global__ void __launch_bounds__(256) combine_dw_kernel(const bf16 *__restrict__ dY, const bf16 *__restrict__ Ye,
+                                                         const int32_t *__restrict__ inv_perm, float *__restrict__ dw,
+                                                         int N, int d, int k) {
+    const int a = (blockIdx.x * blockDim.x + threadIdx.x) / 32, lane = threadIdx.x % 32;
+    if (a >= N) return;
+    const int t = a / k, p = inv_perm[a];
+    const uint4 *src = reinterpret_cast<const uint4 *>(dY + (size_t)t * d);
+    const uint4 *ye = reinterpret_cast<const uint4 *>(Ye + (size_t)p * d);
+    float dot = 0.f;
+    for (int v = lane; v < d / 8; v += 32) {
+        uint4 x = src[v], y = ld_nc(ye + v);
+        const uint32_t *xp = reinterpret_cast<const uint32_t *>(&x), *yp = reinterpret_cast<const uint32_t *>(&y);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            float2 xf = bf16x2_to_float2(xp[q]), yf = bf16x2_to_float2(yp[q]);
+            dot = fmaf(xf.x, yf.x, dot);
+            dot = fmaf(xf.y, yf.y, dot);
+        }
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) dot += __shfl_xor_sync(0xffffffffu, dot, off);
+    if (lane == 0) dw[a] = dot;
+}
+
 // bf16 lookup table of the codebook (fp16 -> bf16, RNE), [256][8]
 __global__ void make_lut_kernel(const __half *__restrict__ cb, bf16 *__restrict__ lut) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -172,6 +197,13 @@ tqp_status launch_combine_bwd(tqp_ctx *c, int T, const bf16 *dY, const bf16 *Ye,
                               const float *topk_w, bf16 *dYe, float *dtopk_w, cudaStream_t s) {
     const int N = T * c->desc.k;
     combine_bwd_kernel<<<(N + 7) / 8, 256, 0, s>>>(dY, Ye, inv_perm, topk_w, dYe, dtopk_w, N, c->desc.d, c->desc.k);
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
+tqp_status launch_combine_dw(tqp_ctx *c, int T, const bf16 *dY, const bf16 *Ye, const int32_t *inv_perm, float *dtopk_w,
+                             cudaStream_t s) {
+    const int N = T * c->desc.k;
+    combine_dw_kernel<<<(N + 7) / 8, 256, 0, s>>>(dY, Ye, inv_perm, dtopk_w, N, c->desc.d, c->desc.k);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }

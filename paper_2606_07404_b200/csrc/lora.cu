@@ -1,73 +1,249 @@
 // Adapter side products of the TQP layer (rank-r adapter on each weight pack, only the adapters train).
-//   lora_down : P[p][0..r) = s * in[p][:] . W_e          (x.A, h.A_d forward;  dy.B^T backward)   -> [N][64] bf16
-//   lora_wgrad: grad[e]    = sum_{p in e} small[p]^T big[p]  (dA = x^T z, dB = (xA)^T dy), fp32, deterministic
-// Both are tall-skinny grouped contractions whose cost is reading the [N][K] operand once from HBM; they use
-// warp-level bf16 MMA (wmma) with fp32 accumulation, operands staged through shared memory with row masking
-// so rows of a neighbouring expert (or beyond N) never enter a sum.
-#include <mma.h>
-
+//   rows_proj : P_w[p][0..r) = s * row(p) . W_w[e]      (x.A_g | x.A_u, h.A_d forward;  dy.B^T backward)  -> [N][64] bf16
+//               row(p) is either in[p] or a GATHERED (and optionally gate-weighted) row in[perm[p]/k] * w[perm[p]],
+//               which the kernel also writes through to the dense permuted tensor (Xp = gather(X), dYe = w . gather(dY)):
+//               the token permutation, the combine backward (a7) and the adapter projections that
+//               follow them read their rows from HBM once instead of two or three times.
+//   rows_wgrad: grad_w[e] = sum_{p in e} small_w[p]^T big[p]   (dA = x^T z, dB = (xA)^T dy), fp32, deterministic
+// Both are tall-skinny grouped contractions whose cost is streaming the [N][K] operand once: bound = HBM.  Rows stream
+// through a cp.async ring; the contraction itself is warp-level bf16 MMA (ldmatrix + mma.sync m16n8k16, fp32
+// accumulate) -- the legacy HMMA path is enough here because the kernels need < 10 % of its rate at HBM speed.
 #include "common.cuh"
+#include "tc_ptx.cuh"
 
 namespace tqp {
-using namespace nvcuda;
 
-constexpr int LD_KC = 128;            // K-chunk staged per iteration in lora_down
-constexpr int LD_LDS = LD_KC + 8;     // padded smem row (bf16)
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src, int src_bytes) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
 
-// grid = (max_tiles, kTileRows/64), block = 128 (4 warps, 16 rows each)
-template <int R>
-__global__ void __launch_bounds__(128) lora_down_kernel(const bf16 *__restrict__ in, int K, const bf16 *__restrict__ W,
-                                                        int w_kr, float s, bf16 *__restrict__ out,
-                                                        const Tile *__restrict__ tiles, const int32_t *__restrict__ num_tiles) {
-    __shared__ __align__(32) bf16 a_s[4][16][LD_LDS];
-    __shared__ __align__(32) float o_s[4][16][R + 4];
+// four 8x8 b16 matrices; lane l supplies the row address of matrix l/8, row l%8 (shared-space address)
+__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t (&r)[4]) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void ldsm_x4_t(uint32_t addr, uint32_t (&r)[4]) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+// D[16x8] += A[16x16] B[16x8]; bf16 operands, fp32 accumulate
+__device__ __forceinline__ void mma16816(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
+// ---- projections ------------------------------------------------------------------------------------------------
+// Rows go global -> registers (LDG.128, two K-chunks ahead) -> shared (+ straight from the registers to the dense
+// permuted tensor in the gathered variants).  cp.async was tried first for the rows: its 16-byte requests cost two
+// 32-byte L2 sectors each (ncu: lts read sectors = 1.9 x the bytes asked for) and made the kernel L2-throughput-bound;
+// 256-byte cp.async.bulk row copies were slower still.  Warp-wide LDG.128 moves exactly the sectors it needs.  The
+// small adapter chunks (shared by the 128 rows of the CTA) keep the cp.async ring: they cost no registers.
+constexpr int PJ_ROWS = 128;         // rows per CTA (8 warps x 16)
+constexpr int PJ_THREADS = 256;
+constexpr int PJ_KC = 64;            // K-chunk per step (128 contiguous bytes of every row)
+constexpr int PJ_LD = PJ_KC + 8;     // padded smem row (bf16): conflict-free ldmatrix
+constexpr int PJ_CH = PJ_ROWS * PJ_KC / 8 / PJ_THREADS;   // 16-byte row chunks per thread per step
+constexpr int PJ_D = 3;              // register sets: chunk kc+2 is in flight while chunk kc is multiplied
+constexpr int PJ_WST = 3;            // adapter-chunk ring
+
+struct ProjArgs {
+    const bf16 *in;        // source rows [*][K]
+    const int32_t *perm;   // != nullptr: row(p) = in[perm[p] / k]   (else in[p])
+    const float *roww;     // != nullptr (needs perm): row(p) *= roww[perm[p]], rounded to bf16
+    bf16 *through;         // != nullptr: row(p) is also written to through[p][K]
+    const bf16 *W[2];      // adapter matrices of all experts
+    bf16 *out[2];          // [N][kLoraPad]
+    int K, k;
+    float s;
+    int ablate;            // timing experiments only (tqp_set_option "ablate"): 256 no write-through, 512 no MMA, 1024 no row loads
+};
+
+template <int R, int NW, bool KR>
+struct ProjCfg {
+    static constexpr int RT = R * NW;
+    static constexpr int WLD = KR ? RT + 8 : PJ_LD;                  // KR: Ws[KC][RT+8]   else: Ws[RT][KC+8]
+    static constexpr int ROWS_BYTES = PJ_ROWS * PJ_LD * 2;
+    static constexpr int W_CHUNKS = KR ? PJ_KC * RT / 8 : RT * PJ_KC / 8;   // 16-byte pieces of the adapter chunk
+    static constexpr int W_BYTES = ((KR ? PJ_KC * WLD : RT * WLD) * 2 + 127) / 128 * 128;
+    static constexpr int OFF_W = 2 * ROWS_BYTES;
+    static constexpr int SMEM = OFF_W + PJ_WST * W_BYTES;
+};
+
+// L2 eviction priorities: gathered source rows (X, dY: 42 MB, each row reused k times) should stay resident while
+// the 0.5 GB of read-once / write-once permuted rows stream through.
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint4 ldg128_hint(const void *p, uint64_t pol) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ void stg128_hint(void *p, const uint4 &v, uint64_t pol) {
+    asm volatile("st.global.L2::cache_hint.v4.u32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(pol)
+                 : "memory");
+}
+
+// grid = (max_tiles, kTileRows / 128), block = 256.  KR: W_e is [K][R] (x.A), else [R][K] (dy.B^T).
+template <int R, int NW, bool KR>
+__global__ void __launch_bounds__(PJ_THREADS, 2) rows_proj_kernel(const __grid_constant__ ProjArgs a, const Tile *__restrict__ tiles,
+                                                                  const int32_t *__restrict__ num_tiles) {
+    using C = ProjCfg<R, NW, KR>;
+    extern __shared__ __align__(128) uint8_t pj_smem[];   // used directly: a pointer rebuilt from an integer would
+                                                          // lose its address space (generic LD.E instead of LDS/ldmatrix)
     if ((int)blockIdx.x >= *num_tiles) return;
     const Tile t = tiles[blockIdx.x];
-    const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
-    const int g = blockIdx.y * 4 + warp;
-    if (g * 16 >= t.rows) return;
-    const int row0 = t.row0 + g * 16, valid = min(16, t.rows - g * 16);
-    const bf16 *We = W + (size_t)t.expert * K * R;
-    wmma::fragment<wmma::accumulator, 16, 16, 16, float> acc[R / 16];
-#pragma unroll
-    for (int n = 0; n < R / 16; ++n) wmma::fill_fragment(acc[n], 0.f);
+    const int rbase = blockIdx.y * PJ_ROWS;
+    const int valid = min(PJ_ROWS, t.rows - rbase);
+    if (valid <= 0) return;
+    const int row0 = t.row0 + rbase;
+    const int tid = threadIdx.x, warp = tid / 32, lane = tid % 32;
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(pj_smem);
+    const int K = a.K;
 
-    for (int k0 = 0; k0 < K; k0 += LD_KC) {
-        // stage 16 rows x 128 k, zero rows >= valid.  2 rows per instruction (16 lanes x 16 B each).
+    // this thread's row chunks: rows rr + RSTEP i (i < PJ_CH), 16-byte chunk rc of every K-chunk
+    constexpr int TPR = PJ_KC / 8, RSTEP = PJ_THREADS / TPR;
+    const int rr = tid / TPR, rc = tid % TPR;
+    const bf16 *src[PJ_CH];
+    float roww[PJ_CH];
 #pragma unroll
-        for (int it = 0; it < 8; ++it) {
-            int r = it * 2 + lane / 16, cv = lane % 16;
-            uint4 v = make_uint4(0, 0, 0, 0);
-            if (r < valid) v = *reinterpret_cast<const uint4 *>(in + (size_t)(row0 + r) * K + k0 + cv * 8);
-            *reinterpret_cast<uint4 *>(&a_s[warp][r][cv * 8]) = v;
+    for (int i = 0; i < PJ_CH; ++i) {
+        const int r = rr + RSTEP * i;
+        src[i] = nullptr;   // rows past `valid` are not loaded (zeros; their outputs are never stored)
+        roww[i] = 1.f;
+        if (r < valid && !(a.ablate & 1024)) {
+            int srow = row0 + r;
+            if (a.perm) {
+                const int as = a.perm[srow];
+                srow = as / a.k;
+                if (a.roww) roww[i] = a.roww[as];
+            }
+            src[i] = a.in + (size_t)srow * K + rc * 8;
         }
-        __syncwarp();
+    }
+    auto issue_w = [&](int kc) {   // adapter chunk kc -> ring slot kc % PJ_WST
+        const uint32_t w_s = sbase + C::OFF_W + (kc % PJ_WST) * C::W_BYTES;
+        for (int v = tid; v < C::W_CHUNKS; v += PJ_THREADS) {
+            if (KR) {   // W_w[e][k][R]: piece = (k, w, 8 columns)
+                const int kk = v / (C::RT / 8), cc = v % (C::RT / 8), w = (cc * 8) / R, q0 = (cc * 8) % R;
+                cp_async16(w_s + (kk * C::WLD + cc * 8) * 2, a.W[w] + ((size_t)t.expert * K + kc * PJ_KC + kk) * R + q0, 16);
+            } else {    // W_w[e][q][K]: piece = (w, q, 8 k)
+                const int n = v / (PJ_KC / 8), cc = v % (PJ_KC / 8), w = n / R, q = n % R;
+                cp_async16(w_s + (n * C::WLD + cc * 8) * 2, a.W[w] + ((size_t)t.expert * R + q) * K + kc * PJ_KC + cc * 8, 16);
+            }
+        }
+    };
+
+    const uint64_t pol_ld = a.perm ? l2_policy_evict_last() : l2_policy_evict_first(), pol_st = l2_policy_evict_first();
+    uint4 pre[PJ_D][PJ_CH];
+    auto fetch = [&](int kc, uint4 (&rows)[PJ_CH]) {
 #pragma unroll
-        for (int kk = 0; kk < LD_KC; kk += 16) {
-            wmma::fragment<wmma::matrix_a, 16, 16, 16, bf16, wmma::row_major> af;
-            wmma::load_matrix_sync(af, &a_s[warp][0][kk], LD_LDS);
+        for (int i = 0; i < PJ_CH; ++i) rows[i] = src[i] ? ldg128_hint(src[i] + (size_t)kc * PJ_KC, pol_ld) : make_uint4(0, 0, 0, 0);
+    };
+
+    float acc[C::RT / 8][4];
 #pragma unroll
-            for (int n = 0; n < R / 16; ++n) {
-                if (w_kr) {   // W_e[K][R]
-                    wmma::fragment<wmma::matrix_b, 16, 16, 16, bf16, wmma::row_major> bfm;
-                    wmma::load_matrix_sync(bfm, We + (size_t)(k0 + kk) * R + n * 16, R);
-                    wmma::mma_sync(acc[n], af, bfm, acc[n]);
-                } else {      // W_e[R][K]  (B^T use)
-                    wmma::fragment<wmma::matrix_b, 16, 16, 16, bf16, wmma::col_major> bfm;
-                    wmma::load_matrix_sync(bfm, We + (size_t)(n * 16) * K + k0 + kk, K);
-                    wmma::mma_sync(acc[n], af, bfm, acc[n]);
+    for (int n = 0; n < C::RT / 8; ++n)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) acc[n][q] = 0.f;
+
+    const int nk = K / PJ_KC;
+    const bool rewrite = a.roww != nullptr, thru = a.through != nullptr && !(a.ablate & 256);
+#pragma unroll
+    for (int s = 0; s < PJ_D - 1; ++s) {
+        if (s < nk) { fetch(s, pre[s]); issue_w(s); }
+        cp_async_commit();
+    }
+
+    auto step = [&](int kc, uint4 (&rows)[PJ_CH], uint4 (&rows_nx)[PJ_CH]) {
+        if (kc + PJ_D - 1 < nk) fetch(kc + PJ_D - 1, rows_nx);
+        const uint32_t rows_s = sbase + (kc & 1) * C::ROWS_BYTES;
+#pragma unroll
+        for (int i = 0; i < PJ_CH; ++i) {
+            const int r = rr + RSTEP * i;
+            uint4 v = rows[i];
+            if (rewrite) {   // gate weight, rounded to bf16 (the value the dH GEMM reads back from dYe)
+                uint32_t *vp = reinterpret_cast<uint32_t *>(&v);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    float2 f = bf16x2_to_float2(vp[q]);
+                    vp[q] = float2_to_bf16x2(roww[i] * f.x, roww[i] * f.y);
+                }
+            }
+            ptx::sts128(rows_s + (r * PJ_LD + rc * 8) * 2, v);
+            if (thru && r < valid) stg128_hint(a.through + (size_t)(row0 + r) * K + kc * PJ_KC + rc * 8, v, pol_st);
+        }
+        cp_async_wait<PJ_WST - 2>();   // adapter chunk kc has landed (chunk kc + 1 may still be in flight)
+        __syncthreads();               // rows + adapter chunk kc visible; everyone is past the MMAs of step kc - 1
+        if (kc + PJ_WST - 1 < nk) issue_w(kc + PJ_WST - 1);
+        cp_async_commit();
+        if (warp * 16 < valid && !(a.ablate & 512)) {
+            const uint32_t w_s = sbase + C::OFF_W + (kc % PJ_WST) * C::W_BYTES;
+            const uint32_t a_addr = rows_s + ((warp * 16 + lane % 16) * PJ_LD + (lane / 16) * 8) * 2;
+            const uint32_t b_addr = KR ? w_s + ((lane % 8 + ((lane / 8) % 2) * 8) * C::WLD + (lane / 16) * 8) * 2
+                                       : w_s + (((lane / 16) * 8 + lane % 8) * C::WLD + ((lane / 8) % 2) * 8) * 2;
+#pragma unroll
+            for (int kk = 0; kk < PJ_KC; kk += 16) {
+                uint32_t af[4];
+                ldsm_x4(a_addr + kk * 2, af);
+#pragma unroll
+                for (int np = 0; np < C::RT / 16; ++np) {
+                    uint32_t bq[4];
+                    if (KR) ldsm_x4_t(b_addr + (kk * C::WLD + np * 16) * 2, bq);
+                    else ldsm_x4(b_addr + (np * 16 * C::WLD + kk) * 2, bq);
+                    mma16816(acc[2 * np], af, bq[0], bq[1]);
+                    mma16816(acc[2 * np + 1], af, bq[2], bq[3]);
                 }
             }
         }
-        __syncwarp();
+    };
+    for (int kc = 0; kc < nk; kc += PJ_D) {   // register sets rotate with compile-time indices
+        step(kc, pre[0], pre[2]);
+        if (kc + 1 < nk) step(kc + 1, pre[1], pre[0]);
+        if (kc + 2 < nk) step(kc + 2, pre[2], pre[1]);
     }
+    cp_async_wait<0>();
+    if (warp * 16 < valid) {   // accumulator layout: rows lane/4 (+8), columns 8 n + 2 (lane%4) + {0,1}
 #pragma unroll
-    for (int n = 0; n < R / 16; ++n) wmma::store_matrix_sync(&o_s[warp][0][n * 16], acc[n], R + 4, wmma::mem_row_major);
-    __syncwarp();
-    for (int v = lane; v < 16 * R; v += 32) {
-        int r = v / R, q = v % R;
-        if (r < valid) out[(size_t)(row0 + r) * kLoraPad + q] = __float2bfloat16_rn(s * o_s[warp][r][q]);
+        for (int n = 0; n < C::RT / 8; ++n) {
+            const int col = n * 8 + (lane % 4) * 2, w = col / R, q = col % R;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int r = warp * 16 + lane / 4 + 8 * h;
+                if (r < valid)
+                    *reinterpret_cast<uint32_t *>(a.out[w] + (size_t)(row0 + r) * kLoraPad + q) =
+                        float2_to_bf16x2(a.s * acc[n][2 * h], a.s * acc[n][2 * h + 1]);
+            }
+        }
     }
+}
+
+template <int R, int NW, bool KR>
+static tqp_status launch_proj_t(tqp_ctx *c, const ProjArgs &a, cudaStream_t st) {
+    using C = ProjCfg<R, NW, KR>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        TQP_CUDA_OK(c, cudaFuncSetAttribute(rows_proj_kernel<R, NW, KR>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+        attr_set = true;
+    }
+    dim3 grid(c->max_tiles, kTileRows / PJ_ROWS);
+    rows_proj_kernel<R, NW, KR><<<grid, PJ_THREADS, C::SMEM, st>>>(a, c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles));
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
 }
 
 // r = 8 (config 0): plain CUDA-core version, one warp per row.
@@ -93,71 +269,146 @@ __global__ void __launch_bounds__(128) lora_down_small_kernel(const bf16 *__rest
     }
 }
 
-tqp_status launch_lora_down(tqp_ctx *c, const bf16 *in, int K, const bf16 *W, int w_kr, float s, bf16 *out, cudaStream_t st) {
-    const Tile *tiles = c->p<Tile>(c->ws.tiles);
-    const int32_t *nt = c->p<int32_t>(c->ws.num_tiles);
-    dim3 grid(c->max_tiles, kTileRows / 64);
-    const int r = c->desc.r;
-    if (r == 16) lora_down_kernel<16><<<grid, 128, 0, st>>>(in, K, W, w_kr, s, out, tiles, nt);
-    else if (r == 32) lora_down_kernel<32><<<grid, 128, 0, st>>>(in, K, W, w_kr, s, out, tiles, nt);
-    else lora_down_small_kernel<<<grid, 128, 0, st>>>(in, K, r, W, w_kr, s, out, tiles, nt);
-    TQP_LAUNCH_OK(c);
-    return TQP_OK;
+// nw projections of the same rows in one pass.  perm/roww/through select the gathered (fused dispatch / combine-bwd)
+// variants; rank 8 (config 0) runs on CUDA cores from an already dense `in`.
+tqp_status launch_rows_proj(tqp_ctx *c, const bf16 *in, int K, const int32_t *perm, const float *roww, bf16 *through,
+                            const bf16 *W0, const bf16 *W1, int w_kr, float s, bf16 *out0, bf16 *out1, cudaStream_t st) {
+    const int r = c->desc.r, nw = W1 ? 2 : 1;
+    if (r != 16 && r != 32) {
+        if (perm || roww || through) { c->err = "rows_proj: gathered variants need r = 16 or 32"; return TQP_ERR_ARG; }
+        const Tile *tiles = c->p<Tile>(c->ws.tiles);
+        const int32_t *nt = c->p<int32_t>(c->ws.num_tiles);
+        dim3 grid(c->max_tiles, kTileRows / 64);
+        lora_down_small_kernel<<<grid, 128, 0, st>>>(in, K, r, W0, w_kr, s, out0, tiles, nt);
+        TQP_LAUNCH_OK(c);
+        if (W1) {
+            lora_down_small_kernel<<<grid, 128, 0, st>>>(in, K, r, W1, w_kr, s, out1, tiles, nt);
+            TQP_LAUNCH_OK(c);
+        }
+        return TQP_OK;
+    }
+    ProjArgs a;
+    a.in = in; a.perm = perm; a.roww = roww; a.through = through; a.W[0] = W0; a.W[1] = W1; a.out[0] = out0; a.out[1] = out1;
+    a.K = K; a.k = c->desc.k; a.s = s; a.ablate = c->ablate;
+#define TQP_PJ(R_, NW_, KR_) if (r == R_ && nw == NW_ && (w_kr != 0) == KR_) return launch_proj_t<R_, NW_, KR_>(c, a, st)
+    TQP_PJ(16, 1, true); TQP_PJ(16, 2, true); TQP_PJ(16, 1, false); TQP_PJ(16, 2, false);
+    TQP_PJ(32, 1, true); TQP_PJ(32, 2, true); TQP_PJ(32, 1, false); TQP_PJ(32, 2, false);
+#undef TQP_PJ
+    return TQP_ERR_ARG;
 }
 
-// ---- weight gradients -----------------------------------------------------------------------------------------
-constexpr int WG_P = 32;   // rows per iteration
-constexpr int WG_A = 64;   // columns of `big` per block
+// ---- weight gradients -------------------------------------------------------------------------------------------
+constexpr int WG_ROWS = 32;             // rows per stage
+constexpr int WG_COLS = 128;            // columns of `big` per CTA (4 warps x 32)
+constexpr int WG_LD = WG_COLS + 8;
+constexpr int WG_NST = 4;
 
-// grid = (E, width/64), block = 128.  acc tile per warp: [R x 16 a-columns].
-template <int R>
-__global__ void __launch_bounds__(128) lora_wgrad_kernel(const bf16 *__restrict__ big, int width, const bf16 *__restrict__ small_,
-                                                         const int32_t *__restrict__ offsets, int out_ar, float *__restrict__ grad) {
-    __shared__ __align__(32) bf16 big_s[WG_P][WG_A + 8];
-    __shared__ __align__(32) bf16 sm_s[WG_P][R + 8];
-    const int e = blockIdx.x, a0 = blockIdx.y * WG_A;
-    const int warp = threadIdx.x / 32, tid = threadIdx.x;
+struct WgradArgs {
+    const bf16 *big;         // [N][width]
+    const bf16 *small_[2];   // [N][kLoraPad]
+    float *grad[2];          // out_ar: [E][width][R] (dA) else [E][R][width] (dB)
+    int width, out_ar;
+};
+
+template <int R, int NS>
+struct WgradCfg {
+    static constexpr int RT = R * NS;
+    static constexpr int SLD = RT + 8;
+    static constexpr int BIG_BYTES = WG_ROWS * WG_LD * 2;
+    static constexpr int SM_BYTES = (WG_ROWS * SLD * 2 + 127) / 128 * 128;
+    static constexpr int STAGE = BIG_BYTES + SM_BYTES;
+    static constexpr int SMEM = WG_NST * STAGE + 128;
+};
+
+// grid = (E, width / 128), block = 128.  Warp w owns columns [32 w, 32 w + 32) of the slab and all RT adapter columns.
+template <int R, int NS>
+__global__ void __launch_bounds__(128) rows_wgrad_kernel(const __grid_constant__ WgradArgs a, const int32_t *__restrict__ offsets) {
+    using C = WgradCfg<R, NS>;
+    extern __shared__ __align__(128) uint8_t wg_smem[];
+    uint8_t *smem = wg_smem;
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem);
+    const int e = blockIdx.x, a0 = blockIdx.y * WG_COLS;
+    const int tid = threadIdx.x, warp = tid / 32;
     const int p0 = offsets[e], p1 = offsets[e + 1];
-    wmma::fragment<wmma::accumulator, 16, 16, 16, float> acc[R / 16];
+    const int width = a.width;
+    const int nit = (p1 - p0 + WG_ROWS - 1) / WG_ROWS;
+
+    auto issue = [&](int it, int st) {
+        const int p = p0 + it * WG_ROWS;
+        const uint32_t big_s = sbase + st * C::STAGE, sm_s = big_s + C::BIG_BYTES;
+        // rows at or past p1 belong to the next expert: zero-filled (src-size 0), address clamped to a valid row
 #pragma unroll
-    for (int n = 0; n < R / 16; ++n) wmma::fill_fragment(acc[n], 0.f);
-    for (int p = p0; p < p1; p += WG_P) {
-        // big tile: 32 rows x 64 cols = 256 uint4, 2 per thread
+        for (int i = 0; i < 4; ++i) {
+            const int r = tid / 16 + 8 * i, cc = tid % 16;
+            const bool ok = p + r < p1;
+            cp_async16(big_s + (r * WG_LD + cc * 8) * 2, a.big + (size_t)(ok ? p + r : p1 - 1) * width + a0 + cc * 8, ok ? 16 : 0);
+        }
+        for (int v = tid; v < WG_ROWS * C::RT / 8; v += 128) {
+            const int r = v / (C::RT / 8), cc = v % (C::RT / 8), w = (cc * 8) / R, q0 = (cc * 8) % R;
+            const bool ok = p + r < p1;
+            cp_async16(sm_s + (r * C::SLD + cc * 8) * 2, a.small_[w] + (size_t)(ok ? p + r : p1 - 1) * kLoraPad + q0, ok ? 16 : 0);
+        }
+    };
+
+    float acc[C::RT / 16][4][4];   // [16 adapter columns][8 big columns][fragment]
 #pragma unroll
-        for (int it = 0; it < 2; ++it) {
-            int v = tid + it * 128, r = v / 8, cv = v % 8;
-            uint4 x = make_uint4(0, 0, 0, 0);
-            if (p + r < p1) x = *reinterpret_cast<const uint4 *>(big + (size_t)(p + r) * width + a0 + cv * 8);
-            *reinterpret_cast<uint4 *>(&big_s[r][cv * 8]) = x;
-        }
-        // small tile: 32 rows x R cols
-        for (int v = tid; v < WG_P * R / 8; v += 128) {
-            int r = v / (R / 8), cv = v % (R / 8);
-            uint4 x = make_uint4(0, 0, 0, 0);
-            if (p + r < p1) x = *reinterpret_cast<const uint4 *>(small_ + (size_t)(p + r) * kLoraPad + cv * 8);
-            *reinterpret_cast<uint4 *>(&sm_s[r][cv * 8]) = x;
-        }
+    for (int m = 0; m < C::RT / 16; ++m)
+#pragma unroll
+        for (int n = 0; n < 4; ++n)
+#pragma unroll
+            for (int q = 0; q < 4; ++q) acc[m][n][q] = 0.f;
+    const int lane = tid % 32;
+    for (int s = 0; s < WG_NST - 1; ++s) {
+        if (s < nit) issue(s, s);
+        cp_async_commit();
+    }
+    // A = small^T (stored [p][q]) and B = big (stored [p][a]) are both read with ldmatrix.trans
+    const uint32_t a_off = (((lane / 16) * 8 + lane % 8) * C::SLD + ((lane / 8) % 2) * 8) * 2;
+    const uint32_t b_off = ((((lane / 8) % 2) * 8 + lane % 8) * WG_LD + warp * 32 + (lane / 16) * 8) * 2;
+    for (int it = 0; it < nit; ++it) {
+        const int st = it % WG_NST;
+        cp_async_wait<WG_NST - 2>();
         __syncthreads();
+        if (it + WG_NST - 1 < nit) issue(it + WG_NST - 1, (it + WG_NST - 1) % WG_NST);
+        cp_async_commit();
+        const uint32_t big_s = sbase + st * C::STAGE, sm_s = big_s + C::BIG_BYTES;
 #pragma unroll
-        for (int pp = 0; pp < WG_P; pp += 16) {
-            wmma::fragment<wmma::matrix_b, 16, 16, 16, bf16, wmma::row_major> bfm;   // big[p][a]
-            wmma::load_matrix_sync(bfm, &big_s[pp][warp * 16], WG_A + 8);
+        for (int pp = 0; pp < WG_ROWS; pp += 16) {
+            uint32_t af[C::RT / 16][4];
 #pragma unroll
-            for (int n = 0; n < R / 16; ++n) {
-                wmma::fragment<wmma::matrix_a, 16, 16, 16, bf16, wmma::col_major> af;  // small^T[q][p]
-                wmma::load_matrix_sync(af, &sm_s[pp][n * 16], R + 8);
-                wmma::mma_sync(acc[n], af, bfm, acc[n]);
+            for (int m = 0; m < C::RT / 16; ++m) ldsm_x4_t(sm_s + a_off + (pp * C::SLD + m * 16) * 2, af[m]);
+#pragma unroll
+            for (int np = 0; np < 2; ++np) {
+                uint32_t bq[4];
+                ldsm_x4_t(big_s + b_off + (pp * WG_LD + np * 16) * 2, bq);
+#pragma unroll
+                for (int m = 0; m < C::RT / 16; ++m) {
+                    mma16816(acc[m][2 * np], af[m], bq[0], bq[1]);
+                    mma16816(acc[m][2 * np + 1], af[m], bq[2], bq[3]);
+                }
             }
         }
-        __syncthreads();
     }
-    const int a = a0 + warp * 16;
+    cp_async_wait<0>();
 #pragma unroll
-    for (int n = 0; n < R / 16; ++n) {
-        if (out_ar)   // grad[e][a][q], ld = R: element (q, a) at a*R + q
-            wmma::store_matrix_sync(grad + ((size_t)e * width + a) * R + n * 16, acc[n], R, wmma::mem_col_major);
-        else          // grad[e][q][a], ld = width
-            wmma::store_matrix_sync(grad + ((size_t)e * R + n * 16) * width + a, acc[n], width, wmma::mem_row_major);
+    for (int m = 0; m < C::RT / 16; ++m) {
+        const int w = (m * 16) / R;
+#pragma unroll
+        for (int n = 0; n < 4; ++n) {
+            const int col = a0 + warp * 32 + n * 8 + (lane % 4) * 2;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int q = (m * 16) % R + lane / 4 + 8 * h;
+                if (a.out_ar) {   // grad[e][col][q]
+                    float *g = a.grad[w] + ((size_t)e * width + col) * R + q;
+                    g[0] = acc[m][n][2 * h];
+                    g[R] = acc[m][n][2 * h + 1];
+                } else {          // grad[e][q][col]
+                    *reinterpret_cast<float2 *>(a.grad[w] + ((size_t)e * R + q) * width + col) =
+                        make_float2(acc[m][n][2 * h], acc[m][n][2 * h + 1]);
+                }
+            }
+        }
     }
 }
 
@@ -177,14 +428,40 @@ __global__ void __launch_bounds__(256) lora_wgrad_small_kernel(const bf16 *__res
     }
 }
 
-tqp_status launch_lora_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 *small_, const int32_t *offsets,
-                             int out_ar, float *grad, cudaStream_t st) {
-    const int r = c->desc.r, E = c->desc.E;
-    if (r == 16) lora_wgrad_kernel<16><<<dim3(E, width / WG_A), 128, 0, st>>>(big, width, small_, offsets, out_ar, grad);
-    else if (r == 32) lora_wgrad_kernel<32><<<dim3(E, width / WG_A), 128, 0, st>>>(big, width, small_, offsets, out_ar, grad);
-    else lora_wgrad_small_kernel<<<dim3(E, 8), 256, 0, st>>>(big, width, r, small_, offsets, out_ar, grad);
+template <int R, int NS>
+static tqp_status launch_wgrad_t(tqp_ctx *c, const WgradArgs &a, const int32_t *offsets, cudaStream_t st) {
+    using C = WgradCfg<R, NS>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        TQP_CUDA_OK(c, cudaFuncSetAttribute(rows_wgrad_kernel<R, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+        attr_set = true;
+    }
+    rows_wgrad_kernel<R, NS><<<dim3(c->desc.E, a.width / WG_COLS), 128, C::SMEM, st>>>(a, offsets);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
+}
+
+// ns weight gradients that share the streamed operand `big` (e.g. dA_gate and dA_up both contract Xp) in one pass.
+tqp_status launch_rows_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 *small0, const bf16 *small1,
+                             const int32_t *offsets, int out_ar, float *grad0, float *grad1, cudaStream_t st) {
+    const int r = c->desc.r, E = c->desc.E;
+    if (r != 16 && r != 32) {
+        lora_wgrad_small_kernel<<<dim3(E, 8), 256, 0, st>>>(big, width, r, small0, offsets, out_ar, grad0);
+        TQP_LAUNCH_OK(c);
+        if (small1) {
+            lora_wgrad_small_kernel<<<dim3(E, 8), 256, 0, st>>>(big, width, r, small1, offsets, out_ar, grad1);
+            TQP_LAUNCH_OK(c);
+        }
+        return TQP_OK;
+    }
+    WgradArgs a;
+    a.big = big; a.small_[0] = small0; a.small_[1] = small1; a.grad[0] = grad0; a.grad[1] = grad1;
+    a.width = width; a.out_ar = out_ar;
+    const int ns = small1 ? 2 : 1;
+    if (r == 16 && ns == 1) return launch_wgrad_t<16, 1>(c, a, offsets, st);
+    if (r == 16 && ns == 2) return launch_wgrad_t<16, 2>(c, a, offsets, st);
+    if (r == 32 && ns == 1) return launch_wgrad_t<32, 1>(c, a, offsets, st);
+    return launch_wgrad_t<32, 2>(c, a, offsets, st);
 }
 
 }  // namespace tqp

@@ -6,66 +6,107 @@
 namespace tqp {
 
 // logits[t][e] = fmaf-chain over i ascending (bit-exact against the oracle: one accumulator per (t,e),
-// no split-K).  Register-tiled fp32 "SGEMM" on the FMA pipes: block = 128 tokens x 64 experts, 256 threads,
-// each thread 8 tokens x 4 experts.  X is bf16 (widened exactly), W_r fp32.
-constexpr int RT_TOK = 128, RT_EXP = 64, RT_K = 32;
+// no split-K).  Register-tiled fp32 "SGEMM" on the FMA pipes: block = 64 tokens x 96 experts, 128 threads,
+// each thread 8 tokens x 6 experts (48 FMAs per 5 shared-memory loads), K-chunks of 32 double-buffered in shared
+// memory (W_r by cp.async, X through registers: bf16 widened exactly and stored transposed).  Bound: fp32 FMA
+// issue rate (R1 forbids tensor cores and any re-association of the sum).
+constexpr int RT_TOK = 64, RT_EXP = 96, RT_K = 32, RT_XLD = RT_TOK + 4;
 
-__global__ void __launch_bounds__(256) route_logits_kernel(const bf16 *__restrict__ X, const float *__restrict__ W_r,
+__global__ void __launch_bounds__(128) route_logits_kernel(const bf16 *__restrict__ X, const float *__restrict__ W_r,
                                                            const float *__restrict__ bias, float *__restrict__ logits,
                                                            int T, int d, int E) {
-    __shared__ float xs[RT_K][RT_TOK + 4];   // [i][token]
-    __shared__ float wsm[RT_K][RT_EXP];      // [i][expert]
+    __shared__ __align__(16) float xs[2][RT_K][RT_XLD];   // [buf][i][token]
+    __shared__ __align__(16) float wsm[2][RT_K][RT_EXP];  // [buf][i][expert]
     const int tid = threadIdx.x;
     const int t0 = blockIdx.x * RT_TOK, e0 = blockIdx.y * RT_EXP;
-    const int tx = tid % 16, ty = tid / 16;  // tx -> experts (4 each), ty -> tokens (8 each)
-    float acc[8][4];
+    const int tx = tid % 16, ty = tid / 16;   // tx -> experts (6 each), ty -> tokens (8 each)
+    const bool w_vec = (E % 4) == 0;          // 16-byte cp.async needs aligned rows and whole chunks
+    float acc[8][6];
 #pragma unroll
     for (int a = 0; a < 8; ++a)
 #pragma unroll
-        for (int b = 0; b < 4; ++b) acc[a][b] = 0.f;
+        for (int b = 0; b < 6; ++b) acc[a][b] = 0.f;
 
-    for (int i0 = 0; i0 < d; i0 += RT_K) {
-        // X tile: 128 tokens x 32 i (bf16).  Each thread loads 16 contiguous bytes (8 values) x 2.
-        for (int v = tid; v < RT_TOK * RT_K / 8; v += 256) {
-            int tok = v / (RT_K / 8), seg = v % (RT_K / 8);
-            uint4 raw = make_uint4(0, 0, 0, 0);
-            if (t0 + tok < T) raw = *reinterpret_cast<const uint4 *>(X + (size_t)(t0 + tok) * d + i0 + seg * 8);
-            const uint32_t *r = reinterpret_cast<const uint32_t *>(&raw);
+    // X tile: 64 tokens x 32 i (bf16) = 256 chunks of 8 values; thread owns chunks (token = tid % 64, seg = tid / 64 + 2 j)
+    const int xtok = tid % RT_TOK, xseg = tid / RT_TOK;
+    const bool x_ok = t0 + xtok < T;
+    const bf16 *xsrc = X + (size_t)(x_ok ? t0 + xtok : 0) * d + xseg * 8;
+    uint4 xr[2];
+    auto load_x = [&](int i0) {
+#pragma unroll
+        for (int j = 0; j < 2; ++j)
+            xr[j] = x_ok ? *reinterpret_cast<const uint4 *>(xsrc + i0 + j * 16) : make_uint4(0, 0, 0, 0);
+    };
+    auto store_x = [&](int buf) {
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const uint32_t *r = reinterpret_cast<const uint32_t *>(&xr[j]);
+            const int ib = (xseg + 2 * j) * 8;
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 float2 f = bf16x2_to_float2(r[q]);
-                xs[seg * 8 + 2 * q][tok] = f.x;
-                xs[seg * 8 + 2 * q + 1][tok] = f.y;
+                xs[buf][ib + 2 * q][xtok] = f.x;
+                xs[buf][ib + 2 * q + 1][xtok] = f.y;
             }
         }
-        for (int v = tid; v < RT_K * RT_EXP; v += 256) {
-            int i = v / RT_EXP, e = v % RT_EXP;
-            wsm[i][e] = (e0 + e < E) ? W_r[(size_t)(i0 + i) * E + e0 + e] : 0.f;
+    };
+    auto load_w = [&](int i0, int buf) {
+        if (w_vec) {
+            for (int v = tid; v < RT_K * RT_EXP / 4; v += 128) {
+                const int i = v / (RT_EXP / 4), e = (v % (RT_EXP / 4)) * 4;
+                const bool ok = e0 + e < E;
+                const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&wsm[buf][i][e]);
+                const float *src = W_r + (size_t)(i0 + i) * E + (ok ? e0 + e : 0);
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(ok ? 16 : 0) : "memory");
+            }
+        } else {
+            for (int v = tid; v < RT_K * RT_EXP; v += 128) {
+                const int i = v / RT_EXP, e = v % RT_EXP;
+                wsm[buf][i][e] = (e0 + e < E) ? W_r[(size_t)(i0 + i) * E + e0 + e] : 0.f;
+            }
         }
-        __syncthreads();
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    load_x(0);
+    load_w(0, 0);
+    store_x(0);
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncthreads();
+    const int nc = d / RT_K;
+    for (int c = 0; c < nc; ++c) {
+        const int buf = c & 1;
+        if (c + 1 < nc) {
+            load_x((c + 1) * RT_K);
+            load_w((c + 1) * RT_K, buf ^ 1);
+        }
 #pragma unroll 8
         for (int i = 0; i < RT_K; ++i) {
-            float xv[8], wv[4];
-            float4 x0 = *reinterpret_cast<const float4 *>(&xs[i][ty * 8]);
-            float4 x1 = *reinterpret_cast<const float4 *>(&xs[i][ty * 8 + 4]);
-            xv[0] = x0.x; xv[1] = x0.y; xv[2] = x0.z; xv[3] = x0.w;
-            xv[4] = x1.x; xv[5] = x1.y; xv[6] = x1.z; xv[7] = x1.w;
-            float4 w0 = *reinterpret_cast<const float4 *>(&wsm[i][tx * 4]);
-            wv[0] = w0.x; wv[1] = w0.y; wv[2] = w0.z; wv[3] = w0.w;
+            const float4 x0 = *reinterpret_cast<const float4 *>(&xs[buf][i][ty * 8]);
+            const float4 x1 = *reinterpret_cast<const float4 *>(&xs[buf][i][ty * 8 + 4]);
+            const float2 w0 = *reinterpret_cast<const float2 *>(&wsm[buf][i][tx * 6]);
+            const float2 w1 = *reinterpret_cast<const float2 *>(&wsm[buf][i][tx * 6 + 2]);
+            const float2 w2 = *reinterpret_cast<const float2 *>(&wsm[buf][i][tx * 6 + 4]);
+            const float xv[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
+            const float wv[6] = {w0.x, w0.y, w1.x, w1.y, w2.x, w2.y};
 #pragma unroll
             for (int a = 0; a < 8; ++a)
 #pragma unroll
-                for (int b = 0; b < 4; ++b) acc[a][b] = fmaf(xv[a], wv[b], acc[a][b]);
+                for (int b = 0; b < 6; ++b) acc[a][b] = fmaf(xv[a], wv[b], acc[a][b]);
+        }
+        if (c + 1 < nc) {
+            store_x(buf ^ 1);
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
         }
         __syncthreads();
     }
 #pragma unroll
     for (int a = 0; a < 8; ++a) {
-        int t = t0 + ty * 8 + a;
+        const int t = t0 + ty * 8 + a;
         if (t >= T) continue;
 #pragma unroll
-        for (int b = 0; b < 4; ++b) {
-            int e = e0 + tx * 4 + b;
+        for (int b = 0; b < 6; ++b) {
+            const int e = e0 + tx * 6 + b;
             if (e < E) {
                 float v = acc[a][b];
                 if (bias) v = v + bias[e];
@@ -125,7 +166,7 @@ tqp_status launch_route(tqp_ctx *c, int T, const bf16 *X, const float *W_r, cons
                         float *topk_w, float *logits, cudaStream_t s) {
     const int d = c->desc.d, E = c->desc.E, k = c->desc.k;
     dim3 grid((T + RT_TOK - 1) / RT_TOK, (E + RT_EXP - 1) / RT_EXP);
-    route_logits_kernel<<<grid, 256, 0, s>>>(X, W_r, bias, logits, T, d, E);
+    route_logits_kernel<<<grid, 128, 0, s>>>(X, W_r, bias, logits, T, d, E);
     TQP_LAUNCH_OK(c);
     route_topk_kernel<<<(T + 3) / 4, 128, 0, s>>>(logits, topk_idx, topk_w, T, E, k);
     TQP_LAUNCH_OK(c);

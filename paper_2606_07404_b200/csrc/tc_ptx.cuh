@@ -74,6 +74,12 @@ __device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const void *tmap,
         "l"(tmap), "r"(c0), "r"(c1), "r"(cluster_bar) : "memory");
 }
 
+// 1-D bulk copy global -> this CTA's shared memory (TMA engine, no tensor map); bytes % 16 == 0, 16-byte aligned ends
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+                 "r"(bytes), "r"(bar) : "memory");
+}
+
 // explicit shared-space accesses (a generic pointer derived from an integer cast compiles to LD.E/ST.E, not LDS/STS)
 __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     uint4 v;
