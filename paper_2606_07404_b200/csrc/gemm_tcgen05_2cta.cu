@@ -26,8 +26,9 @@ constexpr int BM = 128, BK = 64, TN = kTileRows, HN = kTileRows / 2;
 constexpr int NSTAGE = 5, IDXQ = 8;
 constexpr int X_BYTES = HN * 128, A_BYTES = BM * 128, IDX_BYTES = 128 * 16, LUT_BYTES = 256 * 8 * 16;
 constexpr int OFF_X = 0, OFF_A = OFF_X + NSTAGE * X_BYTES, OFF_LUT = OFF_A + NSTAGE * A_BYTES,
-              OFF_IDX = OFF_LUT + LUT_BYTES, OFF_BAR = OFF_IDX + IDXQ * IDX_BYTES;
-constexpr int SMEM_BYTES = OFF_BAR + 512 + 1024;
+              OFF_IDX = OFF_LUT + LUT_BYTES, OFF_BAR = OFF_IDX + IDXQ * IDX_BYTES, OFF_EPI = OFF_BAR + 512;
+constexpr int EPI_ROWS = 32, EPI_BYTES = EPI_ROWS * BM * 2;   // output staging: [32 rows][128 channels] bf16, two buffers
+constexpr int SMEM_BYTES = OFF_EPI + 2 * EPI_BYTES + 1024;
 constexpr int NTHREADS = 480;
 constexpr int W_DEQ0 = 3, W_EPI0 = 11;
 
@@ -298,9 +299,12 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
         }
     } else if (warp >= W_EPI0) {
         // =========================== epilogue (128 threads) ===========================
+        // TMEM (lane = output channel, column = routed row) -> registers in the fragment layout -> bf16 ->
+        // stmatrix.trans into a [32 rows][128 channels] staging tile (16-byte chunks XOR-swizzled by row) ->
+        // 16-byte coalesced global stores (a half-warp writes one 256-byte row segment).
         const int q = warp & 3;             // TMEM lane quadrant this warp may access
-        const int m = q * 32 + lane;        // output channel inside this CTA's 128-row half
-        int cnt = 0;
+        const int et = threadIdx.x - W_EPI0 * 32;
+        int cnt = 0, gcount = 0;
         for (long long item = cid; item < total; item += ncl) {
             Item it;
             get_item(item, it);
@@ -312,15 +316,34 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
             ++cnt;
             mbar_wait(tmem_full(ab), aph);
             tc_fence_after();
-            bf16 *outp = pb.out + (size_t)it.t.row0 * M + it.m0 + m;
+            bf16 *outp = pb.out + (size_t)it.t.row0 * M + it.m0;
             const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + ab * TN;
-            for (int c0 = 0; c0 < it.t.rows; c0 += 16) {
-                uint32_t v[16];
-                tmem_ld16(taddr + c0, v);
+            for (int c0 = 0; c0 < it.t.rows; c0 += EPI_ROWS, ++gcount) {
+                uint32_t v[2][16];
+                tmem_ld_16x256b_x4(taddr + c0, v[0]);
+                tmem_ld_16x256b_x4(taddr + (16u << 16) + c0, v[1]);
                 tmem_ld_wait();
+                const uint32_t ebuf = sbase + OFF_EPI + (gcount & 1) * EPI_BYTES;
 #pragma unroll
-                for (int j = 0; j < 16; ++j)
-                    if (c0 + j < it.t.rows && !(ablate & 16)) outp[(size_t)(c0 + j) * M] = __float2bfloat16_rn(__uint_as_float(v[j]));
+                for (int g8 = 0; g8 < 4; ++g8) {   // 8 routed rows per stmatrix.x4: channels 8j..8j+7 of this warp, j = lane/8
+                    const int tok = g8 * 8 + (lane & 7);
+                    const uint32_t addr = ebuf + tok * (BM * 2) + (((q * 4 + (lane >> 3)) ^ (tok & 7)) << 4);
+                    stsm_x4_t(addr, float2_to_bf16x2(__uint_as_float(v[0][4 * g8]), __uint_as_float(v[0][4 * g8 + 1])),
+                              float2_to_bf16x2(__uint_as_float(v[0][4 * g8 + 2]), __uint_as_float(v[0][4 * g8 + 3])),
+                              float2_to_bf16x2(__uint_as_float(v[1][4 * g8]), __uint_as_float(v[1][4 * g8 + 1])),
+                              float2_to_bf16x2(__uint_as_float(v[1][4 * g8 + 2]), __uint_as_float(v[1][4 * g8 + 3])));
+                }
+                named_bar_sync(1, 128);   // staging tile complete; also orders the reuse of the other buffer
+                if (!(ablate & 16)) {
+#pragma unroll
+                    for (int i = 0; i < EPI_ROWS * 16 / 128; ++i) {
+                        const int r = et / 16 + 8 * i, ch = et % 16;
+                        if (c0 + r < it.t.rows) {
+                            const uint4 val = lds128(ebuf + r * (BM * 2) + ((ch ^ (r & 7)) << 4));
+                            *reinterpret_cast<uint4 *>(outp + (size_t)(c0 + r) * M + ch * 8) = val;
+                        }
+                    }
+                }
             }
             tc_fence_before();
             __syncwarp();
