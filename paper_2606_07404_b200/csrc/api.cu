@@ -267,6 +267,7 @@ tqp_status tqp_set_option(tqp_ctx *c, const char *name, int value) {
     }
     if (!strcmp(name, "trace")) {
         c->trace = value;
+        c->trace_seq = 0;
         return TQP_OK;
     }
     if (!strcmp(name, "ablate")) {

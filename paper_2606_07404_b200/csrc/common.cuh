@@ -86,7 +86,8 @@ struct tqp_ctx {
     int max_tiles = 0;
     std::string err;
     int ablate = 0;             // timing experiments only (tqp_set_option "ablate")
-    int trace = 0;              // debug: clock64 timeline of one cluster of the CTA-pair GEMM
+    int trace = 0;              // debug: n > 0 records a clock64 timeline of one cluster in the n-th CTA-pair GEMM launch from now
+    int trace_seq = 0;
     int time_gemm = 0;          // bracket GEMM launches with events (tqp_gemm_time)
     std::vector<cudaEvent_t> ev; // pairs (start, stop)
     int ev_used = 0;

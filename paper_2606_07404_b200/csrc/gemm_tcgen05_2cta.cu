@@ -216,6 +216,24 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
             if (it.t.rows <= 0) continue;
             const GemmProblem &pb = args.p[it.prob];
             const int m0 = it.m0, M = pb.M, e = it.t.expert;
+            // adapter rows of this item's K-step(s): fetched now, consumed after the k-loop (latency hidden behind it)
+            const int r = pb.r, nch = 2 * max(1, r / 16);
+            uint4 ch[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) ch[j] = make_uint4(0, 0, 0, 0);
+            for (int l = 0; l < pb.nlora; ++l) {
+                if ((l & 1) == g) {   // at most one adapter step per group and item (nlora <= 2)
+                    const GemmLora &L = pb.lora[l];
+                    if (L.mk_layout) {
+                        const uint4 *src = reinterpret_cast<const uint4 *>(L.lw + ((size_t)e * M + m0 + tid) * r);
+                        for (int j = 0; j < r / 8; ++j) ch[j] = src[j];
+                    } else {
+                        const bf16 *src = L.lw + (size_t)e * r * M + m0 + tid;
+                        uint16_t *h = reinterpret_cast<uint16_t *>(ch);
+                        for (int q = 0; q < r; ++q) h[q] = *reinterpret_cast<const uint16_t *>(src + (size_t)q * M);
+                    }
+                }
+            }
             for (int sg = 0; sg < pb.nseg; ++sg) {
                 const GemmSeg &S = pb.seg[sg];
                 const int nkb = S.K / BK;
@@ -270,21 +288,8 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                 }
             }
             // adapter K-steps: A tile = lw[m0 + tid][0..r) as a K-major row (chunks beyond r zeroed)
-            const int r = pb.r, nch = 2 * max(1, r / 16);
             for (int l = 0; l < pb.nlora; ++l) {
                 if ((l & 1) == g) {
-                    const GemmLora &L = pb.lora[l];
-                    uint4 ch[4];
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) ch[j] = make_uint4(0, 0, 0, 0);
-                    if (L.mk_layout) {
-                        const uint4 *src = reinterpret_cast<const uint4 *>(L.lw + ((size_t)e * M + m0 + tid) * r);
-                        for (int j = 0; j < r / 8; ++j) ch[j] = src[j];
-                    } else {
-                        const bf16 *src = L.lw + (size_t)e * r * M + m0 + tid;
-                        uint16_t *h = reinterpret_cast<uint16_t *>(ch);
-                        for (int q = 0; q < r; ++q) h[q] = *reinterpret_cast<const uint16_t *>(src + (size_t)q * M);
-                    }
                     mbar_wait(empty(st.s), st.ph ^ 1);
                     const uint32_t as = sbase + OFF_A + st.s * A_BYTES + tid * 128;
 #pragma unroll
@@ -375,8 +380,9 @@ tqp_status launch_gemm_tcgen05_2cta(tqp_ctx *c, const GemmProblem *probs, int np
     for (int i = 0; i < nprob; ++i) args.p[i] = probs[i];
     args.nprob = nprob;
     const int grid = (c->num_sms / 2) * 2;
+    const bool tr = c->trace > 0 && ++c->trace_seq == c->trace;
     g2::gemm_tcgen05_2cta_kernel<<<grid, g2::NTHREADS, g2::SMEM_BYTES, st>>>(
-        args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), c->ablate, c->trace ? c->p<long long>(c->ws.trace) : nullptr);
+        args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), c->ablate, tr ? c->p<long long>(c->ws.trace) : nullptr);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }
