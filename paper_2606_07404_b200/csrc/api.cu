@@ -131,7 +131,8 @@ tqp_status run_gemm(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_
     if (timed) TQP_CUDA_OK(c, cudaEventRecord(c->ev[c->ev_used], st));
     tqp_status r = c->gemm_impl == 1   ? launch_gemm_scaffold(c, probs, nprob, st)
                    : c->gemm_impl == 2 ? launch_gemm_tcgen05(c, probs, nprob, st)
-                                       : launch_gemm_tcgen05_2cta(c, probs, nprob, st);
+                   : c->gemm_impl == 3 ? launch_gemm_tcgen05_2cta(c, probs, nprob, st)
+                                       : launch_gemm_tcgen05_ts(c, probs, nprob, st);   // falls back to 2cta for MN-major
     if (timed) {
         TQP_CUDA_OK(c, cudaEventRecord(c->ev[c->ev_used + 1], st));
         c->ev_used += 2;
@@ -261,7 +262,7 @@ tqp_status tqp_bind_weights(tqp_ctx *c, const tqp_weights *w, void *stream) {
 tqp_status tqp_set_option(tqp_ctx *c, const char *name, int value) {
     if (!c || !name) return TQP_ERR_ARG;
     if (!strcmp(name, "gemm_impl")) {
-        REQ(c, value >= 0 && value <= 2, TQP_ERR_ARG, "gemm_impl must be 0, 1 or 2");
+        REQ(c, value >= 0 && value <= 3, TQP_ERR_ARG, "gemm_impl must be 0..3");
         c->gemm_impl = value;
         return TQP_OK;
     }

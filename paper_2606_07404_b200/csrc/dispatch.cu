@@ -48,11 +48,11 @@ __global__ void __launch_bounds__(256) dispatch_scan_chunks_kernel(int32_t *__re
 
 __global__ void __launch_bounds__(1024) dispatch_scan_experts_kernel(const int32_t *__restrict__ counts, int E,
                                                                      int32_t *__restrict__ offsets, Tile *__restrict__ tiles,
-                                                                     int32_t *__restrict__ num_tiles) {
+                                                                     int32_t *__restrict__ num_tiles, int tile_rows) {
     __shared__ int32_t w_off[32], w_til[32];
     const int e = threadIdx.x, lane = e % 32, warp = e / 32;
     const int cnt = (e < E) ? counts[e] : 0;
-    const int nt = (cnt + kTileRows - 1) / kTileRows;
+    const int nt = (cnt + tile_rows - 1) / tile_rows;
     int io = cnt, it = nt;   // inclusive scans inside the warp
 #pragma unroll
     for (int off = 1; off < 32; off <<= 1) {
@@ -134,7 +134,7 @@ tqp_status launch_dispatch(tqp_ctx *c, int T, const int32_t *topk_idx, int32_t *
     TQP_LAUNCH_OK(c);
     dispatch_scan_chunks_kernel<<<(E + 7) / 8, 256, 0, s>>>(blk, nchunks, E, counts);
     TQP_LAUNCH_OK(c);
-    dispatch_scan_experts_kernel<<<1, 1024, 0, s>>>(counts, E, offsets, c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles));
+    dispatch_scan_experts_kernel<<<1, 1024, 0, s>>>(counts, E, offsets, c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), kTileRows);
     TQP_LAUNCH_OK(c);
     dispatch_scatter_kernel<<<nblk, 128, smem, s>>>(topk_idx, N, E, blk, offsets, perm, inv_perm);
     TQP_LAUNCH_OK(c);

@@ -29,6 +29,12 @@ constexpr int NTHREADS = 320;
 
 // ---- PTX wrappers ----------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+// one lane of a converged warp (ptxas then keeps the tcgen05.mma operands in uniform registers; see tc_ptx.cuh)
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
 }
@@ -188,7 +194,7 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmArgs args, const uint4 *__restri
         }
     } else if (warp == 1) {
         // =========================== MMA issuer ===========================
-        if (lane == 0) {
+        if (elect_one()) {
             Pipe st;
             int it = 0;
             for (long long item = blockIdx.x; item < total; item += gridDim.x) {

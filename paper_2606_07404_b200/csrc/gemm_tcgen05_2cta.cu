@@ -143,7 +143,7 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
         }
     } else if (warp == 1) {
         // =========================== MMA issuer (leader CTA) ===========================
-        if (rank == 0 && lane == 0) {
+        if (rank == 0 && elect_one()) {
             Pipe st;
             int cnt = 0, tcount = 0;
             for (long long item = cid; item < total; item += ncl) {

@@ -1,0 +1,404 @@
+// Grouped dequant GEMM of the FORWARD projections on CTA pairs with the weight operand in TENSOR MEMORY, sm_100a.
+//
+//   out[p][m] = sum_k act[p][k] * W[m][k]  +  sum_l lact_l[p][q] * lw_l[m][q]
+//   W[m][k] = bf16( bf16(codebook[code[m][k/8]][k%8]) * bf16(scale[m]) )      (look up, rescale by the norm)
+//
+// Same swap-AB mapping as gemm_tcgen05_2cta.cu (UMMA M = 256 weight output channels over two SMs, N = routed rows of
+// one expert), but the dequantised A tile never touches shared memory: the forward GEMMs contract ALONG the code
+// vectors, so the thread that owns output channel m produces exactly row m of the A tile -- which is TMEM lane m.
+// It gathers 8 codebook rows per K-block, scales them and writes them with tcgen05.st; tcgen05.mma reads A from TMEM
+// and only the activations (B) from shared memory.  The CTA-pair kernel was bound by shared-memory bandwidth
+// (LUT gathers + A-tile stores + UMMA A reads + activation writes + UMMA B reads ~ 600 of 780 clk per K-block against
+// 448 clk of tensor work); this removes the A-tile stores and reads (~250 clk).
+// TMEM budget (512 columns): ONE 256-column accumulator + 6 A slots of 32 columns.  A first version kept two 224-column
+// accumulators and only 2 A slots: the slot turn-around (tcgen05.st -> remote mbarrier arrive -> MMA -> commit ->
+// producer wake-up, ~900 clk measured even with the MMAs removed) was then fully exposed (637 clk per K-block).  With six
+// slots that latency is hidden; the price is that the tensor pipe idles while the epilogue drains the accumulator into
+// a 64 KB bf16 staging tile (the global stores themselves overlap the next item's mainloop, and the producers keep
+// filling slots meanwhile).  The backward GEMMs contract ACROSS the code vectors (a thread's gather yields 8 channels
+// of one k) and stay on the shared-memory kernel.
+//
+// Warp roles per CTA (480 threads, 1 CTA/SM, persistent over work items, cluster = 2 CTAs):
+//   warp 0  TMA producer of the activation / adapter-projection tiles (signals the LEADER's barrier)
+//   warp 1  MMA issuer (leader CTA only) + TMEM allocation
+//   warp 2  TMA producer of the code-index tiles
+//   warps 3-10  dequant producers, two groups of four that alternate K-blocks (K-block j -> stage j % 6 -> its A slot)
+//   warps 11-14 epilogue (TMEM -> registers -> bf16 -> staging tile -> 16-byte global stores)
+#include "common.cuh"
+#include "tc_ptx.cuh"
+
+namespace tqp {
+namespace gts {
+using namespace ptx;
+
+constexpr int BM = 128, BK = 64, TN = kTileRows, HN = kTileRows / 2;
+constexpr int NSTAGE = 6, IDXQ = 8;                       // NSTAGE even: K-block j -> stage j % NSTAGE, dequant group j % 2
+constexpr int X_BYTES = HN * 128, IDX_BYTES = 128 * 16, LUT_BYTES = 256 * 8 * 16;
+constexpr int OFF_X = 0, OFF_LUT = OFF_X + NSTAGE * X_BYTES, OFF_IDX = OFF_LUT + LUT_BYTES,
+              OFF_BAR = OFF_IDX + IDXQ * IDX_BYTES, OFF_EPI = OFF_BAR + 512;
+constexpr int EPI_ROWS = 32, EPI_BYTES = TN * BM * 2;      // staging: the whole [256 rows][128 channels] bf16 output tile
+constexpr int SMEM_BYTES = OFF_EPI + EPI_BYTES + 1024;
+constexpr int NTHREADS = 480;
+constexpr int W_DEQ0 = 3, W_EPI0 = 11;
+constexpr bool kFullWaitCluster = true;                  // scope of the MMA issuer's acquire on the stage barrier (experiment)
+constexpr int TM_ACC = 0, TM_A = TN;                      // TMEM columns: accumulator [0, 256), A slots [256, 256 + 32 NSTAGE)
+
+struct Item {
+    Tile t;
+    int prob, m0;
+};
+
+// 32 consecutive 32-bit TMEM columns of this thread's lane
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t *v) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
+        "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};" ::"r"(taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]), "r"(v[10]),
+        "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]),
+        "r"(v[21]), "r"(v[22]), "r"(v[23]), "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]),
+        "r"(v[31])
+        : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t *v) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]), "r"(v[10]),
+        "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
+        : "memory");
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
+gemm_tcgen05_ts_kernel(const __grid_constant__ GemmArgs args, const uint4 *__restrict__ lut_g, const Tile *__restrict__ tiles,
+                       const int32_t *__restrict__ num_tiles_p, int ablate, long long *__restrict__ trace) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    const uint32_t sbase = smem_u32(smem);
+    const uint32_t bar0 = sbase + OFF_BAR;
+    // full[s] (the LEADER's is used): 1 arrival + 2 x X_BYTES of TMA from the activation producers, 8 dequant-warp arrivals
+    auto full = [&](int s) { return bar0 + 8u * s; };
+    auto empty = [&](int s) { return bar0 + 8u * (NSTAGE + s); };                    // local, multicast commit
+    auto idx_full = [&](int s) { return bar0 + 8u * (2 * NSTAGE + s); };             // local
+    auto idx_empty = [&](int s) { return bar0 + 8u * (2 * NSTAGE + IDXQ + s); };     // local
+    const uint32_t tmem_full = bar0 + 8u * (2 * NSTAGE + 2 * IDXQ);        // local, multicast commit
+    const uint32_t tmem_empty = bar0 + 8u * (2 * NSTAGE + 2 * IDXQ + 1);   // the leader's is used
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + OFF_BAR + 8 * (2 * NSTAGE + 2 * IDXQ + 4));
+
+    const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+    const uint32_t rank = cluster_ctarank();
+    const uint32_t full_remote = mapa(full(0), 0), tmem_empty_remote = mapa(tmem_empty, 0);   // the leader's barriers
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NSTAGE; ++s) { mbar_init(full(s), 9); mbar_init(empty(s), 1); }
+        for (int s = 0; s < IDXQ; ++s) { mbar_init(idx_full(s), 1); mbar_init(idx_empty(s), 8); }
+        mbar_init(tmem_full, 1);
+        mbar_init(tmem_empty, 8);
+        mbar_init_fence();
+    }
+    if (warp == 1) tmem_alloc<2>(smem_u32(tmem_slot), 512);
+    {   // replicated LUT: entry e, copy c at (e*8 + c) * 16 B  ->  lane c of every quarter-warp hits bank group c
+        uint4 *lut_s = reinterpret_cast<uint4 *>(smem + OFF_LUT);
+        for (int i = threadIdx.x; i < 256 * 8; i += NTHREADS) lut_s[i] = lut_g[i >> 3];
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync();   // both CTAs' barriers are initialised before any remote arrive / TMA completion
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    const int num_tiles = *num_tiles_p;
+    const int nprob = args.nprob;
+    const int MTP = args.p[0].M / (2 * BM);
+    const long long total = (long long)num_tiles * nprob * MTP;
+    const int cid = blockIdx.x >> 1, ncl = gridDim.x >> 1;
+
+    auto get_item = [&](long long item, Item &it) {
+        const int tile_id = (int)(item / (nprob * MTP)), rem = (int)(item % (nprob * MTP));
+        it.t = tiles[tile_id];
+        it.prob = rem / MTP;
+        it.m0 = ((rem % MTP) * 2 + (int)rank) * BM;
+    };
+
+    if (warp == 0) {
+        // =========================== activation TMA producer ===========================
+        if (lane == 0) {
+            Pipe st;
+            for (long long item = cid; item < total; item += ncl) {
+                Item it;
+                get_item(item, it);
+                if (it.t.rows <= 0) continue;
+                const GemmProblem &pb = args.p[it.prob];
+                const int n = max(16, (it.t.rows + 15) & ~15);
+                const int row = it.t.row0 + (int)rank * (n >> 1);
+                const GemmSeg &S = pb.seg[0];
+                const int nkb = S.K / BK;
+                for (int kb = 0; kb < nkb; ++kb) {
+                    mbar_wait(empty(st.s), st.ph ^ 1);
+                    if (rank == 0) mbar_expect_tx(full(st.s), 2 * X_BYTES);
+                    tma_load_2d_pair(sbase + OFF_X + st.s * X_BYTES, &S.act_map2, kb * BK, row, full_remote + 8u * st.s);
+                    st.next(NSTAGE);
+                }
+                for (int l = 0; l < pb.nlora; ++l) {
+                    mbar_wait(empty(st.s), st.ph ^ 1);
+                    if (rank == 0) mbar_expect_tx(full(st.s), 2 * X_BYTES);
+                    tma_load_2d_pair(sbase + OFF_X + st.s * X_BYTES, &pb.lora[l].lact_map2, 0, row, full_remote + 8u * st.s);
+                    st.next(NSTAGE);
+                }
+            }
+        }
+    } else if (warp == 2) {
+        // =========================== code-index TMA producer ===========================
+        if (lane == 0) {
+            Pipe iq;
+            for (long long item = cid; item < total; item += ncl) {
+                Item it;
+                get_item(item, it);
+                if (it.t.rows <= 0) continue;
+                const GemmProblem &pb = args.p[it.prob];
+                const GemmSeg &S = pb.seg[0];
+                const int npair = S.K / (2 * BK);
+                for (int kp = 0; kp < npair; ++kp) {
+                    mbar_wait(idx_empty(iq.s), iq.ph ^ 1);
+                    mbar_expect_tx(idx_full(iq.s), IDX_BYTES);
+                    tma_load_2d(sbase + OFF_IDX + iq.s * IDX_BYTES, &S.idx_map, kp * 16, it.t.expert * pb.M + it.m0, idx_full(iq.s));
+                    iq.next(IDXQ);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // =========================== MMA issuer (leader CTA) ===========================
+        if (rank == 0 && elect_one()) {
+            Pipe st;
+            int cnt = 0, tcount = 0;
+            const uint32_t hi_k = desc_hi(1024), lo_k = desc_lo_const(16);          // K-major SW128: SBO = 8 rows x 128 B
+            const uint32_t x16 = (sbase + OFF_X) >> 4;
+            for (long long item = cid; item < total; item += ncl) {
+                Item it;
+                get_item(item, it);
+                if (it.t.rows <= 0) continue;
+                const GemmProblem &pb = args.p[it.prob];
+                const uint32_t aph = cnt & 1;
+                ++cnt;
+                const int n = max(16, (it.t.rows + 15) & ~15);
+                mbar_wait<true>(tmem_empty, aph ^ 1);   // the epilogue has drained the previous item's accumulator
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + TM_ACC;
+                const uint32_t idesc = make_idesc(2 * BM, n, 0);
+                uint32_t accum = 0;
+                const int nkb = pb.seg[0].K / BK;
+                const int nmma_l = max(1, pb.r / 16);
+                const int nst = nkb + pb.nlora;
+                for (int j = 0; j < nst; ++j) {
+                    const bool tr = trace && cid == 0 && tcount < 1000;
+                    long long t0 = 0, t1 = 0;
+                    if (tr) t0 = clock64();
+                    mbar_wait<kFullWaitCluster>(full(st.s), st.ph);
+                    tc_fence_after();
+                    if (tr) t1 = clock64();
+                    const uint32_t xs = x16 + st.s * (X_BYTES >> 4), a_tmem = tmem_base + TM_A + st.s * 32;
+                    const int nmma = j < nkb ? BK / 16 : nmma_l;
+                    for (int kk = 0; kk < nmma; ++kk) {
+                        if (ablate & 32) break;
+                        umma_bf16_ts<2>(d_tmem, a_tmem + kk * 8, desc_from(hi_k, lo_k, xs + kk * 2), idesc, accum);
+                        accum = 1;
+                    }
+                    umma_commit_pair(empty(st.s), 3);
+                    if (tr) {
+                        trace[8000 + tcount * 4] = t0; trace[8000 + tcount * 4 + 1] = t1; trace[8000 + tcount * 4 + 2] = clock64();
+                        trace[8000 + tcount * 4 + 3] = j;
+                        ++tcount;
+                    }
+                    st.next(NSTAGE);
+                }
+                umma_commit_pair(tmem_full, 3);
+            }
+        }
+    } else if (warp >= W_DEQ0 && warp < W_EPI0) {
+        // =========================== dequant producers: 2 groups x 128 threads ===========================
+        // Thread = output channel (warp % 4 selects the TMEM lane quadrant this warp may write).  K-block j belongs to
+        // group j % 2 and to A slot j % 2; the gathers and multiplies run ahead of the slot becoming free.
+        const int g = (warp - W_DEQ0) >> 2;
+        const int row = (warp & 3) * 32 + lane;
+        const uint32_t lut_a = sbase + OFF_LUT + (lane & 7) * 16;
+        const uint32_t a_lane = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + TM_A;
+        Pipe st, iq;
+        int dcount = 0;
+        const bool trw = trace && cid == 0 && threadIdx.x == W_DEQ0 * 32;   // debug timeline: group 0, first thread, cluster 0
+        auto wait_slot_free = [&](const Pipe &p) {   // MMAs of the previous use of this stage (A slot + B tile) have completed
+            mbar_wait(empty(p.s), p.ph ^ 1);
+            tc_fence_after();
+        };
+        for (long long item = cid; item < total; item += ncl) {
+            Item it;
+            get_item(item, it);
+            if (it.t.rows <= 0) continue;
+            const GemmProblem &pb = args.p[it.prob];
+            const int m0 = it.m0, M = pb.M, e = it.t.expert;
+            const GemmSeg &S = pb.seg[0];
+            const int nkb = S.K / BK;   // even (K % 128 == 0)
+            const __nv_bfloat162 s2 = __float2bfloat162_rn(__half2float(S.scale[(size_t)e * M + m0 + row]));
+            // adapter row of this channel for the item's last K-step: fetched now, consumed after the k-loop
+            const int r = pb.r;
+            uint32_t ch[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) ch[j] = 0;
+            for (int l = 0; l < pb.nlora; ++l) {
+                if (((st.s + l) & 1) == g) {   // nkb is even, so the parity of the adapter step is known here
+                    const GemmLora &L = pb.lora[l];
+                    if (L.mk_layout) {
+                        const uint4 *src = reinterpret_cast<const uint4 *>(L.lw + ((size_t)e * M + m0 + row) * r);
+                        for (int j = 0; j < r / 8; ++j) *reinterpret_cast<uint4 *>(&ch[4 * j]) = src[j];
+                    } else {
+                        const bf16 *src = L.lw + (size_t)e * r * M + m0 + row;
+                        uint16_t *h = reinterpret_cast<uint16_t *>(ch);
+                        for (int q = 0; q < r; ++q) h[q] = *reinterpret_cast<const uint16_t *>(src + (size_t)q * M);
+                    }
+                }
+            }
+            uint2 codes = make_uint2(0, 0);
+            for (int kb = 0; kb < nkb; ++kb) {
+                const bool tr = trw && dcount < 1000 && (st.s & 1) == g;
+                long long tq[6];
+                if (tr) tq[0] = clock64();
+                if ((kb & 1) == 0) {   // one index tile = 16 codes per channel = this K-block and the next
+                    mbar_wait(idx_full(iq.s), iq.ph);
+                    const int half = ((st.s & 1) == g) ? 0 : 1;
+                    codes = lds64(sbase + OFF_IDX + iq.s * IDX_BYTES + row * 16 + half * 8);
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(idx_empty(iq.s));
+                    iq.next(IDXQ);
+                }
+                if (tr) tq[1] = clock64();
+                if ((st.s & 1) == g) {
+                    uint32_t a[32];   // 64 bf16 of this channel's row = 32 TMEM columns
+                    const uint32_t c01[2] = {codes.x, codes.y};
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const uint32_t code = (c01[j >> 2] >> ((j & 3) * 8)) & 0xffu;
+                        uint4 v = (ablate & 1) ? make_uint4(code, code, code, code) : lds128(lut_a + code * 128);
+                        __nv_bfloat162 *pv = reinterpret_cast<__nv_bfloat162 *>(&v);
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) pv[q] = __hmul2(pv[q], s2);
+                        a[4 * j] = v.x; a[4 * j + 1] = v.y; a[4 * j + 2] = v.z; a[4 * j + 3] = v.w;
+                    }
+                    if (tr) tq[2] = clock64();
+                    wait_slot_free(st);
+                    if (tr) tq[3] = clock64();
+                    if (!(ablate & 2)) tmem_st32(a_lane + st.s * 32, a);
+                    tmem_st_wait();
+                    if (tr) tq[4] = clock64();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_cluster(full_remote + 8u * st.s);
+                    if (tr) {
+                        tq[5] = clock64();
+                        for (int z = 0; z < 6; ++z) trace[dcount * 8 + z] = tq[z];
+                        trace[dcount * 8 + 6] = kb;
+                        ++dcount;
+                    }
+                }
+                st.next(NSTAGE);
+            }
+            for (int l = 0; l < pb.nlora; ++l) {
+                if ((st.s & 1) == g) {
+                    wait_slot_free(st);
+                    tmem_st16(a_lane + st.s * 32, ch);   // columns beyond r/2 are zero
+                    tmem_st_wait();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_cluster(full_remote + 8u * st.s);
+                }
+                st.next(NSTAGE);
+            }
+        }
+    } else if (warp >= W_EPI0) {
+        // =========================== epilogue (128 threads) ===========================
+        // Drain: TMEM (lane = output channel, column = routed row) -> registers in the fragment layout -> bf16 ->
+        // stmatrix.trans into the [rows][128 channels] staging tile (16-byte chunks XOR-swizzled by row); the
+        // accumulator is handed back to the MMA issuer as soon as it has been read.  Then 16-byte coalesced global
+        // stores (a half-warp writes one 256-byte row segment) overlap the next item's mainloop.
+        const int q = warp & 3;             // TMEM lane quadrant this warp may access
+        const int et = threadIdx.x - W_EPI0 * 32;
+        const uint32_t ebuf = sbase + OFF_EPI;
+        int cnt = 0;
+        for (long long item = cid; item < total; item += ncl) {
+            Item it;
+            get_item(item, it);
+            if (it.t.rows <= 0) continue;
+            const GemmProblem &pb = args.p[it.prob];
+            const int M = pb.M;
+            const uint32_t aph = cnt & 1;
+            ++cnt;
+            mbar_wait(tmem_full, aph);
+            tc_fence_after();
+            const bool tre = trace && cid == 0 && et == 0 && cnt <= 100;
+            if (tre) trace[12000 + cnt * 4] = clock64();
+            named_bar_sync(1, 128);   // every epilogue warp has finished storing the previous item out of the staging tile
+            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + TM_ACC;
+            for (int c0 = 0; c0 < it.t.rows; c0 += EPI_ROWS) {
+                uint32_t v[2][16];
+                tmem_ld_16x256b_x4(taddr + c0, v[0]);
+                tmem_ld_16x256b_x4(taddr + (16u << 16) + c0, v[1]);
+                tmem_ld_wait();
+#pragma unroll
+                for (int g8 = 0; g8 < 4; ++g8) {   // 8 routed rows per stmatrix.x4: channels 8j..8j+7 of this warp, j = lane/8
+                    const int tok = c0 + g8 * 8 + (lane & 7);
+                    const uint32_t addr = ebuf + tok * (BM * 2) + (((q * 4 + (lane >> 3)) ^ (tok & 7)) << 4);
+                    stsm_x4_t(addr, float2_to_bf16x2(__uint_as_float(v[0][4 * g8]), __uint_as_float(v[0][4 * g8 + 1])),
+                              float2_to_bf16x2(__uint_as_float(v[0][4 * g8 + 2]), __uint_as_float(v[0][4 * g8 + 3])),
+                              float2_to_bf16x2(__uint_as_float(v[1][4 * g8]), __uint_as_float(v[1][4 * g8 + 1])),
+                              float2_to_bf16x2(__uint_as_float(v[1][4 * g8 + 2]), __uint_as_float(v[1][4 * g8 + 3])));
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(tmem_empty_remote);
+            if (tre) trace[12000 + cnt * 4 + 1] = clock64();
+            named_bar_sync(1, 128);   // staging tile complete
+            if (!(ablate & 16)) {
+                bf16 *outp = pb.out + (size_t)it.t.row0 * M + it.m0;
+                for (int r = et / 16; r < it.t.rows; r += 8) {
+                    const int chk = et % 16;
+                    const uint4 val = lds128(ebuf + r * (BM * 2) + ((chk ^ (r & 7)) << 4));
+                    *reinterpret_cast<uint4 *>(outp + (size_t)r * M + chk * 8) = val;
+                }
+            }
+            if (tre) trace[12000 + cnt * 4 + 2] = clock64();
+        }
+    }
+
+    __syncwarp();
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync();   // the peer may still read this CTA's smem / signal its barriers until both are done
+    if (warp == 1) {
+        tc_fence_after();
+        tmem_dealloc<2>(tmem_base, 512);
+    }
+}
+
+}  // namespace gts
+
+tqp_status launch_gemm_tcgen05_ts(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st) {
+    for (int i = 0; i < nprob; ++i) {   // K-major single-segment problems with an even number of 128-channel tiles only
+        const GemmProblem &p = probs[i];
+        if (p.M % (2 * gts::BM) != 0 || p.nseg != 1 || !p.seg[0].kmajor || p.seg[0].K % (2 * gts::BK) != 0 || p.nlora > 2)
+            return launch_gemm_tcgen05_2cta(c, probs, nprob, st);
+    }
+    static bool attr_set = false;
+    if (!attr_set) {
+        TQP_CUDA_OK(c, cudaFuncSetAttribute(gts::gemm_tcgen05_ts_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, gts::SMEM_BYTES));
+        attr_set = true;
+    }
+    GemmArgs args;
+    for (int i = 0; i < nprob; ++i) args.p[i] = probs[i];
+    args.nprob = nprob;
+    const int grid = (c->num_sms / 2) * 2;
+    const bool tr = c->trace > 0 && ++c->trace_seq == c->trace;
+    gts::gemm_tcgen05_ts_kernel<<<grid, gts::NTHREADS, gts::SMEM_BYTES, st>>>(
+        args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), c->ablate,
+        tr ? c->p<long long>(c->ws.trace) : nullptr);
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
+
+}  // namespace tqp

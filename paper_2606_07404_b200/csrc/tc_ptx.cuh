@@ -19,6 +19,14 @@ __device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t rank) {
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
     return r;
 }
+// One lane of a converged warp.  ptxas knows that code guarded by elect.sync runs in a single thread and moves its
+// operands to uniform registers with a plain R2UR; behind a `lane == 0` test it wraps every tcgen05.mma in an
+// ELECT / R2UR.BROADCAST / BRA.U.ANY loop (~100 clk per MMA measured).
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void cluster_sync() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
