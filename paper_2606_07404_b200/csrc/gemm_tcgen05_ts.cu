@@ -129,13 +129,15 @@ gemm_tcgen05_ts_kernel(const __grid_constant__ GemmArgs args, const uint4 *__res
                 const GemmProblem &pb = args.p[it.prob];
                 const int n = max(16, (it.t.rows + 15) & ~15);
                 const int row = it.t.row0 + (int)rank * (n >> 1);
-                const GemmSeg &S = pb.seg[0];
-                const int nkb = S.K / BK;
-                for (int kb = 0; kb < nkb; ++kb) {
-                    mbar_wait(empty(st.s), st.ph ^ 1);
-                    if (rank == 0) mbar_expect_tx(full(st.s), 2 * X_BYTES);
-                    tma_load_2d_pair(sbase + OFF_X + st.s * X_BYTES, &S.act_map2, kb * BK, row, full_remote + 8u * st.s);
-                    st.next(NSTAGE);
+                for (int sg = 0; sg < pb.nseg; ++sg) {
+                    const GemmSeg &S = pb.seg[sg];
+                    const int nkb = S.K / BK;
+                    for (int kb = 0; kb < nkb; ++kb) {
+                        mbar_wait(empty(st.s), st.ph ^ 1);
+                        if (rank == 0) mbar_expect_tx(full(st.s), 2 * X_BYTES);
+                        tma_load_2d_pair(sbase + OFF_X + st.s * X_BYTES, &S.act_map2, kb * BK, row, full_remote + 8u * st.s);
+                        st.next(NSTAGE);
+                    }
                 }
                 for (int l = 0; l < pb.nlora; ++l) {
                     mbar_wait(empty(st.s), st.ph ^ 1);
@@ -154,13 +156,17 @@ gemm_tcgen05_ts_kernel(const __grid_constant__ GemmArgs args, const uint4 *__res
                 get_item(item, it);
                 if (it.t.rows <= 0) continue;
                 const GemmProblem &pb = args.p[it.prob];
-                const GemmSeg &S = pb.seg[0];
-                const int npair = S.K / (2 * BK);
-                for (int kp = 0; kp < npair; ++kp) {
-                    mbar_wait(idx_empty(iq.s), iq.ph ^ 1);
-                    mbar_expect_tx(idx_full(iq.s), IDX_BYTES);
-                    tma_load_2d(sbase + OFF_IDX + iq.s * IDX_BYTES, &S.idx_map, kp * 16, it.t.expert * pb.M + it.m0, idx_full(iq.s));
-                    iq.next(IDXQ);
+                for (int sg = 0; sg < pb.nseg; ++sg) {
+                    const GemmSeg &S = pb.seg[sg];
+                    const int npair = S.K / (2 * BK);
+                    for (int kp = 0; kp < npair; ++kp) {   // K-major: [128 channels][16 codes]; MN-major: [128 k][16 channel groups]
+                        mbar_wait(idx_empty(iq.s), iq.ph ^ 1);
+                        mbar_expect_tx(idx_full(iq.s), IDX_BYTES);
+                        const int c0 = S.kmajor ? kp * 16 : it.m0 / 8;
+                        const int c1 = S.kmajor ? it.t.expert * pb.M + it.m0 : it.t.expert * S.K + kp * 2 * BK;
+                        tma_load_2d(sbase + OFF_IDX + iq.s * IDX_BYTES, &S.idx_map, c0, c1, idx_full(iq.s));
+                        iq.next(IDXQ);
+                    }
                 }
             }
         }
@@ -184,7 +190,8 @@ gemm_tcgen05_ts_kernel(const __grid_constant__ GemmArgs args, const uint4 *__res
                 const uint32_t d_tmem = tmem_base + TM_ACC;
                 const uint32_t idesc = make_idesc(2 * BM, n, 0);
                 uint32_t accum = 0;
-                const int nkb = pb.seg[0].K / BK;
+                int nkb = 0;
+                for (int sg = 0; sg < pb.nseg; ++sg) nkb += pb.seg[sg].K / BK;
                 const int nmma_l = max(1, pb.r / 16);
                 const int nst = nkb + pb.nlora;
                 for (int j = 0; j < nst; ++j) {
@@ -233,9 +240,6 @@ gemm_tcgen05_ts_kernel(const __grid_constant__ GemmArgs args, const uint4 *__res
             if (it.t.rows <= 0) continue;
             const GemmProblem &pb = args.p[it.prob];
             const int m0 = it.m0, M = pb.M, e = it.t.expert;
-            const GemmSeg &S = pb.seg[0];
-            const int nkb = S.K / BK;   // even (K % 128 == 0)
-            const __nv_bfloat162 s2 = __float2bfloat162_rn(__half2float(S.scale[(size_t)e * M + m0 + row]));
             // adapter row of this channel for the item's last K-step: fetched now, consumed after the k-loop
             const int r = pb.r;
             uint32_t ch[16];
@@ -254,49 +258,122 @@ gemm_tcgen05_ts_kernel(const __grid_constant__ GemmArgs args, const uint4 *__res
                     }
                 }
             }
-            uint2 codes = make_uint2(0, 0);
-            for (int kb = 0; kb < nkb; ++kb) {
-                const bool tr = trw && dcount < 1000 && (st.s & 1) == g;
-                long long tq[6];
-                if (tr) tq[0] = clock64();
-                if ((kb & 1) == 0) {   // one index tile = 16 codes per channel = this K-block and the next
-                    mbar_wait(idx_full(iq.s), iq.ph);
-                    const int half = ((st.s & 1) == g) ? 0 : 1;
-                    codes = lds64(sbase + OFF_IDX + iq.s * IDX_BYTES + row * 16 + half * 8);
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(idx_empty(iq.s));
-                    iq.next(IDXQ);
-                }
-                if (tr) tq[1] = clock64();
-                if ((st.s & 1) == g) {
-                    uint32_t a[32];   // 64 bf16 of this channel's row = 32 TMEM columns
-                    const uint32_t c01[2] = {codes.x, codes.y};
+            for (int sg = 0; sg < pb.nseg; ++sg) {
+                const GemmSeg &S = pb.seg[sg];
+                const int nkb = S.K / BK;   // even (K % 128 == 0)
+                if (S.kmajor) {
+                    // ---- forward: codes run along k; this thread owns TMEM lane `row` and writes its 64 k-values itself
+                    const __nv_bfloat162 s2 = __float2bfloat162_rn(__half2float(S.scale[(size_t)e * M + m0 + row]));
+                    uint2 codes = make_uint2(0, 0);
+                    for (int kb = 0; kb < nkb; ++kb) {
+                        const bool tr = trw && dcount < 1000;
+                        long long tq[6] = {0, 0, 0, 0, 0, 0};
+                        if (tr) tq[0] = clock64();
+                        if ((kb & 1) == 0) {   // one index tile = 16 codes per channel = this K-block and the next
+                            mbar_wait(idx_full(iq.s), iq.ph);
+                            const int half = ((st.s & 1) == g) ? 0 : 1;
+                            codes = lds64(sbase + OFF_IDX + iq.s * IDX_BYTES + row * 16 + half * 8);
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(idx_empty(iq.s));
+                            iq.next(IDXQ);
+                        }
+                        if (tr) tq[1] = clock64();
+                        if ((st.s & 1) == g) {
+                            uint32_t a[32];   // 64 bf16 of this channel's row = 32 TMEM columns
+                            const uint32_t c01[2] = {codes.x, codes.y};
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        const uint32_t code = (c01[j >> 2] >> ((j & 3) * 8)) & 0xffu;
-                        uint4 v = (ablate & 1) ? make_uint4(code, code, code, code) : lds128(lut_a + code * 128);
-                        __nv_bfloat162 *pv = reinterpret_cast<__nv_bfloat162 *>(&v);
+                            for (int j = 0; j < 8; ++j) {
+                                const uint32_t code = (c01[j >> 2] >> ((j & 3) * 8)) & 0xffu;
+                                uint4 v = (ablate & 1) ? make_uint4(code, code, code, code) : lds128(lut_a + code * 128);
+                                __nv_bfloat162 *pv = reinterpret_cast<__nv_bfloat162 *>(&v);
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) pv[q] = __hmul2(pv[q], s2);
-                        a[4 * j] = v.x; a[4 * j + 1] = v.y; a[4 * j + 2] = v.z; a[4 * j + 3] = v.w;
+                                for (int q = 0; q < 4; ++q) pv[q] = __hmul2(pv[q], s2);
+                                a[4 * j] = v.x; a[4 * j + 1] = v.y; a[4 * j + 2] = v.z; a[4 * j + 3] = v.w;
+                            }
+                            if (tr) tq[2] = clock64();
+                            wait_slot_free(st);
+                            if (tr) tq[3] = clock64();
+                            if (!(ablate & 2)) tmem_st32(a_lane + st.s * 32, a);
+                            tmem_st_wait();
+                            if (tr) tq[4] = clock64();
+                            tc_fence_before();
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive_cluster(full_remote + 8u * st.s);
+                            if (tr) tq[5] = clock64();
+                        }
+                        if (tr) {
+                            for (int z = 0; z < 6; ++z) trace[dcount * 8 + z] = tq[z];
+                            trace[dcount * 8 + 6] = kb;
+                            trace[dcount * 8 + 7] = clock64();
+                            ++dcount;
+                        }
+                        st.next(NSTAGE);
                     }
-                    if (tr) tq[2] = clock64();
-                    wait_slot_free(st);
-                    if (tr) tq[3] = clock64();
-                    if (!(ablate & 2)) tmem_st32(a_lane + st.s * 32, a);
-                    tmem_st_wait();
-                    if (tr) tq[4] = clock64();
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive_cluster(full_remote + 8u * st.s);
-                    if (tr) {
-                        tq[5] = clock64();
-                        for (int z = 0; z < 6; ++z) trace[dcount * 8 + z] = tq[z];
-                        trace[dcount * 8 + 6] = kb;
-                        ++dcount;
+                } else {
+                    // ---- backward: codes run along the OUTPUT channels; one codebook row holds 8 channels of one k.
+                    // Thread t = (rk = t / 4, j = t % 4) gathers 4-byte pieces (2 channels) of the rows of 8 k-values, and
+                    // movmatrix turns each 8 (k) x 8 (channel) block into the accumulator-fragment layout of
+                    // tcgen05.st.16x256b: lane = channel, register = k pair.  Source row rk of a block carries
+                    // k = 16 x + 4 (rk / 2) + rk % 2 + 2 i, so that the transposed pairs land in TMEM columns 8 x + 2 j + i.
+                    const int rk = lane >> 2, jj = lane & 3;
+                    const int kofs = 4 * (rk >> 1) + (rk & 1);
+                    const uint32_t lut_b = sbase + OFF_LUT + rk * 16 + jj * 4;   // replica rk: all 32 lanes hit distinct banks
+                    uint32_t cw[8];              // code words (4 channel groups each) of this thread's 8 k-values of its own stage
+                    __nv_bfloat162 sc[8];        // and their per-k scales (the weight's output channel is k here)
+                    __half sraw[8];              // raw scales of the NEXT pair of K-blocks: fetched one pair ahead
+                    const int half = ((st.s & 1) == g) ? 0 : 1;   // which K-block of every pair is this group's (nkb is even)
+                    const __half *scp = S.scale + (size_t)e * S.K + half * BK + kofs;
+#pragma unroll
+                    for (int x = 0; x < 4; ++x)
+#pragma unroll
+                        for (int i = 0; i < 2; ++i) sraw[2 * x + i] = scp[16 * x + 2 * i];
+                    for (int kb = 0; kb < nkb; ++kb) {
+                        if ((kb & 1) == 0) {   // one index tile = 128 k x 16 channel groups = this K-block and the next
+                            mbar_wait(idx_full(iq.s), iq.ph);
+                            const uint32_t is = sbase + OFF_IDX + iq.s * IDX_BYTES + (half * 64 + kofs) * 16 + (warp & 3) * 4;
+#pragma unroll
+                            for (int x = 0; x < 4; ++x)
+#pragma unroll
+                                for (int i = 0; i < 2; ++i) {
+                                    cw[2 * x + i] = lds32(is + (16 * x + 2 * i) * 16);
+                                    sc[2 * x + i] = __float2bfloat162_rn(__half2float(sraw[2 * x + i]));
+                                }
+                            if (kb + 2 < nkb) {
+#pragma unroll
+                                for (int x = 0; x < 4; ++x)
+#pragma unroll
+                                    for (int i = 0; i < 2; ++i) sraw[2 * x + i] = scp[(kb + 2) * BK + 16 * x + 2 * i];
+                            }
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(idx_empty(iq.s));
+                            iq.next(IDXQ);
+                        }
+                        if ((st.s & 1) == g) {
+#pragma unroll
+                            for (int hs = 0; hs < 2; ++hs) {   // lanes +0..15 / +16..31 of this warp's quadrant
+                                uint32_t rg[16];
+#pragma unroll
+                                for (int x = 0; x < 4; ++x)
+#pragma unroll
+                                    for (int i = 0; i < 2; ++i)
+#pragma unroll
+                                        for (int mbi = 0; mbi < 2; ++mbi) {
+                                            const uint32_t code = (cw[2 * x + i] >> ((2 * hs + mbi) * 8)) & 0xffu;
+                                            uint32_t v = lds32(lut_b + code * 128);
+                                            __nv_bfloat162 w2 = __hmul2(*reinterpret_cast<__nv_bfloat162 *>(&v), sc[2 * x + i]);
+                                            rg[4 * x + 2 * mbi + i] = movmatrix_t(*reinterpret_cast<uint32_t *>(&w2));
+                                        }
+                                if (hs == 0) wait_slot_free(st);
+                                if (!(ablate & 2)) tmem_st_16x256b_x4(a_lane + ((uint32_t)(16 * hs) << 16) + st.s * 32, rg);
+                            }
+                            tmem_st_wait();
+                            tc_fence_before();
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive_cluster(full_remote + 8u * st.s);
+                        }
+                        st.next(NSTAGE);
                     }
                 }
-                st.next(NSTAGE);
             }
             for (int l = 0; l < pb.nlora; ++l) {
                 if ((st.s & 1) == g) {
@@ -379,10 +456,11 @@ gemm_tcgen05_ts_kernel(const __grid_constant__ GemmArgs args, const uint4 *__res
 }  // namespace gts
 
 tqp_status launch_gemm_tcgen05_ts(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st) {
-    for (int i = 0; i < nprob; ++i) {   // K-major single-segment problems with an even number of 128-channel tiles only
+    for (int i = 0; i < nprob; ++i) {   // an even number of 128-channel tiles and of 64-wide K-blocks per segment
         const GemmProblem &p = probs[i];
-        if (p.M % (2 * gts::BM) != 0 || p.nseg != 1 || !p.seg[0].kmajor || p.seg[0].K % (2 * gts::BK) != 0 || p.nlora > 2)
-            return launch_gemm_tcgen05_2cta(c, probs, nprob, st);
+        bool ok = p.M % (2 * gts::BM) == 0 && p.nlora <= 2;
+        for (int sg = 0; sg < p.nseg; ++sg) ok = ok && p.seg[sg].K % (2 * gts::BK) == 0;
+        if (!ok) return launch_gemm_tcgen05_2cta(c, probs, nprob, st);
     }
     static bool attr_set = false;
     if (!attr_set) {

@@ -6,58 +6,76 @@
 namespace tqp {
 
 // logits[t][e] = fmaf-chain over i ascending (bit-exact against the oracle: one accumulator per (t,e),
-// no split-K).  Register-tiled fp32 "SGEMM" on the FMA pipes: block = 64 tokens x 96 experts, 128 threads,
-// each thread 8 tokens x 6 experts (48 FMAs per 5 shared-memory loads), K-chunks of 32 double-buffered in shared
-// memory (W_r by cp.async, X through registers: bf16 widened exactly and stored transposed).  Bound: fp32 FMA
-// issue rate (R1 forbids tensor cores and any re-association of the sum).
-constexpr int RT_TOK = 64, RT_EXP = 96, RT_K = 32, RT_XLD = RT_TOK + 4;
+// no split-K).  Register-tiled fp32 "SGEMM" on the FMA pipes: block = 96 tokens x 96 experts, 128 threads,
+// each thread 12 tokens x 6 experts (72 FMAs per 6 shared-memory loads), K-chunks of 32 double-buffered in shared
+// memory (W_r by cp.async, X through registers: bf16 widened exactly and stored transposed).  96-token tiles make
+// 430 CTAs at T = 8192, E = 460: one wave of 3 CTAs per SM on 148 SMs with 97 % of the slots filled (64-token tiles
+// gave 640 CTAs on 740 slots: 4 or 5 per SM, 86 %).  Bound: fp32 FMA issue rate (R1 forbids tensor cores and any
+// re-association of the sum).
+constexpr int RT_TM = 12, RT_EN = 6;                       // per-thread tile
+constexpr int RT_TOK = 8 * RT_TM, RT_EXP = 16 * RT_EN, RT_K = 32, RT_XLD = RT_TOK;   // 96 floats per row: transposed stores and broadcast loads are conflict-free unpadded
+constexpr int RT_XCH = RT_TOK * RT_K / 8 / 128;            // 16-byte X chunks per thread per K-chunk
+constexpr int RT_WCH = RT_K * RT_EXP / 4 / 128;            // 16-byte W_r chunks per thread per K-chunk
 
-__global__ void __launch_bounds__(128) route_logits_kernel(const bf16 *__restrict__ X, const float *__restrict__ W_r,
-                                                           const float *__restrict__ bias, float *__restrict__ logits,
-                                                           int T, int d, int E) {
+__global__ void __launch_bounds__(128, 3) route_logits_kernel(const bf16 *__restrict__ X, const float *__restrict__ W_r,
+                                                              const float *__restrict__ bias, float *__restrict__ logits,
+                                                              int T, int d, int E) {
     __shared__ __align__(16) float xs[2][RT_K][RT_XLD];   // [buf][i][token]
     __shared__ __align__(16) float wsm[2][RT_K][RT_EXP];  // [buf][i][expert]
     const int tid = threadIdx.x;
     const int t0 = blockIdx.x * RT_TOK, e0 = blockIdx.y * RT_EXP;
-    const int tx = tid % 16, ty = tid / 16;   // tx -> experts (6 each), ty -> tokens (8 each)
+    const int tx = tid % 16, ty = tid / 16;   // tx -> experts (6 each), ty -> tokens (12 each)
     const bool w_vec = (E % 4) == 0;          // 16-byte cp.async needs aligned rows and whole chunks
-    float acc[8][6];
+    float acc[RT_TM][RT_EN];
 #pragma unroll
-    for (int a = 0; a < 8; ++a)
+    for (int a = 0; a < RT_TM; ++a)
 #pragma unroll
-        for (int b = 0; b < 6; ++b) acc[a][b] = 0.f;
+        for (int b = 0; b < RT_EN; ++b) acc[a][b] = 0.f;
 
-    // X tile: 64 tokens x 32 i (bf16) = 256 chunks of 8 values; thread owns chunks (token = tid % 64, seg = tid / 64 + 2 j)
-    const int xtok = tid % RT_TOK, xseg = tid / RT_TOK;
-    const bool x_ok = t0 + xtok < T;
-    const bf16 *xsrc = X + (size_t)(x_ok ? t0 + xtok : 0) * d + xseg * 8;
-    uint4 xr[2];
+    // X tile: 96 tokens x 32 i (bf16) = 384 chunks of 8 values; chunk v = tid + 128 j: token v % 96, segment v / 96
+    const bf16 *xsrc[RT_XCH];
+    int xtok[RT_XCH], xseg[RT_XCH];
+#pragma unroll
+    for (int j = 0; j < RT_XCH; ++j) {
+        const int v = tid + 128 * j;
+        xtok[j] = v % RT_TOK;
+        xseg[j] = v / RT_TOK;
+        xsrc[j] = (t0 + xtok[j] < T) ? X + (size_t)(t0 + xtok[j]) * d + xseg[j] * 8 : nullptr;
+    }
+    // W_r tile: 32 i x 96 experts (fp32) = 768 chunks of 4 values; chunk v: row v / 24, experts 4 (v % 24) ..
+    const float *wsrc[RT_WCH];
+    uint32_t wdst[RT_WCH];
+#pragma unroll
+    for (int j = 0; j < RT_WCH; ++j) {
+        const int v = tid + 128 * j, i = v / (RT_EXP / 4), e = (v % (RT_EXP / 4)) * 4;
+        wsrc[j] = (e0 + e < E) ? W_r + (size_t)i * E + e0 + e : nullptr;   // past E: zero-filled
+        wdst[j] = (uint32_t)__cvta_generic_to_shared(&wsm[0][i][e]);
+    }
+    uint4 xr[RT_XCH];
     auto load_x = [&](int i0) {
 #pragma unroll
-        for (int j = 0; j < 2; ++j)
-            xr[j] = x_ok ? *reinterpret_cast<const uint4 *>(xsrc + i0 + j * 16) : make_uint4(0, 0, 0, 0);
+        for (int j = 0; j < RT_XCH; ++j)
+            xr[j] = xsrc[j] ? *reinterpret_cast<const uint4 *>(xsrc[j] + i0) : make_uint4(0, 0, 0, 0);
     };
     auto store_x = [&](int buf) {
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
+        for (int j = 0; j < RT_XCH; ++j) {
             const uint32_t *r = reinterpret_cast<const uint32_t *>(&xr[j]);
-            const int ib = (xseg + 2 * j) * 8;
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 float2 f = bf16x2_to_float2(r[q]);
-                xs[buf][ib + 2 * q][xtok] = f.x;
-                xs[buf][ib + 2 * q + 1][xtok] = f.y;
+                xs[buf][xseg[j] * 8 + 2 * q][xtok[j]] = f.x;
+                xs[buf][xseg[j] * 8 + 2 * q + 1][xtok[j]] = f.y;
             }
         }
     };
     auto load_w = [&](int i0, int buf) {
         if (w_vec) {
-            for (int v = tid; v < RT_K * RT_EXP / 4; v += 128) {
-                const int i = v / (RT_EXP / 4), e = (v % (RT_EXP / 4)) * 4;
-                const bool ok = e0 + e < E;
-                const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&wsm[buf][i][e]);
-                const float *src = W_r + (size_t)(i0 + i) * E + (ok ? e0 + e : 0);
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(ok ? 16 : 0) : "memory");
+#pragma unroll
+            for (int j = 0; j < RT_WCH; ++j) {
+                const float *src = wsrc[j] ? wsrc[j] + (size_t)i0 * E : W_r;
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(wdst[j] + buf * (uint32_t)sizeof(wsm[0])), "l"(src),
+                             "r"(wsrc[j] ? 16 : 0) : "memory");
             }
         } else {
             for (int v = tid; v < RT_K * RT_EXP; v += 128) {
@@ -80,19 +98,23 @@ __global__ void __launch_bounds__(128) route_logits_kernel(const bf16 *__restric
             load_x((c + 1) * RT_K);
             load_w((c + 1) * RT_K, buf ^ 1);
         }
-#pragma unroll 8
+#pragma unroll 4
         for (int i = 0; i < RT_K; ++i) {
-            const float4 x0 = *reinterpret_cast<const float4 *>(&xs[buf][i][ty * 8]);
-            const float4 x1 = *reinterpret_cast<const float4 *>(&xs[buf][i][ty * 8 + 4]);
-            const float2 w0 = *reinterpret_cast<const float2 *>(&wsm[buf][i][tx * 6]);
-            const float2 w1 = *reinterpret_cast<const float2 *>(&wsm[buf][i][tx * 6 + 2]);
-            const float2 w2 = *reinterpret_cast<const float2 *>(&wsm[buf][i][tx * 6 + 4]);
-            const float xv[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
-            const float wv[6] = {w0.x, w0.y, w1.x, w1.y, w2.x, w2.y};
+            float xv[RT_TM], wv[RT_EN];
 #pragma unroll
-            for (int a = 0; a < 8; ++a)
+            for (int a = 0; a < RT_TM / 4; ++a) {
+                const float4 x4 = *reinterpret_cast<const float4 *>(&xs[buf][i][ty * RT_TM + 4 * a]);
+                xv[4 * a] = x4.x; xv[4 * a + 1] = x4.y; xv[4 * a + 2] = x4.z; xv[4 * a + 3] = x4.w;
+            }
 #pragma unroll
-                for (int b = 0; b < 6; ++b) acc[a][b] = fmaf(xv[a], wv[b], acc[a][b]);
+            for (int b = 0; b < RT_EN / 2; ++b) {
+                const float2 w2 = *reinterpret_cast<const float2 *>(&wsm[buf][i][tx * RT_EN + 2 * b]);
+                wv[2 * b] = w2.x; wv[2 * b + 1] = w2.y;
+            }
+#pragma unroll
+            for (int a = 0; a < RT_TM; ++a)
+#pragma unroll
+                for (int b = 0; b < RT_EN; ++b) acc[a][b] = fmaf(xv[a], wv[b], acc[a][b]);
         }
         if (c + 1 < nc) {
             store_x(buf ^ 1);
@@ -101,12 +123,12 @@ __global__ void __launch_bounds__(128) route_logits_kernel(const bf16 *__restric
         __syncthreads();
     }
 #pragma unroll
-    for (int a = 0; a < 8; ++a) {
-        const int t = t0 + ty * 8 + a;
+    for (int a = 0; a < RT_TM; ++a) {
+        const int t = t0 + ty * RT_TM + a;
         if (t >= T) continue;
 #pragma unroll
-        for (int b = 0; b < 6; ++b) {
-            const int e = e0 + tx * 6 + b;
+        for (int b = 0; b < RT_EN; ++b) {
+            const int e = e0 + tx * RT_EN + b;
             if (e < E) {
                 float v = acc[a][b];
                 if (bias) v = v + bias[e];
