@@ -40,6 +40,11 @@ def flops(cfg, T):
     return dict(total=base + lora + router, base=base, lora=lora, router=router, gemm=gemm)
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per grouped-GEMM launch (average of the four launches of a step) from the
+# `ncu --set full` capture summarised in profiles/r1b_gemm_ncu_cfg2.md; None for workloads without a capture.
+NCU_GEMM_TRAFFIC = {"cfg2_120b": 1.072e9}
+
+
 def peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -290,7 +295,8 @@ def run_ours(args, cfg):
                      "frac": gemm_tflops / pk["tensor_sustained"], "frac_of_burst": gemm_tflops / pk["tensor_burst"],
                      "frac_of_datasheet_2250": gemm_tflops / 2250.0, "peak_source": pk["source"] + ", sustained bf16",
                      "gemm_ms_per_step": gemm_ms_step, "gemm_share_of_step": gemm_ms_step / ms_per_step,
-                     "gemm_launches": gemm_launches, "flops_per_step": fl["gemm"], "traffic": None},
+                     "gemm_launches": gemm_launches, "flops_per_step": fl["gemm"],
+                     "flops_per_launch": fl["gemm"] / 4.0, "traffic": NCU_GEMM_TRAFFIC.get(cfg.name)},
     }
     if world == 1 and not args.no_cpu_baseline:
         cb = time_oracle(cfg, args.cpu_tokens, 1, 0)
