@@ -1,4 +1,4 @@
-"""GPU parity at BASELINE.json's FULL sizes (configs 1-4), in the launch configuration bench.py times.
+"""GPU parity at BASELINE.json's FULL sizes (configs 1-4, plus the paper-width shape 5), in the launch configuration bench.py times.
 
 Routing, permutation, combine and the HBM-bound backward steps are compared over the whole tensors (the oracle is
 cheap there).  The grouped expert FFN — too slow to run through the oracle for 460 experts inside a test — is compared
@@ -39,7 +39,7 @@ def sub_problem(inp, S, offsets, perm):
     return sub, rows, offs, np.ascontiguousarray(perm[rows])
 
 
-@pytest.mark.parametrize("cfg_id", [1, 2, 3, 4])
+@pytest.mark.parametrize("cfg_id", [1, 2, 3, 4, 5])
 def test_full_size_config(cfg_id):
     cfg = ti.CONFIGS[cfg_id]
     inp = ti.make_inputs(cfg)

@@ -2,7 +2,7 @@
 
 This module holds none of the method's arithmetic: it only draws random tensors in the storage
 formats the layer's boundary uses (bf16 / fp16 bit patterns, uint8 codes, fp32 router weights) and
-names the five BASELINE.json configs.  Recipe: SURVEY.md §8(d) / DESIGN.md "Input recipe".
+names the five BASELINE.json configs (plus one extra measurement shape).  Recipe: SURVEY.md §8(d) / DESIGN.md "Input recipe".
 
 bf16 tensors are carried as numpy uint16 bit patterns (numpy has no bf16); fp16 as numpy float16.
 """
@@ -39,6 +39,9 @@ CONFIGS = {
     2: Config("cfg2_120b", T=8192, d=2560, F=1024, E=460, k=12, r=16, seed=2),
     3: Config("cfg3_120b_skew", T=8192, d=2560, F=1024, E=460, k=12, r=16, seed=3, skew=True),
     4: Config("cfg4_120b_mb", T=16384, d=2560, F=1024, E=460, k=12, r=32, seed=4, router_grad=True),
+    # extra measurement shape (not a BASELINE.json config): the paper's own 120B layer width, d_model = 4096
+    # (Table 33)
+    5: Config("cfg5_120b_d4096", T=8192, d=4096, F=1024, E=460, k=12, r=16, seed=5),
 }
 
 
