@@ -168,6 +168,10 @@ tqp_status tqp_create(tqp_ctx **out, const tqp_layer_desc *desc) {
 void tqp_destroy(tqp_ctx *ctx) {
     if (!ctx) return;
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+    for (cudaEvent_t e : {ctx->ev_start, ctx->ev_x, ctx->ev_dy, ctx->ev_y, ctx->ev_yout})
+        if (e) cudaEventDestroy(e);
+    if (ctx->copy_in) cudaStreamDestroy(ctx->copy_in);
+    if (ctx->copy_out) cudaStreamDestroy(ctx->copy_out);
     delete ctx;
 }
 
@@ -452,19 +456,38 @@ tqp_status tqp_step_host(tqp_ctx *c, int T, const void *X_host, const void *dY_h
     bf16 *Ye = c->p<bf16>(c->ws.Ye), *dYe = c->p<bf16>(c->ws.dYe), *dXp = c->p<bf16>(c->ws.dXp);
     int total = 0;
 #define CK(x) do { st = (x); total += c->launches; if (st != TQP_OK) return st; } while (0)
-    TQP_CUDA_OK(c, cudaMemcpyAsync(X, X_host, row_bytes, cudaMemcpyHostToDevice, s));
-    TQP_CUDA_OK(c, cudaMemcpyAsync(dY, dY_host, row_bytes, cudaMemcpyHostToDevice, s));
+    if (!c->copy_in) {
+        TQP_CUDA_OK(c, cudaStreamCreateWithFlags(&c->copy_in, cudaStreamNonBlocking));
+        TQP_CUDA_OK(c, cudaStreamCreateWithFlags(&c->copy_out, cudaStreamNonBlocking));
+        for (cudaEvent_t *e : {&c->ev_start, &c->ev_x, &c->ev_dy, &c->ev_y, &c->ev_yout})
+            TQP_CUDA_OK(c, cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+    }
+    // X goes up first; dY follows on the same copy stream while the forward pass already runs on `s`; Y comes down on a
+    // second copy stream under the backward pass (PCIe is full duplex).  Everything is ordered after what `s` held before.
+    TQP_CUDA_OK(c, cudaEventRecord(c->ev_start, s));
+    TQP_CUDA_OK(c, cudaStreamWaitEvent(c->copy_in, c->ev_start, 0));
+    TQP_CUDA_OK(c, cudaStreamWaitEvent(c->copy_out, c->ev_start, 0));
+    TQP_CUDA_OK(c, cudaMemcpyAsync(X, X_host, row_bytes, cudaMemcpyHostToDevice, c->copy_in));
+    TQP_CUDA_OK(c, cudaEventRecord(c->ev_x, c->copy_in));
+    TQP_CUDA_OK(c, cudaMemcpyAsync(dY, dY_host, row_bytes, cudaMemcpyHostToDevice, c->copy_in));
+    TQP_CUDA_OK(c, cudaEventRecord(c->ev_dy, c->copy_in));
+    TQP_CUDA_OK(c, cudaStreamWaitEvent(s, c->ev_x, 0));
     CK(tqp_route(c, T, X, W_r, logit_bias, ti, tw, nullptr, s));
     CK(tqp_dispatch(c, T, ti, counts, offs, perm, inv, s));
     CK(tqp_expert_fwd(c, T, X, offs, perm, Ye, s));
     CK(tqp_combine(c, T, Ye, inv, tw, Y, s));
-    TQP_CUDA_OK(c, cudaMemcpyAsync(Y_host, Y, row_bytes, cudaMemcpyDeviceToHost, s));
+    TQP_CUDA_OK(c, cudaEventRecord(c->ev_y, s));
+    TQP_CUDA_OK(c, cudaStreamWaitEvent(c->copy_out, c->ev_y, 0));
+    TQP_CUDA_OK(c, cudaMemcpyAsync(Y_host, Y, row_bytes, cudaMemcpyDeviceToHost, c->copy_out));
+    TQP_CUDA_OK(c, cudaEventRecord(c->ev_yout, c->copy_out));
+    TQP_CUDA_OK(c, cudaStreamWaitEvent(s, c->ev_dy, 0));
     CK(tqp_combine_bwd(c, T, dY, Ye, inv, tw, dYe, dW_r ? dtw : nullptr, s));
     CK(tqp_expert_bwd(c, T, X, dYe, offs, perm, dXp, dA_gate, dB_gate, dA_up, dB_up, dA_down, dB_down, s));
     CK(tqp_dispatch_bwd(c, T, dXp, inv, dX, s));
     if (dW_r) CK(tqp_route_bwd(c, T, X, W_r, ti, tw, dtw, offs, perm, dX, dW_r, s));
 #undef CK
     TQP_CUDA_OK(c, cudaMemcpyAsync(dX_host, dX, row_bytes, cudaMemcpyDeviceToHost, s));
+    TQP_CUDA_OK(c, cudaStreamWaitEvent(s, c->ev_yout, 0));   // `s` (and its events) now also cover the Y download
     TQP_CUDA_OK(c, cudaStreamSynchronize(s));
     c->launches = total;
     return TQP_OK;

@@ -89,6 +89,9 @@ struct tqp_ctx {
     int trace = 0;              // debug: n > 0 records a clock64 timeline of one cluster in the n-th CTA-pair GEMM launch from now
     int trace_seq = 0;
     int time_gemm = 0;          // bracket GEMM launches with events (tqp_gemm_time)
+    // tqp_step_host: copy streams + events so that dY uploads and Y downloads overlap the compute on `stream`
+    cudaStream_t copy_in = nullptr, copy_out = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_x = nullptr, ev_dy = nullptr, ev_y = nullptr, ev_yout = nullptr;
     std::vector<cudaEvent_t> ev; // pairs (start, stop)
     int ev_used = 0;
     // tensor maps over weights / workspace (built in bind_weights)

@@ -57,7 +57,7 @@ def test_cfg0_tiny_full_chain(gemm_impl):
     check_all(inp, backward=True, router_grad=True, gemm_impl=gemm_impl)
 
 
-@pytest.mark.parametrize("gemm_impl", [1, 2, 0], ids=["scaffold", "tcgen05_1cta", "tcgen05"])
+@pytest.mark.parametrize("gemm_impl", [1, 2, 3, 0], ids=["scaffold", "tcgen05_1cta", "tcgen05_2cta_smemA", "tcgen05"])
 @pytest.mark.parametrize("cfg", [MID, MID32], ids=lambda c: c.name)
 def test_mid_ragged_multi_tile(cfg, gemm_impl):
     inp = _skewed(cfg)
@@ -94,3 +94,28 @@ def test_error_codes_on_device():
     with pytest.raises(tq.TqpError) as e:
         layer.route(torch.zeros(65 * 128 + 1, dtype=torch.bfloat16, device="cuda")[1:].view(65, 128)[:64], W)
     assert e.value.code == 3                           # misaligned pointer
+
+
+@pytest.mark.parametrize("cfg", [ti.CONFIGS[0], MID], ids=lambda c: c.name)
+def test_step_host_end_to_end(cfg):
+    """tqp_step_host (pinned host X/dY in, Y/dX out, copies overlapped with compute on internal streams) against the
+    oracle; called twice so that a stale event or buffer from the first call would show."""
+    import torch
+    from parity_util import make_layer, to_np
+    inp = _skewed(cfg) if cfg is MID else ti.make_inputs(cfg)
+    ref = oracle_ref(inp, True, True)
+    layer, dev = make_layer(inp, training=True)
+    T, d = inp["T"], inp["d"]
+    Xh, dYh = dev["X"].cpu().pin_memory(), dev["dY"].cpu().pin_memory()
+    Yh = torch.zeros((T, d), dtype=torch.bfloat16).pin_memory()
+    dXh = torch.zeros((T, d), dtype=torch.bfloat16).pin_memory()
+    grads = layer.alloc_grads()
+    dW_r = torch.zeros((d, inp["E"]), dtype=torch.float32, device="cuda")
+    for _ in range(2):
+        Yh.zero_(); dXh.zero_()
+        layer.step_host(Xh, dYh, dev["W_r"], dev.get("logit_bias"), Yh, dXh, grads, dW_r)
+    assert_close("Y", to_np(Yh), ref["Y"])
+    assert_close("dX", to_np(dXh), ref["dX"])
+    assert_close("dW_r", to_np(dW_r), ref["dW_r"])
+    for key in ("dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down"):
+        assert_close(key, to_np(grads[key]), ref[key])
