@@ -119,3 +119,43 @@ def test_step_host_end_to_end(cfg):
     assert_close("dW_r", to_np(dW_r), ref["dW_r"])
     for key in ("dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down"):
         assert_close(key, to_np(grads[key]), ref[key])
+
+
+def test_layer_reuse_smaller_batch_and_foreign_dYe():
+    """One ctx, two calls: a full batch, then a smaller batch with different data (stale workspace rows, tile list and
+    cached dispatch pointers must not leak), and an expert_bwd fed a dYe tensor that did NOT come from the fused
+    tqp_combine_bwd of this step (the library must then project it itself)."""
+    import torch
+    from parity_util import make_layer, to_dev, to_np
+    big = _skewed(MID)
+    layer, dev = make_layer(big, training=True)
+    for _ in range(2):   # warm the ctx with the big batch (fused combine_bwd path, cached Zd)
+        idx, w = layer.route(dev["X"], dev["W_r"], dev.get("logit_bias"))
+        counts, offsets, perm, inv = layer.dispatch(idx)
+        Ye = layer.expert_fwd(dev["X"], offsets, perm)
+        dYe, _ = layer.combine_bwd(dev["dY"], Ye, inv, w, want_dw=False)
+        layer.expert_bwd(dev["X"], dYe, offsets, perm)
+    small_cfg = ti.Config("small_after_big", T=200, d=MID.d, F=MID.F, E=MID.E, k=MID.k, r=MID.r, seed=77)
+    small = ti.make_inputs(small_cfg)
+    for key in ("idx_gate", "idx_up", "idx_down", "scale_gate", "scale_up", "scale_down", "codebook",
+                "A_gate", "A_up", "B_gate", "B_up", "A_down", "B_down"):
+        small[key] = big[key]                      # same bound weights
+    ref = oracle_ref(small, True, False)
+    sd = to_dev(small)
+    idx, w = layer.route(sd["X"], sd["W_r"], None)
+    counts, offsets, perm, inv = layer.dispatch(idx)
+    Ye = layer.expert_fwd(sd["X"], offsets, perm)
+    Y = layer.combine(Ye, inv, w)
+    dYe_fused, dw = layer.combine_bwd(sd["dY"], Ye, inv, w, want_dw=True)
+    dYe_foreign = dYe_fused.clone()                # a different tensor: the cached projection must not be trusted
+    dXp, grads = layer.expert_bwd(sd["X"], dYe_foreign, offsets, perm)
+    dX = layer.dispatch_bwd(dXp, inv)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(to_np(idx), ref["topk_idx"])
+    np.testing.assert_array_equal(to_np(perm), ref["perm"])
+    assert_close("Y", to_np(Y), ref["Y"])
+    assert_close("dYe", to_np(dYe_fused), ref["dYe"])
+    assert_close("dtopk_w", to_np(dw), ref["dtopk_w"])
+    assert_close("dX_experts", to_np(dX), ref["dX_experts"])
+    for key in ("dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down"):
+        assert_close(key, to_np(grads[key]), ref[key])
