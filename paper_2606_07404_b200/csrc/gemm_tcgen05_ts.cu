@@ -328,6 +328,9 @@ gemm_tcgen05_ts_kernel(const __grid_constant__ GemmArgs args, const uint4 *__res
 #pragma unroll
                         for (int i = 0; i < 2; ++i) sraw[2 * x + i] = scp[16 * x + 2 * i];
                     for (int kb = 0; kb < nkb; ++kb) {
+                        const bool tr = trw && dcount < 1000;
+                        long long tq[6] = {0, 0, 0, 0, 0, 0};
+                        if (tr) tq[0] = clock64();
                         if ((kb & 1) == 0) {   // one index tile = 128 k x 16 channel groups = this K-block and the next
                             mbar_wait(idx_full(iq.s), iq.ph);
                             const uint32_t is = sbase + OFF_IDX + iq.s * IDX_BYTES + (half * 64 + kofs) * 16 + (warp & 3) * 4;
@@ -348,6 +351,7 @@ gemm_tcgen05_ts_kernel(const __grid_constant__ GemmArgs args, const uint4 *__res
                             if (lane == 0) mbar_arrive(idx_empty(iq.s));
                             iq.next(IDXQ);
                         }
+                        if (tr) tq[1] = clock64();
                         if ((st.s & 1) == g) {
 #pragma unroll
                             for (int hs = 0; hs < 2; ++hs) {   // lanes +0..15 / +16..31 of this warp's quadrant
@@ -363,13 +367,25 @@ gemm_tcgen05_ts_kernel(const __grid_constant__ GemmArgs args, const uint4 *__res
                                             __nv_bfloat162 w2 = __hmul2(*reinterpret_cast<__nv_bfloat162 *>(&v), sc[2 * x + i]);
                                             rg[4 * x + 2 * mbi + i] = movmatrix_t(*reinterpret_cast<uint32_t *>(&w2));
                                         }
-                                if (hs == 0) wait_slot_free(st);
+                                if (hs == 0) {
+                                    if (tr) tq[2] = clock64();
+                                    wait_slot_free(st);
+                                    if (tr) tq[3] = clock64();
+                                }
                                 if (!(ablate & 2)) tmem_st_16x256b_x4(a_lane + ((uint32_t)(16 * hs) << 16) + st.s * 32, rg);
                             }
                             tmem_st_wait();
+                            if (tr) tq[4] = clock64();
                             tc_fence_before();
                             __syncwarp();
                             if (lane == 0) mbar_arrive_cluster(full_remote + 8u * st.s);
+                            if (tr) tq[5] = clock64();
+                        }
+                        if (tr) {
+                            for (int z = 0; z < 6; ++z) trace[dcount * 8 + z] = tq[z];
+                            trace[dcount * 8 + 6] = kb;
+                            trace[dcount * 8 + 7] = clock64();
+                            ++dcount;
                         }
                         st.next(NSTAGE);
                     }

@@ -60,19 +60,52 @@ __global__ void __launch_bounds__(256) route_dx_kernel(const float *__restrict__
     *reinterpret_cast<uint4 *>(dX + (size_t)t * d + col) = o;
 }
 
-// dW_r[i][e] = sum_{p in [offsets[e], offsets[e+1])} X[perm[p]/k][i] * dl[perm[p]];  block = (expert, 256 i's)
-__global__ void __launch_bounds__(256) route_dwr_kernel(const bf16 *__restrict__ X, const float *__restrict__ dl,
-                                                        const int32_t *__restrict__ offsets, const int32_t *__restrict__ perm,
-                                                        float *__restrict__ dW_r, int d, int E, int k) {
-    const int e = blockIdx.x, i = blockIdx.y * 256 + threadIdx.x;
+// dW_r[i][e] = sum_{p in [offsets[e], offsets[e+1])} X[perm[p]/k][i] * dl[perm[p]];  block = (expert, 512 columns):
+// 64 threads x 8 columns (16-byte loads of the gathered X rows, which stay L2-resident), row indices and dl staged
+// through shared memory 64 rows at a time, rows in ascending p (deterministic), four rows of loads in flight.
+constexpr int DWR_COLS = 512, DWR_CHUNK = 64;
+__global__ void __launch_bounds__(64) route_dwr_kernel(const bf16 *__restrict__ X, const float *__restrict__ dl,
+                                                       const int32_t *__restrict__ offsets, const int32_t *__restrict__ perm,
+                                                       float *__restrict__ dW_r, int d, int E, int k) {
+    __shared__ int s_tok[DWR_CHUNK];
+    __shared__ float s_dl[DWR_CHUNK];
+    const int e = blockIdx.x, col = blockIdx.y * DWR_COLS + threadIdx.x * 8;
     const int p0 = offsets[e], p1 = offsets[e + 1];
-    float acc = 0.f;
-    if (i < d) {
-        for (int p = p0; p < p1; ++p) {
-            const int a = perm[p];
-            acc = fmaf(__bfloat162float(X[(size_t)(a / k) * d + i]), dl[a], acc);
+    const bool ok = col < d;
+    float acc[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) acc[q] = 0.f;
+    for (int pc = p0; pc < p1; pc += DWR_CHUNK) {
+        const int n = min(DWR_CHUNK, p1 - pc);
+        __syncthreads();
+        if ((int)threadIdx.x < n) {
+            const int a = perm[pc + threadIdx.x];
+            s_tok[threadIdx.x] = a / k;
+            s_dl[threadIdx.x] = dl[a];
         }
-        dW_r[(size_t)i * E + e] = acc;
+        __syncthreads();
+        if (!ok) continue;
+        for (int r0 = 0; r0 < n; r0 += 4) {
+            uint4 v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                v[u] = (r0 + u < n) ? *reinterpret_cast<const uint4 *>(X + (size_t)s_tok[r0 + u] * d + col) : make_uint4(0, 0, 0, 0);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const float g = (r0 + u < n) ? s_dl[r0 + u] : 0.f;
+                const uint32_t *vp = reinterpret_cast<const uint32_t *>(&v[u]);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    float2 f = bf16x2_to_float2(vp[q]);
+                    acc[2 * q] = fmaf(f.x, g, acc[2 * q]);
+                    acc[2 * q + 1] = fmaf(f.y, g, acc[2 * q + 1]);
+                }
+            }
+        }
+    }
+    if (ok) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) dW_r[(size_t)(col + q) * E + e] = acc[q];
     }
 }
 
@@ -89,7 +122,7 @@ tqp_status launch_route_bwd(tqp_ctx *c, int T, const bf16 *X, const float *W_r, 
     const size_t warps = (size_t)T * slabs;
     route_dx_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, s>>>(WrT, topk_idx, dl, dX, T, d, k);
     TQP_LAUNCH_OK(c);
-    route_dwr_kernel<<<dim3(E, (d + 255) / 256), 256, 0, s>>>(X, dl, offsets, perm, dW_r, d, E, k);
+    route_dwr_kernel<<<dim3(E, (d + DWR_COLS - 1) / DWR_COLS), 64, 0, s>>>(X, dl, offsets, perm, dW_r, d, E, k);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }
