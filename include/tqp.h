@@ -141,6 +141,30 @@ tqp_status tqp_step_host(tqp_ctx *ctx, int T, const void *X_host, const void *dY
                          float *dB_gate, float *dA_up, float *dB_up, float *dA_down, float *dB_down,
                          float *dW_r, void *stream);
 
+/* --- paper-faithful router variant and loss-free balance controller -------------- */
+/* PAPER.md L224 (§3.4): "Routing scores are produced by a sigmoid, expert selection is biased by a per-expert routing
+ * logit bias".  logits as in tqp_route (canonical fmaf chain, NO bias added); selection = the k largest keys
+ * logits[t][e] + select_bias[e] (fp32 add; ties -> lower id; select_bias fp32 [E] or NULL); topk_s[t][j] =
+ * sigmoid(logit) of the UNBIASED selected logit; topk_w = topk_s / sum_j topk_s (summed in ascending j) -- DESIGN.md
+ * R21, R22.  topk_idx int32 [T][k]; topk_w, topk_s fp32 [T][k]; logits_out fp32 [T][E] or NULL.  All DEVICE pointers. */
+tqp_status tqp_route_sigmoid(tqp_ctx *ctx, int T, const void *X, const float *W_r, const float *select_bias,
+                             int32_t *topk_idx, float *topk_w, float *topk_s, float *logits_out, void *stream);
+/* Router backward for tqp_route_sigmoid (selection held constant, the bias has no gradient):
+ * dl_j = (dtopk_w_j - sum_i topk_w_i dtopk_w_i) * topk_w_j * (1 - topk_s_j), then as tqp_route_bwd:
+ * dX[t] += sum_j dl_j W_r[:,e_j] (dX bf16 [T][d], accumulated in place), dW_r[:,e] = sum_{rows of e} X[t] dl
+ * (fp32 [d][E], overwritten). */
+tqp_status tqp_route_sigmoid_bwd(tqp_ctx *ctx, int T, const void *X, const float *W_r, const int32_t *topk_idx,
+                                 const float *topk_w, const float *topk_s, const float *dtopk_w, const int32_t *offsets,
+                                 const int32_t *perm, void *dX, float *dW_r, void *stream);
+/* One step of the loss-free bias controller over the dispatch counts of a batch (§10.5, L1097 Table 29,
+ * L1516 Table 37): load_e = counts[e] / sum(counts), tau = 1/E.
+ * mode 0 (sign-based, 5B/9B):  bias[e] += gamma * sign(tau - load_e).
+ * mode 1 (three-tier band with quadratic boost, 120B; R23): inside [cap_lo, cap_hi] as mode 0; load > cap_hi:
+ *   bias[e] -= gamma * (1 + ((load - cap_hi)/tau)^2); load < cap_lo: bias[e] += gamma * (1 + ((cap_lo - load)/tau)^2);
+ *   cap_lo <= 0 selects tau^2 / cap_hi.  counts int32 [E] (device, e.g. from tqp_dispatch); bias fp32 [E], in place. */
+tqp_status tqp_bias_update(tqp_ctx *ctx, const int32_t *counts, float *bias, int mode, float gamma, float cap_hi,
+                           float cap_lo, void *stream);
+
 /* --- introspection ------------------------------------------------------------------------------------- */
 /* Device pointers of workspace tensors, for tests: "G","U","H" bf16 [N][F]; "Xp" bf16 [N][d];
  * "dH","dG","dU" bf16 [N][F]; "num_tiles" int32 [1].  NULL if unknown. */

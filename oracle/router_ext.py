@@ -76,3 +76,16 @@ def bias_update(counts, bias, mode: str, gamma: float, cap_hi: float = 0.0, cap_
     elif mode != "sign":
         raise ValueError(mode)
     return (np.asarray(bias, dtype=np.float64) + delta).astype(np.float32)
+
+
+def route_bwd_from_dl(X: np.ndarray, W_r: np.ndarray, topk_idx: np.ndarray, dl: np.ndarray, dX: np.ndarray):
+    """Chain rule through logits = X W_r for the selected entries only (the router is trained):
+    dX[t] += sum_j dl[t,j] W_r[:, e_j]  (in place);  returns dW_r with dW_r[:, e_j] += X[t] dl[t,j]."""
+    T, k = topk_idx.shape
+    dW_r = np.zeros_like(W_r, dtype=dX.dtype)
+    for t in range(T):
+        for j in range(k):
+            e = int(topk_idx[t, j])
+            dX[t] += dl[t, j] * W_r[:, e]
+            dW_r[:, e] += X[t] * dl[t, j]
+    return dW_r

@@ -66,6 +66,9 @@ def load_library() -> ctypes.CDLL:
         lib.tqp_dispatch_bwd.argtypes = [vp, ci] + [vp] * 4
         lib.tqp_route_bwd.argtypes = [vp, ci] + [vp] * 10
         lib.tqp_step_host.argtypes = [vp, ci] + [vp] * 14
+        lib.tqp_route_sigmoid.argtypes = [vp, ci] + [vp] * 8
+        lib.tqp_route_sigmoid_bwd.argtypes = [vp, ci] + [vp] * 11
+        lib.tqp_bias_update.argtypes = [vp, vp, vp, ci, ctypes.c_float, ctypes.c_float, ctypes.c_float, vp]
         lib.tqp_debug_buffer.argtypes = [vp, ctypes.c_char_p]
         lib.tqp_debug_buffer.restype = vp
         lib.tqp_gemm_time.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_int)]
@@ -215,6 +218,32 @@ class TqpLayer:
         self._check(self.lib.tqp_route_bwd(self.ctx, T, _ptr(X), _ptr(W_r), _ptr(topk_idx), _ptr(topk_w), _ptr(dtopk_w),
                                            _ptr(offsets), _ptr(perm), _ptr(dX), _ptr(dW_r), self._stream()))
         return dW_r
+
+    # ---- paper-faithful router variant and balance controller ----
+    def route_sigmoid(self, X, W_r, select_bias=None, want_logits=False):
+        t = self.torch
+        T = X.shape[0]
+        idx = t.empty((T, self.k), dtype=t.int32, device=self.device)
+        w = t.empty((T, self.k), dtype=t.float32, device=self.device)
+        sc = t.empty((T, self.k), dtype=t.float32, device=self.device)
+        lg = t.empty((T, self.E), dtype=t.float32, device=self.device) if want_logits else None
+        self._check(self.lib.tqp_route_sigmoid(self.ctx, T, _ptr(X), _ptr(W_r), _ptr(select_bias), _ptr(idx), _ptr(w),
+                                               _ptr(sc), _ptr(lg), self._stream()))
+        return (idx, w, sc, lg) if want_logits else (idx, w, sc)
+
+    def route_sigmoid_bwd(self, X, W_r, topk_idx, topk_w, topk_s, dtopk_w, offsets, perm, dX):
+        t = self.torch
+        T = X.shape[0]
+        dW_r = t.empty((self.d, self.E), dtype=t.float32, device=self.device)
+        self._check(self.lib.tqp_route_sigmoid_bwd(self.ctx, T, _ptr(X), _ptr(W_r), _ptr(topk_idx), _ptr(topk_w),
+                                                   _ptr(topk_s), _ptr(dtopk_w), _ptr(offsets), _ptr(perm), _ptr(dX),
+                                                   _ptr(dW_r), self._stream()))
+        return dW_r
+
+    def bias_update(self, counts, bias, mode, gamma, cap_hi=0.0, cap_lo=0.0):
+        self._check(self.lib.tqp_bias_update(self.ctx, _ptr(counts), _ptr(bias), int(mode), float(gamma), float(cap_hi),
+                                             float(cap_lo), self._stream()))
+        return bias
 
     def step_host(self, X_host, dY_host, W_r, logit_bias, Y_host, dX_host, grads, dW_r=None):
         """Whole forward+backward through HOST (pinned) X/dY/Y/dX buffers; grads / dW_r stay on the device."""

@@ -436,8 +436,38 @@ tqp_status tqp_route_bwd(tqp_ctx *c, int T, const void *X, const float *W_r, con
     if (st != TQP_OK) return st;
     PTR_OK(c, X); PTR_OK(c, W_r); PTR_OK(c, topk_idx); PTR_OK(c, topk_w); PTR_OK(c, dtopk_w); PTR_OK(c, offsets);
     PTR_OK(c, perm); PTR_OK(c, dX); PTR_OK(c, dW_r);
-    return launch_route_bwd(c, T, (const bf16 *)X, W_r, topk_idx, topk_w, dtopk_w, offsets, perm, (bf16 *)dX, dW_r,
+    return launch_route_bwd(c, T, (const bf16 *)X, W_r, topk_idx, topk_w, nullptr, dtopk_w, offsets, perm, (bf16 *)dX, dW_r,
                             (cudaStream_t)stream);
+}
+
+tqp_status tqp_route_sigmoid(tqp_ctx *c, int T, const void *X, const float *W_r, const float *select_bias, int32_t *topk_idx,
+                             float *topk_w, float *topk_s, float *logits_out, void *stream) {
+    tqp_status st = common_checks(c, T, false);
+    if (st != TQP_OK) return st;
+    PTR_OK(c, X); PTR_OK(c, W_r); PTR_OK(c, topk_idx); PTR_OK(c, topk_w); PTR_OK(c, topk_s);
+    float *lg = logits_out ? logits_out : c->p<float>(c->ws.logits);
+    return launch_route_sigmoid(c, T, (const bf16 *)X, W_r, select_bias, topk_idx, topk_w, topk_s, lg, (cudaStream_t)stream);
+}
+
+tqp_status tqp_route_sigmoid_bwd(tqp_ctx *c, int T, const void *X, const float *W_r, const int32_t *topk_idx,
+                                 const float *topk_w, const float *topk_s, const float *dtopk_w, const int32_t *offsets,
+                                 const int32_t *perm, void *dX, float *dW_r, void *stream) {
+    tqp_status st = common_checks(c, T, false);
+    if (st != TQP_OK) return st;
+    PTR_OK(c, X); PTR_OK(c, W_r); PTR_OK(c, topk_idx); PTR_OK(c, topk_w); PTR_OK(c, topk_s); PTR_OK(c, dtopk_w);
+    PTR_OK(c, offsets); PTR_OK(c, perm); PTR_OK(c, dX); PTR_OK(c, dW_r);
+    return launch_route_bwd(c, T, (const bf16 *)X, W_r, topk_idx, topk_w, topk_s, dtopk_w, offsets, perm, (bf16 *)dX, dW_r,
+                            (cudaStream_t)stream);
+}
+
+tqp_status tqp_bias_update(tqp_ctx *c, const int32_t *counts, float *bias, int mode, float gamma, float cap_hi, float cap_lo,
+                           void *stream) {
+    if (!c) return TQP_ERR_ARG;
+    c->launches = 0;
+    PTR_OK(c, counts); PTR_OK(c, bias);
+    REQ(c, mode == 0 || mode == 1, TQP_ERR_ARG, "mode must be 0 (sign-based) or 1 (three-tier)");
+    REQ(c, mode == 0 || cap_hi > 0.f, TQP_ERR_ARG, "three-tier controller needs cap_hi > 0");
+    return launch_bias_update(c, counts, bias, mode, gamma, cap_hi, cap_lo, (cudaStream_t)stream);
 }
 
 tqp_status tqp_step_host(tqp_ctx *c, int T, const void *X_host, const void *dY_host, const float *W_r,

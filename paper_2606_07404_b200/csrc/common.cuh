@@ -135,8 +135,12 @@ tqp_status launch_combine(tqp_ctx *c, int T, const bf16 *Ye, const int32_t *inv_
 tqp_status launch_combine_bwd(tqp_ctx *c, int T, const bf16 *dY, const bf16 *Ye, const int32_t *inv_perm,
                               const float *topk_w, bf16 *dYe, float *dtopk_w, cudaStream_t s);
 tqp_status launch_route_bwd(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const int32_t *topk_idx,
-                            const float *topk_w, const float *dtopk_w, const int32_t *offsets, const int32_t *perm,
-                            bf16 *dX, float *dW_r, cudaStream_t s);
+                            const float *topk_w, const float *topk_s, const float *dtopk_w, const int32_t *offsets,
+                            const int32_t *perm, bf16 *dX, float *dW_r, cudaStream_t s);
+tqp_status launch_route_sigmoid(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const float *select_bias, int32_t *topk_idx,
+                                float *topk_w, float *topk_s, float *logits, cudaStream_t s);
+tqp_status launch_bias_update(tqp_ctx *c, const int32_t *counts, float *bias, int mode, float gamma, float cap_hi, float cap_lo,
+                              cudaStream_t s);
 tqp_status launch_combine_dw(tqp_ctx *c, int T, const bf16 *dY, const bf16 *Ye, const int32_t *inv_perm, float *dtopk_w,
                              cudaStream_t s);
 tqp_status launch_make_lut(tqp_ctx *c, const __half *codebook, bf16 *lut, cudaStream_t s);

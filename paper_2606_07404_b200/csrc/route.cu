@@ -184,6 +184,96 @@ __global__ void __launch_bounds__(128) route_topk_kernel(const float *__restrict
     }
 }
 
+// Paper-faithful variant: selection by logit + bias, gate values from the sigmoid of the UNBIASED logit,
+// normalised over the selected set.  Same warp arg-max as above on the biased keys.
+__global__ void __launch_bounds__(128) route_topk_sigmoid_kernel(const float *__restrict__ logits, const float *__restrict__ bias,
+                                                                 int32_t *__restrict__ topk_idx, float *__restrict__ topk_w,
+                                                                 float *__restrict__ topk_s, int T, int E, int k) {
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) / 32, lane = threadIdx.x % 32;
+    if (warp >= T) return;
+    const float *l = logits + (size_t)warp * E;
+    constexpr int PER = 32;  // E <= 1024
+    float v[PER];
+#pragma unroll
+    for (int q = 0; q < PER; ++q) {
+        int e = q * 32 + lane;
+        v[q] = (e < E) ? (bias ? l[e] + bias[e] : l[e]) : -INFINITY;
+    }
+    uint32_t taken = 0;
+    int sel_e = 0;
+    for (int j = 0; j < k; ++j) {
+        float bv = -INFINITY;
+        int be = 0x7fffffff;
+#pragma unroll
+        for (int q = 0; q < PER; ++q) {
+            int e = q * 32 + lane;
+            bool ok = (e < E) && !((taken >> q) & 1u);
+            if (ok && (v[q] > bv || be == 0x7fffffff)) { bv = v[q]; be = e; }
+        }
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            float ov = __shfl_xor_sync(0xffffffffu, bv, off);
+            int oe = __shfl_xor_sync(0xffffffffu, be, off);
+            bool better = (oe != 0x7fffffff) && (be == 0x7fffffff || ov > bv || (ov == bv && oe < be));
+            if (better) { bv = ov; be = oe; }
+        }
+        if ((be % 32) == lane) taken |= 1u << (be / 32);
+        if (lane == j) sel_e = be;
+    }
+    const float sc = (lane < k) ? 1.f / (1.f + expf(-l[sel_e])) : 0.f;
+    float sum = 0.f;
+    for (int j = 0; j < k; ++j) sum = sum + __shfl_sync(0xffffffffu, sc, j);
+    if (lane < k) {
+        topk_idx[(size_t)warp * k + lane] = sel_e;
+        topk_s[(size_t)warp * k + lane] = sc;
+        topk_w[(size_t)warp * k + lane] = sc / sum;
+    }
+}
+
+// Loss-free bias controller (Table 29): one thread per expert; the total is the sum of the counts.
+__global__ void bias_update_kernel(const int32_t *__restrict__ counts, float *__restrict__ bias, int E, int mode, float gamma,
+                                   float cap_hi, float cap_lo) {
+    __shared__ float s_tot[32];
+    float part = 0.f;
+    for (int e = threadIdx.x; e < E; e += blockDim.x) part += (float)counts[e];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) part += __shfl_xor_sync(0xffffffffu, part, off);
+    if (threadIdx.x % 32 == 0) s_tot[threadIdx.x / 32] = part;
+    __syncthreads();
+    float total = 0.f;
+    for (int w = 0; w < (int)blockDim.x / 32; ++w) total += s_tot[w];
+    const float tau = 1.f / (float)E;
+    for (int e = threadIdx.x; e < E; e += blockDim.x) {
+        const float load = total > 0.f ? (float)counts[e] / total : 0.f;
+        const float err = tau - load;
+        float delta = gamma * (err > 0.f ? 1.f : (err < 0.f ? -1.f : 0.f));
+        if (mode == 1) {
+            const float lo = cap_lo > 0.f ? cap_lo : tau * tau / cap_hi;
+            if (load > cap_hi) { const float z = (load - cap_hi) / tau; delta = -gamma * (1.f + z * z); }
+            else if (load < lo) { const float z = (lo - load) / tau; delta = gamma * (1.f + z * z); }
+        }
+        bias[e] += delta;
+    }
+}
+
+tqp_status launch_route_sigmoid(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const float *select_bias, int32_t *topk_idx,
+                                float *topk_w, float *topk_s, float *logits, cudaStream_t s) {
+    const int d = c->desc.d, E = c->desc.E, k = c->desc.k;
+    dim3 grid((T + RT_TOK - 1) / RT_TOK, (E + RT_EXP - 1) / RT_EXP);
+    route_logits_kernel<<<grid, 128, 0, s>>>(X, W_r, nullptr, logits, T, d, E);
+    TQP_LAUNCH_OK(c);
+    route_topk_sigmoid_kernel<<<(T + 3) / 4, 128, 0, s>>>(logits, select_bias, topk_idx, topk_w, topk_s, T, E, k);
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
+
+tqp_status launch_bias_update(tqp_ctx *c, const int32_t *counts, float *bias, int mode, float gamma, float cap_hi, float cap_lo,
+                              cudaStream_t s) {
+    bias_update_kernel<<<1, 256, 0, s>>>(counts, bias, c->desc.E, mode, gamma, cap_hi, cap_lo);
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
+
 tqp_status launch_route(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const float *bias, int32_t *topk_idx,
                         float *topk_w, float *logits, cudaStream_t s) {
     const int d = c->desc.d, E = c->desc.E, k = c->desc.k;

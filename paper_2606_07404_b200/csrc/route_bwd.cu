@@ -5,12 +5,19 @@
 
 namespace tqp {
 
-__global__ void route_dl_kernel(const float *__restrict__ w, const float *__restrict__ dw, float *__restrict__ dl, int T, int k) {
+// sc == nullptr: softmax over the selected logits.  sc != nullptr: normalised sigmoid scores (tqp_route_sigmoid):
+// dl_j = (dw_j - sum_i w_i dw_i) w_j (1 - s_j).
+__global__ void route_dl_kernel(const float *__restrict__ w, const float *__restrict__ dw, const float *__restrict__ sc,
+                                float *__restrict__ dl, int T, int k) {
     int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= T) return;
     float dotp = 0.f;
     for (int j = 0; j < k; ++j) dotp = fmaf(w[(size_t)t * k + j], dw[(size_t)t * k + j], dotp);
-    for (int j = 0; j < k; ++j) dl[(size_t)t * k + j] = w[(size_t)t * k + j] * (dw[(size_t)t * k + j] - dotp);
+    for (int j = 0; j < k; ++j) {
+        float g = w[(size_t)t * k + j] * (dw[(size_t)t * k + j] - dotp);
+        if (sc) g *= 1.f - sc[(size_t)t * k + j];
+        dl[(size_t)t * k + j] = g;
+    }
 }
 
 __global__ void transpose_wr_kernel(const float *__restrict__ W_r, float *__restrict__ WrT, int d, int E) {
@@ -110,11 +117,11 @@ __global__ void __launch_bounds__(64) route_dwr_kernel(const bf16 *__restrict__ 
 }
 
 tqp_status launch_route_bwd(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const int32_t *topk_idx,
-                            const float *topk_w, const float *dtopk_w, const int32_t *offsets, const int32_t *perm,
-                            bf16 *dX, float *dW_r, cudaStream_t s) {
+                            const float *topk_w, const float *topk_s, const float *dtopk_w, const int32_t *offsets,
+                            const int32_t *perm, bf16 *dX, float *dW_r, cudaStream_t s) {
     const int d = c->desc.d, E = c->desc.E, k = c->desc.k;
     float *dl = c->p<float>(c->ws.dl), *WrT = c->p<float>(c->ws.WrT);
-    route_dl_kernel<<<(T + 127) / 128, 128, 0, s>>>(topk_w, dtopk_w, dl, T, k);
+    route_dl_kernel<<<(T + 127) / 128, 128, 0, s>>>(topk_w, dtopk_w, topk_s, dl, T, k);
     TQP_LAUNCH_OK(c);
     transpose_wr_kernel<<<dim3((d + 31) / 32, (E + 31) / 32), dim3(32, 8), 0, s>>>(W_r, WrT, d, E);
     TQP_LAUNCH_OK(c);

@@ -135,3 +135,32 @@ def test_controller_drives_a_skewed_router_towards_balance():
         bias = rx.bias_update(counts, bias, "three_tier", 2e-2, cap_hi=1.5 / E)
     c1 = np.bincount(rx.route_sigmoid(lg, bias, k)[0].ravel(), minlength=E)
     assert c1.max() < 0.5 * c0.max() and c1.min() > 4 * max(1, c0.min())
+
+
+def test_router_chain_gradients_against_finite_differences():
+    """L(X, W_r) = sum_t sum_j w_j(X W_r)[t] c[t,j]: dX and dW_r from route_sigmoid_dl + route_bwd_from_dl against
+    central differences in fp64 (selection unchanged under the perturbation)."""
+    rng = np.random.default_rng(8)
+    T, d, E, k, h = 5, 7, 9, 3, 1e-6
+    X = rng.standard_normal((T, d)); W = rng.standard_normal((d, E)); c = rng.standard_normal((T, k))
+
+    def loss(Xv, Wv, idx_ref=None):
+        idx, w, s = rx.route_sigmoid(Xv @ Wv, None, k)
+        if idx_ref is not None:
+            assert (idx == idx_ref).all()
+        return float(np.sum(w * c)), idx, w, s
+
+    _, idx, w, s = loss(X, W)
+    dl = rx.route_sigmoid_dl(w, s, c)
+    dX = np.zeros_like(X)
+    dW = rx.route_bwd_from_dl(X, W, idx, dl, dX)
+    for (t, i) in [(0, 0), (2, 3), (4, 6)]:
+        Xp, Xm = X.copy(), X.copy(); Xp[t, i] += h; Xm[t, i] -= h
+        fd = (loss(Xp, W, idx)[0] - loss(Xm, W, idx)[0]) / (2 * h)
+        assert abs(fd - dX[t, i]) <= 1e-6 * max(1.0, abs(fd))
+    for (i, e) in [(0, int(idx[0, 0])), (3, int(idx[1, 1])), (6, int(idx[4, 2]))]:
+        Wp, Wm = W.copy(), W.copy(); Wp[i, e] += h; Wm[i, e] -= h
+        fd = (loss(X, Wp, idx)[0] - loss(X, Wm, idx)[0]) / (2 * h)
+        assert abs(fd - dW[i, e]) <= 1e-6 * max(1.0, abs(fd))
+    unsel = np.setdiff1d(np.arange(E), idx.ravel())
+    assert (dW[:, unsel] == 0).all()
