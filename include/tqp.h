@@ -82,10 +82,12 @@ tqp_status tqp_bind_workspace(tqp_ctx *ctx, void *dev_ptr, size_t bytes, void *s
 /* Records the weight pointers, builds the TMA descriptors over the code indices and converts the codebook
  * to the bf16 lookup table the GEMM mainloop gathers from.  One-time, untimed; needs a bound workspace. */
 tqp_status tqp_bind_weights(tqp_ctx *ctx, const tqp_weights *w, void *stream);
-/* Options (debug / ablation).  "gemm_impl": 0 = tcgen05 grouped GEMM on CTA pairs (default), 1 = CUDA-core scaffold,
- * 2 = tcgen05 grouped GEMM, one CTA per tile.
- * "time_gemm": 0/1, see tqp_gemm_time.  "ablate": bit mask that disables parts of the dequant producer (results
- * become wrong; timing experiments only; 0 = off). */
+/* Options (debug / ablation).  "gemm_impl": 0 = tcgen05 grouped GEMM on CTA pairs with the dequantised weight
+ * operand in tensor memory (default), 1 = CUDA-core scaffold, 2 = tcgen05 grouped GEMM, one CTA per tile, weight operand
+ * through shared memory, 3 = CTA pairs, weight operand through shared memory.
+ * "time_gemm": 0/1, see tqp_gemm_time.  "ablate": bit mask that disables parts of the kernels (results become
+ * wrong; timing experiments only; 0 = off).  "trace": n > 0 records a clock64 timeline of one CTA pair in the n-th
+ * grouped-GEMM launch from now into the workspace tensor "trace" (tqp_debug_buffer). */
 tqp_status tqp_set_option(tqp_ctx *ctx, const char *name, int value);
 
 /* --- forward ------------------------------------------------------------------------------------------ */
