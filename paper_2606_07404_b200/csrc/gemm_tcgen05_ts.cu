@@ -267,8 +267,8 @@ gemm_tcgen05_ts_kernel(const __grid_constant__ GemmArgs args, const uint4 *__res
                     uint2 codes = make_uint2(0, 0);
                     for (int kb = 0; kb < nkb; ++kb) {
                         const bool tr = trw && dcount < 1000;
-                        long long tq[6] = {0, 0, 0, 0, 0, 0};
-                        if (tr) tq[0] = clock64();
+                        long long tq[6];
+                        if (tr) { tq[0] = clock64(); tq[5] = 0; }
                         if ((kb & 1) == 0) {   // one index tile = 16 codes per channel = this K-block and the next
                             mbar_wait(idx_full(iq.s), iq.ph);
                             const int half = ((st.s & 1) == g) ? 0 : 1;
@@ -329,8 +329,8 @@ gemm_tcgen05_ts_kernel(const __grid_constant__ GemmArgs args, const uint4 *__res
                         for (int i = 0; i < 2; ++i) sraw[2 * x + i] = scp[16 * x + 2 * i];
                     for (int kb = 0; kb < nkb; ++kb) {
                         const bool tr = trw && dcount < 1000;
-                        long long tq[6] = {0, 0, 0, 0, 0, 0};
-                        if (tr) tq[0] = clock64();
+                        long long tq[6];
+                        if (tr) { tq[0] = clock64(); tq[5] = 0; }
                         if ((kb & 1) == 0) {   // one index tile = 128 k x 16 channel groups = this K-block and the next
                             mbar_wait(idx_full(iq.s), iq.ph);
                             const uint32_t is = sbase + OFF_IDX + iq.s * IDX_BYTES + (half * 64 + kofs) * 16 + (warp & 3) * 4;
