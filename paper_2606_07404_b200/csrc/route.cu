@@ -140,12 +140,12 @@ __global__ void __launch_bounds__(128, 3) route_logits_kernel(const bf16 *__rest
 
 // One warp per token: k rounds of a warp arg-max under the total order (-logit, id); then the softmax over
 // the k selected logits with the sum taken in ascending j (the oracle's order).  E <= 1024.
+template <int PER>   // PER = ceil(E / 32) rounded up to a power of two: logits held per lane
 __global__ void __launch_bounds__(128) route_topk_kernel(const float *__restrict__ logits, int32_t *__restrict__ topk_idx,
                                                          float *__restrict__ topk_w, int T, int E, int k) {
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) / 32, lane = threadIdx.x % 32;
     if (warp >= T) return;
     const float *l = logits + (size_t)warp * E;
-    constexpr int PER = 32;  // E <= 1024
     float v[PER];
 #pragma unroll
     for (int q = 0; q < PER; ++q) {
@@ -186,13 +186,13 @@ __global__ void __launch_bounds__(128) route_topk_kernel(const float *__restrict
 
 // Paper-faithful variant: selection by logit + bias, gate values from the sigmoid of the UNBIASED logit,
 // normalised over the selected set.  Same warp arg-max as above on the biased keys.
+template <int PER>
 __global__ void __launch_bounds__(128) route_topk_sigmoid_kernel(const float *__restrict__ logits, const float *__restrict__ bias,
                                                                  int32_t *__restrict__ topk_idx, float *__restrict__ topk_w,
                                                                  float *__restrict__ topk_s, int T, int E, int k) {
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) / 32, lane = threadIdx.x % 32;
     if (warp >= T) return;
     const float *l = logits + (size_t)warp * E;
-    constexpr int PER = 32;  // E <= 1024
     float v[PER];
 #pragma unroll
     for (int q = 0; q < PER; ++q) {
@@ -262,7 +262,9 @@ tqp_status launch_route_sigmoid(tqp_ctx *c, int T, const bf16 *X, const float *W
     dim3 grid((T + RT_TOK - 1) / RT_TOK, (E + RT_EXP - 1) / RT_EXP);
     route_logits_kernel<<<grid, 128, 0, s>>>(X, W_r, nullptr, logits, T, d, E);
     TQP_LAUNCH_OK(c);
-    route_topk_sigmoid_kernel<<<(T + 3) / 4, 128, 0, s>>>(logits, select_bias, topk_idx, topk_w, topk_s, T, E, k);
+#define TQP_TOPK(P) route_topk_sigmoid_kernel<P><<<(T + 3) / 4, 128, 0, s>>>(logits, select_bias, topk_idx, topk_w, topk_s, T, E, k)
+    if (E <= 64) TQP_TOPK(2); else if (E <= 128) TQP_TOPK(4); else if (E <= 256) TQP_TOPK(8); else if (E <= 512) TQP_TOPK(16); else TQP_TOPK(32);
+#undef TQP_TOPK
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }
@@ -280,7 +282,9 @@ tqp_status launch_route(tqp_ctx *c, int T, const bf16 *X, const float *W_r, cons
     dim3 grid((T + RT_TOK - 1) / RT_TOK, (E + RT_EXP - 1) / RT_EXP);
     route_logits_kernel<<<grid, 128, 0, s>>>(X, W_r, bias, logits, T, d, E);
     TQP_LAUNCH_OK(c);
-    route_topk_kernel<<<(T + 3) / 4, 128, 0, s>>>(logits, topk_idx, topk_w, T, E, k);
+#define TQP_TOPK(P) route_topk_kernel<P><<<(T + 3) / 4, 128, 0, s>>>(logits, topk_idx, topk_w, T, E, k)
+    if (E <= 64) TQP_TOPK(2); else if (E <= 128) TQP_TOPK(4); else if (E <= 256) TQP_TOPK(8); else if (E <= 512) TQP_TOPK(16); else TQP_TOPK(32);
+#undef TQP_TOPK
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }
