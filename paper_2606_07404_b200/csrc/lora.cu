@@ -211,10 +211,17 @@ __global__ void __launch_bounds__(PJ_THREADS, 2) rows_proj_kernel(const __grid_c
             }
         }
     };
-    for (int kc = 0; kc < nk; kc += PJ_D) {   // register sets rotate with compile-time indices
+    // Register sets rotate with compile-time indices.  The main loop runs whole triples without conditions so that the
+    // three sets keep fixed registers (guarding every step made the compiler merge the sets with moves at the joins).
+    int kc = 0;
+    for (; kc + PJ_D <= nk; kc += PJ_D) {
+        step(kc, pre[0], pre[2]);
+        step(kc + 1, pre[1], pre[0]);
+        step(kc + 2, pre[2], pre[1]);
+    }
+    if (kc < nk) {
         step(kc, pre[0], pre[2]);
         if (kc + 1 < nk) step(kc + 1, pre[1], pre[0]);
-        if (kc + 2 < nk) step(kc + 2, pre[2], pre[1]);
     }
     cp_async_wait<0>();
     if (warp * 16 < valid) {   // accumulator layout: rows lane/4 (+8), columns 8 n + 2 (lane%4) + {0,1}
