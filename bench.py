@@ -37,6 +37,8 @@ def flops(cfg, T):
     lora = 18.0 * N * cfg.r * (cfg.d + cfg.F)            # fwd, activation-grad, weight-grad of the adapters
     router = 2.0 * T * cfg.d * cfg.E
     gemm = base + 6.0 * N * cfg.r * (cfg.d + cfg.F)      # what the grouped-GEMM kernels themselves execute
+    if not cfg.backward:                                 # forward-only config (configs[1]): half of the base, a third of the adapters
+        base, lora, gemm = base / 2, lora / 3, gemm / 2
     return dict(total=base + lora + router, base=base, lora=lora, router=router, gemm=gemm)
 
 
@@ -215,6 +217,9 @@ def run_ours(args, cfg):
         counts, offsets, perm, inv = layer.dispatch(idx); n += layer.last_launch_count()
         layer.expert_fwd(X, offsets, perm, out=Ye); n += layer.last_launch_count()
         layer.combine(Ye, inv, w, out=Y); n += layer.last_launch_count()
+        if not cfg.backward:
+            launches[0] = n
+            return
         _, dw = layer.combine_bwd(dY, Ye, inv, w, want_dw=cfg.router_grad, out=dYe); n += layer.last_launch_count()
         layer.expert_bwd(X, dYe, offsets, perm, grads=grads, out=dXp); n += layer.last_launch_count()
         layer.dispatch_bwd(dXp, inv, out=dX); n += layer.last_launch_count()
@@ -249,7 +254,7 @@ def run_ours(args, cfg):
 
     # ---- end to end through the C ABI with HOST buffers (H2D + whole chain + D2H inside the timed region) ----
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and cfg.backward:   # tqp_step_host runs forward + backward
         Xh = X.cpu().pin_memory(); dYh = dY.cpu().pin_memory()
         Yh = torch.empty((T, d), dtype=bf).pin_memory(); dXh = torch.empty((T, d), dtype=bf).pin_memory()
         dW_r = torch.empty((d, cfg.E), dtype=torch.float32, device=dev) if cfg.router_grad else None
@@ -280,7 +285,7 @@ def run_ours(args, cfg):
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
         "data": "synthetic",
         "config": {"workload": cfg.name, "T": T, "d": cfg.d, "F": cfg.F, "E": cfg.E, "k": cfg.k, "r": cfg.r,
-                   "passes": "fwd+bwd" + ("+router_grad" if cfg.router_grad else ""), "routing": "zipf1.1" if cfg.skew else "near-uniform",
+                   "passes": ("fwd+bwd" if cfg.backward else "fwd") + ("+router_grad" if cfg.router_grad else ""), "routing": "zipf1.1" if cfg.skew else "near-uniform",
                    "l2": f"inputs larger than L2 ({3 * cfg.E * cfg.d * cfg.F / 8 / 1e6:.0f} MB code indices + "
                          f"{T * cfg.k * cfg.d * 2 / 1e6:.0f} MB permuted rows per step), no flush",
                    "gemm_impl": "scaffold" if args.gemm_impl else "tcgen05", "parallelism": f"replicas x{world}, no collective"},
@@ -297,7 +302,7 @@ def run_ours(args, cfg):
                      "frac_of_datasheet_2250": gemm_tflops / 2250.0, "peak_source": pk["source"] + ", sustained bf16",
                      "gemm_ms_per_step": gemm_ms_step, "gemm_share_of_step": gemm_ms_step / ms_per_step,
                      "gemm_launches": gemm_launches, "flops_per_step": fl["gemm"],
-                     "flops_per_launch": fl["gemm"] / 4.0, "traffic": NCU_GEMM_TRAFFIC.get(cfg.name)},
+                     "flops_per_launch": fl["gemm"] / (4.0 if cfg.backward else 2.0), "traffic": NCU_GEMM_TRAFFIC.get(cfg.name)},
     }
     if world == 1 and not args.no_cpu_baseline:
         cb = time_oracle(cfg, args.cpu_tokens, 1, 0)
