@@ -35,6 +35,11 @@ Workspace layout(const tqp_layer_desc &d) {
     w.blk_counts = take(((N + kDispChunk - 1) / kDispChunk + 4) * E * 4);
     w.tiles = take((E + N / kTileRows + 2) * sizeof(Tile));
     w.num_tiles = take(16);
+    w.xsegs = take((N / kWgradSeg + 2) * sizeof(Tile));
+    w.xfirst = take((E + 1) * 4);
+    // partial weight gradients of split experts: first segments indexed by expert, extra segments by list position;
+    // widest use: two rank-r gradients over d columns in one pass (dA_gate + dA_up)
+    w.wg_scratch = d.training ? take((E + N / kWgradSeg + 2) * (size_t)2 * d.r * (dm > F ? dm : F) * 4) : take(16);
     w.lut = take(256 * 8 * 2);
     w.WrT = take(E * dm * 4);
     w.dl = take(N * 4);
@@ -160,6 +165,7 @@ tqp_status tqp_create(tqp_ctx **out, const tqp_layer_desc *desc) {
     c->ws = layout(*desc);
     c->num_sms = sms > 0 ? sms : 148;
     c->max_tiles = desc->E + (desc->T_max * desc->k) / kTileRows + 1;
+    c->max_xsegs = (desc->T_max * desc->k) / kWgradSeg + 1;
     memset(&c->w, 0, sizeof(c->w));
     *out = c;
     return TQP_OK;

@@ -20,6 +20,7 @@ constexpr int kTileRows = 256;   // max routed rows (UMMA N) of one grouped-GEMM
 constexpr int kRowPad = 512;     // rows of slack after N in every [N][*] workspace tensor (TMA boxes / 16-row groups over-read)
 constexpr int kLoraPad = 64;     // adapter projections are stored [N][64] bf16 (one 128-byte swizzle row)
 constexpr int kDispChunk = 256;  // assignments per warp in the dispatch kernels
+constexpr int kWgradSeg = 512;   // rows per CTA of the adapter weight-gradient kernels; longer experts are split and reduced in order
 
 struct Tile {          // one token tile of the grouped GEMMs: rows [row0, row0+rows) all belong to `expert`
     int32_t expert, row0, rows, pad;
@@ -62,7 +63,7 @@ struct Workspace {
     // sizes
     size_t total = 0;
     // offsets (bytes) into the bound buffer
-    size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, lut, WrT, dl,
+    size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, xsegs, xfirst, wg_scratch, lut, WrT, dl,
         // tqp_step_host staging
         trace, hX, hdY, hY, hdX, topk_idx, topk_w, counts, offsets, perm, inv_perm, Ye, dYe, dXp, dtopk_w;
 };
@@ -84,6 +85,7 @@ struct tqp_ctx {
     int launches = 0;
     int num_sms = 148;
     int max_tiles = 0;
+    int max_xsegs = 0;          // upper bound of the extra weight-gradient segments (N / kWgradSeg)
     std::string err;
     int ablate = 0;             // timing experiments only (tqp_set_option "ablate")
     int trace = 0;              // debug: n > 0 records a clock64 timeline of one cluster in the n-th CTA-pair GEMM launch from now

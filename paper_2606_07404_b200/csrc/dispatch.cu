@@ -48,32 +48,48 @@ __global__ void __launch_bounds__(256) dispatch_scan_chunks_kernel(int32_t *__re
 
 __global__ void __launch_bounds__(1024) dispatch_scan_experts_kernel(const int32_t *__restrict__ counts, int E,
                                                                      int32_t *__restrict__ offsets, Tile *__restrict__ tiles,
-                                                                     int32_t *__restrict__ num_tiles, int tile_rows) {
-    __shared__ int32_t w_off[32], w_til[32];
+                                                                     int32_t *__restrict__ num_tiles, int tile_rows,
+                                                                     Tile *__restrict__ xsegs, int32_t *__restrict__ xfirst) {
+    __shared__ int32_t w_off[32], w_til[32], w_xs[32];
     const int e = threadIdx.x, lane = e % 32, warp = e / 32;
     const int cnt = (e < E) ? counts[e] : 0;
     const int nt = (cnt + tile_rows - 1) / tile_rows;
-    int io = cnt, it = nt;   // inclusive scans inside the warp
+    const int nx = max(0, (cnt + kWgradSeg - 1) / kWgradSeg - 1);   // row segments of this expert beyond its first (weight gradients)
+    int io = cnt, it = nt, ix = nx;   // inclusive scans inside the warp
 #pragma unroll
     for (int off = 1; off < 32; off <<= 1) {
         int a = __shfl_up_sync(0xffffffffu, io, off), b = __shfl_up_sync(0xffffffffu, it, off);
-        if (lane >= off) { io += a; it += b; }
+        int c = __shfl_up_sync(0xffffffffu, ix, off);
+        if (lane >= off) { io += a; it += b; ix += c; }
     }
-    if (lane == 31) { w_off[warp] = io; w_til[warp] = it; }
+    if (lane == 31) { w_off[warp] = io; w_til[warp] = it; w_xs[warp] = ix; }
     __syncthreads();
     if (warp == 0) {
-        int a = w_off[lane], b = w_til[lane], ia = a, ib = b;
+        int a = w_off[lane], b = w_til[lane], c = w_xs[lane], ia = a, ib = b, ic = c;
 #pragma unroll
         for (int off = 1; off < 32; off <<= 1) {
             int x = __shfl_up_sync(0xffffffffu, ia, off), y = __shfl_up_sync(0xffffffffu, ib, off);
-            if (lane >= off) { ia += x; ib += y; }
+            int z = __shfl_up_sync(0xffffffffu, ic, off);
+            if (lane >= off) { ia += x; ib += y; ic += z; }
         }
         w_off[lane] = ia - a;   // exclusive prefix of the warp totals
         w_til[lane] = ib - b;
+        w_xs[lane] = ic - c;
     }
     __syncthreads();
-    const int off_e = w_off[warp] + io - cnt, til_e = w_til[warp] + it - nt;
+    const int off_e = w_off[warp] + io - cnt, til_e = w_til[warp] + it - nt, xs_e = w_xs[warp] + ix - nx;
     if (e < E) {
+        // extra row segments of experts with more than kWgradSeg rows: segment i+1 covers rows [(i+1) S, (i+2) S) of the expert
+        xfirst[e] = xs_e;
+        if (e == E - 1) xfirst[E] = xs_e + nx;
+        for (int i = 0; i < nx; ++i) {
+            Tile t;
+            t.expert = e;
+            t.row0 = off_e + (i + 1) * kWgradSeg;
+            t.rows = min(kWgradSeg, cnt - (i + 1) * kWgradSeg);
+            t.pad = i + 1;
+            xsegs[xs_e + i] = t;
+        }
         offsets[e] = off_e;
         if (e == E - 1) { offsets[E] = off_e + cnt; *num_tiles = til_e + nt; }
         if (nt > 0) {
@@ -134,7 +150,8 @@ tqp_status launch_dispatch(tqp_ctx *c, int T, const int32_t *topk_idx, int32_t *
     TQP_LAUNCH_OK(c);
     dispatch_scan_chunks_kernel<<<(E + 7) / 8, 256, 0, s>>>(blk, nchunks, E, counts);
     TQP_LAUNCH_OK(c);
-    dispatch_scan_experts_kernel<<<1, 1024, 0, s>>>(counts, E, offsets, c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), kTileRows);
+    dispatch_scan_experts_kernel<<<1, 1024, 0, s>>>(counts, E, offsets, c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), kTileRows,
+                                                    c->p<Tile>(c->ws.xsegs), c->p<int32_t>(c->ws.xfirst));
     TQP_LAUNCH_OK(c);
     dispatch_scatter_kernel<<<nblk, 128, smem, s>>>(topk_idx, N, E, blk, offsets, perm, inv_perm);
     TQP_LAUNCH_OK(c);

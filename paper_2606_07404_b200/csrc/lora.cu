@@ -315,6 +315,14 @@ struct WgradArgs {
     const bf16 *small_[2];   // [N][kLoraPad]
     float *grad[2];          // out_ar: [E][width][R] (dA) else [E][R][width] (dB)
     int width, out_ar;
+    // experts with more than kWgradSeg rows are split into row segments (one CTA each); their partial gradients go to
+    // `scratch` (entry e: first segment of expert e; entry E + j: extra segment j of the device-built list) and are
+    // summed in segment order by wgrad_reduce_kernel -- deterministic, no atomics
+    const Tile *xsegs;
+    const int32_t *xfirst;   // [E + 1]: first extra segment of every expert; xfirst[E] = number of extra segments
+    float *scratch;
+    int E;
+    size_t entry;            // floats per scratch entry = ns * R * width
 };
 
 template <int R, int NS>
@@ -327,17 +335,37 @@ struct WgradCfg {
     static constexpr int SMEM = WG_NST * STAGE + 128;
 };
 
-// grid = (E, width / 128), block = 128.  Warp w owns columns [32 w, 32 w + 32) of the slab and all RT adapter columns.
+// grid = (E + max extra segments, width / 128), block = 128.  Warp w owns columns [32 w, 32 w + 32) of the slab and all RT
+// adapter columns.  Blocks [0, E): the first kWgradSeg rows of expert blockIdx.x; blocks >= E: one extra segment each.
 template <int R, int NS>
 __global__ void __launch_bounds__(128) rows_wgrad_kernel(const __grid_constant__ WgradArgs a, const int32_t *__restrict__ offsets) {
     using C = WgradCfg<R, NS>;
     extern __shared__ __align__(128) uint8_t wg_smem[];
     uint8_t *smem = wg_smem;
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem);
-    const int e = blockIdx.x, a0 = blockIdx.y * WG_COLS;
+    const int a0 = blockIdx.y * WG_COLS;
     const int tid = threadIdx.x, warp = tid / 32;
-    const int p0 = offsets[e], p1 = offsets[e + 1];
     const int width = a.width;
+    int e, p0, p1;
+    float *dst[2];
+    if ((int)blockIdx.x < a.E) {
+        e = blockIdx.x;
+        p0 = offsets[e];
+        const int cnt = offsets[e + 1] - p0;
+        p1 = p0 + min(cnt, kWgradSeg);
+#pragma unroll
+        for (int w = 0; w < NS; ++w)
+            dst[w] = cnt > kWgradSeg ? a.scratch + (size_t)e * a.entry + (size_t)w * R * width : a.grad[w] + (size_t)e * R * width;
+    } else {
+        const int j = blockIdx.x - a.E;
+        if (j >= a.xfirst[a.E]) return;
+        const Tile t = a.xsegs[j];
+        e = t.expert;
+        p0 = t.row0;
+        p1 = p0 + t.rows;
+#pragma unroll
+        for (int w = 0; w < NS; ++w) dst[w] = a.scratch + (size_t)(a.E + j) * a.entry + (size_t)w * R * width;
+    }
     const int nit = (p1 - p0 + WG_ROWS - 1) / WG_ROWS;
 
     auto issue = [&](int it, int st) {
@@ -406,15 +434,35 @@ __global__ void __launch_bounds__(128) rows_wgrad_kernel(const __grid_constant__
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 const int q = (m * 16) % R + lane / 4 + 8 * h;
-                if (a.out_ar) {   // grad[e][col][q]
-                    float *g = a.grad[w] + ((size_t)e * width + col) * R + q;
+                if (a.out_ar) {   // [col][q]
+                    float *g = dst[w] + (size_t)col * R + q;
                     g[0] = acc[m][n][2 * h];
                     g[R] = acc[m][n][2 * h + 1];
-                } else {          // grad[e][q][col]
-                    *reinterpret_cast<float2 *>(a.grad[w] + ((size_t)e * R + q) * width + col) =
+                } else {          // [q][col]
+                    *reinterpret_cast<float2 *>(dst[w] + (size_t)q * width + col) =
                         make_float2(acc[m][n][2 * h], acc[m][n][2 * h + 1]);
                 }
             }
+        }
+    }
+}
+
+// Sum of the partial gradients of split experts, in segment order.  grid = (E, 4), block = 512; float4 elements.
+__global__ void __launch_bounds__(512) wgrad_reduce_kernel(const __grid_constant__ WgradArgs a, int ns, int R) {
+    const int e = blockIdx.x;
+    const int x0 = a.xfirst[e], nx = a.xfirst[e + 1] - x0;
+    if (nx <= 0) return;
+    const size_t per = (size_t)R * a.width;   // floats per gradient of one expert
+    for (int w = 0; w < ns; ++w) {
+        const float4 *first = reinterpret_cast<const float4 *>(a.scratch + (size_t)e * a.entry + (size_t)w * per);
+        float4 *out = reinterpret_cast<float4 *>(a.grad[w] + (size_t)e * per);
+        for (size_t i = blockIdx.y * blockDim.x + threadIdx.x; i < per / 4; i += (size_t)gridDim.y * blockDim.x) {
+            float4 s = first[i];
+            for (int j = 0; j < nx; ++j) {
+                const float4 v = reinterpret_cast<const float4 *>(a.scratch + (size_t)(a.E + x0 + j) * a.entry + (size_t)w * per)[i];
+                s.x += v.x; s.y += v.y; s.z += v.z; s.w += v.w;
+            }
+            out[i] = s;
         }
     }
 }
@@ -443,7 +491,9 @@ static tqp_status launch_wgrad_t(tqp_ctx *c, const WgradArgs &a, const int32_t *
         TQP_CUDA_OK(c, cudaFuncSetAttribute(rows_wgrad_kernel<R, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
         attr_set = true;
     }
-    rows_wgrad_kernel<R, NS><<<dim3(c->desc.E, a.width / WG_COLS), 128, C::SMEM, st>>>(a, offsets);
+    rows_wgrad_kernel<R, NS><<<dim3(c->desc.E + c->max_xsegs, a.width / WG_COLS), 128, C::SMEM, st>>>(a, offsets);
+    TQP_LAUNCH_OK(c);
+    wgrad_reduce_kernel<<<dim3(c->desc.E, 4), 512, 0, st>>>(a, NS, R);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }
@@ -465,6 +515,8 @@ tqp_status launch_rows_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 
     a.big = big; a.small_[0] = small0; a.small_[1] = small1; a.grad[0] = grad0; a.grad[1] = grad1;
     a.width = width; a.out_ar = out_ar;
     const int ns = small1 ? 2 : 1;
+    a.xsegs = c->p<Tile>(c->ws.xsegs); a.xfirst = c->p<int32_t>(c->ws.xfirst); a.scratch = c->p<float>(c->ws.wg_scratch);
+    a.E = E; a.entry = (size_t)ns * r * width;
     if (r == 16 && ns == 1) return launch_wgrad_t<16, 1>(c, a, offsets, st);
     if (r == 16 && ns == 2) return launch_wgrad_t<16, 2>(c, a, offsets, st);
     if (r == 32 && ns == 1) return launch_wgrad_t<32, 1>(c, a, offsets, st);
