@@ -1,4 +1,5 @@
 // C-ABI entry points (include/tqp.h): argument validation, workspace layout, TMA descriptors, call chains.
+#include <algorithm>
 #include <cstring>
 #include <new>
 
@@ -174,7 +175,8 @@ tqp_status tqp_create(tqp_ctx **out, const tqp_layer_desc *desc) {
 void tqp_destroy(tqp_ctx *ctx) {
     if (!ctx) return;
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
-    for (cudaEvent_t e : {ctx->ev_start, ctx->ev_x, ctx->ev_dy, ctx->ev_y, ctx->ev_yout})
+    for (cudaEvent_t e : {ctx->ev_start, ctx->ev_x, ctx->ev_dy, ctx->ev_y, ctx->ev_yout, ctx->ev_dx, ctx->ev_xc[0], ctx->ev_xc[1],
+                          ctx->ev_xc[2], ctx->ev_xc[3]})
         if (e) cudaEventDestroy(e);
     if (ctx->copy_in) cudaStreamDestroy(ctx->copy_in);
     if (ctx->copy_out) cudaStreamDestroy(ctx->copy_out);
@@ -413,17 +415,41 @@ tqp_status tqp_expert_bwd(tqp_ctx *c, int T, const void *X, const void *dYe, con
     CK(act_map(c, &ph.seg[0].act_map2, dye, (uint64_t)N, D.d, kTileRows / 2));
     CK(run_gemm(c, &ph, 1, s));
     CK(launch_swiglu_bwd(c, N, dH, G, U, dG, dU, s));
-    CK(launch_rows_wgrad(c, dye, D.d, c->p<bf16>(c->ws.HAd), nullptr, offsets, 0, dB_down, nullptr, s));
-    CK(launch_rows_wgrad(c, H, D.F, Zd, nullptr, offsets, 1, dA_down, nullptr, s));
+    if (!c->defer_tail) {
+        CK(launch_rows_wgrad(c, dye, D.d, c->p<bf16>(c->ws.HAd), nullptr, offsets, 0, dB_down, nullptr, s));
+        CK(launch_rows_wgrad(c, H, D.F, Zd, nullptr, offsets, 1, dA_down, nullptr, s));
+    }
     // gate / up projections: dXp = dG . Wg_eff^T + dU . Wu_eff^T and their adapter gradients
     CK(launch_rows_proj(c, dG, D.F, nullptr, nullptr, nullptr, (const bf16 *)c->w.B_gate, nullptr, 0, ls, Zg, nullptr, s));
     CK(launch_rows_proj(c, dU, D.F, nullptr, nullptr, nullptr, (const bf16 *)c->w.B_up, nullptr, 0, ls, Zu, nullptr, s));
     GemmProblem px = c->prob_dx;
     px.out = (bf16 *)dXp;
     CK(run_gemm(c, &px, 1, s));
+    if (c->defer_tail) {   // tqp_step_host: dX leaves for the host first (nothing below feeds it)
+        c->tail = {dA_gate, dB_gate, dA_up, dB_up, dA_down, dB_down, dye, offsets, true};
+        return TQP_OK;
+    }
     CK(launch_rows_wgrad(c, dG, D.F, c->p<bf16>(c->ws.XAg), nullptr, offsets, 0, dB_gate, nullptr, s));
     CK(launch_rows_wgrad(c, dU, D.F, c->p<bf16>(c->ws.XAu), nullptr, offsets, 0, dB_up, nullptr, s));
     CK(launch_rows_wgrad(c, Xp, D.d, Zg, Zu, offsets, 1, dA_gate, dA_up, s));   // one pass over Xp for both
+#undef CK
+    return TQP_OK;
+}
+
+// the adapter weight gradients that tqp_expert_bwd left pending (defer_tail)
+static tqp_status expert_bwd_tail(tqp_ctx *c, cudaStream_t s) {
+    if (!c->tail.pending) return TQP_OK;
+    c->tail.pending = false;
+    c->launches = 0;
+    const tqp_layer_desc &D = c->desc;
+    tqp_status st;
+#define CK(x) do { st = (x); if (st != TQP_OK) return st; } while (0)
+    CK(launch_rows_wgrad(c, c->tail.dYe, D.d, c->p<bf16>(c->ws.HAd), nullptr, c->tail.offsets, 0, c->tail.dB_down, nullptr, s));
+    CK(launch_rows_wgrad(c, c->p<bf16>(c->ws.H), D.F, c->p<bf16>(c->ws.Zd), nullptr, c->tail.offsets, 1, c->tail.dA_down, nullptr, s));
+    CK(launch_rows_wgrad(c, c->p<bf16>(c->ws.dG), D.F, c->p<bf16>(c->ws.XAg), nullptr, c->tail.offsets, 0, c->tail.dB_gate, nullptr, s));
+    CK(launch_rows_wgrad(c, c->p<bf16>(c->ws.dU), D.F, c->p<bf16>(c->ws.XAu), nullptr, c->tail.offsets, 0, c->tail.dB_up, nullptr, s));
+    CK(launch_rows_wgrad(c, c->p<bf16>(c->ws.Xp), D.d, c->p<bf16>(c->ws.Zg), c->p<bf16>(c->ws.Zu), c->tail.offsets, 1, c->tail.dA_gate,
+                         c->tail.dA_up, s));
 #undef CK
     return TQP_OK;
 }
@@ -495,20 +521,32 @@ tqp_status tqp_step_host(tqp_ctx *c, int T, const void *X_host, const void *dY_h
     if (!c->copy_in) {
         TQP_CUDA_OK(c, cudaStreamCreateWithFlags(&c->copy_in, cudaStreamNonBlocking));
         TQP_CUDA_OK(c, cudaStreamCreateWithFlags(&c->copy_out, cudaStreamNonBlocking));
-        for (cudaEvent_t *e : {&c->ev_start, &c->ev_x, &c->ev_dy, &c->ev_y, &c->ev_yout})
+        for (cudaEvent_t *e : {&c->ev_start, &c->ev_x, &c->ev_dy, &c->ev_y, &c->ev_yout, &c->ev_dx, &c->ev_xc[0], &c->ev_xc[1],
+                               &c->ev_xc[2], &c->ev_xc[3]})
             TQP_CUDA_OK(c, cudaEventCreateWithFlags(e, cudaEventDisableTiming));
     }
-    // X goes up first; dY follows on the same copy stream while the forward pass already runs on `s`; Y comes down on a
-    // second copy stream under the backward pass (PCIe is full duplex).  Everything is ordered after what `s` held before.
+    // X goes up in four token chunks and the router (token-wise) starts on each chunk as it lands; dY follows on the same
+    // copy stream while the forward pass already runs on `s`; Y comes down on a second copy stream under the backward
+    // pass (PCIe is full duplex); dX leaves before the last adapter weight gradients are computed.  Everything is ordered
+    // after what `s` held before.
     TQP_CUDA_OK(c, cudaEventRecord(c->ev_start, s));
     TQP_CUDA_OK(c, cudaStreamWaitEvent(c->copy_in, c->ev_start, 0));
     TQP_CUDA_OK(c, cudaStreamWaitEvent(c->copy_out, c->ev_start, 0));
-    TQP_CUDA_OK(c, cudaMemcpyAsync(X, X_host, row_bytes, cudaMemcpyHostToDevice, c->copy_in));
-    TQP_CUDA_OK(c, cudaEventRecord(c->ev_x, c->copy_in));
+    {
+        const int nch = T >= 1024 ? 4 : 1, per = ((T + nch - 1) / nch + 3) & ~3;   // chunk starts stay 16-byte aligned in every array
+        float *lg = c->p<float>(c->ws.logits);
+        for (int ch = 0; ch < nch; ++ch) {
+            const int t0 = ch * per, tc = std::min(per, T - t0);
+            if (tc <= 0) break;
+            const size_t eo = (size_t)t0 * D.d;
+            TQP_CUDA_OK(c, cudaMemcpyAsync(X + eo, (const bf16 *)X_host + eo, (size_t)tc * D.d * 2, cudaMemcpyHostToDevice, c->copy_in));
+            TQP_CUDA_OK(c, cudaEventRecord(c->ev_xc[ch], c->copy_in));
+            TQP_CUDA_OK(c, cudaStreamWaitEvent(s, c->ev_xc[ch], 0));
+            CK(tqp_route(c, tc, X + eo, W_r, logit_bias, ti + (size_t)t0 * D.k, tw + (size_t)t0 * D.k, lg + (size_t)t0 * D.E, s));
+        }
+    }
     TQP_CUDA_OK(c, cudaMemcpyAsync(dY, dY_host, row_bytes, cudaMemcpyHostToDevice, c->copy_in));
     TQP_CUDA_OK(c, cudaEventRecord(c->ev_dy, c->copy_in));
-    TQP_CUDA_OK(c, cudaStreamWaitEvent(s, c->ev_x, 0));
-    CK(tqp_route(c, T, X, W_r, logit_bias, ti, tw, nullptr, s));
     CK(tqp_dispatch(c, T, ti, counts, offs, perm, inv, s));
     CK(tqp_expert_fwd(c, T, X, offs, perm, Ye, s));
     CK(tqp_combine(c, T, Ye, inv, tw, Y, s));
@@ -518,12 +556,20 @@ tqp_status tqp_step_host(tqp_ctx *c, int T, const void *X_host, const void *dY_h
     TQP_CUDA_OK(c, cudaEventRecord(c->ev_yout, c->copy_out));
     TQP_CUDA_OK(c, cudaStreamWaitEvent(s, c->ev_dy, 0));
     CK(tqp_combine_bwd(c, T, dY, Ye, inv, tw, dYe, dW_r ? dtw : nullptr, s));
-    CK(tqp_expert_bwd(c, T, X, dYe, offs, perm, dXp, dA_gate, dB_gate, dA_up, dB_up, dA_down, dB_down, s));
+    c->defer_tail = 1;
+    st = tqp_expert_bwd(c, T, X, dYe, offs, perm, dXp, dA_gate, dB_gate, dA_up, dB_up, dA_down, dB_down, s);
+    c->defer_tail = 0;
+    total += c->launches;
+    if (st != TQP_OK) { c->tail.pending = false; return st; }
     CK(tqp_dispatch_bwd(c, T, dXp, inv, dX, s));
     if (dW_r) CK(tqp_route_bwd(c, T, X, W_r, ti, tw, dtw, offs, perm, dX, dW_r, s));
+    TQP_CUDA_OK(c, cudaEventRecord(c->ev_dx, s));
+    TQP_CUDA_OK(c, cudaStreamWaitEvent(c->copy_out, c->ev_dx, 0));   // after the Y download on the same copy stream
+    TQP_CUDA_OK(c, cudaMemcpyAsync(dX_host, dX, row_bytes, cudaMemcpyDeviceToHost, c->copy_out));
+    TQP_CUDA_OK(c, cudaEventRecord(c->ev_yout, c->copy_out));
+    CK(expert_bwd_tail(c, s));
 #undef CK
-    TQP_CUDA_OK(c, cudaMemcpyAsync(dX_host, dX, row_bytes, cudaMemcpyDeviceToHost, s));
-    TQP_CUDA_OK(c, cudaStreamWaitEvent(s, c->ev_yout, 0));   // `s` (and its events) now also cover the Y download
+    TQP_CUDA_OK(c, cudaStreamWaitEvent(s, c->ev_yout, 0));   // `s` (and its events) now also cover both downloads
     TQP_CUDA_OK(c, cudaStreamSynchronize(s));
     c->launches = total;
     return TQP_OK;

@@ -93,7 +93,11 @@ struct tqp_ctx {
     int time_gemm = 0;          // bracket GEMM launches with events (tqp_gemm_time)
     // tqp_step_host: copy streams + events so that dY uploads and Y downloads overlap the compute on `stream`
     cudaStream_t copy_in = nullptr, copy_out = nullptr;
-    cudaEvent_t ev_start = nullptr, ev_x = nullptr, ev_dy = nullptr, ev_y = nullptr, ev_yout = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_x = nullptr, ev_dy = nullptr, ev_y = nullptr, ev_yout = nullptr, ev_dx = nullptr;
+    cudaEvent_t ev_xc[4] = {nullptr, nullptr, nullptr, nullptr};   // X arrives in token chunks; the router starts on the first
+    // tqp_step_host defers all adapter weight gradients (nothing else depends on them) until dX is on its way to the host
+    int defer_tail = 0;
+    struct { float *dA_gate, *dB_gate, *dA_up, *dB_up, *dA_down, *dB_down; const tqp::bf16 *dYe; const int32_t *offsets; bool pending; } tail = {};
     std::vector<cudaEvent_t> ev; // pairs (start, stop)
     int ev_used = 0;
     // tensor maps over weights / workspace (built in bind_weights)
