@@ -296,7 +296,7 @@ def run_ours(args, cfg):
         "clocks": sampler.summary(),
         "e2e": e2e,
         "gpu_launches": launches[0] * args.steps,
-        "roofline": {"kernel": "grouped dequant GEMM gemm_tcgen05_ts_kernel (4 launches/step: gate+up, down, dH, dXp)", "bound": "tensor",
+        "roofline": {"kernel": "grouped dequant GEMM gemm_tcgen05_ts2_kernel (4 launches/step: gate+up, down, dH, dXp)", "bound": "tensor",
                      "achieved": gemm_tflops, "peak": pk["tensor_sustained"], "unit": "TFLOP/s",
                      "frac": gemm_tflops / pk["tensor_sustained"], "frac_of_burst": gemm_tflops / pk["tensor_burst"],
                      "frac_of_datasheet_2250": gemm_tflops / 2250.0, "peak_source": pk["source"] + ", sustained bf16",

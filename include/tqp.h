@@ -83,8 +83,9 @@ tqp_status tqp_bind_workspace(tqp_ctx *ctx, void *dev_ptr, size_t bytes, void *s
  * to the bf16 lookup table the GEMM mainloop gathers from.  One-time, untimed; needs a bound workspace. */
 tqp_status tqp_bind_weights(tqp_ctx *ctx, const tqp_weights *w, void *stream);
 /* Options (debug / ablation).  "gemm_impl": 0 = tcgen05 grouped GEMM on CTA pairs with the dequantised weight
- * operand in tensor memory (default), 1 = CUDA-core scaffold, 2 = tcgen05 grouped GEMM, one CTA per tile, weight operand
- * through shared memory, 3 = CTA pairs, weight operand through shared memory.
+ * operand in tensor memory, 128-wide producer stages (default), 1 = CUDA-core scaffold, 2 = tcgen05 grouped GEMM, one
+ * CTA per tile, weight operand through shared memory, 3 = CTA pairs, weight operand through shared memory, 4 = as 0
+ * with 64-wide producer stages.
  * "time_gemm": 0/1, see tqp_gemm_time.  "ablate": bit mask that disables parts of the kernels (results become
  * wrong; timing experiments only; 0 = off).  "trace": n > 0 records a clock64 timeline of one CTA pair in the n-th
  * grouped-GEMM launch from now into the workspace tensor "trace" (tqp_debug_buffer). */

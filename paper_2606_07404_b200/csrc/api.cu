@@ -138,7 +138,8 @@ tqp_status run_gemm(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_
     tqp_status r = c->gemm_impl == 1   ? launch_gemm_scaffold(c, probs, nprob, st)
                    : c->gemm_impl == 2 ? launch_gemm_tcgen05(c, probs, nprob, st)
                    : c->gemm_impl == 3 ? launch_gemm_tcgen05_2cta(c, probs, nprob, st)
-                                       : launch_gemm_tcgen05_ts(c, probs, nprob, st);   // falls back to 2cta for MN-major
+                   : c->gemm_impl == 4 ? launch_gemm_tcgen05_ts(c, probs, nprob, st)
+                                       : launch_gemm_tcgen05_ts2(c, probs, nprob, st);
     if (timed) {
         TQP_CUDA_OK(c, cudaEventRecord(c->ev[c->ev_used + 1], st));
         c->ev_used += 2;
@@ -274,7 +275,7 @@ tqp_status tqp_bind_weights(tqp_ctx *c, const tqp_weights *w, void *stream) {
 tqp_status tqp_set_option(tqp_ctx *c, const char *name, int value) {
     if (!c || !name) return TQP_ERR_ARG;
     if (!strcmp(name, "gemm_impl")) {
-        REQ(c, value >= 0 && value <= 3, TQP_ERR_ARG, "gemm_impl must be 0..3");
+        REQ(c, value >= 0 && value <= 4, TQP_ERR_ARG, "gemm_impl must be 0..4");
         c->gemm_impl = value;
         return TQP_OK;
     }

@@ -164,7 +164,8 @@ tqp_status launch_rows_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 
 tqp_status launch_gemm_scaffold(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);
 tqp_status launch_gemm_tcgen05(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);       // 1 CTA / tile
 tqp_status launch_gemm_tcgen05_2cta(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);  // CTA pair / tile
-tqp_status launch_gemm_tcgen05_ts(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);    // CTA pair, A in TMEM (K-major only)
+tqp_status launch_gemm_tcgen05_ts(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);
+tqp_status launch_gemm_tcgen05_ts2(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);   // ... 128-wide A stages    // CTA pair, A in TMEM (K-major only)
 
 // ---- device helpers ------------------------------------------------------------------------------------
 __device__ __forceinline__ float bf16_bits_to_float(uint16_t b) { return __uint_as_float(((uint32_t)b) << 16); }

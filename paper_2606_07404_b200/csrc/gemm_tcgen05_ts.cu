@@ -283,7 +283,7 @@ gemm_tcgen05_ts_kernel(const __grid_constant__ GemmArgs args, const uint4 *__res
                             const uint32_t c01[2] = {codes.x, codes.y};
 #pragma unroll
                             for (int j = 0; j < 8; ++j) {
-                                const uint32_t code = (c01[j >> 2] >> ((j & 3) * 8)) & 0xffu;
+                                const uint32_t code = __byte_perm(c01[j >> 2], 0, 0x4440 | (j & 3));   // one PRMT
                                 uint4 v = (ablate & 1) ? make_uint4(code, code, code, code) : lds128(lut_a + code * 128);
                                 __nv_bfloat162 *pv = reinterpret_cast<__nv_bfloat162 *>(&v);
 #pragma unroll

@@ -1,0 +1,469 @@
+// Grouped dequant GEMM on CTA pairs with the weight operand in TENSOR MEMORY, 128-wide A stages (sm_100a) -- the default.
+//
+//   out[p][m] = sum_seg sum_k act_seg[p][k] * W_seg[m][k]  +  sum_l lact_l[p][q] * lw_l[m][q]
+//   W[m][k] = bf16( bf16(codebook[code]) * bf16(scale) )                      (look up, rescale by the norm)
+//
+// Mapping, operands and epilogue are those of gemm_tcgen05_ts.cu (swap-AB: UMMA M = 256 weight output channels over two
+// SMs, N = routed rows of one expert; dequantised A tile written to TMEM with tcgen05.st -- row-wise by the channel's own
+// thread in the forward GEMMs, through movmatrix in the backward GEMMs; activations by TMA; one 256-column accumulator
+// drained into a bf16 staging tile).  What differs is the granularity of the producer hand-shake: one A stage is 128 k
+// (one code-index tile, 64 TMEM columns, two 64-wide activation stages), so the fixed cost per hand-shake (index-tile
+// wait, slot wait, tcgen05.wait::st, fence, remote arrive: ~400 of the ~1000 clk a backward producer spent per 64 k) is
+// paid half as often.  The backward GEMMs were producer-bound at ~600 clk per 64 k against ~455 clk of MMA issue.
+// TMEM: accumulator [0, 256) + 3 A slots of 64 columns.  Barriers: fullB/emptyB per activation stage (TMA <-> MMA),
+// fullA/emptyA per A slot (dequant warps <-> MMA), index ring, accumulator full/empty.
+//
+// Warp roles per CTA (480 threads, 1 CTA/SM, persistent over work items, cluster = 2 CTAs):
+//   warp 0  TMA producer of the activation / adapter-projection tiles (signals the LEADER's barrier)
+//   warp 1  MMA issuer (leader CTA only, one elected lane) + TMEM allocation
+//   warp 2  TMA producer of the code-index tiles
+//   warps 3-10  dequant producers, two groups of four that alternate A stages
+//   warps 11-14 epilogue (TMEM -> registers -> bf16 -> staging tile -> 16-byte global stores)
+#include "common.cuh"
+#include "tc_ptx.cuh"
+
+namespace tqp {
+namespace gt2 {
+using namespace ptx;
+
+constexpr int BM = 128, BK = 64, TN = kTileRows, HN = kTileRows / 2;
+constexpr int AK = 128;                                   // K of one A stage (one index tile, one producer hand-shake) = two B stages
+constexpr int NSTAGE = 6, NASLOT = 3, IDXQ = 8;           // B (activation) ring, A (weight) slots of 64 TMEM columns, index ring
+constexpr int X_BYTES = HN * 128, IDX_BYTES = 128 * 16, LUT_BYTES = 256 * 8 * 16;
+constexpr int OFF_X = 0, OFF_LUT = OFF_X + NSTAGE * X_BYTES, OFF_IDX = OFF_LUT + LUT_BYTES,
+              OFF_BAR = OFF_IDX + IDXQ * IDX_BYTES, OFF_EPI = OFF_BAR + 512;
+constexpr int EPI_ROWS = 32, EPI_BYTES = TN * BM * 2;      // staging: the whole [256 rows][128 channels] bf16 output tile
+constexpr int SMEM_BYTES = OFF_EPI + EPI_BYTES + 1024;
+constexpr int NTHREADS = 480;
+constexpr int W_DEQ0 = 3, W_EPI0 = 11;
+constexpr int TM_ACC = 0, TM_A = TN;                      // TMEM columns: accumulator [0, 256), A slots [256, 256 + 64 NASLOT)
+
+struct Item {
+    Tile t;
+    int prob, m0;
+};
+
+// 32 consecutive 32-bit TMEM columns of this thread's lane
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t *v) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
+        "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};" ::"r"(taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]), "r"(v[10]),
+        "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]),
+        "r"(v[21]), "r"(v[22]), "r"(v[23]), "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]),
+        "r"(v[31])
+        : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t *v) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]), "r"(v[10]),
+        "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
+        : "memory");
+}
+
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
+gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__restrict__ lut_g, const Tile *__restrict__ tiles,
+                        const int32_t *__restrict__ num_tiles_p, int ablate) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    const uint32_t sbase = smem_u32(smem);
+    const uint32_t bar0 = sbase + OFF_BAR;
+    auto fullB = [&](int s) { return bar0 + 8u * s; };                               // the LEADER's: expect_tx + 2 x X_BYTES of TMA
+    auto emptyB = [&](int s) { return bar0 + 8u * (NSTAGE + s); };                   // local, multicast commit
+    auto fullA = [&](int s) { return bar0 + 8u * (2 * NSTAGE + s); };                // the LEADER's: 8 dequant-warp arrivals
+    auto emptyA = [&](int s) { return bar0 + 8u * (2 * NSTAGE + NASLOT + s); };      // local, multicast commit
+    auto idx_full = [&](int s) { return bar0 + 8u * (2 * NSTAGE + 2 * NASLOT + s); };            // local
+    auto idx_empty = [&](int s) { return bar0 + 8u * (2 * NSTAGE + 2 * NASLOT + IDXQ + s); };    // local, the owning group's 4 warps
+    const uint32_t tmem_full = bar0 + 8u * (2 * NSTAGE + 2 * NASLOT + 2 * IDXQ);       // local, multicast commit
+    const uint32_t tmem_empty = bar0 + 8u * (2 * NSTAGE + 2 * NASLOT + 2 * IDXQ + 1);  // the leader's is used
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + OFF_BAR + 8 * (2 * NSTAGE + 2 * NASLOT + 2 * IDXQ + 4));
+
+    const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+    const uint32_t rank = cluster_ctarank();
+    const uint32_t fullB_remote = mapa(fullB(0), 0), fullA_remote = mapa(fullA(0), 0), tmem_empty_remote = mapa(tmem_empty, 0);
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NSTAGE; ++s) { mbar_init(fullB(s), 1); mbar_init(emptyB(s), 1); }
+        for (int s = 0; s < NASLOT; ++s) { mbar_init(fullA(s), 8); mbar_init(emptyA(s), 1); }
+        for (int s = 0; s < IDXQ; ++s) { mbar_init(idx_full(s), 1); mbar_init(idx_empty(s), 4); }
+        mbar_init(tmem_full, 1);
+        mbar_init(tmem_empty, 8);
+        mbar_init_fence();
+    }
+    if (warp == 1) tmem_alloc<2>(smem_u32(tmem_slot), 512);
+    {   // replicated LUT: entry e, copy c at (e*8 + c) * 16 B  ->  lane c of every quarter-warp hits bank group c
+        uint4 *lut_s = reinterpret_cast<uint4 *>(smem + OFF_LUT);
+        for (int i = threadIdx.x; i < 256 * 8; i += NTHREADS) lut_s[i] = lut_g[i >> 3];
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync();   // both CTAs' barriers are initialised before any remote arrive / TMA completion
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    const int num_tiles = *num_tiles_p;
+    const int nprob = args.nprob;
+    const int MTP = args.p[0].M / (2 * BM);
+    const long long total = (long long)num_tiles * nprob * MTP;
+    const int cid = blockIdx.x >> 1, ncl = gridDim.x >> 1;
+
+    auto get_item = [&](long long item, Item &it) {
+        const int tile_id = (int)(item / (nprob * MTP)), rem = (int)(item % (nprob * MTP));
+        it.t = tiles[tile_id];
+        it.prob = rem / MTP;
+        it.m0 = ((rem % MTP) * 2 + (int)rank) * BM;
+    };
+
+    if (warp == 0) {
+        // =========================== activation TMA producer ===========================
+        if (lane == 0) {
+            Pipe st;
+            for (long long item = cid; item < total; item += ncl) {
+                Item it;
+                get_item(item, it);
+                if (it.t.rows <= 0) continue;
+                const GemmProblem &pb = args.p[it.prob];
+                const int n = max(16, (it.t.rows + 15) & ~15);
+                const int row = it.t.row0 + (int)rank * (n >> 1);
+                for (int sg = 0; sg < pb.nseg; ++sg) {
+                    const GemmSeg &S = pb.seg[sg];
+                    const int nkb = S.K / BK;
+                    for (int kb = 0; kb < nkb; ++kb) {
+                        mbar_wait(emptyB(st.s), st.ph ^ 1);
+                        if (rank == 0) mbar_expect_tx(fullB(st.s), 2 * X_BYTES);
+                        tma_load_2d_pair(sbase + OFF_X + st.s * X_BYTES, &S.act_map2, kb * BK, row, fullB_remote + 8u * st.s);
+                        st.next(NSTAGE);
+                    }
+                }
+                for (int l = 0; l < pb.nlora; ++l) {
+                    mbar_wait(emptyB(st.s), st.ph ^ 1);
+                    if (rank == 0) mbar_expect_tx(fullB(st.s), 2 * X_BYTES);
+                    tma_load_2d_pair(sbase + OFF_X + st.s * X_BYTES, &pb.lora[l].lact_map2, 0, row, fullB_remote + 8u * st.s);
+                    st.next(NSTAGE);
+                }
+            }
+        }
+    } else if (warp == 2) {
+        // =========================== code-index TMA producer ===========================
+        if (lane == 0) {
+            Pipe iq;
+            for (long long item = cid; item < total; item += ncl) {
+                Item it;
+                get_item(item, it);
+                if (it.t.rows <= 0) continue;
+                const GemmProblem &pb = args.p[it.prob];
+                for (int sg = 0; sg < pb.nseg; ++sg) {
+                    const GemmSeg &S = pb.seg[sg];
+                    const int nka = S.K / AK;
+                    for (int ka = 0; ka < nka; ++ka) {   // K-major: [128 channels][16 codes]; MN-major: [128 k][16 channel groups]
+                        mbar_wait(idx_empty(iq.s), iq.ph ^ 1);
+                        mbar_expect_tx(idx_full(iq.s), IDX_BYTES);
+                        const int c0 = S.kmajor ? ka * 16 : it.m0 / 8;
+                        const int c1 = S.kmajor ? it.t.expert * pb.M + it.m0 : it.t.expert * S.K + ka * AK;
+                        tma_load_2d(sbase + OFF_IDX + iq.s * IDX_BYTES, &S.idx_map, c0, c1, idx_full(iq.s));
+                        iq.next(IDXQ);
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // =========================== MMA issuer (leader CTA) ===========================
+        if (rank == 0 && elect_one()) {
+            Pipe st, sa;
+            int cnt = 0;
+            const uint32_t hi_k = desc_hi(1024), lo_k = desc_lo_const(16);          // K-major SW128: SBO = 8 rows x 128 B
+            const uint32_t x16 = (sbase + OFF_X) >> 4;
+            for (long long item = cid; item < total; item += ncl) {
+                Item it;
+                get_item(item, it);
+                if (it.t.rows <= 0) continue;
+                const GemmProblem &pb = args.p[it.prob];
+                const uint32_t aph = cnt & 1;
+                ++cnt;
+                const int n = max(16, (it.t.rows + 15) & ~15);
+                mbar_wait<true>(tmem_empty, aph ^ 1);   // the epilogue has drained the previous item's accumulator
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + TM_ACC;
+                const uint32_t idesc = make_idesc(2 * BM, n, 0);
+                uint32_t accum = 0;
+                int nka = 0;
+                for (int sg = 0; sg < pb.nseg; ++sg) nka += pb.seg[sg].K / AK;
+                const int nmma_l = max(1, pb.r / 16);
+                for (int ja = 0; ja < nka + pb.nlora; ++ja) {
+                    const bool lora = ja >= nka;
+                    mbar_wait<true>(fullA(sa.s), sa.ph);
+                    const uint32_t a_tmem = tmem_base + TM_A + sa.s * 64;
+                    for (int h = 0; h < (lora ? 1 : 2); ++h) {
+                        mbar_wait<true>(fullB(st.s), st.ph);
+                        tc_fence_after();
+                        const uint32_t xs = x16 + st.s * (X_BYTES >> 4);
+                        if (!lora) {
+#pragma unroll
+                            for (int kk = 0; kk < BK / 16; ++kk) {
+                                umma_bf16_ts<2>(d_tmem, a_tmem + h * 32 + kk * 8, desc_from(hi_k, lo_k, xs + kk * 2), idesc, accum);
+                                accum = 1;
+                            }
+                        } else {
+                            for (int kk = 0; kk < nmma_l; ++kk) {
+                                umma_bf16_ts<2>(d_tmem, a_tmem + kk * 8, desc_from(hi_k, lo_k, xs + kk * 2), idesc, accum);
+                                accum = 1;
+                            }
+                        }
+                        umma_commit_pair(emptyB(st.s), 3);
+                        st.next(NSTAGE);
+                    }
+                    umma_commit_pair(emptyA(sa.s), 3);
+                    sa.next(NASLOT);
+                }
+                umma_commit_pair(tmem_full, 3);
+            }
+        }
+    } else if (warp >= W_DEQ0 && warp < W_EPI0) {
+        // =========================== dequant producers: 2 groups x 128 threads ===========================
+        // A stage ja (128 k, counted over the whole run of this cluster) belongs to group ja % 2 and to A slot ja % 3.
+        const int g = (warp - W_DEQ0) >> 2;
+        const int row = (warp & 3) * 32 + lane;                       // K-major: this thread's channel = its TMEM lane
+        const uint32_t lut_a = sbase + OFF_LUT + (lane & 7) * 16;
+        const uint32_t a_lane = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + TM_A;
+        const int rk = lane >> 2, jj = lane & 3;                       // MN-major: source row / channel pair of a movmatrix block
+        const int kofs = 4 * (rk >> 1) + (rk & 1);
+        const uint32_t lut_b = sbase + OFF_LUT + rk * 16 + jj * 4;   // replica rk: all 32 lanes hit distinct banks
+        Pipe sa, iq;
+        int ja = 0;
+        auto wait_slot_free = [&]() {   // MMAs of the previous use of this A slot have completed
+            mbar_wait(emptyA(sa.s), sa.ph ^ 1);
+            tc_fence_after();
+        };
+        auto publish = [&]() {          // the A stage is in TMEM: tell the MMA issuer (the leader CTA's barrier)
+            tmem_st_wait();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(fullA_remote + 8u * sa.s);
+        };
+        for (long long item = cid; item < total; item += ncl) {
+            Item it;
+            get_item(item, it);
+            if (it.t.rows <= 0) continue;
+            const GemmProblem &pb = args.p[it.prob];
+            const int m0 = it.m0, M = pb.M, e = it.t.expert;
+            int nka_tot = 0;
+            for (int sg = 0; sg < pb.nseg; ++sg) nka_tot += pb.seg[sg].K / AK;
+            // adapter row of this channel for the item's last K-step(s): fetched now, consumed after the k-loop
+            const int r = pb.r;
+            uint32_t ch[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) ch[j] = 0;
+            for (int l = 0; l < pb.nlora; ++l) {
+                if (((ja + nka_tot + l) & 1) == g) {
+                    const GemmLora &L = pb.lora[l];
+                    if (L.mk_layout) {
+                        const uint4 *src = reinterpret_cast<const uint4 *>(L.lw + ((size_t)e * M + m0 + row) * r);
+                        for (int j = 0; j < r / 8; ++j) *reinterpret_cast<uint4 *>(&ch[4 * j]) = src[j];
+                    } else {
+                        const bf16 *src = L.lw + (size_t)e * r * M + m0 + row;
+                        uint16_t *h = reinterpret_cast<uint16_t *>(ch);
+                        for (int q = 0; q < r; ++q) h[q] = *reinterpret_cast<const uint16_t *>(src + (size_t)q * M);
+                    }
+                }
+            }
+            for (int sg = 0; sg < pb.nseg; ++sg) {
+                const GemmSeg &S = pb.seg[sg];
+                const int nka = S.K / AK;
+                if (S.kmajor) {
+                    // ---- forward: codes run along k; this thread owns TMEM lane `row` and writes its 128 k-values itself
+                    const __nv_bfloat162 s2 = __float2bfloat162_rn(__half2float(S.scale[(size_t)e * M + m0 + row]));
+                    for (int ka = 0; ka < nka; ++ka) {
+                        const bool own = (ja & 1) == g;
+                        uint4 codes = make_uint4(0, 0, 0, 0);
+                        if (own) {   // one index tile = 16 codes per channel = this A stage
+                            mbar_wait(idx_full(iq.s), iq.ph);
+                            codes = lds128(sbase + OFF_IDX + iq.s * IDX_BYTES + row * 16);
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(idx_empty(iq.s));
+                        }
+                        iq.next(IDXQ);
+                        if (own) {
+                            const uint32_t cwd[4] = {codes.x, codes.y, codes.z, codes.w};
+#pragma unroll
+                            for (int h = 0; h < 2; ++h) {
+                                uint32_t a[32];   // 64 bf16 of this channel's row = 32 TMEM columns
+#pragma unroll
+                                for (int j = 0; j < 8; ++j) {
+                                    const uint32_t code = __byte_perm(cwd[2 * h + (j >> 2)], 0, 0x4440 | (j & 3));   // one PRMT
+                                    uint4 v = lds128(lut_a + code * 128);
+                                    __nv_bfloat162 *pv = reinterpret_cast<__nv_bfloat162 *>(&v);
+#pragma unroll
+                                    for (int q = 0; q < 4; ++q) pv[q] = __hmul2(pv[q], s2);
+                                    a[4 * j] = v.x; a[4 * j + 1] = v.y; a[4 * j + 2] = v.z; a[4 * j + 3] = v.w;
+                                }
+                                if (h == 0) wait_slot_free();
+                                tmem_st32(a_lane + sa.s * 64 + h * 32, a);
+                            }
+                            publish();
+                        }
+                        sa.next(NASLOT);
+                        ++ja;
+                    }
+                } else {
+                    // ---- backward: codes run along the OUTPUT channels; one codebook row holds 8 channels of one k.
+                    // Thread t = (rk = t / 4, jj = t % 4) gathers 4-byte pieces (2 channels) of the rows of its k-values, and
+                    // movmatrix turns each 8 (k) x 8 (channel) block into the accumulator-fragment layout of
+                    // tcgen05.st.16x256b: lane = channel, register = k pair.  Source row rk of a block carries
+                    // k = 16 x + 4 (rk / 2) + rk % 2 + 2 i, so that the transposed pairs land in TMEM columns 8 x + 2 jj + i.
+                    uint32_t cw[16];             // code words (4 channel groups each) of this thread's 16 k-values of its A stage
+                    __nv_bfloat162 sc[16];       // and their per-k scales (the weight's output channel is k here)
+                    __half sraw[16];             // raw scales of this group's NEXT A stage: fetched one own-stage ahead
+                    const __half *scp = S.scale + (size_t)e * S.K + kofs;
+                    {
+                        const int ka0 = ((ja & 1) == g) ? 0 : 1;
+                        if (ka0 < nka) {
+#pragma unroll
+                            for (int z = 0; z < 16; ++z) sraw[z] = scp[ka0 * AK + (z >> 3) * 64 + ((z >> 1) & 3) * 16 + (z & 1) * 2];
+                        }
+                    }
+                    for (int ka = 0; ka < nka; ++ka) {
+                        const bool own = (ja & 1) == g;
+                        if (own) {   // one index tile = 128 k x 16 channel groups = this A stage
+                            mbar_wait(idx_full(iq.s), iq.ph);
+                            const uint32_t is = sbase + OFF_IDX + iq.s * IDX_BYTES + kofs * 16 + (warp & 3) * 4;
+#pragma unroll
+                            for (int z = 0; z < 16; ++z) {   // z = 8 h + 2 x + i  ->  k = 64 h + 16 x + kofs + 2 i
+                                cw[z] = lds32(is + ((z >> 3) * 64 + ((z >> 1) & 3) * 16 + (z & 1) * 2) * 16);
+                                sc[z] = __float2bfloat162_rn(__half2float(sraw[z]));
+                            }
+                            if (ka + 2 < nka) {
+#pragma unroll
+                                for (int z = 0; z < 16; ++z) sraw[z] = scp[(ka + 2) * AK + (z >> 3) * 64 + ((z >> 1) & 3) * 16 + (z & 1) * 2];
+                            }
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(idx_empty(iq.s));
+                        }
+                        iq.next(IDXQ);
+                        if (own) {
+#pragma unroll
+                            for (int h = 0; h < 2; ++h) {
+#pragma unroll
+                                for (int hs = 0; hs < 2; ++hs) {   // lanes +0..15 / +16..31 of this warp's quadrant
+                                    uint32_t rg[16];
+#pragma unroll
+                                    for (int x = 0; x < 4; ++x)
+#pragma unroll
+                                        for (int i = 0; i < 2; ++i)
+#pragma unroll
+                                            for (int mbi = 0; mbi < 2; ++mbi) {
+                                                const int z = 8 * h + 2 * x + i;
+                                                const uint32_t code = __byte_perm(cw[z], 0, 0x4440 | (2 * hs + mbi));   // one PRMT
+                                                uint32_t v = lds32(lut_b + code * 128);
+                                                __nv_bfloat162 w2 = __hmul2(*reinterpret_cast<__nv_bfloat162 *>(&v), sc[z]);
+                                                rg[4 * x + 2 * mbi + i] = movmatrix_t(*reinterpret_cast<uint32_t *>(&w2));
+                                            }
+                                    if (h == 0 && hs == 0) wait_slot_free();
+                                    tmem_st_16x256b_x4(a_lane + ((uint32_t)(16 * hs) << 16) + sa.s * 64 + h * 32, rg);
+                                }
+                            }
+                            publish();
+                        }
+                        sa.next(NASLOT);
+                        ++ja;
+                    }
+                }
+            }
+            for (int l = 0; l < pb.nlora; ++l) {
+                if ((ja & 1) == g) {
+                    wait_slot_free();
+                    tmem_st16(a_lane + sa.s * 64, ch);   // columns beyond r/2 are zero
+                    publish();
+                }
+                sa.next(NASLOT);
+                ++ja;
+            }
+        }
+    } else if (warp >= W_EPI0) {
+        // =========================== epilogue (128 threads) ===========================
+        // Drain: TMEM (lane = output channel, column = routed row) -> registers in the fragment layout -> bf16 ->
+        // stmatrix.trans into the [rows][128 channels] staging tile (16-byte chunks XOR-swizzled by row); the
+        // accumulator is handed back to the MMA issuer as soon as it has been read.  Then 16-byte coalesced global
+        // stores (a half-warp writes one 256-byte row segment) overlap the next item's mainloop.
+        const int q = warp & 3;             // TMEM lane quadrant this warp may access
+        const int et = threadIdx.x - W_EPI0 * 32;
+        const uint32_t ebuf = sbase + OFF_EPI;
+        int cnt = 0;
+        for (long long item = cid; item < total; item += ncl) {
+            Item it;
+            get_item(item, it);
+            if (it.t.rows <= 0) continue;
+            const GemmProblem &pb = args.p[it.prob];
+            const int M = pb.M;
+            const uint32_t aph = cnt & 1;
+            ++cnt;
+            mbar_wait(tmem_full, aph);
+            tc_fence_after();
+            named_bar_sync(1, 128);   // every epilogue warp has finished storing the previous item out of the staging tile
+            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + TM_ACC;
+            for (int c0 = 0; c0 < it.t.rows; c0 += EPI_ROWS) {
+                uint32_t v[2][16];
+                tmem_ld_16x256b_x4(taddr + c0, v[0]);
+                tmem_ld_16x256b_x4(taddr + (16u << 16) + c0, v[1]);
+                tmem_ld_wait();
+#pragma unroll
+                for (int g8 = 0; g8 < 4; ++g8) {   // 8 routed rows per stmatrix.x4: channels 8j..8j+7 of this warp, j = lane/8
+                    const int tok = c0 + g8 * 8 + (lane & 7);
+                    const uint32_t addr = ebuf + tok * (BM * 2) + (((q * 4 + (lane >> 3)) ^ (tok & 7)) << 4);
+                    stsm_x4_t(addr, float2_to_bf16x2(__uint_as_float(v[0][4 * g8]), __uint_as_float(v[0][4 * g8 + 1])),
+                              float2_to_bf16x2(__uint_as_float(v[0][4 * g8 + 2]), __uint_as_float(v[0][4 * g8 + 3])),
+                              float2_to_bf16x2(__uint_as_float(v[1][4 * g8]), __uint_as_float(v[1][4 * g8 + 1])),
+                              float2_to_bf16x2(__uint_as_float(v[1][4 * g8 + 2]), __uint_as_float(v[1][4 * g8 + 3])));
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(tmem_empty_remote);
+            named_bar_sync(1, 128);   // staging tile complete
+            if (!(ablate & 16)) {
+                bf16 *outp = pb.out + (size_t)it.t.row0 * M + it.m0;
+                for (int r = et / 16; r < it.t.rows; r += 8) {
+                    const int chk = et % 16;
+                    const uint4 val = lds128(ebuf + r * (BM * 2) + ((chk ^ (r & 7)) << 4));
+                    *reinterpret_cast<uint4 *>(outp + (size_t)r * M + chk * 8) = val;
+                }
+            }
+        }
+    }
+
+    __syncwarp();
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync();   // the peer may still read this CTA's smem / signal its barriers until both are done
+    if (warp == 1) {
+        tc_fence_after();
+        tmem_dealloc<2>(tmem_base, 512);
+    }
+}
+
+}  // namespace gt2
+
+tqp_status launch_gemm_tcgen05_ts2(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st) {
+    for (int i = 0; i < nprob; ++i) {   // an even number of 128-channel tiles and whole 128-wide A stages per segment
+        const GemmProblem &p = probs[i];
+        bool ok = p.M % (2 * gt2::BM) == 0 && p.nlora <= 2;
+        for (int sg = 0; sg < p.nseg; ++sg) ok = ok && p.seg[sg].K % gt2::AK == 0;
+        if (!ok) return launch_gemm_tcgen05_2cta(c, probs, nprob, st);
+    }
+    static bool attr_set = false;
+    if (!attr_set) {
+        TQP_CUDA_OK(c, cudaFuncSetAttribute(gt2::gemm_tcgen05_ts2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, gt2::SMEM_BYTES));
+        attr_set = true;
+    }
+    GemmArgs args;
+    for (int i = 0; i < nprob; ++i) args.p[i] = probs[i];
+    args.nprob = nprob;
+    const int grid = (c->num_sms / 2) * 2;
+    gt2::gemm_tcgen05_ts2_kernel<<<grid, gt2::NTHREADS, gt2::SMEM_BYTES, st>>>(
+        args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), c->ablate);
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
+
+}  // namespace tqp

@@ -57,7 +57,8 @@ def test_cfg0_tiny_full_chain(gemm_impl):
     check_all(inp, backward=True, router_grad=True, gemm_impl=gemm_impl)
 
 
-@pytest.mark.parametrize("gemm_impl", [1, 2, 3, 0], ids=["scaffold", "tcgen05_1cta", "tcgen05_2cta_smemA", "tcgen05"])
+@pytest.mark.parametrize("gemm_impl", [1, 2, 3, 4, 0],
+                         ids=["scaffold", "tcgen05_1cta", "tcgen05_2cta_smemA", "tcgen05_tmemA_64", "tcgen05"])
 @pytest.mark.parametrize("cfg", [MID, MID32], ids=lambda c: c.name)
 def test_mid_ragged_multi_tile(cfg, gemm_impl):
     inp = _skewed(cfg)
