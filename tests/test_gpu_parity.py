@@ -160,3 +160,20 @@ def test_layer_reuse_smaller_batch_and_foreign_dYe():
     assert_close("dX_experts", to_np(dX), ref["dX_experts"])
     for key in ("dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down"):
         assert_close(key, to_np(grads[key]), ref[key])
+
+
+EDGE = [
+    ti.Config("edge_T1", T=1, d=128, F=128, E=4, k=2, r=16, seed=31),   # 2 dot products: dtopk_w too ill-conditioned to compare
+    ti.Config("edge_k_eq_E", T=37, d=256, F=128, E=4, k=4, r=16, seed=32, router_grad=True),
+    ti.Config("edge_E1", T=50, d=128, F=256, E=1, k=1, r=32, seed=33, router_grad=True),
+    ti.Config("edge_k1_many_empty", T=9, d=128, F=128, E=64, k=1, r=16, seed=34, router_grad=True),
+    ti.Config("edge_max_E_k", T=96, d=128, F=128, E=1024, k=32, r=16, seed=35, router_grad=True),   # API maxima of E and k
+]
+
+
+@pytest.mark.parametrize("cfg", EDGE, ids=lambda c: c.name)
+def test_degenerate_shapes(cfg):
+    """A single token, k = E (every expert selected, softmax over all logits), one expert, and far more experts than
+    assignments (most experts empty): full chain against the oracle."""
+    inp = ti.make_inputs(cfg)
+    check_all(inp, backward=True, router_grad=cfg.router_grad, gemm_impl=0)
