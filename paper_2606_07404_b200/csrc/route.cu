@@ -12,14 +12,17 @@ namespace tqp {
 // 430 CTAs at T = 8192, E = 460: one wave of 3 CTAs per SM on 148 SMs with 97 % of the slots filled (64-token tiles
 // gave 640 CTAs on 740 slots: 4 or 5 per SM, 86 %).  Bound: fp32 FMA issue rate (R1 forbids tensor cores and any
 // re-association of the sum).
-constexpr int RT_TM = 12, RT_EN = 6;                       // per-thread tile
-constexpr int RT_TOK = 8 * RT_TM, RT_EXP = 16 * RT_EN, RT_K = 32, RT_XLD = RT_TOK;   // 96 floats per row: transposed stores and broadcast loads are conflict-free unpadded
-constexpr int RT_XCH = RT_TOK * RT_K / 8 / 128;            // 16-byte X chunks per thread per K-chunk
-constexpr int RT_WCH = RT_K * RT_EXP / 4 / 128;            // 16-byte W_r chunks per thread per K-chunk
+// A second instantiation (4 x 4 per thread: 32 tokens x 64 experts per CTA) serves small problems, where the large tile
+// would leave most SMs idle (configs[1]: T = 4096, E = 64 -> 43 large CTAs on 148 SMs, 148 us; 128 small CTAs: see DESIGN).
+constexpr int RT_K = 32;
 
+template <int RT_TM, int RT_EN>   // per-thread tile: RT_TM tokens x RT_EN experts; 8 x 16 threads per CTA
 __global__ void __launch_bounds__(128, 3) route_logits_kernel(const bf16 *__restrict__ X, const float *__restrict__ W_r,
                                                               const float *__restrict__ bias, float *__restrict__ logits,
                                                               int T, int d, int E) {
+    constexpr int RT_TOK = 8 * RT_TM, RT_EXP = 16 * RT_EN, RT_XLD = RT_TOK;   // unpadded rows: transposed stores and broadcast loads are conflict-free
+    constexpr int RT_XCH = (RT_TOK * RT_K / 8 + 127) / 128;    // 16-byte X chunks per thread per K-chunk
+    constexpr int RT_WCH = RT_K * RT_EXP / 4 / 128;            // 16-byte W_r chunks per thread per K-chunk
     __shared__ __align__(16) float xs[2][RT_K][RT_XLD];   // [buf][i][token]
     __shared__ __align__(16) float wsm[2][RT_K][RT_EXP];  // [buf][i][expert]
     const int tid = threadIdx.x;
@@ -39,8 +42,8 @@ __global__ void __launch_bounds__(128, 3) route_logits_kernel(const bf16 *__rest
     for (int j = 0; j < RT_XCH; ++j) {
         const int v = tid + 128 * j;
         xtok[j] = v % RT_TOK;
-        xseg[j] = v / RT_TOK;
-        xsrc[j] = (t0 + xtok[j] < T) ? X + (size_t)(t0 + xtok[j]) * d + xseg[j] * 8 : nullptr;
+        xseg[j] = v / RT_TOK;   // segments past the K-chunk (small tile: fewer chunks than threads) load nothing
+        xsrc[j] = (xseg[j] < RT_K / 8 && t0 + xtok[j] < T) ? X + (size_t)(t0 + xtok[j]) * d + xseg[j] * 8 : nullptr;
     }
     // W_r tile: 32 i x 96 experts (fp32) = 768 chunks of 4 values; chunk v: row v / 24, experts 4 (v % 24) ..
     const float *wsrc[RT_WCH];
@@ -60,6 +63,7 @@ __global__ void __launch_bounds__(128, 3) route_logits_kernel(const bf16 *__rest
     auto store_x = [&](int buf) {
 #pragma unroll
         for (int j = 0; j < RT_XCH; ++j) {
+            if (xseg[j] >= RT_K / 8) continue;
             const uint32_t *r = reinterpret_cast<const uint32_t *>(&xr[j]);
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
@@ -256,11 +260,21 @@ __global__ void bias_update_kernel(const int32_t *__restrict__ counts, float *__
     }
 }
 
+// Picks the tile: the large one (96 x 96) unless it cannot fill the SMs (few tokens or few experts).
+static void launch_logits(const bf16 *X, const float *W_r, const float *bias, float *logits, int T, int d, int E, int num_sms,
+                          cudaStream_t s) {
+    const long big = (long)((T + 95) / 96) * ((E + 95) / 96);
+    if (big >= 2L * num_sms) {
+        route_logits_kernel<12, 6><<<dim3((T + 95) / 96, (E + 95) / 96), 128, 0, s>>>(X, W_r, bias, logits, T, d, E);
+    } else {
+        route_logits_kernel<4, 4><<<dim3((T + 31) / 32, (E + 63) / 64), 128, 0, s>>>(X, W_r, bias, logits, T, d, E);
+    }
+}
+
 tqp_status launch_route_sigmoid(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const float *select_bias, int32_t *topk_idx,
                                 float *topk_w, float *topk_s, float *logits, cudaStream_t s) {
     const int d = c->desc.d, E = c->desc.E, k = c->desc.k;
-    dim3 grid((T + RT_TOK - 1) / RT_TOK, (E + RT_EXP - 1) / RT_EXP);
-    route_logits_kernel<<<grid, 128, 0, s>>>(X, W_r, nullptr, logits, T, d, E);
+    launch_logits(X, W_r, nullptr, logits, T, d, E, c->num_sms, s);
     TQP_LAUNCH_OK(c);
 #define TQP_TOPK(P) route_topk_sigmoid_kernel<P><<<(T + 3) / 4, 128, 0, s>>>(logits, select_bias, topk_idx, topk_w, topk_s, T, E, k)
     if (E <= 64) TQP_TOPK(2); else if (E <= 128) TQP_TOPK(4); else if (E <= 256) TQP_TOPK(8); else if (E <= 512) TQP_TOPK(16); else TQP_TOPK(32);
@@ -279,8 +293,7 @@ tqp_status launch_bias_update(tqp_ctx *c, const int32_t *counts, float *bias, in
 tqp_status launch_route(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const float *bias, int32_t *topk_idx,
                         float *topk_w, float *logits, cudaStream_t s) {
     const int d = c->desc.d, E = c->desc.E, k = c->desc.k;
-    dim3 grid((T + RT_TOK - 1) / RT_TOK, (E + RT_EXP - 1) / RT_EXP);
-    route_logits_kernel<<<grid, 128, 0, s>>>(X, W_r, bias, logits, T, d, E);
+    launch_logits(X, W_r, bias, logits, T, d, E, c->num_sms, s);
     TQP_LAUNCH_OK(c);
 #define TQP_TOPK(P) route_topk_kernel<P><<<(T + 3) / 4, 128, 0, s>>>(logits, topk_idx, topk_w, T, E, k)
     if (E <= 64) TQP_TOPK(2); else if (E <= 128) TQP_TOPK(4); else if (E <= 256) TQP_TOPK(8); else if (E <= 512) TQP_TOPK(16); else TQP_TOPK(32);
