@@ -347,8 +347,9 @@ tqp_status tqp_expert_fwd(tqp_ctx *c, int T, const void *X, const int32_t *offse
     GemmProblem pr[2] = {c->prob_gate, c->prob_up};
     CK(run_gemm(c, pr, 2, s));
     CK(launch_swiglu_fwd(c, N, G, U, H, s));
-    CK(launch_rows_proj(c, H, D.F, nullptr, nullptr, nullptr, (const bf16 *)c->w.A_down, nullptr, 1, ls,
-                        c->p<bf16>(c->ws.HAd), nullptr, s));
+    if (fused) CK(launch_rows_proj_tma(c, &c->prob_down.seg[0].act_map2, D.F, (const bf16 *)c->w.A_down, 1, ls, c->p<bf16>(c->ws.HAd), s));
+    else CK(launch_rows_proj(c, H, D.F, nullptr, nullptr, nullptr, (const bf16 *)c->w.A_down, nullptr, 1, ls,
+                             c->p<bf16>(c->ws.HAd), nullptr, s));
     GemmProblem pd = c->prob_down;
     pd.out = (bf16 *)Ye;
     CK(run_gemm(c, &pd, 1, s));
@@ -421,8 +422,13 @@ tqp_status tqp_expert_bwd(tqp_ctx *c, int T, const void *X, const void *dYe, con
         CK(launch_rows_wgrad(c, H, D.F, Zd, nullptr, offsets, 1, dA_down, nullptr, s));
     }
     // gate / up projections: dXp = dG . Wg_eff^T + dU . Wu_eff^T and their adapter gradients
-    CK(launch_rows_proj(c, dG, D.F, nullptr, nullptr, nullptr, (const bf16 *)c->w.B_gate, nullptr, 0, ls, Zg, nullptr, s));
-    CK(launch_rows_proj(c, dU, D.F, nullptr, nullptr, nullptr, (const bf16 *)c->w.B_up, nullptr, 0, ls, Zu, nullptr, s));
+    if (D.r == 16 || D.r == 32) {   // dG, dU are workspace tensors the dXp GEMM already has tensor maps for
+        CK(launch_rows_proj_tma(c, &c->prob_dx.seg[0].act_map2, D.F, (const bf16 *)c->w.B_gate, 0, ls, Zg, s));
+        CK(launch_rows_proj_tma(c, &c->prob_dx.seg[1].act_map2, D.F, (const bf16 *)c->w.B_up, 0, ls, Zu, s));
+    } else {
+        CK(launch_rows_proj(c, dG, D.F, nullptr, nullptr, nullptr, (const bf16 *)c->w.B_gate, nullptr, 0, ls, Zg, nullptr, s));
+        CK(launch_rows_proj(c, dU, D.F, nullptr, nullptr, nullptr, (const bf16 *)c->w.B_up, nullptr, 0, ls, Zu, nullptr, s));
+    }
     GemmProblem px = c->prob_dx;
     px.out = (bf16 *)dXp;
     CK(run_gemm(c, &px, 1, s));

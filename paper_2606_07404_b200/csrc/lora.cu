@@ -253,6 +253,147 @@ static tqp_status launch_proj_t(tqp_ctx *c, const ProjArgs &a, cudaStream_t st) 
     return TQP_OK;
 }
 
+// ---- plain projections of a dense workspace tensor, rows by TMA --------------------------------------------------------
+// h.A_d, dG.B_g^T, dU.B_u^T: the rows are a dense [N][K] tensor the grouped GEMM already has a tensor map for (box
+// 64 columns x 128 rows, 128-byte swizzle).  One thread issues one TMA load per K-chunk into a 5-deep ring (16 KB a stage,
+// two CTAs per SM: 128 KB of rows in flight per SM against 64 KB in the register-staged kernel, which these HBM-latency-
+// bound passes need); ldmatrix reads the swizzled tile (16-byte chunk c of row r sits at chunk c ^ (r & 7)).
+constexpr int PT_NST = 5;
+template <int R, bool KR>
+struct ProjTmaCfg {
+    static constexpr int WLD = KR ? R + 8 : PJ_LD;
+    static constexpr int ROWS_BYTES = PJ_ROWS * PJ_KC * 2;                                   // 16 KB, unpadded (swizzled)
+    static constexpr int W_CHUNKS = KR ? PJ_KC * R / 8 : R * PJ_KC / 8;
+    static constexpr int W_BYTES = ((KR ? PJ_KC * WLD : R * WLD) * 2 + 127) / 128 * 128;
+    static constexpr int OFF_W = PT_NST * ROWS_BYTES;
+    static constexpr int SMEM = OFF_W + PT_NST * W_BYTES + 1024;
+};
+
+struct ProjTmaArgs {
+    CUtensorMap map;       // rows [*][K], box {64, 128}, SWIZZLE_128B
+    const bf16 *W;         // adapter matrix of all experts
+    bf16 *out;             // [N][kLoraPad]
+    int K;
+    float s;
+};
+
+template <int R, bool KR>
+__global__ void __launch_bounds__(PJ_THREADS, 2) rows_proj_tma_kernel(const __grid_constant__ ProjTmaArgs a, const Tile *__restrict__ tiles,
+                                                                      const int32_t *__restrict__ num_tiles) {
+    using C = ProjTmaCfg<R, KR>;
+    using namespace ptx;
+    extern __shared__ uint8_t pt_smem_raw[];
+    __shared__ __align__(8) uint64_t s_full[PT_NST];
+    if ((int)blockIdx.x >= *num_tiles) return;
+    const Tile t = tiles[blockIdx.x];
+    const int rbase = blockIdx.y * PJ_ROWS;
+    const int valid = min(PJ_ROWS, t.rows - rbase);
+    if (valid <= 0) return;
+    const int row0 = t.row0 + rbase;
+    const int tid = threadIdx.x, warp = tid / 32, lane = tid % 32;
+    const uint32_t sbase = (smem_u32(pt_smem_raw) + 1023u) & ~1023u;   // shared-space ADDRESS arithmetic only (TMA / ldmatrix / cp.async)
+    const uint32_t bar0 = smem_u32(s_full);
+    const int K = a.K, nk = K / PJ_KC;
+    if (tid == 0) {
+        for (int s = 0; s < PT_NST; ++s) mbar_init(bar0 + 8 * s, 1);
+        mbar_init_fence();
+    }
+    __syncthreads();
+    auto issue = [&](int kc) {   // rows by TMA (one thread), adapter chunk by cp.async (everyone)
+        const int st = kc % PT_NST;
+        if (tid == 0) {
+            mbar_expect_tx(bar0 + 8 * st, C::ROWS_BYTES);
+            tma_load_2d(sbase + st * C::ROWS_BYTES, &a.map, kc * PJ_KC, row0, bar0 + 8 * st);
+        }
+        const uint32_t w_s = sbase + C::OFF_W + st * C::W_BYTES;
+        for (int v = tid; v < C::W_CHUNKS; v += PJ_THREADS) {
+            if (KR) {   // W[e][k][R]
+                const int kk = v / (R / 8), cc = v % (R / 8);
+                cp_async16(w_s + (kk * C::WLD + cc * 8) * 2, a.W + ((size_t)t.expert * K + kc * PJ_KC + kk) * R + cc * 8, 16);
+            } else {    // W[e][q][K]
+                const int q = v / (PJ_KC / 8), cc = v % (PJ_KC / 8);
+                cp_async16(w_s + (q * C::WLD + cc * 8) * 2, a.W + ((size_t)t.expert * R + q) * K + kc * PJ_KC + cc * 8, 16);
+            }
+        }
+    };
+    float acc[R / 8][4];
+#pragma unroll
+    for (int n = 0; n < R / 8; ++n)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) acc[n][q] = 0.f;
+    for (int s = 0; s < PT_NST - 1; ++s) {
+        if (s < nk) issue(s);
+        cp_async_commit();
+    }
+    const int arow = warp * 16 + lane % 16;   // this lane's row of the A fragment (ldmatrix x4)
+    for (int kc = 0; kc < nk; ++kc) {
+        const int st = kc % PT_NST;
+        mbar_wait(bar0 + 8 * st, (kc / PT_NST) & 1);
+        cp_async_wait<PT_NST - 2>();
+        __syncthreads();   // chunk kc visible to everyone; everyone is past the MMAs of chunk kc - 1 (its stage is refilled below)
+        if (kc + PT_NST - 1 < nk) issue(kc + PT_NST - 1);
+        cp_async_commit();
+        if (warp * 16 < valid) {
+            const uint32_t rows_s = sbase + st * C::ROWS_BYTES, w_s = sbase + C::OFF_W + st * C::W_BYTES;
+            const uint32_t b_addr = KR ? w_s + ((lane % 8 + ((lane / 8) % 2) * 8) * C::WLD + (lane / 16) * 8) * 2
+                                       : w_s + (((lane / 16) * 8 + lane % 8) * C::WLD + ((lane / 8) % 2) * 8) * 2;
+#pragma unroll
+            for (int kk = 0; kk < PJ_KC; kk += 16) {
+                uint32_t af[4];
+                ldsm_x4(rows_s + arow * 128 + ((((kk >> 3) + (lane >> 4)) ^ (arow & 7)) << 4), af);
+#pragma unroll
+                for (int np = 0; np < R / 16; ++np) {
+                    uint32_t bq[4];
+                    if (KR) ldsm_x4_t(b_addr + (kk * C::WLD + np * 16) * 2, bq);
+                    else ldsm_x4(b_addr + (np * 16 * C::WLD + kk) * 2, bq);
+                    mma16816(acc[2 * np], af, bq[0], bq[1]);
+                    mma16816(acc[2 * np + 1], af, bq[2], bq[3]);
+                }
+            }
+        }
+    }
+    cp_async_wait<0>();
+    if (warp * 16 < valid) {
+#pragma unroll
+        for (int n = 0; n < R / 8; ++n) {
+            const int q = n * 8 + (lane % 4) * 2;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int r = warp * 16 + lane / 4 + 8 * h;
+                if (r < valid)
+                    *reinterpret_cast<uint32_t *>(a.out + (size_t)(row0 + r) * kLoraPad + q) =
+                        float2_to_bf16x2(a.s * acc[n][2 * h], a.s * acc[n][2 * h + 1]);
+            }
+        }
+    }
+}
+
+template <int R, bool KR>
+static tqp_status launch_proj_tma_t(tqp_ctx *c, const ProjTmaArgs &a, cudaStream_t st) {
+    using C = ProjTmaCfg<R, KR>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        TQP_CUDA_OK(c, cudaFuncSetAttribute(rows_proj_tma_kernel<R, KR>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+        attr_set = true;
+    }
+    dim3 grid(c->max_tiles, kTileRows / PJ_ROWS);
+    rows_proj_tma_kernel<R, KR><<<grid, PJ_THREADS, C::SMEM, st>>>(a, c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles));
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
+
+// One adapter projection of a dense workspace tensor whose tensor map (box {64, 128}, 128-byte swizzle) is `map`.
+tqp_status launch_rows_proj_tma(tqp_ctx *c, const CUtensorMap *map, int K, const bf16 *W, int w_kr, float s, bf16 *out, cudaStream_t st) {
+    const int r = c->desc.r;
+    ProjTmaArgs a;
+    a.map = *map; a.W = W; a.out = out; a.K = K; a.s = s;
+    if (r == 16 && w_kr) return launch_proj_tma_t<16, true>(c, a, st);
+    if (r == 16) return launch_proj_tma_t<16, false>(c, a, st);
+    if (r == 32 && w_kr) return launch_proj_tma_t<32, true>(c, a, st);
+    if (r == 32) return launch_proj_tma_t<32, false>(c, a, st);
+    return TQP_ERR_ARG;
+}
+
 // r = 8 (config 0): plain CUDA-core version, one warp per row.
 __global__ void __launch_bounds__(128) lora_down_small_kernel(const bf16 *__restrict__ in, int K, int R, const bf16 *__restrict__ W,
                                                               int w_kr, float s, bf16 *__restrict__ out,
