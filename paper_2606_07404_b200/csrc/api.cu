@@ -88,6 +88,16 @@ tqp_status act_map(tqp_ctx *c, CUtensorMap *m, const void *ptr, uint64_t rows, u
     return make_map(c, m, ptr, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, rows, K, 64, box_rows, CU_TENSOR_MAP_SWIZZLE_128B);
 }
 
+// Unswizzled maps of the gathered projections (lora.cu): m[0] = source rows, box {256, 1} (gather4);  m[1], m[2] = the
+// permuted destination, box {256, 128} (tile store) and {256, 1} (scatter4 of a ragged tile).
+tqp_status gather_maps(tqp_ctx *c, CUtensorMap *m, const void *in, uint64_t in_rows, const void *through, uint64_t out_rows, uint64_t K) {
+    const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
+    tqp_status st = make_map(c, &m[0], in, dt, 2, in_rows, K, 256, 1, CU_TENSOR_MAP_SWIZZLE_NONE);
+    if (st == TQP_OK) st = make_map(c, &m[1], through, dt, 2, out_rows, K, 256, 128, CU_TENSOR_MAP_SWIZZLE_NONE);
+    if (st == TQP_OK) st = make_map(c, &m[2], through, dt, 2, out_rows, K, 256, 1, CU_TENSOR_MAP_SWIZZLE_NONE);
+    return st;
+}
+
 tqp_status set_seg(tqp_ctx *c, GemmSeg *s, const bf16 *act, uint64_t act_rows, const uint8_t *idx, const void *scale, int K,
                    int M, int kmajor) {
     s->act = act; s->idx = idx; s->scale = (const __half *)scale; s->K = K; s->kmajor = kmajor;
@@ -337,8 +347,15 @@ tqp_status tqp_expert_fwd(tqp_ctx *c, int T, const void *X, const int32_t *offse
 #define CK(x) do { st = (x); if (st != TQP_OK) return st; } while (0)
     const bool fused = D.r == 16 || D.r == 32;   // rank 8 (config 0) keeps the separate CUDA-core kernels
     if (fused) {   // Xp = gather(X) and both adapter projections x.A_g | x.A_u in one pass over the rows
-        CK(launch_rows_proj(c, (const bf16 *)X, D.d, perm, nullptr, Xp, (const bf16 *)c->w.A_gate, (const bf16 *)c->w.A_up, 1,
-                            ls, c->p<bf16>(c->ws.XAg), c->p<bf16>(c->ws.XAu), s));
+        if (D.d % 256 == 0) {   // rows by TMA gather4 (X is the caller's: its maps are encoded per call)
+            CUtensorMap gm[3];
+            CK(gather_maps(c, gm, X, (uint64_t)T, Xp, (uint64_t)N, D.d));
+            CK(launch_rows_gather_proj(c, &gm[0], T, &gm[1], &gm[2], N, D.d, perm, nullptr, (const bf16 *)c->w.A_gate,
+                                       (const bf16 *)c->w.A_up, 1, ls, c->p<bf16>(c->ws.XAg), c->p<bf16>(c->ws.XAu), s));
+        } else {
+            CK(launch_rows_proj(c, (const bf16 *)X, D.d, perm, nullptr, Xp, (const bf16 *)c->w.A_gate, (const bf16 *)c->w.A_up, 1,
+                                ls, c->p<bf16>(c->ws.XAg), c->p<bf16>(c->ws.XAu), s));
+        }
     } else {
         CK(launch_gather_rows(c, N, (const bf16 *)X, perm, Xp, s));
         CK(launch_rows_proj(c, Xp, D.d, nullptr, nullptr, nullptr, (const bf16 *)c->w.A_gate, (const bf16 *)c->w.A_up, 1, ls,
@@ -377,8 +394,16 @@ tqp_status tqp_combine_bwd(tqp_ctx *c, int T, const void *dY, const void *Ye, co
     if ((D.r == 16 || D.r == 32) && D.training && c->have_weights && c->disp_T == T && c->disp_inv_perm == inv_perm) {
         // Fused: dYe[p] = w[a] dY[t] by sorted position (a = perm[p]) and, from the same rows, Zd = s dYe . B_d^T, the
         // adapter projection tqp_expert_bwd needs.  dw = <dY, Ye> is a separate reduction when asked for.
-        st = launch_rows_proj(c, (const bf16 *)dY, D.d, c->disp_perm, topk_w, (bf16 *)dYe, (const bf16 *)c->w.B_down, nullptr,
-                              0, D.lora_scale, c->p<bf16>(c->ws.Zd), nullptr, (cudaStream_t)stream);
+        if (D.d % 256 == 0) {
+            CUtensorMap gm[3];
+            st = gather_maps(c, gm, dY, (uint64_t)T, dYe, (uint64_t)T * D.k, D.d);
+            if (st == TQP_OK)
+                st = launch_rows_gather_proj(c, &gm[0], T, &gm[1], &gm[2], T * D.k, D.d, c->disp_perm, topk_w, (const bf16 *)c->w.B_down,
+                                             nullptr, 0, D.lora_scale, c->p<bf16>(c->ws.Zd), nullptr, (cudaStream_t)stream);
+        } else {
+            st = launch_rows_proj(c, (const bf16 *)dY, D.d, c->disp_perm, topk_w, (bf16 *)dYe, (const bf16 *)c->w.B_down, nullptr, 0,
+                                  D.lora_scale, c->p<bf16>(c->ws.Zd), nullptr, (cudaStream_t)stream);
+        }
         if (st != TQP_OK) return st;
         c->zd_src = dYe;
         if (dtopk_w) st = launch_combine_dw(c, T, (const bf16 *)dY, (const bf16 *)Ye, inv_perm, dtopk_w, (cudaStream_t)stream);

@@ -158,6 +158,11 @@ tqp_status launch_rows_proj(tqp_ctx *c, const bf16 *in, int K, const int32_t *pe
                             const bf16 *W0, const bf16 *W1, int w_kr, float s, bf16 *out0, bf16 *out1, cudaStream_t st);
 // the same for ONE adapter matrix and a dense workspace tensor read through its GEMM tensor map (r = 16 / 32 only)
 tqp_status launch_rows_proj_tma(tqp_ctx *c, const CUtensorMap *map, int K, const bf16 *W, int w_kr, float s, bf16 *out, cudaStream_t st);
+// the gathered variants (perm != nullptr) with rows by TMA gather4 and the write-through by TMA store (lora.cu); needs
+// K % 256 == 0 and r = 16 / 32; maps as built by gather_maps() in api.cu
+tqp_status launch_rows_gather_proj(tqp_ctx *c, const CUtensorMap *in_map, int in_rows, const CUtensorMap *out_map, const CUtensorMap *sc_map,
+                                   int out_rows, int K, const int32_t *perm, const float *roww, const bf16 *W0, const bf16 *W1, int w_kr,
+                                   float s, bf16 *out0, bf16 *out1, cudaStream_t st);
 // grad_w[e] = sum_{p in e} small_w[p][q] * big[p][a]; stored [a][q] (out_ar=1: dA) or [q][a] (out_ar=0: dB), fp32
 tqp_status launch_rows_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 *small0, const bf16 *small1,
                              const int32_t *offsets, int out_ar, float *grad0, float *grad1, cudaStream_t st);

@@ -394,6 +394,305 @@ tqp_status launch_rows_proj_tma(tqp_ctx *c, const CUtensorMap *map, int K, const
     return TQP_ERR_ARG;
 }
 
+// ---- gathered projections: rows by TMA gather4, write-through by TMA store -------------------------------------------
+// Xp = gather(X) with x.A_g | x.A_u, and dYe = w . gather(dY) with dYe.B_d^T, for K % 256 == 0.
+//
+// What bounds the register-staged kernel above is not bytes but requests: it (and a first TMA version with 128-byte
+// swizzled rows) moves the rows in 128-byte pieces and stays at ~2.6 TB/s.  A gather4 instruction costs the TMA unit the
+// same ~70 clocks whether its four rows are 128 or 512 bytes wide, so this kernel gathers 256 columns (512 B) of a row
+// at a time: a stage is 128 rows x 256 columns, DENSE (swizzling stops at 128-byte rows), 64 KB, three stages, one CTA
+// per SM.  Warp 8 issues the gathers (lane l owns rows 4l..4l+3), warp 9 sends each landed stage to `through` (one
+// tile store; a ragged last tile goes out with scatter4 so that the next expert's rows are never touched), warps 0-7
+// multiply.
+//
+// Dense 512-byte rows put every row of one column in the same bank, which rules out ldmatrix for the row operand.  The
+// A fragments are read with LDS.128 instead, in a PERMUTED k order: thread (g = lane/4, t = lane%4) takes the 16-byte
+// chunks t and t+4 of every 64-column span of rows g and g+8 (odd g in the opposite order: the eight lanes of a
+// quarter-warp then hit eight different bank groups), and feeds chunk words (0,1), (2,3) of chunk t to MMAs 0, 1 and
+// those of chunk t+4 to MMAs 2, 3.  A sum over k does not care which physical column sits in which slot of the MMA as
+// long as the adapter operand uses the same assignment: slot (2t+e) of MMA m holds column 32 (m/2) + 8t + 4 (m%2) + e,
+// slot (8+2t+e) the column two further.  The adapter chunk is laid out in shared memory so that this read is
+// conflict-free too: [R][K] matrices with a 96-element row (LDS.128 per thread), [K][R] matrices with ldmatrix.trans
+// over hand-picked rows and a 32-byte skew every 8 rows.
+// SCALE: the consumers first multiply their own 16 rows by the gate weight in place (bf16-rounded: the value the dH GEMM
+// reads back), so the projection and the store both see the scaled rows.
+constexpr int GP_THREADS = 320;   // 8 consumer warps, producer warp, store warp
+constexpr int GP_COLS = 256;      // columns per stage
+constexpr int GP_NST = 3;
+template <int R, int NW, bool KR>
+struct GatherCfg {
+    static constexpr int RT = R * NW;
+    static constexpr int WST = RT <= 32 ? 4 : 3;                      // adapter ring (64-k chunks)
+    static constexpr int WLD = KR ? RT + 8 : 96;                      // KR: Ws[64][RT+8] (+16 elements every 8 rows), else Ws[RT][96]
+    static constexpr int ROWS_BYTES = PJ_ROWS * GP_COLS * 2;          // 64 KB
+    static constexpr int W_CHUNKS = KR ? PJ_KC * RT / 8 : RT * PJ_KC / 8;
+    static constexpr int W_BYTES = KR ? PJ_KC * WLD * 2 + 256 : RT * WLD * 2;
+    static constexpr int OFF_W = GP_NST * ROWS_BYTES;
+    static constexpr int SMEM = OFF_W + WST * W_BYTES + 1024;
+    static_assert(SMEM <= 232448, "shared memory");
+};
+
+struct GatherArgs {
+    CUtensorMap in_map;    // source rows [in_rows][K], box {256, 1}, no swizzle (gather4)
+    CUtensorMap out_map;   // through [out_rows][K], box {256, 128}, no swizzle (tile store)
+    CUtensorMap sc_map;    // through, box {256, 1} (scatter4, ragged tiles)
+    const int32_t *perm;   // row(p) = in[perm[p] / k]
+    const float *roww;     // SCALE: row(p) *= roww[perm[p]]
+    const bf16 *W[2];
+    bf16 *out[2];
+    int K, k, in_rows, out_rows;
+    float s;
+    int ablate;            // timing experiments only, as in ProjArgs: 256 no write-through, 512 no MMA
+};
+
+// One work item = 128 rows of one expert tile.  The kernel is persistent (one CTA per SM, items round-robin): every role
+// walks the same item sequence on its own, stage and adapter-ring counters run on across items, so the gathers of the
+// next item are in flight while the consumers finish the current one.
+struct GatherItem { int expert, row0, valid; };
+
+template <int R, int NW, bool KR, bool SCALE>
+__global__ void __launch_bounds__(GP_THREADS, 1) rows_gather_proj_kernel(const __grid_constant__ GatherArgs a, const Tile *__restrict__ tiles,
+                                                                         const int32_t *__restrict__ num_tiles) {
+    using C = GatherCfg<R, NW, KR>;
+    using namespace ptx;
+    constexpr int NST = GP_NST, WST = C::WST, HALVES = kTileRows / PJ_ROWS;
+    extern __shared__ uint8_t gp_smem_raw[];
+    __shared__ __align__(8) uint64_t s_bar[3 * NST];   // full | empty | ready
+    const int nt = *num_tiles, n_items = nt * HALVES;
+    const int tid = threadIdx.x, warp = tid / 32, lane = tid % 32;
+    const uint32_t sbase = (smem_u32(gp_smem_raw) + 1023u) & ~1023u;
+    const uint32_t full0 = smem_u32(s_bar), empty0 = full0 + 8 * NST, ready0 = full0 + 16 * NST;
+    const int K = a.K, nst = K / GP_COLS, nq = K / PJ_KC;
+    if (tid == 0) {
+        for (int s = 0; s < NST; ++s) {
+            mbar_init(full0 + 8 * s, 1);
+            mbar_init(empty0 + 8 * s, 9);    // 8 consumer warps + the store warp
+            mbar_init(ready0 + 8 * s, 8);
+        }
+        mbar_init_fence();
+    }
+    __syncthreads();
+    // first non-empty item at or after `it` in this CTA's sequence (valid = 0: none left)
+    auto find = [&](int &it) {
+        GatherItem g{0, 0, 0};
+        for (; it < n_items; it += gridDim.x) {
+            const Tile t = tiles[it % nt];   // all first halves (whole), then the ragged second halves: with (tile, half)
+                                             // interleaved, the even CTAs of an even-sized grid would get every whole one
+            const int rbase = (it / nt) * PJ_ROWS, v = min(PJ_ROWS, t.rows - rbase);
+            if (v > 0) { g.expert = t.expert; g.row0 = t.row0 + rbase; g.valid = v; break; }
+        }
+        return g;
+    };
+
+    if (warp == 8) {   // ---- producer: gather4 of this lane's four rows, 256 columns per stage
+        const uint64_t pol = l2_policy_evict_last();
+        int n = 0;     // stages issued so far
+        for (int it = blockIdx.x;; it += gridDim.x) {
+            const GatherItem g = find(it);
+            if (!g.valid) break;
+            const int nl = (g.valid + 3) / 4;
+            int sr[4];     // rows past `valid`: an index past the tensor (zero fill, no traffic)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) sr[j] = 4 * lane + j < g.valid ? a.perm[g.row0 + 4 * lane + j] / a.k : a.in_rows;
+            for (int kc = 0; kc < nst; ++kc, ++n) {
+                const int st = n % NST;
+                if (n >= NST) mbar_wait(empty0 + 8 * st, ((n / NST) - 1) & 1);
+                if (lane == 0) mbar_expect_tx(full0 + 8 * st, nl * 4 * GP_COLS * 2);
+                __syncwarp();
+                if (lane < nl)
+                    tma_gather4(sbase + st * C::ROWS_BYTES + lane * (4 * GP_COLS * 2), &a.in_map, kc * GP_COLS, sr[0], sr[1], sr[2], sr[3],
+                                full0 + 8 * st, pol);
+            }
+        }
+        return;
+    }
+    if (warp == 9) {   // ---- store: stage -> through[row0 .. row0 + valid)
+        const uint64_t pol = l2_policy_evict_first();
+        int n = 0;
+        for (int it = blockIdx.x;; it += gridDim.x) {
+            const GatherItem g = find(it);
+            if (!g.valid) break;
+            const int nl = (g.valid + 3) / 4;
+            int dr[4];     // ragged tile: rows past `valid` get an index past the tensor (clipped, never written)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) dr[j] = 4 * lane + j < g.valid ? g.row0 + 4 * lane + j : a.out_rows;
+            const bool whole = g.valid == PJ_ROWS;
+            for (int kc = 0; kc < nst; ++kc, ++n) {
+                const int st = n % NST;
+                mbar_wait((SCALE ? ready0 : full0) + 8 * st, (n / NST) & 1);
+                const uint32_t rows_s = sbase + st * C::ROWS_BYTES;
+                if (!(a.ablate & 256) && (whole ? lane == 0 : lane < nl)) {
+                    if (whole) tma_store_2d(&a.out_map, kc * GP_COLS, g.row0, rows_s, pol);
+                    else tma_scatter4(&a.sc_map, kc * GP_COLS, dr[0], dr[1], dr[2], dr[3], rows_s + lane * (4 * GP_COLS * 2), pol);
+                    bulk_commit_group();
+                    bulk_wait_group_read<0>();   // the stage has been read: it may be refilled
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty0 + 8 * st);
+            }
+        }
+        return;
+    }
+
+    // ---- consumers (256 threads): adapter chunks by cp.async, MMAs on the gathered rows
+    auto issue_w = [&](int expert, int q, int slot) {   // 64-k adapter chunk q of `expert` -> ring slot
+        const uint32_t w_s = sbase + C::OFF_W + slot * C::W_BYTES;
+        for (int v = tid; v < C::W_CHUNKS; v += PJ_THREADS) {
+            if (KR) {   // W_w[e][k][R] -> Ws[k][w R + q], rows skewed by 16 elements every 8
+                const int kk = v / (C::RT / 8), cc = v % (C::RT / 8), w = (cc * 8) / R, q0 = (cc * 8) % R;
+                cp_async16(w_s + (kk * C::WLD + (kk / 8) * 16 + cc * 8) * 2, a.W[w] + ((size_t)expert * K + q * PJ_KC + kk) * R + q0, 16);
+            } else {    // W_w[e][q][K] -> Ws[w R + q][k]
+                const int n = v / (PJ_KC / 8), cc = v % (PJ_KC / 8), w = n / R, qq = n % R;
+                cp_async16(w_s + (n * C::WLD + cc * 8) * 2, a.W[w] + ((size_t)expert * R + qq) * K + q * PJ_KC + cc * 8, 16);
+            }
+        }
+    };
+    const int g8 = lane >> 2, tq = lane & 3, odd = g8 & 1;
+    const uint32_t a_off = (warp * 16 + g8) * (GP_COLS * 2) + (tq + 4 * odd) * 16;   // first chunk of this lane in a span
+    const int a_sw = odd ? -64 : 64;                                                 // byte offset of its second chunk
+    // [K][R] adapters: lane (i = lane%8, j = (lane/8)%2, nb = lane/16) addresses row 8 (i/2) + i%2 + 2 j of the chunk
+    const int li = lane & 7, lj = (lane >> 3) & 1;
+    const int kl = 8 * (li >> 1) + (li & 1) + 2 * lj;
+    const uint32_t bk_off = (kl * C::WLD + (li >> 1) * 16 + (lane >> 4) * 8) * 2;
+    const uint32_t bn_off = (g8 * C::WLD + 8 * tq) * 2;                               // [R][K] adapters
+
+    int it = blockIdx.x;
+    GatherItem cur = find(it);
+    int n = 0, wq = 0;   // stages / adapter chunks consumed so far
+    if (cur.valid)
+        for (int s = 0; s < WST - 1; ++s) { issue_w(cur.expert, s, s); cp_async_commit(); }   // nq >= 4 > WST - 1
+    while (cur.valid) {
+        int itn = it + gridDim.x;
+        const GatherItem nxt = find(itn);
+        float acc[C::RT / 8][4];
+#pragma unroll
+        for (int i = 0; i < C::RT / 8; ++i)
+#pragma unroll
+            for (int q = 0; q < 4; ++q) acc[i][q] = 0.f;
+        const bool active = warp * 16 < cur.valid;
+        float roww = 1.f;   // SCALE: lane l (< 16) holds the gate weight of row 16 warp + l
+        if (SCALE && lane < 16 && warp * 16 + lane < cur.valid) roww = a.roww[a.perm[cur.row0 + warp * 16 + lane]];
+        for (int q = 0; q < nq; ++q, ++wq) {
+            const int ss = q % 4, st = n % NST;
+            const uint32_t rows_s = sbase + st * C::ROWS_BYTES, w_s = sbase + C::OFF_W + (wq % WST) * C::W_BYTES;
+            cp_async_wait<WST - 2>();
+            named_bar_sync(1, PJ_THREADS);   // adapter chunk wq visible; every consumer is past the MMAs of chunk wq - 1
+            {   // refill the slot chunk wq - 1 used: the chunk WST - 1 ahead, of this item or the first of the next
+                const int qa = q + WST - 1, slot = (wq + WST - 1) % WST;
+                if (qa < nq) issue_w(cur.expert, qa, slot);
+                else if (nxt.valid) issue_w(nxt.expert, qa - nq, slot);
+                cp_async_commit();
+            }
+            if (ss == 0) {
+                mbar_wait(full0 + 8 * st, (n / NST) & 1);
+                if (SCALE) {
+                    if (active) {
+                        const uint32_t mine = rows_s + warp * 16 * (GP_COLS * 2) + lane * 16;
+#pragma unroll 4
+                        for (int i = 0; i < 16; ++i) {   // row 16 warp + i: 32 lanes x 16 bytes
+                            const float wr = __shfl_sync(0xffffffffu, roww, i);
+                            uint4 v = lds128(mine + i * (GP_COLS * 2));
+                            uint32_t *vp = reinterpret_cast<uint32_t *>(&v);
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) {
+                                const float2 f = bf16x2_to_float2(vp[e]);
+                                vp[e] = float2_to_bf16x2(wr * f.x, wr * f.y);
+                            }
+                            sts128(mine + i * (GP_COLS * 2), v);
+                        }
+                        fence_async_smem();   // the TMA store (async proxy) must see the scaled rows
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(ready0 + 8 * st);
+                }
+            }
+            if (active && !(a.ablate & 512)) {
+                const uint32_t ra = rows_s + a_off + ss * 128;
+                const uint4 x0 = lds128(ra), x1 = lds128(ra + a_sw), y0 = lds128(ra + 8 * GP_COLS * 2), y1 = lds128(ra + 8 * GP_COLS * 2 + a_sw);
+                const uint4 P = odd ? x1 : x0, Q = odd ? x0 : x1, P8 = odd ? y1 : y0, Q8 = odd ? y0 : y1;   // chunk t | t+4 of rows g | g+8
+                const uint32_t af[4][4] = {{P.x, P8.x, P.y, P8.y}, {P.z, P8.z, P.w, P8.w}, {Q.x, Q8.x, Q.y, Q8.y}, {Q.z, Q8.z, Q.w, Q8.w}};
+                if (KR) {
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) {
+                        const uint32_t bm = w_s + bk_off + ((32 * (m / 2) + 4 * (m % 2)) * C::WLD + 4 * (m / 2) * 16) * 2;
+#pragma unroll
+                        for (int np = 0; np < C::RT / 16; ++np) {
+                            uint32_t bq[4];
+                            ldsm_x4_t(bm + np * 32, bq);
+                            mma16816(acc[2 * np], af[m], bq[0], bq[1]);
+                            mma16816(acc[2 * np + 1], af[m], bq[2], bq[3]);
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int nb = 0; nb < C::RT / 8; ++nb) {
+                        const uint4 w0 = lds128(w_s + bn_off + nb * 8 * C::WLD * 2), w1 = lds128(w_s + bn_off + nb * 8 * C::WLD * 2 + 64);
+                        mma16816(acc[nb], af[0], w0.x, w0.y);
+                        mma16816(acc[nb], af[1], w0.z, w0.w);
+                        mma16816(acc[nb], af[2], w1.x, w1.y);
+                        mma16816(acc[nb], af[3], w1.z, w1.w);
+                    }
+                }
+            }
+            if (ss == 3) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty0 + 8 * st);
+                ++n;
+            }
+        }
+        if (active) {
+#pragma unroll
+            for (int i = 0; i < C::RT / 8; ++i) {
+                const int col = i * 8 + (lane % 4) * 2, w = col / R, q = col % R;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int r = warp * 16 + lane / 4 + 8 * h;
+                    if (r < cur.valid)
+                        *reinterpret_cast<uint32_t *>(a.out[w] + (size_t)(cur.row0 + r) * kLoraPad + q) =
+                            float2_to_bf16x2(a.s * acc[i][2 * h], a.s * acc[i][2 * h + 1]);
+                }
+            }
+        }
+        cur = nxt;
+        it = itn;
+    }
+    cp_async_wait<0>();
+}
+
+template <int R, int NW, bool KR, bool SCALE>
+static tqp_status launch_gather_t(tqp_ctx *c, const GatherArgs &a, cudaStream_t st) {
+    using C = GatherCfg<R, NW, KR>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        TQP_CUDA_OK(c, cudaFuncSetAttribute(rows_gather_proj_kernel<R, NW, KR, SCALE>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+        attr_set = true;
+    }
+    const int grid = std::min(c->num_sms, c->max_tiles * (kTileRows / PJ_ROWS));
+    rows_gather_proj_kernel<R, NW, KR, SCALE><<<grid, GP_THREADS, C::SMEM, st>>>(a, c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles));
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
+
+// through[p] = (roww ? roww[perm[p]] : 1) . in[perm[p] / k]  and  out_w[p] = s . through[p] . W_w[e(p)]   (r = 16 / 32,
+// K % 256 == 0).  Unswizzled maps: in_map = the source with box {256, 1}; out_map / sc_map = `through` with box
+// {256, 128} / {256, 1}.
+tqp_status launch_rows_gather_proj(tqp_ctx *c, const CUtensorMap *in_map, int in_rows, const CUtensorMap *out_map, const CUtensorMap *sc_map,
+                                   int out_rows, int K, const int32_t *perm, const float *roww, const bf16 *W0, const bf16 *W1, int w_kr,
+                                   float s, bf16 *out0, bf16 *out1, cudaStream_t st) {
+    const int r = c->desc.r;
+    GatherArgs a;
+    a.in_map = *in_map; a.out_map = *out_map; a.sc_map = *sc_map; a.perm = perm; a.roww = roww;
+    a.W[0] = W0; a.W[1] = W1; a.out[0] = out0; a.out[1] = out1; a.K = K; a.k = c->desc.k; a.in_rows = in_rows; a.out_rows = out_rows; a.s = s; a.ablate = c->ablate;
+    const bool kr = w_kr != 0, two = W1 != nullptr, sc = roww != nullptr;
+    if (K % GP_COLS) return TQP_ERR_ARG;
+    // the two shapes the layer uses: x.A_g | x.A_u (two [K][R] matrices, no scale) and w dY . B_d^T (one [R][K] matrix, scaled)
+    if (r == 16 && two && kr && !sc) return launch_gather_t<16, 2, true, false>(c, a, st);
+    if (r == 32 && two && kr && !sc) return launch_gather_t<32, 2, true, false>(c, a, st);
+    if (r == 16 && !two && !kr && sc) return launch_gather_t<16, 1, false, true>(c, a, st);
+    if (r == 32 && !two && !kr && sc) return launch_gather_t<32, 1, false, true>(c, a, st);
+    return TQP_ERR_ARG;
+}
+
 // r = 8 (config 0): plain CUDA-core version, one warp per row.
 __global__ void __launch_bounds__(128) lora_down_small_kernel(const bf16 *__restrict__ in, int K, int R, const bf16 *__restrict__ W,
                                                               int w_kr, float s, bf16 *__restrict__ out,

@@ -82,6 +82,26 @@ __device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const void *tmap,
         "l"(tmap), "r"(c0), "r"(c1), "r"(cluster_bar) : "memory");
 }
 
+// tile::gather4: four rows r0..r3 of a 2-D tensor (map box {cols, 1}), columns c0.., land as four consecutive box rows at dst
+__device__ __forceinline__ void tma_gather4(uint32_t dst, const void *tmap, int c0, int r0, int r1, int r2, int r3, uint32_t bar, uint64_t pol) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile::gather4.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%2, %3, %4, %5, %6}], [%7], %8;" ::"r"(dst),
+        "l"(tmap), "r"(c0), "r"(r0), "r"(r1), "r"(r2), "r"(r3), "r"(bar), "l"(pol) : "memory");
+}
+// shared -> global tile store (bulk async-group completion); rows / columns past the tensor's extent are clipped
+__device__ __forceinline__ void tma_store_2d(const void *tmap, int c0, int c1, uint32_t src, uint64_t pol) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%1, %2}], [%3], %4;" ::"l"(tmap), "r"(c0),
+                 "r"(c1), "r"(src), "l"(pol) : "memory");
+}
+// tile::scatter4: four consecutive box rows at src go to rows r0..r3 (map box {cols, 1}); rows past the extent are clipped
+__device__ __forceinline__ void tma_scatter4(const void *tmap, int c0, int r0, int r1, int r2, int r3, uint32_t src, uint64_t pol) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile::scatter4.bulk_group.L2::cache_hint [%0, {%1, %2, %3, %4, %5}], [%6], %7;" ::"l"(tmap),
+                 "r"(c0), "r"(r0), "r"(r1), "r"(r2), "r"(r3), "r"(src), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void bulk_commit_group() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_group_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
 // 1-D bulk copy global -> this CTA's shared memory (TMA engine, no tensor map); bytes % 16 == 0, 16-byte aligned ends
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),

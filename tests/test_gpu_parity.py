@@ -68,6 +68,17 @@ def test_mid_ragged_multi_tile(cfg, gemm_impl):
         assert (gpu[key][cfg.E - 1] == 0).all()        # empty expert: exactly zero gradients
 
 
+# d % 256 == 0 with r = 32: the TMA-gather projections (rows_gather_proj_kernel) in their rank-32 instantiations, two
+# 256-column stages per row, whole and ragged 128-row items, an expert with several tiles and an empty one
+MID32_D512 = ti.Config("mid_r32_d512", T=700, d=512, F=256, E=5, k=2, r=32, seed=23, router_grad=True)
+
+
+def test_gathered_projections_rank32_multi_stage():
+    inp = _skewed(MID32_D512)
+    gpu, ref = check_all(inp, backward=True, router_grad=True, gemm_impl=0)
+    assert ref["counts"].max() > 256 and ref["counts"].min() == 0
+
+
 def test_routing_ties_lower_id_wins():
     cfg = ti.CONFIGS[0]
     inp = ti.make_inputs(cfg)
