@@ -168,6 +168,17 @@ tqp_status tqp_route_sigmoid_bwd(tqp_ctx *ctx, int T, const void *X, const float
 tqp_status tqp_bias_update(tqp_ctx *ctx, const int32_t *counts, float *bias, int mode, float gamma, float cap_hi,
                            float cap_lo, void *stream);
 
+/* --- consolidation ---------------------------------------------------------- */
+/* PAPER.md L1110 (10.6) "The trained adapter is merged into the base weights, the result is materialized as bf16";
+ * L1481.  Writes the merged, ordinary bf16 weights of experts e0 .. e0 + n_experts - 1 of one pack
+ * (0 = gate, 1 = up, 2 = down):
+ *   W_out[e - e0][out][in] = bf16( scale[out] * codebook[idx[out][in/8]][in%8] + lora_scale * sum_q A[in][q] B[q][out] )
+ * computed in fp32 with one rounding; row = output channel, so that y = x . W^T is the dense layer (gate / up:
+ * out = F, in = d; down: out = d, in = F).  W_out: DEVICE bf16 [n_experts][out][in], caller-owned (5.2 MB per expert
+ * and pack at d = 2560, F = 1024: consolidate in expert ranges).  Needs bound weights; reads them, writes nothing else.
+ * Errors: TQP_ERR_STATE without weights, TQP_ERR_ARG for a bad pack / range / NULL. */
+tqp_status tqp_consolidate(tqp_ctx *ctx, int pack, int e0, int n_experts, void *W_out, void *stream);
+
 /* --- introspection ------------------------------------------------------------------------------------- */
 /* Device pointers of workspace tensors, for tests: "G","U","H" bf16 [N][F]; "Xp" bf16 [N][d];
  * "dH","dG","dU" bf16 [N][F]; "num_tiles" int32 [1].  NULL if unknown. */

@@ -69,6 +69,7 @@ def load_library() -> ctypes.CDLL:
         lib.tqp_route_sigmoid.argtypes = [vp, ci] + [vp] * 8
         lib.tqp_route_sigmoid_bwd.argtypes = [vp, ci] + [vp] * 11
         lib.tqp_bias_update.argtypes = [vp, vp, vp, ci, ctypes.c_float, ctypes.c_float, ctypes.c_float, vp]
+        lib.tqp_consolidate.argtypes = [vp, ci, ci, ci, vp, vp]
         lib.tqp_debug_buffer.argtypes = [vp, ctypes.c_char_p]
         lib.tqp_debug_buffer.restype = vp
         lib.tqp_gemm_time.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_int)]
@@ -244,6 +245,16 @@ class TqpLayer:
         self._check(self.lib.tqp_bias_update(self.ctx, _ptr(counts), _ptr(bias), int(mode), float(gamma), float(cap_hi),
                                              float(cap_lo), self._stream()))
         return bias
+
+    def consolidate(self, pack, e0=0, n_experts=None, out=None):
+        """Merged bf16 weights [n_experts][out][in] of pack 0 (gate) / 1 (up) / 2 (down) for experts e0 .. e0 + n_experts."""
+        pack = {"gate": 0, "up": 1, "down": 2}.get(pack, pack)
+        n = self.E - e0 if n_experts is None else n_experts
+        out_dim, in_dim = (self.d, self.F) if pack == 2 else (self.F, self.d)
+        if out is None:
+            out = self.torch.empty((n, out_dim, in_dim), dtype=self.torch.bfloat16, device=self.device)
+        self._check(self.lib.tqp_consolidate(self.ctx, int(pack), int(e0), int(n), _ptr(out), self._stream()))
+        return out
 
     def step_host(self, X_host, dY_host, W_r, logit_bias, Y_host, dX_host, grads, dW_r=None):
         """Whole forward+backward through HOST (pinned) X/dY/Y/dX buffers; grads / dW_r stay on the device."""

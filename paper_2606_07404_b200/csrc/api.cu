@@ -534,6 +534,17 @@ tqp_status tqp_bias_update(tqp_ctx *c, const int32_t *counts, float *bias, int m
     return launch_bias_update(c, counts, bias, mode, gamma, cap_hi, cap_lo, (cudaStream_t)stream);
 }
 
+tqp_status tqp_consolidate(tqp_ctx *c, int pack, int e0, int n_experts, void *W_out, void *stream) {
+    if (!c) return TQP_ERR_ARG;
+    c->launches = 0;
+    REQ(c, c->have_weights, TQP_ERR_STATE, "tqp_consolidate needs tqp_bind_weights first");
+    REQ(c, pack >= 0 && pack <= 2, TQP_ERR_ARG, "pack must be 0 (gate), 1 (up) or 2 (down)");
+    REQ(c, e0 >= 0 && n_experts >= 0 && e0 + n_experts <= c->desc.E, TQP_ERR_ARG, "expert range outside [0, E)");
+    if (n_experts == 0) return TQP_OK;
+    PTR_OK(c, W_out);
+    return launch_consolidate(c, pack, e0, n_experts, (bf16 *)W_out, (cudaStream_t)stream);
+}
+
 tqp_status tqp_step_host(tqp_ctx *c, int T, const void *X_host, const void *dY_host, const float *W_r,
                          const float *logit_bias, void *Y_host, void *dX_host, float *dA_gate, float *dB_gate,
                          float *dA_up, float *dB_up, float *dA_down, float *dB_down, float *dW_r, void *stream) {

@@ -163,6 +163,8 @@ tqp_status launch_rows_proj_tma(tqp_ctx *c, const CUtensorMap *map, int K, const
 tqp_status launch_rows_gather_proj(tqp_ctx *c, const CUtensorMap *in_map, int in_rows, const CUtensorMap *out_map, const CUtensorMap *sc_map,
                                    int out_rows, int K, const int32_t *perm, const float *roww, const bf16 *W0, const bf16 *W1, int w_kr,
                                    float s, bf16 *out0, bf16 *out1, cudaStream_t st);
+// W[e - e0][out][in] = bf16(deq + s A B) for experts e0 .. e0 + n_experts of pack 0 (gate) / 1 (up) / 2 (down) (consolidate.cu)
+tqp_status launch_consolidate(tqp_ctx *c, int pack, int e0, int n_experts, bf16 *W, cudaStream_t st);
 // grad_w[e] = sum_{p in e} small_w[p][q] * big[p][a]; stored [a][q] (out_ar=1: dA) or [q][a] (out_ar=0: dB), fp32
 tqp_status launch_rows_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 *small0, const bf16 *small1,
                              const int32_t *offsets, int out_ar, float *grad0, float *grad1, cudaStream_t st);
