@@ -38,6 +38,7 @@ Workspace layout(const tqp_layer_desc &d) {
     w.num_tiles = take(16);
     w.xsegs = take((N / kWgradSeg + 2) * sizeof(Tile));
     w.xfirst = take((E + 1) * 4);
+    w.sched = take(64);   // work counters of the persistent kernels (zeroed before each launch)
     // partial weight gradients of split experts: first segments indexed by expert, extra segments by list position;
     // widest use: two rank-r gradients over d columns in one pass (dA_gate + dA_up)
     w.wg_scratch = d.training ? take((E + N / kWgradSeg + 2) * (size_t)2 * d.r * (dm > F ? dm : F) * 4) : take(16);

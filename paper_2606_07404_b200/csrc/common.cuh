@@ -63,7 +63,7 @@ struct Workspace {
     // sizes
     size_t total = 0;
     // offsets (bytes) into the bound buffer
-    size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, xsegs, xfirst, wg_scratch, lut, WrT, dl,
+    size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, xsegs, xfirst, wg_scratch, sched, lut, WrT, dl,
         // tqp_step_host staging
         trace, hX, hdY, hY, hdX, topk_idx, topk_w, counts, offsets, perm, inv_perm, Ye, dYe, dXp, dtopk_w;
 };

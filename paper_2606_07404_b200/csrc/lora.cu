@@ -445,17 +445,23 @@ struct GatherArgs {
     int ablate;            // timing experiments only, as in ProjArgs: 256 no write-through, 512 no MMA
 };
 
-// One work item = 128 rows of one expert tile.  The kernel is persistent (one CTA per SM, items round-robin): every role
-// walks the same item sequence on its own, stage and adapter-ring counters run on across items, so the gathers of the
-// next item are in flight while the consumers finish the current one.
+// One work item = 128 rows of one expert tile.  The kernel is persistent (one CTA per SM): the producer warp draws items
+// from a global counter (whole 128-row halves of all tiles first, then the ragged second halves; item sizes differ a lot
+// under skewed routing, so a fixed round-robin left SMs idle) and publishes each id in a small shared-memory queue that
+// the store warp and the consumers follow.  Stage and adapter-ring counters run on across items, so the gathers of the
+// next item are in flight while the consumers finish the current one.  Which CTA takes which item does not affect any
+// result (items write disjoint rows).
 struct GatherItem { int expert, row0, valid; };
+constexpr int GP_QN = 8;   // item queue entries; the producer is at most GP_NST + 1 items ahead of its readers
 
 template <int R, int NW, bool KR, bool SCALE>
 __global__ void __launch_bounds__(GP_THREADS, 1) rows_gather_proj_kernel(const __grid_constant__ GatherArgs a, const Tile *__restrict__ tiles,
-                                                                         const int32_t *__restrict__ num_tiles) {
+                                                                         const int32_t *__restrict__ num_tiles, int32_t *__restrict__ counter) {
     using C = GatherCfg<R, NW, KR>;
     using namespace ptx;
     constexpr int NST = GP_NST, WST = C::WST, HALVES = kTileRows / PJ_ROWS;
+    __shared__ int s_q[GP_QN];   // published item ids (-1: no more)
+    __shared__ int s_pub;        // number of entries published so far
     extern __shared__ uint8_t gp_smem_raw[];
     __shared__ __align__(8) uint64_t s_bar[3 * NST];   // full | empty | ready
     const int nt = *num_tiles, n_items = nt * HALVES;
@@ -464,6 +470,7 @@ __global__ void __launch_bounds__(GP_THREADS, 1) rows_gather_proj_kernel(const _
     const uint32_t full0 = smem_u32(s_bar), empty0 = full0 + 8 * NST, ready0 = full0 + 16 * NST;
     const int K = a.K, nst = K / GP_COLS, nq = K / PJ_KC;
     if (tid == 0) {
+        s_pub = 0;
         for (int s = 0; s < NST; ++s) {
             mbar_init(full0 + 8 * s, 1);
             mbar_init(empty0 + 8 * s, 9);    // 8 consumer warps + the store warp
@@ -472,24 +479,39 @@ __global__ void __launch_bounds__(GP_THREADS, 1) rows_gather_proj_kernel(const _
         mbar_init_fence();
     }
     __syncthreads();
-    // first non-empty item at or after `it` in this CTA's sequence (valid = 0: none left)
-    auto find = [&](int &it) {
+    auto item = [&](int it) {   // item id -> rows; valid <= 0: nothing there (a tile of at most 128 rows has no second half)
         GatherItem g{0, 0, 0};
-        for (; it < n_items; it += gridDim.x) {
-            const Tile t = tiles[it % nt];   // all first halves (whole), then the ragged second halves: with (tile, half)
-                                             // interleaved, the even CTAs of an even-sized grid would get every whole one
-            const int rbase = (it / nt) * PJ_ROWS, v = min(PJ_ROWS, t.rows - rbase);
-            if (v > 0) { g.expert = t.expert; g.row0 = t.row0 + rbase; g.valid = v; break; }
+        if (it >= 0 && it < n_items) {
+            const Tile t = tiles[it % nt];
+            const int rbase = (it / nt) * PJ_ROWS;
+            g.expert = t.expert; g.row0 = t.row0 + rbase; g.valid = min(PJ_ROWS, t.rows - rbase);
         }
         return g;
+    };
+    // the seq-th published item of this CTA (store warp and consumers; valid = 0: the queue has ended)
+    auto published = [&](int seq) {
+        while (*(volatile int *)&s_pub <= seq) {}
+        __threadfence_block();
+        return item(*(volatile int *)&s_q[seq % GP_QN]);
     };
 
     if (warp == 8) {   // ---- producer: gather4 of this lane's four rows, 256 columns per stage
         const uint64_t pol = l2_policy_evict_last();
         int n = 0;     // stages issued so far
-        for (int it = blockIdx.x;; it += gridDim.x) {
-            const GatherItem g = find(it);
-            if (!g.valid) break;
+        for (int seq = 0;; ++seq) {
+            GatherItem g{0, 0, 0};
+            int it = -1;
+            do {   // draw until a non-empty item or the end
+                if (lane == 0) it = atomicAdd(counter, 1);
+                it = __shfl_sync(0xffffffffu, it, 0);
+                g = item(it);
+            } while (it < n_items && g.valid <= 0);
+            if (lane == 0) {
+                s_q[seq % GP_QN] = it < n_items ? it : -1;
+                __threadfence_block();
+                *(volatile int *)&s_pub = seq + 1;
+            }
+            if (it >= n_items) break;
             const int nl = (g.valid + 3) / 4;
             int sr[4];     // rows past `valid`: an index past the tensor (zero fill, no traffic)
 #pragma unroll
@@ -509,9 +531,9 @@ __global__ void __launch_bounds__(GP_THREADS, 1) rows_gather_proj_kernel(const _
     if (warp == 9) {   // ---- store: stage -> through[row0 .. row0 + valid)
         const uint64_t pol = l2_policy_evict_first();
         int n = 0;
-        for (int it = blockIdx.x;; it += gridDim.x) {
-            const GatherItem g = find(it);
-            if (!g.valid) break;
+        for (int seq = 0;; ++seq) {
+            const GatherItem g = published(seq);
+            if (g.valid <= 0) break;
             const int nl = (g.valid + 3) / 4;
             int dr[4];     // ragged tile: rows past `valid` get an index past the tensor (clipped, never written)
 #pragma unroll
@@ -556,14 +578,15 @@ __global__ void __launch_bounds__(GP_THREADS, 1) rows_gather_proj_kernel(const _
     const uint32_t bk_off = (kl * C::WLD + (li >> 1) * 16 + (lane >> 4) * 8) * 2;
     const uint32_t bn_off = (g8 * C::WLD + 8 * tq) * 2;                               // [R][K] adapters
 
-    int it = blockIdx.x;
-    GatherItem cur = find(it);
+    int seq = 0;
+    GatherItem cur = published(seq);
     int n = 0, wq = 0;   // stages / adapter chunks consumed so far
-    if (cur.valid)
+    if (cur.valid > 0)
         for (int s = 0; s < WST - 1; ++s) { issue_w(cur.expert, s, s); cp_async_commit(); }   // nq >= 4 > WST - 1
-    while (cur.valid) {
-        int itn = it + gridDim.x;
-        const GatherItem nxt = find(itn);
+    while (cur.valid > 0) {
+        GatherItem nxt{0, 0, 0};
+        bool have_nxt = false;   // looked up when the adapter ring first reaches past this item: by then the producer has
+                                 // issued this item's last stage and is drawing the next
         float acc[C::RT / 8][4];
 #pragma unroll
         for (int i = 0; i < C::RT / 8; ++i)
@@ -580,7 +603,10 @@ __global__ void __launch_bounds__(GP_THREADS, 1) rows_gather_proj_kernel(const _
             {   // refill the slot chunk wq - 1 used: the chunk WST - 1 ahead, of this item or the first of the next
                 const int qa = q + WST - 1, slot = (wq + WST - 1) % WST;
                 if (qa < nq) issue_w(cur.expert, qa, slot);
-                else if (nxt.valid) issue_w(nxt.expert, qa - nq, slot);
+                else {
+                    if (!have_nxt) { nxt = published(seq + 1); have_nxt = true; }
+                    if (nxt.valid > 0) issue_w(nxt.expert, qa - nq, slot);
+                }
                 cp_async_commit();
             }
             if (ss == 0) {
@@ -653,8 +679,8 @@ __global__ void __launch_bounds__(GP_THREADS, 1) rows_gather_proj_kernel(const _
                 }
             }
         }
-        cur = nxt;
-        it = itn;
+        cur = nxt;   // nq >= WST - 1 chunks: the look-up above has happened
+        ++seq;
     }
     cp_async_wait<0>();
 }
@@ -668,7 +694,9 @@ static tqp_status launch_gather_t(tqp_ctx *c, const GatherArgs &a, cudaStream_t 
         attr_set = true;
     }
     const int grid = std::min(c->num_sms, c->max_tiles * (kTileRows / PJ_ROWS));
-    rows_gather_proj_kernel<R, NW, KR, SCALE><<<grid, GP_THREADS, C::SMEM, st>>>(a, c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles));
+    int32_t *counter = c->p<int32_t>(c->ws.sched);
+    TQP_CUDA_OK(c, cudaMemsetAsync(counter, 0, sizeof(int32_t), st));
+    rows_gather_proj_kernel<R, NW, KR, SCALE><<<grid, GP_THREADS, C::SMEM, st>>>(a, c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), counter);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }
