@@ -144,39 +144,60 @@ __global__ void __launch_bounds__(128, 3) route_logits_kernel(const bf16 *__rest
 
 // One warp per token: k rounds of a warp arg-max under the total order (-logit, id); then the softmax over
 // the k selected logits with the sum taken in ascending j (the oracle's order).  E <= 1024.
+//
+// The arg-max works on order-preserving 32-bit integer keys of the floats (sign bit flipped for positives, all bits for
+// negatives; -0 is first made +0 so that equal floats have equal keys): a lane's best is a max tree over its PER keys,
+// the warp's best one redux.sync (max), the tie-break a second redux.sync (min) over the ids of the slots that hold that
+// key.  Key 0 (a NaN pattern no logit maps to) marks slots past E and slots already taken.  (The first version compared
+// floats through five rounds of shuffles per selection: 35 us at cfg 2, latency-bound.)
+__device__ __forceinline__ uint32_t order_key(float f) {
+    if (f == 0.f) f = 0.f;   // -0 -> +0
+    const uint32_t u = __float_as_uint(f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float key_value(uint32_t key) { return __uint_as_float((key & 0x80000000u) ? (key ^ 0x80000000u) : ~key); }
+
+// Selects the best remaining slot of the warp: returns its expert id, its key in `best`, and retires it.
+template <int PER>
+__device__ __forceinline__ int warp_select(uint32_t (&key)[PER], int lane, uint32_t &best) {
+    uint32_t t[PER];
+#pragma unroll
+    for (int q = 0; q < PER; ++q) t[q] = key[q];
+#pragma unroll
+    for (int s = PER / 2; s > 0; s >>= 1)
+#pragma unroll
+        for (int q = 0; q < s; ++q) t[q] = max(t[q], t[q + s]);
+    const uint32_t m = __reduce_max_sync(0xffffffffu, t[0]);
+    int cand = 0x7fffffff;
+#pragma unroll
+    for (int q = PER - 1; q >= 0; --q)
+        if (key[q] == m) cand = q * 32 + lane;   // descending q: the lowest id of this lane survives
+    const int e = __reduce_min_sync(0xffffffffu, cand);   // ties -> lower expert id
+#pragma unroll
+    for (int q = 0; q < PER; ++q)
+        if (q * 32 + lane == e) key[q] = 0u;
+    best = m;
+    return e;
+}
+
 template <int PER>   // PER = ceil(E / 32) rounded up to a power of two: logits held per lane
 __global__ void __launch_bounds__(128) route_topk_kernel(const float *__restrict__ logits, int32_t *__restrict__ topk_idx,
                                                          float *__restrict__ topk_w, int T, int E, int k) {
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) / 32, lane = threadIdx.x % 32;
     if (warp >= T) return;
     const float *l = logits + (size_t)warp * E;
-    float v[PER];
+    uint32_t key[PER];
 #pragma unroll
     for (int q = 0; q < PER; ++q) {
-        int e = q * 32 + lane;
-        v[q] = (e < E) ? l[e] : -INFINITY;
+        const int e = q * 32 + lane;
+        key[q] = (e < E) ? order_key(l[e]) : 0u;
     }
-    uint32_t taken = 0;  // bit q: slot q of this lane already selected
     float sel_l = 0.f;   // lane j keeps the j-th selected logit
     int sel_e = 0;
     for (int j = 0; j < k; ++j) {
-        float bv = -INFINITY;
-        int be = 0x7fffffff;
-#pragma unroll
-        for (int q = 0; q < PER; ++q) {
-            int e = q * 32 + lane;
-            bool ok = (e < E) && !((taken >> q) & 1u);
-            if (ok && (v[q] > bv || be == 0x7fffffff)) { bv = v[q]; be = e; }   // ascending e: ties keep lower id
-        }
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            float ov = __shfl_xor_sync(0xffffffffu, bv, off);
-            int oe = __shfl_xor_sync(0xffffffffu, be, off);
-            bool better = (oe != 0x7fffffff) && (be == 0x7fffffff || ov > bv || (ov == bv && oe < be));
-            if (better) { bv = ov; be = oe; }
-        }
-        if ((be % 32) == lane) taken |= 1u << (be / 32);
-        if (lane == j) { sel_l = bv; sel_e = be; }
+        uint32_t m;
+        const int e = warp_select<PER>(key, lane, m);
+        if (lane == j) { sel_l = key_value(m); sel_e = e; }
     }
     float m = __shfl_sync(0xffffffffu, sel_l, 0);
     float ex = (lane < k) ? expf(sel_l - m) : 0.f;
@@ -197,32 +218,17 @@ __global__ void __launch_bounds__(128) route_topk_sigmoid_kernel(const float *__
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) / 32, lane = threadIdx.x % 32;
     if (warp >= T) return;
     const float *l = logits + (size_t)warp * E;
-    float v[PER];
+    uint32_t key[PER];
 #pragma unroll
     for (int q = 0; q < PER; ++q) {
-        int e = q * 32 + lane;
-        v[q] = (e < E) ? (bias ? l[e] + bias[e] : l[e]) : -INFINITY;
+        const int e = q * 32 + lane;
+        key[q] = (e < E) ? order_key(bias ? l[e] + bias[e] : l[e]) : 0u;
     }
-    uint32_t taken = 0;
     int sel_e = 0;
     for (int j = 0; j < k; ++j) {
-        float bv = -INFINITY;
-        int be = 0x7fffffff;
-#pragma unroll
-        for (int q = 0; q < PER; ++q) {
-            int e = q * 32 + lane;
-            bool ok = (e < E) && !((taken >> q) & 1u);
-            if (ok && (v[q] > bv || be == 0x7fffffff)) { bv = v[q]; be = e; }
-        }
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            float ov = __shfl_xor_sync(0xffffffffu, bv, off);
-            int oe = __shfl_xor_sync(0xffffffffu, be, off);
-            bool better = (oe != 0x7fffffff) && (be == 0x7fffffff || ov > bv || (ov == bv && oe < be));
-            if (better) { bv = ov; be = oe; }
-        }
-        if ((be % 32) == lane) taken |= 1u << (be / 32);
-        if (lane == j) sel_e = be;
+        uint32_t m;
+        const int e = warp_select<PER>(key, lane, m);
+        if (lane == j) sel_e = e;
     }
     const float sc = (lane < k) ? 1.f / (1.f + expf(-l[sel_e])) : 0.f;
     float sum = 0.f;
