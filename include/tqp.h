@@ -144,6 +144,20 @@ tqp_status tqp_step_host(tqp_ctx *ctx, int T, const void *X_host, const void *dY
                          float *dB_gate, float *dA_up, float *dB_up, float *dA_down, float *dB_down,
                          float *dW_r, void *stream);
 
+/* The same step without the final synchronisation: everything is enqueued (kernels on `stream`, copies on the ctx's
+ * two copy streams) and the call returns.  A second call may follow at once: its uploads use the other of two device
+ * staging sets and travel while the first step's kernels run, its kernels follow on `stream`, and the first step's dX
+ * download overlaps its forward pass - the pipelining a data loader gives a training loop.  The host buffers of a step
+ * belong to the library until tqp_step_host_wait has returned for it: at most two steps may be in flight.
+ * tqp_step_host_wait(ctx, age) blocks the host until the latest (age 0) or the previous (age 1) enqueued step has
+ * delivered Y_host / dX_host and finished its kernels (gradients included); returns at once if there is no such step.
+ * Errors as tqp_step_host; TQP_ERR_ARG for another age. */
+tqp_status tqp_step_host_async(tqp_ctx *ctx, int T, const void *X_host, const void *dY_host, const float *W_r,
+                               const float *logit_bias, void *Y_host, void *dX_host, float *dA_gate,
+                               float *dB_gate, float *dA_up, float *dB_up, float *dA_down, float *dB_down,
+                               float *dW_r, void *stream);
+tqp_status tqp_step_host_wait(tqp_ctx *ctx, int age);
+
 /* --- paper-faithful router variant and loss-free balance controller -------------- */
 /* PAPER.md L224 (§3.4): "Routing scores are produced by a sigmoid, expert selection is biased by a per-expert routing
  * logit bias".  logits as in tqp_route (canonical fmaf chain, NO bias added); selection = the k largest keys

@@ -66,6 +66,8 @@ def load_library() -> ctypes.CDLL:
         lib.tqp_dispatch_bwd.argtypes = [vp, ci] + [vp] * 4
         lib.tqp_route_bwd.argtypes = [vp, ci] + [vp] * 10
         lib.tqp_step_host.argtypes = [vp, ci] + [vp] * 14
+        lib.tqp_step_host_async.argtypes = [vp, ci] + [vp] * 14
+        lib.tqp_step_host_wait.argtypes = [vp, ci]
         lib.tqp_route_sigmoid.argtypes = [vp, ci] + [vp] * 8
         lib.tqp_route_sigmoid_bwd.argtypes = [vp, ci] + [vp] * 11
         lib.tqp_bias_update.argtypes = [vp, vp, vp, ci, ctypes.c_float, ctypes.c_float, ctypes.c_float, vp]
@@ -264,6 +266,20 @@ class TqpLayer:
                                            _ptr(Y_host), _ptr(dX_host), _ptr(g["dA_gate"]), _ptr(g["dB_gate"]),
                                            _ptr(g["dA_up"]), _ptr(g["dB_up"]), _ptr(g["dA_down"]), _ptr(g["dB_down"]),
                                            _ptr(dW_r), self._stream()))
+
+    def step_host_async(self, X_host, dY_host, W_r, logit_bias, Y_host, dX_host, grads, dW_r=None):
+        """step_host without the final wait: returns once everything is enqueued (at most two steps in flight; the host
+        buffers of a step belong to the library until step_host_wait has returned for it)."""
+        T = X_host.shape[0]
+        g = grads
+        self._check(self.lib.tqp_step_host_async(self.ctx, T, _ptr(X_host), _ptr(dY_host), _ptr(W_r), _ptr(logit_bias),
+                                                 _ptr(Y_host), _ptr(dX_host), _ptr(g["dA_gate"]), _ptr(g["dB_gate"]),
+                                                 _ptr(g["dA_up"]), _ptr(g["dB_up"]), _ptr(g["dA_down"]), _ptr(g["dB_down"]),
+                                                 _ptr(dW_r), self._stream()))
+
+    def step_host_wait(self, age=0):
+        """Blocks until the latest (age 0) or the previous (age 1) asynchronous step has delivered its host outputs."""
+        self._check(self.lib.tqp_step_host_wait(self.ctx, int(age)))
 
     def gemm_time(self):
         """(summed grouped-GEMM device ms, launches) since the last call; needs set_option('time_gemm', 1)."""

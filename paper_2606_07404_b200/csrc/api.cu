@@ -47,6 +47,7 @@ Workspace layout(const tqp_layer_desc &d) {
     w.dl = take(N * 4);
     w.trace = take(16384 * 8);
     w.hX = take(T * dm * 2); w.hdY = take(T * dm * 2); w.hY = take(T * dm * 2); w.hdX = take(T * dm * 2);
+    w.hX2 = take(T * dm * 2); w.hdY2 = take(T * dm * 2);   // second upload set (tqp_step_host_async)
     w.topk_idx = take(N * 4); w.topk_w = take(N * 4); w.counts = take(E * 4); w.offsets = take((E + 1) * 4);
     w.perm = take(N * 4); w.inv_perm = take(N * 4);
     w.Ye = take(N * dm * 2); w.dYe = take(N * dm * 2); w.dXp = take(N * dm * 2); w.dtopk_w = take(N * 4);
@@ -188,7 +189,7 @@ void tqp_destroy(tqp_ctx *ctx) {
     if (!ctx) return;
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     for (cudaEvent_t e : {ctx->ev_start, ctx->ev_x, ctx->ev_dy, ctx->ev_y, ctx->ev_yout, ctx->ev_dx, ctx->ev_xc[0], ctx->ev_xc[1],
-                          ctx->ev_xc[2], ctx->ev_xc[3]})
+                          ctx->ev_xc[2], ctx->ev_xc[3], ctx->ev_done[0], ctx->ev_done[1], ctx->ev_comp[0], ctx->ev_comp[1]})
         if (e) cudaEventDestroy(e);
     if (ctx->copy_in) cudaStreamDestroy(ctx->copy_in);
     if (ctx->copy_out) cudaStreamDestroy(ctx->copy_out);
@@ -549,13 +550,39 @@ tqp_status tqp_consolidate(tqp_ctx *c, int pack, int e0, int n_experts, void *W_
 tqp_status tqp_step_host(tqp_ctx *c, int T, const void *X_host, const void *dY_host, const float *W_r,
                          const float *logit_bias, void *Y_host, void *dX_host, float *dA_gate, float *dB_gate,
                          float *dA_up, float *dB_up, float *dA_down, float *dB_down, float *dW_r, void *stream) {
+    tqp_status st = tqp_step_host_async(c, T, X_host, dY_host, W_r, logit_bias, Y_host, dX_host, dA_gate, dB_gate, dA_up, dB_up,
+                                        dA_down, dB_down, dW_r, stream);
+    if (st != TQP_OK) return st;
+    const int launches = c->launches;
+    st = tqp_step_host_wait(c, 0);
+    if (st != TQP_OK) return st;
+    TQP_CUDA_OK(c, cudaStreamSynchronize((cudaStream_t)stream));
+    c->launches = launches;
+    return TQP_OK;
+}
+
+tqp_status tqp_step_host_wait(tqp_ctx *c, int age) {
+    if (!c) return TQP_ERR_ARG;
+    REQ(c, age == 0 || age == 1, TQP_ERR_ARG, "age must be 0 (latest step) or 1 (the one before)");
+    const long long seq = c->host_seq - 1 - age;
+    if (seq < 0 || !c->ev_done[0]) return TQP_OK;   // nothing that old is in flight
+    TQP_CUDA_OK(c, cudaEventSynchronize(c->ev_done[seq & 1]));
+    TQP_CUDA_OK(c, cudaEventSynchronize(c->ev_comp[seq & 1]));
+    return TQP_OK;
+}
+
+tqp_status tqp_step_host_async(tqp_ctx *c, int T, const void *X_host, const void *dY_host, const float *W_r,
+                               const float *logit_bias, void *Y_host, void *dX_host, float *dA_gate, float *dB_gate,
+                               float *dA_up, float *dB_up, float *dA_down, float *dB_down, float *dW_r, void *stream) {
     tqp_status st = common_checks(c, T, true);
     if (st != TQP_OK) return st;
     REQ(c, X_host && dY_host && Y_host && dX_host, TQP_ERR_ARG, "host buffer is NULL");
     cudaStream_t s = (cudaStream_t)stream;
     const tqp_layer_desc &D = c->desc;
     const size_t row_bytes = (size_t)T * D.d * 2;
-    bf16 *X = c->p<bf16>(c->ws.hX), *dY = c->p<bf16>(c->ws.hdY), *Y = c->p<bf16>(c->ws.hY), *dX = c->p<bf16>(c->ws.hdX);
+    const int par = (int)(c->host_seq & 1);   // upload staging set of this step
+    bf16 *X = c->p<bf16>(par ? c->ws.hX2 : c->ws.hX), *dY = c->p<bf16>(par ? c->ws.hdY2 : c->ws.hdY);
+    bf16 *Y = c->p<bf16>(c->ws.hY), *dX = c->p<bf16>(c->ws.hdX);
     int32_t *ti = c->p<int32_t>(c->ws.topk_idx), *counts = c->p<int32_t>(c->ws.counts), *offs = c->p<int32_t>(c->ws.offsets);
     int32_t *perm = c->p<int32_t>(c->ws.perm), *inv = c->p<int32_t>(c->ws.inv_perm);
     float *tw = c->p<float>(c->ws.topk_w), *dtw = c->p<float>(c->ws.dtopk_w);
@@ -566,18 +593,21 @@ tqp_status tqp_step_host(tqp_ctx *c, int T, const void *X_host, const void *dY_h
         TQP_CUDA_OK(c, cudaStreamCreateWithFlags(&c->copy_in, cudaStreamNonBlocking));
         TQP_CUDA_OK(c, cudaStreamCreateWithFlags(&c->copy_out, cudaStreamNonBlocking));
         for (cudaEvent_t *e : {&c->ev_start, &c->ev_x, &c->ev_dy, &c->ev_y, &c->ev_yout, &c->ev_dx, &c->ev_xc[0], &c->ev_xc[1],
-                               &c->ev_xc[2], &c->ev_xc[3]})
+                               &c->ev_xc[2], &c->ev_xc[3], &c->ev_done[0], &c->ev_done[1], &c->ev_comp[0], &c->ev_comp[1]})
             TQP_CUDA_OK(c, cudaEventCreateWithFlags(e, cudaEventDisableTiming));
     }
     // X goes up in four token chunks and the router (token-wise) starts on each chunk as it lands; dY follows on the same
     // copy stream while the forward pass already runs on `s`; Y comes down on a second copy stream under the backward
-    // pass (PCIe is full duplex); dX leaves before the last adapter weight gradients are computed.  Everything is ordered
-    // after what `s` held before.
-    TQP_CUDA_OK(c, cudaEventRecord(c->ev_start, s));
-    TQP_CUDA_OK(c, cudaStreamWaitEvent(c->copy_in, c->ev_start, 0));
-    TQP_CUDA_OK(c, cudaStreamWaitEvent(c->copy_out, c->ev_start, 0));
+    // pass (PCIe is full duplex); dX leaves before the last adapter weight gradients are computed.  The kernels are
+    // ordered after what `s` held before.  The uploads are NOT: they only wait for the step before last, which used the
+    // same staging set (its kernels read X until the end of its backward pass), so that the uploads of a step issued
+    // while the previous one is still running travel under that step's kernels.
+    if (c->host_seq >= 2) TQP_CUDA_OK(c, cudaStreamWaitEvent(c->copy_in, c->ev_comp[par], 0));
     {
-        const int nch = T >= 1024 ? 4 : 1, per = ((T + nch - 1) / nch + 3) & ~3;   // chunk starts stay 16-byte aligned in every array
+        // With the previous step still running its kernels, this step's X will have landed long before `s` gets to the
+        // router: upload and route it in one piece then (four router launches of T / 4 tokens fill the SMs worse than one).
+        const bool behind = c->host_seq >= 1 && cudaEventQuery(c->ev_comp[par ^ 1]) == cudaErrorNotReady;
+        const int nch = (T >= 1024 && !behind) ? 4 : 1, per = ((T + nch - 1) / nch + 3) & ~3;   // chunk starts stay 16-byte aligned in every array
         float *lg = c->p<float>(c->ws.logits);
         for (int ch = 0; ch < nch; ++ch) {
             const int t0 = ch * per, tc = std::min(per, T - t0);
@@ -593,6 +623,7 @@ tqp_status tqp_step_host(tqp_ctx *c, int T, const void *X_host, const void *dY_h
     TQP_CUDA_OK(c, cudaEventRecord(c->ev_dy, c->copy_in));
     CK(tqp_dispatch(c, T, ti, counts, offs, perm, inv, s));
     CK(tqp_expert_fwd(c, T, X, offs, perm, Ye, s));
+    if (c->host_seq >= 1) TQP_CUDA_OK(c, cudaStreamWaitEvent(s, c->ev_done[par ^ 1], 0));   // the previous step's Y and dX have left
     CK(tqp_combine(c, T, Ye, inv, tw, Y, s));
     TQP_CUDA_OK(c, cudaEventRecord(c->ev_y, s));
     TQP_CUDA_OK(c, cudaStreamWaitEvent(c->copy_out, c->ev_y, 0));
@@ -610,11 +641,11 @@ tqp_status tqp_step_host(tqp_ctx *c, int T, const void *X_host, const void *dY_h
     TQP_CUDA_OK(c, cudaEventRecord(c->ev_dx, s));
     TQP_CUDA_OK(c, cudaStreamWaitEvent(c->copy_out, c->ev_dx, 0));   // after the Y download on the same copy stream
     TQP_CUDA_OK(c, cudaMemcpyAsync(dX_host, dX, row_bytes, cudaMemcpyDeviceToHost, c->copy_out));
-    TQP_CUDA_OK(c, cudaEventRecord(c->ev_yout, c->copy_out));
+    TQP_CUDA_OK(c, cudaEventRecord(c->ev_done[par], c->copy_out));
     CK(expert_bwd_tail(c, s));
 #undef CK
-    TQP_CUDA_OK(c, cudaStreamWaitEvent(s, c->ev_yout, 0));   // `s` (and its events) now also cover both downloads
-    TQP_CUDA_OK(c, cudaStreamSynchronize(s));
+    TQP_CUDA_OK(c, cudaEventRecord(c->ev_comp[par], s));
+    ++c->host_seq;
     c->launches = total;
     return TQP_OK;
 }

@@ -65,7 +65,7 @@ struct Workspace {
     // offsets (bytes) into the bound buffer
     size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, xsegs, xfirst, wg_scratch, sched, lut, WrT, dl,
         // tqp_step_host staging
-        trace, hX, hdY, hY, hdX, topk_idx, topk_w, counts, offsets, perm, inv_perm, Ye, dYe, dXp, dtopk_w;
+        trace, hX, hdY, hX2, hdY2, hY, hdX, topk_idx, topk_w, counts, offsets, perm, inv_perm, Ye, dYe, dXp, dtopk_w;
 };
 
 }  // namespace tqp
@@ -95,6 +95,10 @@ struct tqp_ctx {
     cudaStream_t copy_in = nullptr, copy_out = nullptr;
     cudaEvent_t ev_start = nullptr, ev_x = nullptr, ev_dy = nullptr, ev_y = nullptr, ev_yout = nullptr, ev_dx = nullptr;
     cudaEvent_t ev_xc[4] = {nullptr, nullptr, nullptr, nullptr};   // X arrives in token chunks; the router starts on the first
+    // tqp_step_host_async: steps alternate between two upload staging sets so that the next step's X / dY travel while this
+    // step computes; ev_done[p] = the step that used set p has delivered Y and dX to the host, ev_comp[p] = its kernels are done
+    cudaEvent_t ev_done[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr};
+    long long host_seq = 0;
     // tqp_step_host defers all adapter weight gradients (nothing else depends on them) until dX is on its way to the host
     int defer_tail = 0;
     struct { float *dA_gate, *dB_gate, *dA_up, *dB_up, *dA_down, *dB_down; const tqp::bf16 *dYe; const int32_t *offsets; bool pending; } tail = {};

@@ -146,6 +146,45 @@ def test_step_host_end_to_end(cfg):
         assert_close(key, to_np(grads[key]), ref[key])
 
 
+def test_step_host_async_three_steps_in_a_pipeline():
+    """tqp_step_host_async / tqp_step_host_wait: three steps with alternating inputs enqueued back to back (two in flight,
+    so the uploads of a step travel under the previous step's kernels and use the other staging set); every step's Y and
+    dX must be that step's own, and the gradients those of the last step."""
+    import torch
+    from parity_util import make_layer, to_np
+    inpA = _skewed(MID)
+    inpB = dict(inpA)
+    other = ti.make_inputs(ti.Config("mid_other", T=MID.T, d=MID.d, F=MID.F, E=MID.E, k=MID.k, r=MID.r, seed=97, router_grad=True))
+    inpB["X"], inpB["dY"] = other["X"], other["dY"]
+    refA, refB = oracle_ref(inpA, True, True), oracle_ref(inpB, True, True)
+    layer, dev = make_layer(inpA, training=True)
+    T, d = inpA["T"], inpA["d"]
+
+    def pinned(a):
+        return torch.from_numpy(a.view(np.int16)).view(torch.bfloat16).pin_memory()
+
+    host = {"A": (pinned(inpA["X"]), pinned(inpA["dY"])), "B": (pinned(inpB["X"]), pinned(inpB["dY"]))}
+    outs = [(torch.zeros((T, d), dtype=torch.bfloat16).pin_memory(), torch.zeros((T, d), dtype=torch.bfloat16).pin_memory())
+            for _ in range(3)]
+    grads = layer.alloc_grads()
+    dW_r = torch.zeros((d, inpA["E"]), dtype=torch.float32, device="cuda")
+    order = ["A", "B", "A"]
+    refs = {"A": refA, "B": refB}
+    for i, which in enumerate(order):
+        layer.step_host_async(host[which][0], host[which][1], dev["W_r"], dev.get("logit_bias"), outs[i][0], outs[i][1], grads, dW_r)
+        if i >= 1:
+            layer.step_host_wait(1)
+            assert_close(f"Y[{i - 1}]", to_np(outs[i - 1][0]), refs[order[i - 1]]["Y"])
+            assert_close(f"dX[{i - 1}]", to_np(outs[i - 1][1]), refs[order[i - 1]]["dX"])
+    layer.step_host_wait(0)
+    assert_close("Y[2]", to_np(outs[2][0]), refA["Y"])
+    assert_close("dX[2]", to_np(outs[2][1]), refA["dX"])
+    assert_close("dW_r", to_np(dW_r), refA["dW_r"])
+    for key in ("dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down"):
+        assert_close(key, to_np(grads[key]), refA[key])
+    assert np.abs(refA["Y"] - refB["Y"]).max() > 0.1 * np.abs(refA["Y"]).max()     # the two inputs really differ
+
+
 def test_layer_reuse_smaller_batch_and_foreign_dYe():
     """One ctx, two calls: a full batch, then a smaller batch with different data (stale workspace rows, tile list and
     cached dispatch pointers must not leak), and an expert_bwd fed a dYe tensor that did NOT come from the fused
