@@ -29,7 +29,8 @@ using namespace ptx;
 constexpr int BM = 128, BK = 64, TN = kTileRows, HN = kTileRows / 2;
 constexpr int AK = 128;                                   // K of one A stage (one index tile, one producer hand-shake) = two B stages
 constexpr int NSTAGE = 6, NASLOT = 3, IDXQ = 8;           // B (activation) ring, A (weight) slots of 64 TMEM columns, index ring
-constexpr int X_BYTES = HN * 128, IDX_BYTES = 128 * 16, LUT_BYTES = 256 * 8 * 16;
+constexpr int X_BYTES = HN * 128, IDX_TILE = 128 * 16, SCL_BYTES = 128 * 2, LUT_BYTES = 256 * 8 * 16;
+constexpr int IDX_BYTES = IDX_TILE + SCL_BYTES;          // an index ring entry: the code tile + the 128 fp16 scales of its A stage
 constexpr int OFF_X = 0, OFF_LUT = OFF_X + NSTAGE * X_BYTES, OFF_IDX = OFF_LUT + LUT_BYTES,
               OFF_BAR = OFF_IDX + IDXQ * IDX_BYTES, OFF_EPI = OFF_BAR + 512;
 constexpr int EPI_ROWS = 32, EPI_BYTES = TN * BM * 2;      // staging: the whole [256 rows][128 channels] bf16 output tile
@@ -65,7 +66,7 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t *v) {
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
 gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__restrict__ lut_g, const Tile *__restrict__ tiles,
-                        const int32_t *__restrict__ num_tiles_p, int ablate) {
+                        const int32_t *__restrict__ num_tiles_p, int ablate, long long *__restrict__ trace) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     const uint32_t sbase = smem_u32(smem);
@@ -163,6 +164,9 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                         const int c0 = S.kmajor ? ka * 16 : it.m0 / 8;
                         const int c1 = S.kmajor ? it.t.expert * pb.M + it.m0 : it.t.expert * S.K + ka * AK;
                         tma_load_2d(sbase + OFF_IDX + iq.s * IDX_BYTES, &S.idx_map, c0, c1, idx_full(iq.s));
+                        // the stage's scales ride along (K-major: of this CTA's 128 channels; MN-major: of the stage's 128 k), so
+                        // that no producer waits on a global load when an item starts
+                        bulk_g2s(sbase + OFF_IDX + iq.s * IDX_BYTES + IDX_TILE, S.scale + c1, SCL_BYTES, idx_full(iq.s));
                         iq.next(IDXQ);
                     }
                 }
@@ -183,8 +187,12 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                 const uint32_t aph = cnt & 1;
                 ++cnt;
                 const int n = max(16, (it.t.rows + 15) & ~15);
+                const bool trc = trace && cid == 0 && cnt <= 400;   // per item: start | accumulator free | first operands | per-stage waits | end
+                long long ts0 = 0, ts1 = 0, ts2 = 0, twait = 0;
+                if (trc) ts0 = clock64();
                 mbar_wait<true>(tmem_empty, aph ^ 1);   // the epilogue has drained the previous item's accumulator
                 tc_fence_after();
+                if (trc) ts1 = clock64();
                 const uint32_t d_tmem = tmem_base + TM_ACC;
                 const uint32_t idesc = make_idesc(2 * BM, n, 0);
                 uint32_t accum = 0;
@@ -193,11 +201,17 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                 const int nmma_l = max(1, pb.r / 16);
                 for (int ja = 0; ja < nka + pb.nlora; ++ja) {
                     const bool lora = ja >= nka;
+                    long long tw0 = 0;
+                    if (trc) tw0 = clock64();
                     mbar_wait<true>(fullA(sa.s), sa.ph);
                     const uint32_t a_tmem = tmem_base + TM_A + sa.s * 64;
                     for (int h = 0; h < (lora ? 1 : 2); ++h) {
                         mbar_wait<true>(fullB(st.s), st.ph);
                         tc_fence_after();
+                        if (trc && h == 0) {
+                            const long long tw1 = clock64();
+                            if (ja == 0) ts2 = tw1; else twait += tw1 - tw0;
+                        }
                         const uint32_t xs = x16 + st.s * (X_BYTES >> 4);
                         if (!lora) {
 #pragma unroll
@@ -218,6 +232,10 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                     sa.next(NASLOT);
                 }
                 umma_commit_pair(tmem_full, 3);
+                if (trc) {
+                    long long *tp = trace + (cnt - 1) * 8;
+                    tp[0] = ts0; tp[1] = ts1; tp[2] = ts2; tp[3] = twait; tp[4] = clock64(); tp[5] = nka + pb.nlora;
+                }
             }
         }
     } else if (warp >= W_DEQ0 && warp < W_EPI0) {
@@ -273,18 +291,20 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                 const int nka = S.K / AK;
                 if (S.kmajor) {
                     // ---- forward: codes run along k; this thread owns TMEM lane `row` and writes its 128 k-values itself
-                    const __nv_bfloat162 s2 = __float2bfloat162_rn(__half2float(S.scale[(size_t)e * M + m0 + row]));
                     for (int ka = 0; ka < nka; ++ka) {
                         const bool own = (ja & 1) == g;
                         uint4 codes = make_uint4(0, 0, 0, 0);
+                        uint32_t sraw = 0;
                         if (own) {   // one index tile = 16 codes per channel = this A stage
                             mbar_wait(idx_full(iq.s), iq.ph);
                             codes = lds128(sbase + OFF_IDX + iq.s * IDX_BYTES + row * 16);
+                            sraw = lds16(sbase + OFF_IDX + iq.s * IDX_BYTES + IDX_TILE + row * 2);
                             __syncwarp();
                             if (lane == 0) mbar_arrive(idx_empty(iq.s));
                         }
                         iq.next(IDXQ);
                         if (own) {
+                            const __nv_bfloat162 s2 = __float2bfloat162_rn(__half2float(__ushort_as_half((unsigned short)sraw)));
                             const uint32_t cwd[4] = {codes.x, codes.y, codes.z, codes.w};
 #pragma unroll
                             for (int h = 0; h < 2; ++h) {
@@ -314,28 +334,17 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                     // k = 16 x + 4 (rk / 2) + rk % 2 + 2 i, so that the transposed pairs land in TMEM columns 8 x + 2 jj + i.
                     uint32_t cw[16];             // code words (4 channel groups each) of this thread's 16 k-values of its A stage
                     __nv_bfloat162 sc[16];       // and their per-k scales (the weight's output channel is k here)
-                    __half sraw[16];             // raw scales of this group's NEXT A stage: fetched one own-stage ahead
-                    const __half *scp = S.scale + (size_t)e * S.K + kofs;
-                    {
-                        const int ka0 = ((ja & 1) == g) ? 0 : 1;
-                        if (ka0 < nka) {
-#pragma unroll
-                            for (int z = 0; z < 16; ++z) sraw[z] = scp[ka0 * AK + (z >> 3) * 64 + ((z >> 1) & 3) * 16 + (z & 1) * 2];
-                        }
-                    }
                     for (int ka = 0; ka < nka; ++ka) {
                         const bool own = (ja & 1) == g;
                         if (own) {   // one index tile = 128 k x 16 channel groups = this A stage
                             mbar_wait(idx_full(iq.s), iq.ph);
                             const uint32_t is = sbase + OFF_IDX + iq.s * IDX_BYTES + kofs * 16 + (warp & 3) * 4;
+                            const uint32_t ss = sbase + OFF_IDX + iq.s * IDX_BYTES + IDX_TILE + kofs * 2;   // the stage's per-k scales
 #pragma unroll
                             for (int z = 0; z < 16; ++z) {   // z = 8 h + 2 x + i  ->  k = 64 h + 16 x + kofs + 2 i
-                                cw[z] = lds32(is + ((z >> 3) * 64 + ((z >> 1) & 3) * 16 + (z & 1) * 2) * 16);
-                                sc[z] = __float2bfloat162_rn(__half2float(sraw[z]));
-                            }
-                            if (ka + 2 < nka) {
-#pragma unroll
-                                for (int z = 0; z < 16; ++z) sraw[z] = scp[(ka + 2) * AK + (z >> 3) * 64 + ((z >> 1) & 3) * 16 + (z & 1) * 2];
+                                const int kz = (z >> 3) * 64 + ((z >> 1) & 3) * 16 + (z & 1) * 2;
+                                cw[z] = lds32(is + kz * 16);
+                                sc[z] = __float2bfloat162_rn(__half2float(__ushort_as_half((unsigned short)lds16(ss + kz * 2))));
                             }
                             __syncwarp();
                             if (lane == 0) mbar_arrive(idx_empty(iq.s));
@@ -400,6 +409,8 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
             ++cnt;
             mbar_wait(tmem_full, aph);
             tc_fence_after();
+            const bool tre = trace && cid == 0 && rank == 0 && et == 0 && cnt <= 400;
+            if (tre) trace[4000 + (cnt - 1) * 4] = clock64();
             named_bar_sync(1, 128);   // every epilogue warp has finished storing the previous item out of the staging tile
             const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + TM_ACC;
             for (int c0 = 0; c0 < it.t.rows; c0 += EPI_ROWS) {
@@ -420,6 +431,7 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(tmem_empty_remote);
+            if (tre) trace[4000 + (cnt - 1) * 4 + 1] = clock64();
             named_bar_sync(1, 128);   // staging tile complete
             if (!(ablate & 16)) {
                 bf16 *outp = pb.out + (size_t)it.t.row0 * M + it.m0;
@@ -460,8 +472,10 @@ tqp_status launch_gemm_tcgen05_ts2(tqp_ctx *c, const GemmProblem *probs, int npr
     for (int i = 0; i < nprob; ++i) args.p[i] = probs[i];
     args.nprob = nprob;
     const int grid = (c->num_sms / 2) * 2;
+    const bool tr = c->trace > 0 && ++c->trace_seq == c->trace;   // debug timeline of cluster 0 (tqp_set_option "trace")
     gt2::gemm_tcgen05_ts2_kernel<<<grid, gt2::NTHREADS, gt2::SMEM_BYTES, st>>>(
-        args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), c->ablate);
+        args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), c->ablate,
+        tr ? c->p<long long>(c->ws.trace) : nullptr);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }
