@@ -133,6 +133,11 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                     const int nkb = S.K / BK;
                     for (int kb = 0; kb < nkb; ++kb) {
                         mbar_wait(emptyB(st.s), st.ph ^ 1);
+                        if (ablate & 64) {   // timing experiment: no activation traffic (the MMAs read stale tiles)
+                            if (rank == 0) mbar_arrive(fullB(st.s));
+                            st.next(NSTAGE);
+                            continue;
+                        }
                         if (rank == 0) mbar_expect_tx(fullB(st.s), 2 * X_BYTES);
                         tma_load_2d_pair(sbase + OFF_X + st.s * X_BYTES, &S.act_map2, kb * BK, row, fullB_remote + 8u * st.s);
                         st.next(NSTAGE);
@@ -188,7 +193,7 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                 ++cnt;
                 const int n = max(16, (it.t.rows + 15) & ~15);
                 const bool trc = trace && cid == 0 && cnt <= 400;   // per item: start | accumulator free | first operands | per-stage waits | end
-                long long ts0 = 0, ts1 = 0, ts2 = 0, twait = 0;
+                long long ts0 = 0, ts1 = 0, ts2 = 0, twait = 0, twaitb = 0;
                 if (trc) ts0 = clock64();
                 mbar_wait<true>(tmem_empty, aph ^ 1);   // the epilogue has drained the previous item's accumulator
                 tc_fence_after();
@@ -204,14 +209,19 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                     long long tw0 = 0;
                     if (trc) tw0 = clock64();
                     mbar_wait<true>(fullA(sa.s), sa.ph);
+                    long long twa = 0;
+                    if (trc) twa = clock64();
                     const uint32_t a_tmem = tmem_base + TM_A + sa.s * 64;
                     for (int h = 0; h < (lora ? 1 : 2); ++h) {
+                        long long twb = 0;
+                        if (trc && h == 1) twb = clock64();
                         mbar_wait<true>(fullB(st.s), st.ph);
                         tc_fence_after();
                         if (trc && h == 0) {
                             const long long tw1 = clock64();
-                            if (ja == 0) ts2 = tw1; else twait += tw1 - tw0;
+                            if (ja == 0) ts2 = tw1; else { twait += twa - tw0; twaitb += tw1 - twa; }
                         }
+                        if (trc && h == 1) twaitb += clock64() - twb;
                         const uint32_t xs = x16 + st.s * (X_BYTES >> 4);
                         if (!lora) {
 #pragma unroll
@@ -234,7 +244,7 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                 umma_commit_pair(tmem_full, 3);
                 if (trc) {
                     long long *tp = trace + (cnt - 1) * 8;
-                    tp[0] = ts0; tp[1] = ts1; tp[2] = ts2; tp[3] = twait; tp[4] = clock64(); tp[5] = nka + pb.nlora;
+                    tp[0] = ts0; tp[1] = ts1; tp[2] = ts2; tp[3] = twait; tp[4] = clock64(); tp[5] = nka + pb.nlora; tp[6] = twaitb;
                 }
             }
         }
