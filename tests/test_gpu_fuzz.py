@@ -1,0 +1,36 @@
+"""Random-shape parity of the whole chain against the oracle: a fixed set of seeds drawn from the shape space the
+library accepts (T 1..3000, d and F multiples of 128, E 1..200, k 1..16, r in {8, 16, 32}, half of them with a logit
+bias that floods one expert and empties another).  The hand-picked cases elsewhere cover the known corner cases; this
+one looks for the unknown ones (tile / stage / ring boundaries that only some combination of sizes hits)."""
+import numpy as np
+import pytest
+
+import tqp_inputs as ti
+from test_gpu_parity import check_all
+
+pytestmark = pytest.mark.gpu
+
+
+def _case(seed, big):
+    rng = np.random.default_rng(seed)
+    d = int(rng.choice([128, 256, 384, 512, 768, 1024]))
+    F = int(rng.choice([128, 256, 384, 512]))
+    E = int(rng.integers(1, 201 if big else 41))
+    k = int(rng.integers(1, min(E, 16 if big else 8) + 1))
+    r = int(rng.choice([8, 16, 32]))
+    T = int(rng.integers(1, 3000 if big else 1200))
+    cfg = ti.Config(f"fuzz{seed}", T=T, d=d, F=F, E=E, k=k, r=r, seed=seed, router_grad=bool(T * k >= 64))
+    inp = ti.make_inputs(cfg)
+    if rng.random() < 0.5 and E >= 3:
+        bias = np.zeros(E, np.float32)
+        bias[int(rng.integers(0, E))] = 2.5
+        bias[int(rng.integers(0, E))] = -50.0
+        inp["logit_bias"] = bias
+    return cfg, inp
+
+
+@pytest.mark.parametrize("seed,big", [(1000, False), (1003, False), (1017, False), (1020, False), (1036, False),
+                                      (5001, True), (5012, True), (5016, True), (5025, True), (5028, True)])
+def test_random_shape_matches_the_oracle(seed, big):
+    cfg, inp = _case(seed, big)
+    check_all(inp, backward=True, router_grad=cfg.router_grad, gemm_impl=0)
