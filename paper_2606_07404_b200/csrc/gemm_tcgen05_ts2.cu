@@ -160,6 +160,21 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                 get_item(item, it);
                 if (it.t.rows <= 0) continue;
                 const GemmProblem &pb = args.p[it.prob];
+                // This thread runs about one item ahead of the dequant warps: it pulls the item's adapter rows (read once per
+                // step, so cold in HBM) into L2 now; fetched cold by the producers they cost an HBM round trip.
+                for (int l = 0; l < pb.nlora; ++l) {
+                    const GemmLora &L = pb.lora[l];
+                    if (L.mk_layout) {
+                        const char *p0 = reinterpret_cast<const char *>(L.lw + ((size_t)it.t.expert * pb.M + it.m0) * pb.r);
+                        for (int off = 0; off < BM * pb.r * 2; off += 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(p0 + off));
+                    } else {
+                        for (int q = 0; q < pb.r; ++q) {
+                            const char *p0 = reinterpret_cast<const char *>(L.lw + ((size_t)it.t.expert * pb.r + q) * pb.M + it.m0);
+                            asm volatile("prefetch.global.L2 [%0];" ::"l"(p0));
+                            asm volatile("prefetch.global.L2 [%0];" ::"l"(p0 + 128));
+                        }
+                    }
+                }
                 for (int sg = 0; sg < pb.nseg; ++sg) {
                     const GemmSeg &S = pb.seg[sg];
                     const int nka = S.K / AK;
@@ -285,14 +300,27 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
             for (int j = 0; j < 16; ++j) ch[j] = 0;
             for (int l = 0; l < pb.nlora; ++l) {
                 if (((ja + nka_tot + l) & 1) == g) {
+                    // all loads of the row are issued back to back (fixed trip counts, predicated on r)
                     const GemmLora &L = pb.lora[l];
                     if (L.mk_layout) {
                         const uint4 *src = reinterpret_cast<const uint4 *>(L.lw + ((size_t)e * M + m0 + row) * r);
-                        for (int j = 0; j < r / 8; ++j) *reinterpret_cast<uint4 *>(&ch[4 * j]) = src[j];
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            if (8 * j < r) {
+                                const uint4 v = src[j];
+                                ch[4 * j] = v.x; ch[4 * j + 1] = v.y; ch[4 * j + 2] = v.z; ch[4 * j + 3] = v.w;
+                            }
+                        }
                     } else {
-                        const bf16 *src = L.lw + (size_t)e * r * M + m0 + row;
-                        uint16_t *h = reinterpret_cast<uint16_t *>(ch);
-                        for (int q = 0; q < r; ++q) h[q] = *reinterpret_cast<const uint16_t *>(src + (size_t)q * M);
+                        const uint16_t *src = reinterpret_cast<const uint16_t *>(L.lw + (size_t)e * r * M + m0 + row);
+                        uint32_t lo[16], hi[16];
+#pragma unroll
+                        for (int q = 0; q < 16; ++q) {
+                            lo[q] = 2 * q < r ? src[(size_t)(2 * q) * M] : 0u;
+                            hi[q] = 2 * q + 1 < r ? src[(size_t)(2 * q + 1) * M] : 0u;
+                        }
+#pragma unroll
+                        for (int q = 0; q < 16; ++q) ch[q] = lo[q] | (hi[q] << 16);
                     }
                 }
             }
