@@ -43,8 +43,8 @@ def flops(cfg, T):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per grouped-GEMM launch (average of the four launches of a step) from the
-# `ncu --set full` capture summarised in profiles/r1f_gemm_ncu_cfg2.md; None for workloads without a capture.
-NCU_GEMM_TRAFFIC = {"cfg2_120b": 1.067e9}
+# `ncu --set full` capture summarised in profiles/r1g_gemm_ncu_cfg2.md; None for workloads without a capture.
+NCU_GEMM_TRAFFIC = {"cfg2_120b": 1.069e9}
 
 
 def peaks():
