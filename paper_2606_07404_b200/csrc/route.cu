@@ -16,6 +16,18 @@ namespace tqp {
 // would leave most SMs idle (configs[1]: T = 4096, E = 64 -> 43 large CTAs on 148 SMs, 148 us; 128 small CTAs: see DESIGN).
 constexpr int RT_K = 32;
 
+// d.x = fma(a.x, b, d.x), d.y = fma(a.y, b, d.y): two IEEE fp32 FMAs in one instruction (FFMA2 on sm_100: packed
+// register pairs with a scalar third operand).  Each lane rounds exactly like fmaf, so the logits stay bit-identical to the
+// canonical chain; what changes is the number of instructions per FMA, which is what bounds this kernel.
+__device__ __forceinline__ void ffma2(float2 &d, const float2 a, const float b) {
+    uint64_t dd, aa, bb;
+    asm("mov.b64 %0, {%1,%2};" : "=l"(dd) : "f"(d.x), "f"(d.y));
+    asm("mov.b64 %0, {%1,%2};" : "=l"(aa) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1,%1};" : "=l"(bb) : "f"(b));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(dd) : "l"(aa), "l"(bb));
+    asm("mov.b64 {%0,%1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(dd));
+}
+
 template <int RT_TM, int RT_EN>   // per-thread tile: RT_TM tokens x RT_EN experts; 8 x 16 threads per CTA
 __global__ void __launch_bounds__(128, 3) route_logits_kernel(const bf16 *__restrict__ X, const float *__restrict__ W_r,
                                                               const float *__restrict__ bias, float *__restrict__ logits,
@@ -29,11 +41,12 @@ __global__ void __launch_bounds__(128, 3) route_logits_kernel(const bf16 *__rest
     const int t0 = blockIdx.x * RT_TOK, e0 = blockIdx.y * RT_EXP;
     const int tx = tid % 16, ty = tid / 16;   // tx -> experts (6 each), ty -> tokens (12 each)
     const bool w_vec = (E % 4) == 0;          // 16-byte cp.async needs aligned rows and whole chunks
-    float acc[RT_TM][RT_EN];
+    static_assert(RT_TM % 2 == 0, "token pairs");
+    float2 acc[RT_TM / 2][RT_EN];   // (token 2a, token 2a + 1) x expert b
 #pragma unroll
-    for (int a = 0; a < RT_TM; ++a)
+    for (int a = 0; a < RT_TM / 2; ++a)
 #pragma unroll
-        for (int b = 0; b < RT_EN; ++b) acc[a][b] = 0.f;
+        for (int b = 0; b < RT_EN; ++b) acc[a][b] = make_float2(0.f, 0.f);
 
     // X tile: 96 tokens x 32 i (bf16) = 384 chunks of 8 values; chunk v = tid + 128 j: token v % 96, segment v / 96
     const bf16 *xsrc[RT_XCH];
@@ -116,9 +129,9 @@ __global__ void __launch_bounds__(128, 3) route_logits_kernel(const bf16 *__rest
                 wv[2 * b] = w2.x; wv[2 * b + 1] = w2.y;
             }
 #pragma unroll
-            for (int a = 0; a < RT_TM; ++a)
+            for (int a = 0; a < RT_TM / 2; ++a)
 #pragma unroll
-                for (int b = 0; b < RT_EN; ++b) acc[a][b] = fmaf(xv[a], wv[b], acc[a][b]);
+                for (int b = 0; b < RT_EN; ++b) ffma2(acc[a][b], make_float2(xv[2 * a], xv[2 * a + 1]), wv[b]);
         }
         if (c + 1 < nc) {
             store_x(buf ^ 1);
@@ -134,7 +147,7 @@ __global__ void __launch_bounds__(128, 3) route_logits_kernel(const bf16 *__rest
         for (int b = 0; b < RT_EN; ++b) {
             const int e = e0 + tx * RT_EN + b;
             if (e < E) {
-                float v = acc[a][b];
+                float v = (a & 1) ? acc[a / 2][b].y : acc[a / 2][b].x;
                 if (bias) v = v + bias[e];
                 logits[(size_t)t * E + e] = v;
             }
