@@ -14,7 +14,9 @@
  * Pins (tests/test_oracle_pins.py): P1 closed-form dequant, P2 B=0 adapters, P3 brute-force top-k with
  * injected ties, P4 permutation invariants, P5 fp64 finite differences, P6 softmax special cases,
  * P7 E=1 dense FFN vs an independent numpy fp64 matmul, P8 merge identity, P9 linearity /
- * empty experts, P10 fp32-vs-fp64, P12 hand-checkable 0/1 worked example (tests/golden/p12_worked_example.txt).
+ * empty experts, P10 fp32-vs-fp64, P12 hand-checkable 0/1 worked example (tests/golden/p12_worked_example.txt),
+ * P13 hand-computed combine / combine_bwd with k = 3 and distinct rows (tests/golden/p13_combine_worked_example.txt);
+ * P5 also runs at lora_scale 0.5 and 2 with large adapters (the factor s in dA, dB and the adapter term of dX).
  * Parity unpinned: absolute numerical outputs — the paper prints no worked example, codebook or expected
  * value for this layer.
  * ====================================================================================================== */

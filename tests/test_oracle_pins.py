@@ -55,8 +55,8 @@ def test_p1_dequant_is_scale_times_codebook_entry(inp0):
 
 
 # ---------------------------------------------------------------- P12: hand-checkable 0/1 worked example
-def _parse_golden():
-    path = os.path.join(os.path.dirname(__file__), "golden", "p12_worked_example.txt")
+def _parse_golden(name="p12_worked_example.txt"):
+    path = os.path.join(os.path.dirname(__file__), "golden", name)
     vals = {}
     for line in open(path):
         line = line.split("#")[0].strip()
@@ -217,6 +217,39 @@ def test_dispatch_empty_and_single_expert():
     np.testing.assert_array_equal(inv, [3, 0, 4, 1, 2, 5])
 
 
+# ---------------------------------------------------------------- P13: combine / combine_bwd, k > 1, distinct rows
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_p13_combine_worked_example(dtype):
+    """PAPER.md L239 (top-k routing) + north_star "weighted unpermute/combine": which gate weight multiplies which of a
+    token's k rows.  Hand-computed values (tests/golden/p13_combine_worked_example.txt); a swap of the weight/row
+    pairing in combine, dYe or dtopk_w changes every expected number."""
+    g = _parse_golden("p13_combine_worked_example.txt")
+    Ye = np.stack([g[f"Ye{p}"] for p in range(6)]).astype(dtype)
+    inv = g["inv_perm"].astype(np.int32)
+    w = np.stack([g["w0"], g["w1"]]).astype(dtype)
+    dY = np.stack([g["dY0"], g["dY1"]]).astype(dtype)
+    tol = dict(rtol=1e-6, atol=1e-6) if dtype == np.float32 else dict(rtol=1e-14, atol=1e-14)
+    Y = oracle.combine(Ye, inv, w)
+    np.testing.assert_allclose(Y, np.stack([g["Y0"], g["Y1"]]), **tol)
+    dYe, dw = oracle.combine_bwd(dY, Ye, inv, w, dtype)
+    np.testing.assert_allclose(dYe, np.stack([g[f"dYe{p}"] for p in range(6)]), **tol)
+    np.testing.assert_allclose(dw, np.stack([g["dw0"], g["dw1"]]), **tol)
+
+
+def test_p13_combine_on_cfg0_against_numpy_gather(inp0):
+    """The same pairing on the seeded cfg 0 (k = 2, every row distinct): fancy-indexed numpy einsum in fp64."""
+    out = oracle.layer(f64_inputs(inp0), dtype=np.float64, backward=True)
+    T, k = CFG0.T, CFG0.k
+    rows = out["Ye"][out["inv_perm"].reshape(T, k)]                       # [T][k][d]
+    np.testing.assert_allclose(out["Y"], np.einsum("tj,tjd->td", out["topk_w"], rows), rtol=1e-13, atol=1e-15)
+    dY = widen(inp0["dY"]).astype(np.float64)
+    np.testing.assert_allclose(out["dtopk_w"], np.einsum("td,tjd->tj", dY, rows), rtol=1e-13, atol=1e-15)
+    expect = np.empty_like(out["dYe"])
+    expect[out["inv_perm"]] = (out["topk_w"][:, :, None] * dY[:, None, :]).reshape(T * k, -1)
+    np.testing.assert_allclose(out["dYe"], expect, rtol=1e-13, atol=1e-15)
+    assert np.abs(out["topk_w"][:, 0] - out["topk_w"][:, 1]).min() > 1e-6   # weights differ, so a swap would show
+
+
 # ---------------------------------------------------------------- P2 / P8: adapter wiring
 def _with(inp, **kw):
     out = dict(inp); out.update(kw); return out
@@ -268,7 +301,24 @@ def _loss(inp64):
     return float((out["Y"] * inp64["dY"]).sum()), out
 
 
-def test_p5_finite_differences_cfg0(inp0):
+def _big_adapters(inp, lora_scale):
+    """cfg-0 inputs with adapters of order 0.1 (as P7) and the given lora_scale, so that every adapter term and its
+    scale factor s moves the loss far above the finite-difference noise."""
+    out = dict(inp)
+    rng = np.random.default_rng(77)
+    for key in ("A_gate", "B_gate", "A_up", "B_up", "A_down", "B_down"):
+        out[key] = ti.f32_to_bf16_bits(rng.standard_normal(inp[key].shape).astype(np.float32) * 0.1)
+    out["lora_scale"] = lora_scale
+    return out
+
+
+@pytest.mark.parametrize("variant", ["cfg0", "lora_scale_0.5_big_adapters", "lora_scale_2_big_adapters"])
+def test_p5_finite_differences_cfg0(inp0, variant):
+    """Central differences of the (P7-pinned) forward against the analytic backward.  The lora_scale != 1 variants
+    (PAPER.md L938 adapters; `tqp_layer_desc.lora_scale`) catch a dropped or doubled factor s in dA, dB or the
+    adapter term of dX (oracle hole (b))."""
+    if variant != "cfg0":
+        inp0 = _big_adapters(inp0, 0.5 if "0.5" in variant else 2.0)
     inp64 = f64_inputs(inp0)
     ana = oracle.layer(inp64, dtype=np.float64, backward=True, router_grad=True)
     lg = ana["logits"]
