@@ -42,9 +42,12 @@ def flops(cfg, T):
     return dict(total=base + lora + router, base=base, lora=lora, router=router, gemm=gemm)
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per grouped-GEMM launch (average of the four launches of a step) from the
-# `ncu --set full` capture summarised in profiles/r1g_gemm_ncu_cfg2.md; None for workloads without a capture.
-NCU_GEMM_TRAFFIC = {"cfg2_120b": 1.069e9}
+# roofline.traffic is NOT measured by this run (ncu cannot run inside a timed bench): it is dram__bytes_read.sum +
+# dram__bytes_write.sum per grouped-GEMM launch (average over the launches of one step) copied from the committed
+# `ncu --set full` capture named beside it; None for workloads without a capture.
+NCU_GEMM_TRAFFIC = {"cfg2_120b": (1.069e9, "profiles/r1g_gemm_ncu_cfg2.md")}
+GEMM_IMPL_NAMES = {0: "tcgen05 CTA pairs, weight operand in TMEM (gemm_tcgen05_ts2)", 1: "CUDA-core scaffold",
+                   2: "tcgen05 one CTA per tile, smem weight operand", 3: "tcgen05 CTA pairs, smem weight operand"}
 
 
 def peaks():
@@ -151,7 +154,9 @@ def time_oracle(cfg, T_sample, steps, warmup):
         oracle_step(inp, cfg)
     dt = (time.perf_counter() - t0) / max(steps, 1)
     return dict(value=T_sample / dt, unit="tokens/s", cores=oracle.num_threads(), kind="oracle",
-                sample=f"T={T_sample} of {cfg.T} tokens, all {cfg.E} experts, fwd+bwd, fp32, {steps} step(s) of {dt:.2f} s",
+                sample=f"T={T_sample} of {cfg.T} tokens, all {cfg.E} experts (each dequantised once per pass), "
+                       f"{'fwd+bwd' if cfg.backward else 'fwd+bwd (the GPU arm of this config is forward only)'}, fp32, "
+                       f"{steps} step(s) of {dt:.2f} s",
                 seconds_per_step=dt, gflops=flops(cfg, T_sample)["total"] / dt / 1e9)
 
 
@@ -220,8 +225,8 @@ def run_ours(args, cfg):
         if not cfg.backward:
             launches[0] = n
             return
-        _, dw = layer.combine_bwd(dY, Ye, inv, w, want_dw=cfg.router_grad, out=dYe); n += layer.last_launch_count()
-        layer.expert_bwd(X, dYe, offsets, perm, grads=grads, out=dXp); n += layer.last_launch_count()
+        _, dw = layer.combine_bwd(dY, Ye, inv, w, want_dw=cfg.router_grad, out=dYe, perm=perm); n += layer.last_launch_count()
+        layer.expert_bwd(X, dYe, offsets, perm, grads=grads, out=dXp, dYe_unmodified=cfg.r in (16, 32)); n += layer.last_launch_count()
         layer.dispatch_bwd(dXp, inv, out=dX); n += layer.last_launch_count()
         if cfg.router_grad:
             layer.route_bwd(X, W_r, idx, w, dw, offsets, perm, dX); n += layer.last_launch_count()
@@ -234,7 +239,6 @@ def run_ours(args, cfg):
 
     for _ in range(args.warmup):
         step()
-    layer.set_option("time_gemm", 1)
     sampler = ClockSampler(local)
     barrier()
     sampler.start()
@@ -244,9 +248,16 @@ def run_ours(args, cfg):
         step()
     e1.record()
     barrier()
-    sampler.stop_flag = True
     ms = e0.elapsed_time(e1)
-    gemm_ms, gemm_launches = layer.gemm_time()
+    # second pass of the same K steps with every grouped-GEMM launch bracketed by CUDA events on its own stream
+    # (tqp_gemm_time); the headline time above carries no such events.  The clock sampler covers both passes.
+    layer.set_option("time_gemm", 1)
+    for _ in range(args.steps):
+        step()
+    barrier()
+    sampler.stop_flag = True
+    gemm_each = layer.gemm_times()
+    gemm_ms, gemm_launches = float(sum(gemm_each)), len(gemm_each)
     layer.set_option("time_gemm", 0)
     ms = max_over_ranks(ms, dist, dev)
     ms_per_step = ms / args.steps
@@ -302,6 +313,8 @@ def run_ours(args, cfg):
     pk = peaks()
     gemm_ms_step = gemm_ms / args.steps
     gemm_tflops = fl["gemm"] / (gemm_ms_step / 1e3) / 1e12 if gemm_ms_step > 0 else 0.0
+    nl = 4 if cfg.backward else 2
+    traffic = NCU_GEMM_TRAFFIC.get(cfg.name, (None, None))
     line = {
         "metric": METRIC, "value": value, "unit": "tokens/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
@@ -310,7 +323,7 @@ def run_ours(args, cfg):
                    "passes": ("fwd+bwd" if cfg.backward else "fwd") + ("+router_grad" if cfg.router_grad else ""), "routing": "zipf1.1" if cfg.skew else "near-uniform",
                    "l2": f"inputs larger than L2 ({3 * cfg.E * cfg.d * cfg.F / 8 / 1e6:.0f} MB code indices + "
                          f"{T * cfg.k * cfg.d * 2 / 1e6:.0f} MB permuted rows per step), no flush",
-                   "gemm_impl": "scaffold" if args.gemm_impl else "tcgen05", "parallelism": f"replicas x{world}, no collective"},
+                   "gemm_impl": GEMM_IMPL_NAMES.get(args.gemm_impl, str(args.gemm_impl)), "parallelism": f"replicas x{world}, no collective"},
         "tflops": world * fl["total"] / (ms_per_step / 1e3) / 1e12,
         "frac_of_bf16_peak": {"measured_burst": fl["total"] / (ms_per_step / 1e3) / 1e12 / pk["tensor_burst"],
                               "measured_sustained": fl["total"] / (ms_per_step / 1e3) / 1e12 / pk["tensor_sustained"],
@@ -318,16 +331,21 @@ def run_ours(args, cfg):
         "clocks": sampler.summary(),
         "e2e": e2e,
         "gpu_launches": launches[0] * args.steps,
+        # the primary denominator is the MEASURED BURST bf16 peak; sustained and datasheet beside it
         "roofline": {"kernel": "grouped dequant GEMM gemm_tcgen05_ts2_kernel (4 launches/step: gate+up, down, dH, dXp)", "bound": "tensor",
-                     "achieved": gemm_tflops, "peak": pk["tensor_sustained"], "unit": "TFLOP/s",
-                     "frac": gemm_tflops / pk["tensor_sustained"], "frac_of_burst": gemm_tflops / pk["tensor_burst"],
-                     "frac_of_datasheet_2250": gemm_tflops / 2250.0, "peak_source": pk["source"] + ", sustained bf16",
+                     "achieved": gemm_tflops, "peak": pk["tensor_burst"], "unit": "TFLOP/s",
+                     "frac": gemm_tflops / pk["tensor_burst"], "frac_of_sustained": gemm_tflops / pk["tensor_sustained"],
+                     "frac_of_datasheet_2250": gemm_tflops / 2250.0, "peak_source": pk["source"] + ", burst bf16 (bf16_tflops)",
                      "gemm_ms_per_step": gemm_ms_step, "gemm_share_of_step": gemm_ms_step / ms_per_step,
                      "gemm_launches": gemm_launches, "flops_per_step": fl["gemm"],
-                     "flops_per_launch": fl["gemm"] / (4.0 if cfg.backward else 2.0), "traffic": NCU_GEMM_TRAFFIC.get(cfg.name)},
+                     "flops_per_launch": fl["gemm"] / (4.0 if cfg.backward else 2.0),
+                     "launch_ms": [float(np.mean(gemm_each[i::nl])) for i in range(nl)] if gemm_each else [],
+                     "traffic": traffic[0], "traffic_source": traffic[1]},
     }
     if world == 1 and not args.no_cpu_baseline:
-        cb = time_oracle(cfg, args.cpu_tokens, 1, 0)
+        # one full oracle pass over the workload's own batch where that takes about a minute; capped at
+        # 8192 tokens (cfg 4 would need ~2 min); --cpu-tokens overrides
+        cb = time_oracle(cfg, args.cpu_tokens if args.cpu_tokens > 0 else min(cfg.T, 8192), 1, 0)
         line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
     print(json.dumps(line), flush=True)
     if dist is not None:
@@ -344,7 +362,7 @@ def main():
     ap.add_argument("--gemm-impl", type=int, default=0)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-tokens", type=int, default=1024, help="tokens in the bounded cpu_baseline sample")
+    ap.add_argument("--cpu-tokens", type=int, default=0, help="tokens of the cpu_baseline oracle pass (0: the whole batch, at most 8192)")
     ap.add_argument("--ref-tokens", type=int, default=256, help="tokens per step of the --impl reference arm")
     args = ap.parse_args()
     cfg = ti.CONFIGS[args.config]

@@ -14,8 +14,9 @@
  *
  * Conventions for EVERY entry point below unless a comment says otherwise:
  *  - All tensor pointers are DEVICE pointers, row-major, contiguous, 16-byte aligned, caller-owned; the
- *    library never frees or retains them beyond the call, except the tqp_weights pointers and the bound
- *    workspace, which must stay valid while the ctx uses them.
+ *    library never frees them and never dereferences them after the call has been enqueued, except the
+ *    tqp_weights pointers and the bound workspace, which must stay valid while the ctx uses them, and the
+ *    buffers of a tqp_step_host_async step until tqp_step_host_wait has returned for it.
  *  - "bf16" / "fp16" tensors are passed as const void* (2 bytes per element).
  *  - `stream` is a cudaStream_t passed as void*.  Every call only enqueues work on it: no host
  *    synchronisation, no device->host copy.  Expert counts/offsets are consumed on the device.
@@ -82,13 +83,13 @@ tqp_status tqp_bind_workspace(tqp_ctx *ctx, void *dev_ptr, size_t bytes, void *s
 /* Records the weight pointers, builds the TMA descriptors over the code indices and converts the codebook
  * to the bf16 lookup table the GEMM mainloop gathers from.  One-time, untimed; needs a bound workspace. */
 tqp_status tqp_bind_weights(tqp_ctx *ctx, const tqp_weights *w, void *stream);
-/* Options (debug / ablation).  "gemm_impl": 0 = tcgen05 grouped GEMM on CTA pairs with the dequantised weight
- * operand in tensor memory, 128-wide producer stages (default), 1 = CUDA-core scaffold, 2 = tcgen05 grouped GEMM, one
- * CTA per tile, weight operand through shared memory, 3 = CTA pairs, weight operand through shared memory, 4 = as 0
- * with 64-wide producer stages.
- * "time_gemm": 0/1, see tqp_gemm_time.  "ablate": bit mask that disables parts of the kernels (results become
- * wrong; timing experiments only; 0 = off).  "trace": n > 0 records a clock64 timeline of one CTA pair in the n-th
- * grouped-GEMM launch from now into the workspace tensor "trace" (tqp_debug_buffer). */
+/* Options.  "gemm_impl": 0 = tcgen05 grouped GEMM on CTA pairs with the dequantised weight operand in tensor memory
+ * (default), 1 = CUDA-core scaffold (test reference), 2 = tcgen05 grouped GEMM, one CTA per tile, weight operand
+ * through shared memory (fallback for M % 256 != 0), 3 = CTA pairs, weight operand through shared memory (fallback for
+ * K % 128 != 0).
+ * "time_gemm": 0/1, see tqp_gemm_time.  "host_chunks": 0 (default) lets tqp_step_host_async choose at run time
+ * whether X goes up and is routed in one piece or in four token chunks; 1 / 4 pin the choice (same results).  Unknown names return TQP_ERR_ARG.  (Kernel instrumentation -- "trace",
+ * "ablate" -- exists only in builds compiled with -DTQP_TRACE and is not part of this interface.) */
 tqp_status tqp_set_option(tqp_ctx *ctx, const char *name, int value);
 
 /* --- forward ------------------------------------------------------------------------------------------ */
@@ -114,16 +115,25 @@ tqp_status tqp_combine(tqp_ctx *ctx, int T, const void *Ye, const int32_t *inv_p
                        void *Y, void *stream);
 
 /* --- backward (loss L = sum(Y * dY)) -------------------------------------------------------------------- */
-/* dYe[p] = topk_w[a] * dY[t] (bf16 [N][d]);  dtopk_w[a] = <dY[t], Ye[p]> (fp32 [T][k], NULL to skip). */
+/* dYe[p] = topk_w[a] * dY[t] (bf16 [N][d]);  dtopk_w[a] = <dY[t], Ye[p]> (fp32 [T][k], NULL to skip).
+ * perm (int32 [N], the array tqp_dispatch wrote together with inv_perm; NULL allowed): when given, and the ctx is a
+ * training ctx with bound weights and r in {16, 32}, dYe is produced by sorted position with a TMA row gather and the
+ * adapter projection s * dYe . B_down^T that tqp_expert_bwd needs is computed from the same rows into the workspace
+ * (one pass instead of two).  With perm == NULL a plain kernel walks inv_perm; the results are the same. */
 tqp_status tqp_combine_bwd(tqp_ctx *ctx, int T, const void *dY, const void *Ye, const int32_t *inv_perm,
-                           const float *topk_w, void *dYe, float *dtopk_w, void *stream);
+                           const int32_t *perm, const float *topk_w, void *dYe, float *dtopk_w, void *stream);
 /* Activation gradient through the frozen dequantised weights and weight gradients of the adapters only
  * (PAPER.md L938).  Needs training=1 and the preceding tqp_expert_fwd of the same T.  dXp bf16 [N][d];
  * dA_gate/dA_up fp32 [E][d][r]; dB_gate/dB_up fp32 [E][r][F]; dA_down fp32 [E][F][r]; dB_down fp32
- * [E][r][d]; gradients are overwritten (exactly 0 for experts with no rows). */
+ * [E][r][d]; gradients are overwritten (exactly 0 for experts with no rows).
+ * flags: 0, or TQP_BWD_DYE_UNMODIFIED = the caller vouches that dYe is exactly the tensor the directly preceding
+ * tqp_combine_bwd (called with perm) on this ctx wrote, unmodified since: its adapter projection is then reused instead of
+ * being recomputed from dYe.  TQP_ERR_STATE if no such call preceded or dYe is another pointer.  With flags = 0 nothing
+ * from an earlier call is trusted (a caller that adds, say, a shared-expert gradient to dYe in place passes 0). */
+#define TQP_BWD_DYE_UNMODIFIED 1
 tqp_status tqp_expert_bwd(tqp_ctx *ctx, int T, const void *X, const void *dYe, const int32_t *offsets,
                           const int32_t *perm, void *dXp, float *dA_gate, float *dB_gate, float *dA_up,
-                          float *dB_up, float *dA_down, float *dB_down, void *stream);
+                          float *dB_up, float *dA_down, float *dB_down, int flags, void *stream);
 /* dX[t] = sum_j dXp[inv_perm[t*k+j]] (fp32 accumulate, j ascending); dX bf16 [T][d]. */
 tqp_status tqp_dispatch_bwd(tqp_ctx *ctx, int T, const void *dXp, const int32_t *inv_perm, void *dX,
                             void *stream);

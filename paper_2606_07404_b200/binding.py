@@ -61,8 +61,8 @@ def load_library() -> ctypes.CDLL:
         lib.tqp_dispatch.argtypes = [vp, ci] + [vp] * 6
         lib.tqp_expert_fwd.argtypes = [vp, ci] + [vp] * 5
         lib.tqp_combine.argtypes = [vp, ci] + [vp] * 5
-        lib.tqp_combine_bwd.argtypes = [vp, ci] + [vp] * 7
-        lib.tqp_expert_bwd.argtypes = [vp, ci] + [vp] * 12
+        lib.tqp_combine_bwd.argtypes = [vp, ci] + [vp] * 8
+        lib.tqp_expert_bwd.argtypes = [vp, ci] + [vp] * 11 + [ci, vp]
         lib.tqp_dispatch_bwd.argtypes = [vp, ci] + [vp] * 4
         lib.tqp_route_bwd.argtypes = [vp, ci] + [vp] * 10
         lib.tqp_step_host.argtypes = [vp, ci] + [vp] * 14
@@ -181,13 +181,14 @@ class TqpLayer:
         return Y
 
     # ---- backward ----
-    def combine_bwd(self, dY, Ye, inv_perm, topk_w, want_dw=True, out=None):
+    def combine_bwd(self, dY, Ye, inv_perm, topk_w, want_dw=True, out=None, perm=None):
+        """perm (the array dispatch returned) selects the fused row-gather path, see tqp.h."""
         t = self.torch
         T = topk_w.shape[0]
         dYe = out if out is not None else t.empty((T * self.k, self.d), dtype=t.bfloat16, device=self.device)
         dw = t.empty((T, self.k), dtype=t.float32, device=self.device) if want_dw else None
-        self._check(self.lib.tqp_combine_bwd(self.ctx, T, _ptr(dY), _ptr(Ye), _ptr(inv_perm), _ptr(topk_w), _ptr(dYe),
-                                             _ptr(dw), self._stream()))
+        self._check(self.lib.tqp_combine_bwd(self.ctx, T, _ptr(dY), _ptr(Ye), _ptr(inv_perm), _ptr(perm), _ptr(topk_w),
+                                             _ptr(dYe), _ptr(dw), self._stream()))
         return dYe, dw
 
     def alloc_grads(self):
@@ -197,14 +198,16 @@ class TqpLayer:
         return {"dA_gate": mk(E, d, r), "dB_gate": mk(E, r, F), "dA_up": mk(E, d, r), "dB_up": mk(E, r, F),
                 "dA_down": mk(E, F, r), "dB_down": mk(E, r, d)}
 
-    def expert_bwd(self, X, dYe, offsets, perm, grads=None, out=None):
+    def expert_bwd(self, X, dYe, offsets, perm, grads=None, out=None, dYe_unmodified=False):
+        """dYe_unmodified=True passes TQP_BWD_DYE_UNMODIFIED (dYe is the untouched output of the preceding fused combine_bwd)."""
         t = self.torch
         T = X.shape[0]
         g = grads if grads is not None else self.alloc_grads()
         dXp = out if out is not None else t.empty((T * self.k, self.d), dtype=t.bfloat16, device=self.device)
         self._check(self.lib.tqp_expert_bwd(self.ctx, T, _ptr(X), _ptr(dYe), _ptr(offsets), _ptr(perm), _ptr(dXp),
                                             _ptr(g["dA_gate"]), _ptr(g["dB_gate"]), _ptr(g["dA_up"]), _ptr(g["dB_up"]),
-                                            _ptr(g["dA_down"]), _ptr(g["dB_down"]), self._stream()))
+                                            _ptr(g["dA_down"]), _ptr(g["dB_down"]), 1 if dYe_unmodified else 0,
+                                            self._stream()))
         return dXp, g
 
     def dispatch_bwd(self, dXp, inv_perm, out=None):

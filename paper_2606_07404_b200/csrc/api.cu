@@ -150,7 +150,6 @@ tqp_status run_gemm(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_
     tqp_status r = c->gemm_impl == 1   ? launch_gemm_scaffold(c, probs, nprob, st)
                    : c->gemm_impl == 2 ? launch_gemm_tcgen05(c, probs, nprob, st)
                    : c->gemm_impl == 3 ? launch_gemm_tcgen05_2cta(c, probs, nprob, st)
-                   : c->gemm_impl == 4 ? launch_gemm_tcgen05_ts(c, probs, nprob, st)
                                        : launch_gemm_tcgen05_ts2(c, probs, nprob, st);
     if (timed) {
         TQP_CUDA_OK(c, cudaEventRecord(c->ev[c->ev_used + 1], st));
@@ -176,6 +175,7 @@ tqp_status tqp_create(tqp_ctx **out, const tqp_layer_desc *desc) {
     tqp_ctx *c = new (std::nothrow) tqp_ctx();
     if (!c) return TQP_ERR_ARG;
     c->desc = *desc;
+    c->device = dev;
     c->ws = layout(*desc);
     c->num_sms = sms > 0 ? sms : 148;
     c->max_tiles = desc->E + (desc->T_max * desc->k) / kTileRows + 1;
@@ -287,10 +287,11 @@ tqp_status tqp_bind_weights(tqp_ctx *c, const tqp_weights *w, void *stream) {
 tqp_status tqp_set_option(tqp_ctx *c, const char *name, int value) {
     if (!c || !name) return TQP_ERR_ARG;
     if (!strcmp(name, "gemm_impl")) {
-        REQ(c, value >= 0 && value <= 4, TQP_ERR_ARG, "gemm_impl must be 0..4");
+        REQ(c, value >= 0 && value <= 3, TQP_ERR_ARG, "gemm_impl must be 0..3");
         c->gemm_impl = value;
         return TQP_OK;
     }
+#ifdef TQP_TRACE   // instrumented builds only (see common.cuh)
     if (!strcmp(name, "trace")) {
         c->trace = value;
         c->trace_seq = 0;
@@ -298,6 +299,12 @@ tqp_status tqp_set_option(tqp_ctx *c, const char *name, int value) {
     }
     if (!strcmp(name, "ablate")) {
         c->ablate = value;
+        return TQP_OK;
+    }
+#endif
+    if (!strcmp(name, "host_chunks")) {
+        REQ(c, value == 0 || value == 1 || value == 4, TQP_ERR_ARG, "host_chunks must be 0 (auto), 1 or 4");
+        c->host_chunks = value;
         return TQP_OK;
     }
     if (!strcmp(name, "time_gemm")) {
@@ -329,8 +336,6 @@ tqp_status tqp_dispatch(tqp_ctx *c, int T, const int32_t *topk_idx, int32_t *cou
     PTR_OK(c, topk_idx); PTR_OK(c, counts); PTR_OK(c, offsets); PTR_OK(c, perm); PTR_OK(c, inv_perm);
     c->disp_T = T;
     c->fwd_T = -1;
-    c->disp_perm = perm;
-    c->disp_inv_perm = inv_perm;
     c->zd_src = nullptr;
     return launch_dispatch(c, T, topk_idx, counts, offsets, perm, inv_perm, (cudaStream_t)stream);
 }
@@ -385,25 +390,26 @@ tqp_status tqp_combine(tqp_ctx *c, int T, const void *Ye, const int32_t *inv_per
     return launch_combine(c, T, (const bf16 *)Ye, inv_perm, topk_w, (bf16 *)Y, (cudaStream_t)stream);
 }
 
-tqp_status tqp_combine_bwd(tqp_ctx *c, int T, const void *dY, const void *Ye, const int32_t *inv_perm,
+tqp_status tqp_combine_bwd(tqp_ctx *c, int T, const void *dY, const void *Ye, const int32_t *inv_perm, const int32_t *perm,
                            const float *topk_w, void *dYe, float *dtopk_w, void *stream) {
     tqp_status st = common_checks(c, T, false);
     if (st != TQP_OK) return st;
     PTR_OK(c, dY); PTR_OK(c, inv_perm); PTR_OK(c, topk_w); PTR_OK(c, dYe);
     if (dtopk_w) PTR_OK(c, Ye);
+    if (perm) REQ(c, aligned16(perm), TQP_ERR_ALIGN, "perm is not 16-byte aligned");
     const tqp_layer_desc &D = c->desc;
     c->zd_src = nullptr;
-    if ((D.r == 16 || D.r == 32) && D.training && c->have_weights && c->disp_T == T && c->disp_inv_perm == inv_perm) {
+    if (perm && (D.r == 16 || D.r == 32) && D.training && c->have_weights) {
         // Fused: dYe[p] = w[a] dY[t] by sorted position (a = perm[p]) and, from the same rows, Zd = s dYe . B_d^T, the
         // adapter projection tqp_expert_bwd needs.  dw = <dY, Ye> is a separate reduction when asked for.
         if (D.d % 256 == 0) {
             CUtensorMap gm[3];
             st = gather_maps(c, gm, dY, (uint64_t)T, dYe, (uint64_t)T * D.k, D.d);
             if (st == TQP_OK)
-                st = launch_rows_gather_proj(c, &gm[0], T, &gm[1], &gm[2], T * D.k, D.d, c->disp_perm, topk_w, (const bf16 *)c->w.B_down,
+                st = launch_rows_gather_proj(c, &gm[0], T, &gm[1], &gm[2], T * D.k, D.d, perm, topk_w, (const bf16 *)c->w.B_down,
                                              nullptr, 0, D.lora_scale, c->p<bf16>(c->ws.Zd), nullptr, (cudaStream_t)stream);
         } else {
-            st = launch_rows_proj(c, (const bf16 *)dY, D.d, c->disp_perm, topk_w, (bf16 *)dYe, (const bf16 *)c->w.B_down, nullptr, 0,
+            st = launch_rows_proj(c, (const bf16 *)dY, D.d, perm, topk_w, (bf16 *)dYe, (const bf16 *)c->w.B_down, nullptr, 0,
                                   D.lora_scale, c->p<bf16>(c->ws.Zd), nullptr, (cudaStream_t)stream);
         }
         if (st != TQP_OK) return st;
@@ -418,7 +424,7 @@ tqp_status tqp_combine_bwd(tqp_ctx *c, int T, const void *dY, const void *Ye, co
 
 tqp_status tqp_expert_bwd(tqp_ctx *c, int T, const void *X, const void *dYe, const int32_t *offsets, const int32_t *perm,
                           void *dXp, float *dA_gate, float *dB_gate, float *dA_up, float *dB_up, float *dA_down,
-                          float *dB_down, void *stream) {
+                          float *dB_down, int flags, void *stream) {
     tqp_status st = common_checks(c, T, true);
     if (st != TQP_OK) return st;
     PTR_OK(c, X); PTR_OK(c, dYe); PTR_OK(c, offsets); PTR_OK(c, perm); PTR_OK(c, dXp);
@@ -434,8 +440,12 @@ tqp_status tqp_expert_bwd(tqp_ctx *c, int T, const void *X, const void *dYe, con
     bf16 *dH = c->p<bf16>(c->ws.dH), *dG = c->p<bf16>(c->ws.dG), *dU = c->p<bf16>(c->ws.dU);
     bf16 *Zd = c->p<bf16>(c->ws.Zd), *Zg = c->p<bf16>(c->ws.Zg), *Zu = c->p<bf16>(c->ws.Zu);
 #define CK(x) do { st = (x); if (st != TQP_OK) return st; } while (0)
+    REQ(c, (flags & ~TQP_BWD_DYE_UNMODIFIED) == 0, TQP_ERR_ARG, "unknown flag");
+    if (flags & TQP_BWD_DYE_UNMODIFIED)
+        REQ(c, c->zd_src == dYe, TQP_ERR_STATE,
+            "TQP_BWD_DYE_UNMODIFIED: dYe is not the tensor the directly preceding fused tqp_combine_bwd (perm given) wrote");
     // down projection: dH = dYe . Wd_eff^T,  dB_d = (s h A_d)^T dYe,  dA_d = h^T (s dYe B_d^T)
-    if (c->zd_src != dYe)   // not produced by the fused tqp_combine_bwd of this step
+    if (!(flags & TQP_BWD_DYE_UNMODIFIED))   // the caller does not vouch for the projection tqp_combine_bwd may have left
         CK(launch_rows_proj(c, dye, D.d, nullptr, nullptr, nullptr, (const bf16 *)c->w.B_down, nullptr, 0, ls, Zd, nullptr, s));
     c->zd_src = nullptr;
     GemmProblem ph = c->prob_dh;
@@ -602,12 +612,19 @@ tqp_status tqp_step_host_async(tqp_ctx *c, int T, const void *X_host, const void
     // ordered after what `s` held before.  The uploads are NOT: they only wait for the step before last, which used the
     // same staging set (its kernels read X until the end of its backward pass), so that the uploads of a step issued
     // while the previous one is still running travel under that step's kernels.
-    if (c->host_seq >= 2) TQP_CUDA_OK(c, cudaStreamWaitEvent(c->copy_in, c->ev_comp[par], 0));
+    if (c->host_seq >= 2) {
+        TQP_CUDA_OK(c, cudaStreamWaitEvent(c->copy_in, c->ev_comp[par], 0));
+    } else {   // first use of this staging set: order the uploads after what `s` holds now (e.g. tqp_bind_workspace's zero-fill)
+        TQP_CUDA_OK(c, cudaEventRecord(c->ev_start, s));
+        TQP_CUDA_OK(c, cudaStreamWaitEvent(c->copy_in, c->ev_start, 0));
+    }
     {
         // With the previous step still running its kernels, this step's X will have landed long before `s` gets to the
         // router: upload and route it in one piece then (four router launches of T / 4 tokens fill the SMs worse than one).
+        // (Which of the two is taken depends on timing; both give the same bits -- the router is token-wise -- and the option
+        // "host_chunks" = 1 / 4 pins the choice for tests.)
         const bool behind = c->host_seq >= 1 && cudaEventQuery(c->ev_comp[par ^ 1]) == cudaErrorNotReady;
-        const int nch = (T >= 1024 && !behind) ? 4 : 1, per = ((T + nch - 1) / nch + 3) & ~3;   // chunk starts stay 16-byte aligned in every array
+        const int nch = c->host_chunks ? c->host_chunks : (T >= 1024 && !behind) ? 4 : 1, per = ((T + nch - 1) / nch + 3) & ~3;   // chunk starts stay 16-byte aligned in every array
         float *lg = c->p<float>(c->ws.logits);
         for (int ch = 0; ch < nch; ++ch) {
             const int t0 = ch * per, tc = std::min(per, T - t0);
@@ -630,9 +647,10 @@ tqp_status tqp_step_host_async(tqp_ctx *c, int T, const void *X_host, const void
     TQP_CUDA_OK(c, cudaMemcpyAsync(Y_host, Y, row_bytes, cudaMemcpyDeviceToHost, c->copy_out));
     TQP_CUDA_OK(c, cudaEventRecord(c->ev_yout, c->copy_out));
     TQP_CUDA_OK(c, cudaStreamWaitEvent(s, c->ev_dy, 0));
-    CK(tqp_combine_bwd(c, T, dY, Ye, inv, tw, dYe, dW_r ? dtw : nullptr, s));
+    CK(tqp_combine_bwd(c, T, dY, Ye, inv, perm, tw, dYe, dW_r ? dtw : nullptr, s));
     c->defer_tail = 1;
-    st = tqp_expert_bwd(c, T, X, dYe, offs, perm, dXp, dA_gate, dB_gate, dA_up, dB_up, dA_down, dB_down, s);
+    st = tqp_expert_bwd(c, T, X, dYe, offs, perm, dXp, dA_gate, dB_gate, dA_up, dB_up, dA_down, dB_down,
+                        c->zd_src == dYe ? TQP_BWD_DYE_UNMODIFIED : 0, s);
     c->defer_tail = 0;
     total += c->launches;
     if (st != TQP_OK) { c->tail.pending = false; return st; }

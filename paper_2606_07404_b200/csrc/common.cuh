@@ -16,6 +16,14 @@ namespace tqp {
 
 typedef __nv_bfloat16 bf16;
 
+// Debug instrumentation (clock64 timelines of one CTA pair, ablation switches that make results wrong on purpose) exists only
+// in builds compiled with -DTQP_TRACE; in the product build TQP_DBG(x) is the constant 0 and the compiler drops those branches.
+#ifdef TQP_TRACE
+#define TQP_DBG(x) (x)
+#else
+#define TQP_DBG(x) 0
+#endif
+
 constexpr int kTileRows = 256;   // max routed rows (UMMA N) of one grouped-GEMM tile
 constexpr int kRowPad = 512;     // rows of slack after N in every [N][*] workspace tensor (TMA boxes / 16-row groups over-read)
 constexpr int kLoraPad = 64;     // adapter projections are stored [N][64] bf16 (one 128-byte swizzle row)
@@ -80,8 +88,11 @@ struct tqp_ctx {
     int gemm_impl = 0;          // 0 tcgen05 CTA-pair kernel, 1 scaffold, 2 tcgen05 single-CTA kernel
     int fwd_T = -1;             // T of the last training-mode expert_fwd (TQP_ERR_STATE check)
     int disp_T = -1;
-    const int32_t *disp_perm = nullptr, *disp_inv_perm = nullptr;   // arrays written by the last tqp_dispatch
-    const void *zd_src = nullptr;   // dYe tensor whose projection dYe.B_d^T already sits in ws.Zd (fused tqp_combine_bwd)
+    // Set by the fused tqp_combine_bwd: ws.Zd holds s dYe.B_d^T of the dYe tensor it wrote (kept only to VALIDATE the caller's
+    // TQP_BWD_DYE_UNMODIFIED claim in tqp_expert_bwd, never dereferenced); cleared by every other call that could invalidate it
+    const void *zd_src = nullptr;
+    int device = 0;                 // the device the ctx was created on (kernel attributes are per device)
+    std::vector<const void *> smem_attr_done;   // kernels whose dynamic shared-memory limit has been raised on `device`
     int launches = 0;
     int num_sms = 148;
     int max_tiles = 0;
@@ -99,6 +110,7 @@ struct tqp_ctx {
     // step computes; ev_done[p] = the step that used set p has delivered Y and dX to the host, ev_comp[p] = its kernels are done
     cudaEvent_t ev_done[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr};
     long long host_seq = 0;
+    int host_chunks = 0;        // tqp_step_host_async: X upload / router in 1 or 4 token chunks (0: chosen at run time)
     // tqp_step_host defers all adapter weight gradients (nothing else depends on them) until dX is on its way to the host
     int defer_tail = 0;
     struct { float *dA_gate, *dB_gate, *dA_up, *dB_up, *dA_down, *dB_down; const tqp::bf16 *dYe; const int32_t *offsets; bool pending; } tail = {};
@@ -177,8 +189,20 @@ tqp_status launch_rows_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 
 tqp_status launch_gemm_scaffold(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);
 tqp_status launch_gemm_tcgen05(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);       // 1 CTA / tile
 tqp_status launch_gemm_tcgen05_2cta(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);  // CTA pair / tile
-tqp_status launch_gemm_tcgen05_ts(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);
-tqp_status launch_gemm_tcgen05_ts2(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);   // ... 128-wide A stages    // CTA pair, A in TMEM (K-major only)
+tqp_status launch_gemm_tcgen05_ts2(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st);   // CTA pair, weight operand in TMEM, 128-wide A stages (default)
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: raised once per ctx (a ctx lives on one device)
+inline tqp_status ensure_dyn_smem(tqp_ctx *c, const void *func, int bytes) {
+    for (const void *f : c->smem_attr_done)
+        if (f == func) return TQP_OK;
+    cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) {
+        c->err = std::string("cudaFuncSetAttribute(MaxDynamicSharedMemorySize): ") + cudaGetErrorString(e);
+        return TQP_ERR_CUDA;
+    }
+    c->smem_attr_done.push_back(func);
+    return TQP_OK;
+}
 
 // ---- device helpers ------------------------------------------------------------------------------------
 __device__ __forceinline__ float bf16_bits_to_float(uint16_t b) { return __uint_as_float(((uint32_t)b) << 16); }

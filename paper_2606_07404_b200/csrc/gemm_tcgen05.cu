@@ -298,13 +298,13 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmArgs args, const uint4 *__restri
 #pragma unroll
                     for (int j = 0; j < 8; ++j) {
                         const uint32_t code = (c01[j >> 2] >> ((j & 3) * 8)) & 0xffu;
-                        uint4 v = (ablate & 1) ? make_uint4(code, code, code, code) : lut_s[code * 8 + c];
+                        uint4 v = TQP_DBG(ablate & 1) ? make_uint4(code, code, code, code) : lut_s[code * 8 + c];
                         __nv_bfloat162 *pv = reinterpret_cast<__nv_bfloat162 *>(&v);
-                        if (!(ablate & 4)) {
+                        if (!TQP_DBG(ablate & 4)) {
 #pragma unroll
                             for (int q = 0; q < 4; ++q) pv[q] = __hmul2(pv[q], s2);
                         }
-                        if (!(ablate & 2)) *reinterpret_cast<uint4 *>(as + rowoff + ((j ^ sw) << 4)) = v;
+                        if (!TQP_DBG(ablate & 2)) *reinterpret_cast<uint4 *>(as + rowoff + ((j ^ sw) << 4)) = v;
                     }
                     fence_async_smem();
                     __syncwarp();
@@ -382,11 +382,7 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmArgs args, const uint4 *__restri
 }  // namespace g5
 
 tqp_status launch_gemm_tcgen05(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        TQP_CUDA_OK(c, cudaFuncSetAttribute(g5::gemm_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, g5::SMEM_BYTES));
-        attr_set = true;
-    }
+    if (tqp_status st_attr = ensure_dyn_smem(c, reinterpret_cast<const void *>(&g5::gemm_tcgen05_kernel), g5::SMEM_BYTES)) return st_attr;
     GemmArgs args;
     for (int i = 0; i < nprob; ++i) args.p[i] = probs[i];
     args.nprob = nprob;

@@ -103,7 +103,7 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                     const int nkb = S.K / BK;
                     for (int kb = 0; kb < nkb; ++kb) {
                         mbar_wait(empty(st.s), st.ph ^ 1);
-                        if (ablate & 8) { if (rank == 0) mbar_arrive(full(st.s)); st.next(NSTAGE); continue; }
+                        if (TQP_DBG(ablate & 8)) { if (rank == 0) mbar_arrive(full(st.s)); st.next(NSTAGE); continue; }
                         if (rank == 0) mbar_expect_tx(full(st.s), 2 * X_BYTES);
                         tma_load_2d_pair(sbase + OFF_X + st.s * X_BYTES, &S.act_map2, kb * BK, row, full_remote + 8u * st.s);
                         st.next(NSTAGE);
@@ -131,7 +131,7 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                     const int npair = S.K / (2 * BK);
                     for (int kp = 0; kp < npair; ++kp) {
                         mbar_wait(idx_empty(iq.s), iq.ph ^ 1);
-                        if (ablate & 64) { mbar_arrive(idx_full(iq.s)); iq.next(IDXQ); continue; }
+                        if (TQP_DBG(ablate & 64)) { mbar_arrive(idx_full(iq.s)); iq.next(IDXQ); continue; }
                         mbar_expect_tx(idx_full(iq.s), IDX_BYTES);
                         const int c0 = S.kmajor ? kp * 16 : it.m0 / 8;
                         const int c1 = S.kmajor ? it.t.expert * pb.M + it.m0 : it.t.expert * S.K + kp * 2 * BK;
@@ -170,19 +170,19 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                     const uint32_t a_hi = kmajor ? hi_k : hi_mn, a_lo = kmajor ? lo_k : lo_mn, a_step = kmajor ? 2u : 256u;
                     for (int kb = 0; kb < nkb; ++kb) {
                         long long tr0 = 0;
-                        if (trace && cid == 0) tr0 = clock64();
+                        if (TQP_DBG(trace != nullptr) && cid == 0) tr0 = clock64();
                         mbar_wait<true>(full(st.s), st.ph);
                         tc_fence_after();
-                        if (trace && cid == 0 && tcount < 2000) { trace[tcount * 4 + 0] = tr0; trace[tcount * 4 + 1] = clock64(); }
+                        if (TQP_DBG(trace != nullptr) && cid == 0 && tcount < 2000) { trace[tcount * 4 + 0] = tr0; trace[tcount * 4 + 1] = clock64(); }
                         const uint32_t xs = x16 + st.s * (X_BYTES >> 4), as = a16 + st.s * (A_BYTES >> 4);
 #pragma unroll
                         for (int kk = 0; kk < BK / 16; ++kk) {
-                            if (ablate & 32) break;
+                            if (TQP_DBG(ablate & 32)) break;
                             umma_bf16<2>(d_tmem, desc_from(a_hi, a_lo, as + kk * a_step), desc_from(hi_k, lo_k, xs + kk * 2), idesc, accum);
                             accum = 1;
                         }
                         umma_commit_pair(empty(st.s), 3);
-                        if (trace && cid == 0 && tcount < 2000) { trace[tcount * 4 + 2] = clock64(); trace[tcount * 4 + 3] = kb; ++tcount; }
+                        if (TQP_DBG(trace != nullptr) && cid == 0 && tcount < 2000) { trace[tcount * 4 + 2] = clock64(); trace[tcount * 4 + 3] = kb; ++tcount; }
                         st.next(NSTAGE);
                     }
                 }
@@ -259,7 +259,7 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                         const __nv_bfloat162 s2 = __float2bfloat162_rn(__half2float(sc_next));
                         if (!kmajor && kb + 2 < nkb) sc_next = scale_p[(kb + 2 - g) * BK];
                         long long tr0 = 0;
-                        const bool tr = trace && cid == 0 && rank == 0 && threadIdx.x == W_DEQ0 * 32 && dcount < 1000;
+                        const bool tr = TQP_DBG(trace != nullptr) && cid == 0 && rank == 0 && threadIdx.x == W_DEQ0 * 32 && dcount < 1000;
                         if (tr) tr0 = clock64();
                         mbar_wait(empty(st.s), st.ph ^ 1);
                         if (tr) { trace[8000 + dcount * 4] = tr0; trace[8000 + dcount * 4 + 1] = clock64(); }
@@ -268,16 +268,16 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
 #pragma unroll
                         for (int j = 0; j < 8; ++j) {
                             const uint32_t code = (c01[j >> 2] >> ((j & 3) * 8)) & 0xffu;
-                            uint4 v = (ablate & 1) ? make_uint4(code, code, code, code) : lds128(lut_a + code * 128);
+                            uint4 v = TQP_DBG(ablate & 1) ? make_uint4(code, code, code, code) : lds128(lut_a + code * 128);
                             __nv_bfloat162 *pv = reinterpret_cast<__nv_bfloat162 *>(&v);
-                            if (!(ablate & 4)) {
+                            if (!TQP_DBG(ablate & 4)) {
 #pragma unroll
                                 for (int q = 0; q < 4; ++q) pv[q] = __hmul2(pv[q], s2);
                             }
-                            if (!(ablate & 2)) sts128(as + ((j ^ sw) << 4), v);
+                            if (!TQP_DBG(ablate & 2)) sts128(as + ((j ^ sw) << 4), v);
                         }
                         if (tr) trace[12000 + dcount * 2] = clock64();
-                        if (!(ablate & 128)) fence_async_smem();
+                        if (!TQP_DBG(ablate & 128)) fence_async_smem();
                         if (tr) trace[8000 + dcount * 4 + 2] = clock64();
                         __syncwarp();
                         if (tr) trace[12000 + dcount * 2 + 1] = clock64();
@@ -339,7 +339,7 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
                               float2_to_bf16x2(__uint_as_float(v[1][4 * g8 + 2]), __uint_as_float(v[1][4 * g8 + 3])));
                 }
                 named_bar_sync(1, 128);   // staging tile complete; also orders the reuse of the other buffer
-                if (!(ablate & 16)) {
+                if (!TQP_DBG(ablate & 16)) {
 #pragma unroll
                     for (int i = 0; i < EPI_ROWS * 16 / 128; ++i) {
                         const int r = et / 16 + 8 * i, ch = et % 16;
@@ -371,11 +371,7 @@ gemm_tcgen05_2cta_kernel(const __grid_constant__ GemmArgs args, const uint4 *__r
 tqp_status launch_gemm_tcgen05_2cta(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st) {
     for (int i = 0; i < nprob; ++i)
         if (probs[i].M % (2 * g2::BM) != 0) return launch_gemm_tcgen05(c, probs, nprob, st);   // odd number of 128-row tiles
-    static bool attr_set = false;
-    if (!attr_set) {
-        TQP_CUDA_OK(c, cudaFuncSetAttribute(g2::gemm_tcgen05_2cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, g2::SMEM_BYTES));
-        attr_set = true;
-    }
+    if (tqp_status st_attr = ensure_dyn_smem(c, reinterpret_cast<const void *>(&g2::gemm_tcgen05_2cta_kernel), g2::SMEM_BYTES)) return st_attr;
     GemmArgs args;
     for (int i = 0; i < nprob; ++i) args.p[i] = probs[i];
     args.nprob = nprob;

@@ -133,7 +133,7 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                     const int nkb = S.K / BK;
                     for (int kb = 0; kb < nkb; ++kb) {
                         mbar_wait(emptyB(st.s), st.ph ^ 1);
-                        if (ablate & 64) {   // timing experiment: no activation traffic (the MMAs read stale tiles)
+                        if (TQP_DBG(ablate & 64)) {   // timing experiment: no activation traffic (the MMAs read stale tiles)
                             if (rank == 0) mbar_arrive(fullB(st.s));
                             st.next(NSTAGE);
                             continue;
@@ -207,7 +207,7 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                 const uint32_t aph = cnt & 1;
                 ++cnt;
                 const int n = max(16, (it.t.rows + 15) & ~15);
-                const bool trc = trace && cid == 0 && cnt <= 400;   // per item: start | accumulator free | first operands | per-stage waits | end
+                const bool trc = TQP_DBG(trace != nullptr) && cid == 0 && cnt <= 400;   // per item: start | accumulator free | first operands | per-stage waits | end
                 long long ts0 = 0, ts1 = 0, ts2 = 0, twait = 0, twaitb = 0;
                 if (trc) ts0 = clock64();
                 mbar_wait<true>(tmem_empty, aph ^ 1);   // the epilogue has drained the previous item's accumulator
@@ -447,7 +447,7 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
             ++cnt;
             mbar_wait(tmem_full, aph);
             tc_fence_after();
-            const bool tre = trace && cid == 0 && rank == 0 && et == 0 && cnt <= 400;
+            const bool tre = TQP_DBG(trace != nullptr) && cid == 0 && rank == 0 && et == 0 && cnt <= 400;
             if (tre) trace[4000 + (cnt - 1) * 4] = clock64();
             named_bar_sync(1, 128);   // every epilogue warp has finished storing the previous item out of the staging tile
             const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + TM_ACC;
@@ -471,7 +471,7 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
             if (lane == 0) mbar_arrive_cluster(tmem_empty_remote);
             if (tre) trace[4000 + (cnt - 1) * 4 + 1] = clock64();
             named_bar_sync(1, 128);   // staging tile complete
-            if (!(ablate & 16)) {
+            if (!TQP_DBG(ablate & 16)) {
                 bf16 *outp = pb.out + (size_t)it.t.row0 * M + it.m0;
                 for (int r = et / 16; r < it.t.rows; r += 8) {
                     const int chk = et % 16;
@@ -501,11 +501,7 @@ tqp_status launch_gemm_tcgen05_ts2(tqp_ctx *c, const GemmProblem *probs, int npr
         for (int sg = 0; sg < p.nseg; ++sg) ok = ok && p.seg[sg].K % gt2::AK == 0;
         if (!ok) return launch_gemm_tcgen05_2cta(c, probs, nprob, st);
     }
-    static bool attr_set = false;
-    if (!attr_set) {
-        TQP_CUDA_OK(c, cudaFuncSetAttribute(gt2::gemm_tcgen05_ts2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, gt2::SMEM_BYTES));
-        attr_set = true;
-    }
+    if (tqp_status st_attr = ensure_dyn_smem(c, reinterpret_cast<const void *>(&gt2::gemm_tcgen05_ts2_kernel), gt2::SMEM_BYTES)) return st_attr;
     GemmArgs args;
     for (int i = 0; i < nprob; ++i) args.p[i] = probs[i];
     args.nprob = nprob;

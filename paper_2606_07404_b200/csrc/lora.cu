@@ -125,7 +125,7 @@ __global__ void __launch_bounds__(PJ_THREADS, 2) rows_proj_kernel(const __grid_c
         const int r = rr + RSTEP * i;
         src[i] = nullptr;   // rows past `valid` are not loaded (zeros; their outputs are never stored)
         roww[i] = 1.f;
-        if (r < valid && !(a.ablate & 1024)) {
+        if (r < valid && !TQP_DBG(a.ablate & 1024)) {
             int srow = row0 + r;
             if (a.perm) {
                 const int as = a.perm[srow];
@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(PJ_THREADS, 2) rows_proj_kernel(const __grid_c
         for (int q = 0; q < 4; ++q) acc[n][q] = 0.f;
 
     const int nk = K / PJ_KC;
-    const bool rewrite = a.roww != nullptr, thru = a.through != nullptr && !(a.ablate & 256);
+    const bool rewrite = a.roww != nullptr, thru = a.through != nullptr && !TQP_DBG(a.ablate & 256);
 #pragma unroll
     for (int s = 0; s < PJ_D - 1; ++s) {
         if (s < nk) { fetch(s, pre[s]); issue_w(s); }
@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(PJ_THREADS, 2) rows_proj_kernel(const __grid_c
         __syncthreads();               // rows + adapter chunk kc visible; everyone is past the MMAs of step kc - 1
         if (kc + PJ_WST - 1 < nk) issue_w(kc + PJ_WST - 1);
         cp_async_commit();
-        if (warp * 16 < valid && !(a.ablate & 512)) {
+        if (warp * 16 < valid && !TQP_DBG(a.ablate & 512)) {
             const uint32_t w_s = sbase + C::OFF_W + (kc % PJ_WST) * C::W_BYTES;
             const uint32_t a_addr = rows_s + ((warp * 16 + lane % 16) * PJ_LD + (lane / 16) * 8) * 2;
             const uint32_t b_addr = KR ? w_s + ((lane % 8 + ((lane / 8) % 2) * 8) * C::WLD + (lane / 16) * 8) * 2
@@ -242,11 +242,7 @@ __global__ void __launch_bounds__(PJ_THREADS, 2) rows_proj_kernel(const __grid_c
 template <int R, int NW, bool KR>
 static tqp_status launch_proj_t(tqp_ctx *c, const ProjArgs &a, cudaStream_t st) {
     using C = ProjCfg<R, NW, KR>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        TQP_CUDA_OK(c, cudaFuncSetAttribute(rows_proj_kernel<R, NW, KR>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-        attr_set = true;
-    }
+    if (tqp_status st_attr = ensure_dyn_smem(c, reinterpret_cast<const void *>(&rows_proj_kernel<R, NW, KR>), C::SMEM)) return st_attr;
     dim3 grid(c->max_tiles, kTileRows / PJ_ROWS);
     rows_proj_kernel<R, NW, KR><<<grid, PJ_THREADS, C::SMEM, st>>>(a, c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles));
     TQP_LAUNCH_OK(c);
@@ -371,11 +367,7 @@ __global__ void __launch_bounds__(PJ_THREADS, 2) rows_proj_tma_kernel(const __gr
 template <int R, bool KR>
 static tqp_status launch_proj_tma_t(tqp_ctx *c, const ProjTmaArgs &a, cudaStream_t st) {
     using C = ProjTmaCfg<R, KR>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        TQP_CUDA_OK(c, cudaFuncSetAttribute(rows_proj_tma_kernel<R, KR>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-        attr_set = true;
-    }
+    if (tqp_status st_attr = ensure_dyn_smem(c, reinterpret_cast<const void *>(&rows_proj_tma_kernel<R, KR>), C::SMEM)) return st_attr;
     dim3 grid(c->max_tiles, kTileRows / PJ_ROWS);
     rows_proj_tma_kernel<R, KR><<<grid, PJ_THREADS, C::SMEM, st>>>(a, c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles));
     TQP_LAUNCH_OK(c);
@@ -543,7 +535,7 @@ __global__ void __launch_bounds__(GP_THREADS, 1) rows_gather_proj_kernel(const _
                 const int st = n % NST;
                 mbar_wait((SCALE ? ready0 : full0) + 8 * st, (n / NST) & 1);
                 const uint32_t rows_s = sbase + st * C::ROWS_BYTES;
-                if (!(a.ablate & 256) && (whole ? lane == 0 : lane < nl)) {
+                if (!TQP_DBG(a.ablate & 256) && (whole ? lane == 0 : lane < nl)) {
                     if (whole) tma_store_2d(&a.out_map, kc * GP_COLS, g.row0, rows_s, pol);
                     else tma_scatter4(&a.sc_map, kc * GP_COLS, dr[0], dr[1], dr[2], dr[3], rows_s + lane * (4 * GP_COLS * 2), pol);
                     bulk_commit_group();
@@ -632,7 +624,7 @@ __global__ void __launch_bounds__(GP_THREADS, 1) rows_gather_proj_kernel(const _
                     if (lane == 0) mbar_arrive(ready0 + 8 * st);
                 }
             }
-            if (active && !(a.ablate & 512)) {
+            if (active && !TQP_DBG(a.ablate & 512)) {
                 const uint32_t ra = rows_s + a_off + ss * 128;
                 const uint4 x0 = lds128(ra), x1 = lds128(ra + a_sw), y0 = lds128(ra + 8 * GP_COLS * 2), y1 = lds128(ra + 8 * GP_COLS * 2 + a_sw);
                 const uint4 P = odd ? x1 : x0, Q = odd ? x0 : x1, P8 = odd ? y1 : y0, Q8 = odd ? y0 : y1;   // chunk t | t+4 of rows g | g+8
@@ -688,11 +680,7 @@ __global__ void __launch_bounds__(GP_THREADS, 1) rows_gather_proj_kernel(const _
 template <int R, int NW, bool KR, bool SCALE>
 static tqp_status launch_gather_t(tqp_ctx *c, const GatherArgs &a, cudaStream_t st) {
     using C = GatherCfg<R, NW, KR>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        TQP_CUDA_OK(c, cudaFuncSetAttribute(rows_gather_proj_kernel<R, NW, KR, SCALE>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-        attr_set = true;
-    }
+    if (tqp_status st_attr = ensure_dyn_smem(c, reinterpret_cast<const void *>(&rows_gather_proj_kernel<R, NW, KR, SCALE>), C::SMEM)) return st_attr;
     const int grid = std::min(c->num_sms, c->max_tiles * (kTileRows / PJ_ROWS));
     int32_t *counter = c->p<int32_t>(c->ws.sched);
     TQP_CUDA_OK(c, cudaMemsetAsync(counter, 0, sizeof(int32_t), st));
@@ -954,11 +942,7 @@ __global__ void __launch_bounds__(256) lora_wgrad_small_kernel(const bf16 *__res
 template <int R, int NS>
 static tqp_status launch_wgrad_t(tqp_ctx *c, const WgradArgs &a, const int32_t *offsets, cudaStream_t st) {
     using C = WgradCfg<R, NS>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        TQP_CUDA_OK(c, cudaFuncSetAttribute(rows_wgrad_kernel<R, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-        attr_set = true;
-    }
+    if (tqp_status st_attr = ensure_dyn_smem(c, reinterpret_cast<const void *>(&rows_wgrad_kernel<R, NS>), C::SMEM)) return st_attr;
     rows_wgrad_kernel<R, NS><<<dim3(c->desc.E + c->max_xsegs, a.width / WG_COLS), 128, C::SMEM, st>>>(a, offsets);
     TQP_LAUNCH_OK(c);
     wgrad_reduce_kernel<<<dim3(c->desc.E, 4), 512, 0, st>>>(a, NS, R);

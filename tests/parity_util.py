@@ -42,8 +42,10 @@ def make_layer(inp, T_max=None, training=True, gemm_impl=0):
     return layer, dev
 
 
-def run_gpu(inp, backward=True, router_grad=False, gemm_impl=0, keep_dev=False):
-    """The whole chain through the C ABI; returns fp32/int numpy arrays keyed like oracle.layer()."""
+def run_gpu(inp, backward=True, router_grad=False, gemm_impl=0, keep_dev=False, fused_bwd=True):
+    """The whole chain through the C ABI; returns fp32/int numpy arrays keyed like oracle.layer().  fused_bwd: the call
+    sequence bench.py times (tqp_combine_bwd with perm, tqp_expert_bwd with TQP_BWD_DYE_UNMODIFIED); False: the plain
+    combine_bwd kernel and an expert_bwd that trusts nothing from earlier calls."""
     import torch
     layer, dev = make_layer(inp, training=backward, gemm_impl=gemm_impl)
     T, k, F, d = inp["T"], inp["k"], inp["F"], inp["d"]
@@ -59,8 +61,9 @@ def run_gpu(inp, backward=True, router_grad=False, gemm_impl=0, keep_dev=False):
         res[name] = layer.debug_buffer(name, (N, F), torch.bfloat16).clone()
     res["Xp"] = layer.debug_buffer("Xp", (N, d), torch.bfloat16).clone()
     if backward:
-        dYe, dw = layer.combine_bwd(dev["dY"], Ye, inv, w, want_dw=True)
-        dXp, grads = layer.expert_bwd(dev["X"], dYe, offsets, perm)
+        fused = fused_bwd and inp["r"] in (16, 32)
+        dYe, dw = layer.combine_bwd(dev["dY"], Ye, inv, w, want_dw=True, perm=perm if fused_bwd else None)
+        dXp, grads = layer.expert_bwd(dev["X"], dYe, offsets, perm, dYe_unmodified=fused)
         dX = layer.dispatch_bwd(dXp, inv)
         res.update(dYe=dYe, dtopk_w=dw, dXp=dXp, dX_experts=dX.clone(), **grads)
         for name in ("dH", "dG", "dU"):

@@ -29,8 +29,14 @@ def _case(seed, big):
     return cfg, inp
 
 
-@pytest.mark.parametrize("seed,big", [(1000, False), (1003, False), (1017, False), (1020, False), (1036, False),
-                                      (5001, True), (5012, True), (5016, True), (5025, True), (5028, True)])
+# Seeds: the contiguous ranges 1000-1004 (small shapes) and 5000-5004 (big shapes), chosen without looking at results,
+# plus the non-contiguous seeds of round 1 (1017, 1020, 1036, 5012, 5016, 5025, 5028; their selection rule was not recorded),
+# kept as regression cases.
+SEEDS = sorted({(s, False) for s in (1000, 1001, 1002, 1003, 1004, 1017, 1020, 1036)} |
+               {(s, True) for s in (5000, 5001, 5002, 5003, 5004, 5012, 5016, 5025, 5028)})
+
+
+@pytest.mark.parametrize("seed,big", SEEDS)
 def test_random_shape_matches_the_oracle(seed, big):
     cfg, inp = _case(seed, big)
     check_all(inp, backward=True, router_grad=cfg.router_grad, gemm_impl=0)

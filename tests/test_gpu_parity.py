@@ -57,8 +57,8 @@ def test_cfg0_tiny_full_chain(gemm_impl):
     check_all(inp, backward=True, router_grad=True, gemm_impl=gemm_impl)
 
 
-@pytest.mark.parametrize("gemm_impl", [1, 2, 3, 4, 0],
-                         ids=["scaffold", "tcgen05_1cta", "tcgen05_2cta_smemA", "tcgen05_tmemA_64", "tcgen05"])
+@pytest.mark.parametrize("gemm_impl", [1, 2, 3, 0],
+                         ids=["scaffold", "tcgen05_1cta", "tcgen05_2cta_smemA", "tcgen05"])
 @pytest.mark.parametrize("cfg", [MID, MID32], ids=lambda c: c.name)
 def test_mid_ragged_multi_tile(cfg, gemm_impl):
     inp = _skewed(cfg)
@@ -185,6 +185,42 @@ def test_step_host_async_three_steps_in_a_pipeline():
     assert np.abs(refA["Y"] - refB["Y"]).max() > 0.1 * np.abs(refA["Y"]).max()     # the two inputs really differ
 
 
+@pytest.mark.parametrize("T", [1025, 2050])
+@pytest.mark.parametrize("chunks", [4, 1, 0])
+def test_step_host_chunked_upload_is_bitwise_the_stepwise_api(T, chunks):
+    """the path behind the e2e number at T >= 1024.  X goes up and is routed in four ragged token chunks
+    (T = 1025 -> 260 + 260 + 260 + 245, T = 2050 -> 516 x 3 + 502), or in one piece when the previous step is still running;
+    both branches are pinned through the option "host_chunks" and must give, bit for bit, what the stepwise API gives
+    (same kernels, same order of every sum), for Y, dX and all gradients; two async steps in flight."""
+    import torch
+    from parity_util import make_layer, to_np
+    cfg = ti.Config(f"host_T{T}", T=T, d=256, F=256, E=12, k=3, r=16, seed=40 + T, router_grad=True)
+    inp = ti.make_inputs(cfg)
+    step = run_gpu(inp, backward=True, router_grad=True)
+    layer, dev = make_layer(inp, training=True)
+    layer.set_option("host_chunks", chunks)
+    d = cfg.d
+    Xh, dYh = dev["X"].cpu().pin_memory(), dev["dY"].cpu().pin_memory()
+    outs = [(torch.zeros((T, d), dtype=torch.bfloat16).pin_memory(), torch.zeros((T, d), dtype=torch.bfloat16).pin_memory())
+            for _ in range(3)]
+    grads = layer.alloc_grads()
+    dW_r = torch.zeros((d, cfg.E), dtype=torch.float32, device="cuda")
+    for i in range(3):
+        layer.step_host_async(Xh, dYh, dev["W_r"], None, outs[i][0], outs[i][1], grads, dW_r)
+        if i >= 1:
+            layer.step_host_wait(1)
+    layer.step_host_wait(0)
+    for i in range(3):
+        np.testing.assert_array_equal(to_np(outs[i][0]), step["Y"], err_msg=f"Y of step {i}")
+        np.testing.assert_array_equal(to_np(outs[i][1]), step["dX"], err_msg=f"dX of step {i}")
+    np.testing.assert_array_equal(to_np(dW_r), step["dW_r"])
+    for key in ("dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down"):
+        np.testing.assert_array_equal(to_np(grads[key]), step[key], err_msg=key)
+    ref = oracle_ref(inp, True, True)
+    assert_close("Y", to_np(outs[2][0]), ref["Y"])
+    assert_close("dX", to_np(outs[2][1]), ref["dX"])
+
+
 def test_layer_reuse_smaller_batch_and_foreign_dYe():
     """One ctx, two calls: a full batch, then a smaller batch with different data (stale workspace rows, tile list and
     cached dispatch pointers must not leak), and an expert_bwd fed a dYe tensor that did NOT come from the fused
@@ -197,8 +233,8 @@ def test_layer_reuse_smaller_batch_and_foreign_dYe():
         idx, w = layer.route(dev["X"], dev["W_r"], dev.get("logit_bias"))
         counts, offsets, perm, inv = layer.dispatch(idx)
         Ye = layer.expert_fwd(dev["X"], offsets, perm)
-        dYe, _ = layer.combine_bwd(dev["dY"], Ye, inv, w, want_dw=False)
-        layer.expert_bwd(dev["X"], dYe, offsets, perm)
+        dYe, _ = layer.combine_bwd(dev["dY"], Ye, inv, w, want_dw=False, perm=perm)
+        layer.expert_bwd(dev["X"], dYe, offsets, perm, dYe_unmodified=True)
     small_cfg = ti.Config("small_after_big", T=200, d=MID.d, F=MID.F, E=MID.E, k=MID.k, r=MID.r, seed=77)
     small = ti.make_inputs(small_cfg)
     for key in ("idx_gate", "idx_up", "idx_down", "scale_gate", "scale_up", "scale_down", "codebook",
@@ -210,8 +246,12 @@ def test_layer_reuse_smaller_batch_and_foreign_dYe():
     counts, offsets, perm, inv = layer.dispatch(idx)
     Ye = layer.expert_fwd(sd["X"], offsets, perm)
     Y = layer.combine(Ye, inv, w)
-    dYe_fused, dw = layer.combine_bwd(sd["dY"], Ye, inv, w, want_dw=True)
+    dYe_fused, dw = layer.combine_bwd(sd["dY"], Ye, inv, w, want_dw=True, perm=perm)
     dYe_foreign = dYe_fused.clone()                # a different tensor: the cached projection must not be trusted
+    import paper_2606_07404_b200 as tq
+    with pytest.raises(tq.TqpError) as e:          # vouching for a tensor the fused combine_bwd did not write is refused
+        layer.expert_bwd(sd["X"], dYe_foreign, offsets, perm, dYe_unmodified=True)
+    assert e.value.code == 5
     dXp, grads = layer.expert_bwd(sd["X"], dYe_foreign, offsets, perm)
     dX = layer.dispatch_bwd(dXp, inv)
     torch.cuda.synchronize()
@@ -223,6 +263,51 @@ def test_layer_reuse_smaller_batch_and_foreign_dYe():
     assert_close("dX_experts", to_np(dX), ref["dX_experts"])
     for key in ("dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down"):
         assert_close(key, to_np(grads[key]), ref[key])
+
+
+def test_dYe_edited_in_place_between_combine_bwd_and_expert_bwd():
+    """a caller that adds something to dYe in place (a shared-expert or auxiliary gradient) between the fused
+    tqp_combine_bwd and tqp_expert_bwd passes flags = 0; the adapter projection left by combine_bwd must then NOT be
+    used.  Checked against the oracle's expert_bwd on the edited dYe.  Also: the unfused path (perm = NULL) gives the same
+    dYe bits as the fused one."""
+    import torch
+    from parity_util import make_layer, to_np
+    inp = _skewed(MID)
+    ref = oracle_ref(inp, True, False)
+    layer, dev = make_layer(inp, training=True)
+    idx, w = layer.route(dev["X"], dev["W_r"], dev.get("logit_bias"))
+    counts, offsets, perm, inv = layer.dispatch(idx)
+    Ye = layer.expert_fwd(dev["X"], offsets, perm)
+    dYe_plain, dw_plain = layer.combine_bwd(dev["dY"], Ye, inv, w, want_dw=True)             # perm = NULL
+    dYe, dw = layer.combine_bwd(dev["dY"], Ye, inv, w, want_dw=True, perm=perm)              # fused
+    assert torch.equal(dYe_plain, dYe) and torch.equal(dw_plain, dw)
+    extra = torch.randn_like(dYe, dtype=torch.float32).mul_(0.5).to(torch.bfloat16)
+    dYe.add_(extra)                                                                          # in-place edit
+    dXp, grads = layer.expert_bwd(dev["X"], dYe, offsets, perm)                              # flags = 0
+    torch.cuda.synchronize()
+    dYe_ref = to_np(dYe)
+    dXp_ref, g_ref = oracle.expert_bwd(inp, dYe_ref, ref["G"], ref["U"], ref["H"], ref["offsets"], ref["perm"])
+    assert_close("dXp", to_np(dXp), dXp_ref)
+    for key in ("dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down"):
+        assert_close(key, to_np(grads[key]), g_ref[key])
+
+
+@pytest.mark.parametrize("lora_scale,r", [(0.5, 16), (2.0, 32), (0.25, 8)])
+def test_lora_scale_not_one_full_chain(lora_scale, r):
+    """the whole chain including all six adapter gradients at lora_scale != 1 with adapters large
+    enough (N(0, 0.1), as pin P7) that a dropped or doubled factor s in the forward, in dA / dB or in the adapter term of
+    dX is far outside the tolerance (`tqp_layer_desc.lora_scale`)."""
+    cfg = ti.Config(f"mid_ls{lora_scale}_r{r}", T=640, d=256, F=384, E=6, k=3, r=r, seed=24, router_grad=True, lora_scale=lora_scale)
+    inp = _skewed(cfg)
+    rng = np.random.default_rng(5)
+    for key in ("A_gate", "B_gate", "A_up", "B_up", "A_down", "B_down"):
+        inp[key] = ti.f32_to_bf16_bits(rng.standard_normal(inp[key].shape).astype(np.float32) * 0.1)
+    gpu, ref = check_all(inp, backward=True, router_grad=True, gemm_impl=0)
+    base = oracle.layer(dict(inp, lora_scale=0.0), dtype=np.float32, backward=False)["Y"]
+    assert np.linalg.norm(ref["Y"] - base) > 0.3 * np.linalg.norm(base)      # the adapter term is a large part of Y
+    one = oracle.layer(dict(inp, lora_scale=1.0), dtype=np.float32, backward=True, router_grad=True)
+    for key in ("Y", "dX", "dA_gate", "dB_down"):                            # and s = 1 would be far outside the tolerance
+        assert np.linalg.norm(one[key] - ref[key]) > 0.05 * np.linalg.norm(ref[key]), key
 
 
 EDGE = [

@@ -1,58 +1,122 @@
-"""GPU parity at BASELINE.json's FULL sizes (configs 1-4, plus the paper-width shape 5), in the launch configuration bench.py times.
+"""GPU parity at BASELINE.json's FULL sizes (configs 1-4, plus the paper-width shape 5), in the launch configuration
+bench.py times, over ALL experts and end to end.
 
-Routing, permutation, combine and the HBM-bound backward steps are compared over the whole tensors (the oracle is
-cheap there).  The grouped expert FFN — too slow to run through the oracle for 460 experts inside a test — is compared
-on a SAMPLE of experts the oracle computes one by one (largest, smallest, an empty one if any, and seeded random
-ones): every routed row, every output element and every adapter-gradient element of the sampled experts."""
+The oracle runs the whole layer once per config (`oracle.layer`, fp32, as it stands: ~45 s for cfg 2 / 3, ~2 min for
+cfg 4 on the GPU box's 16 host cores) and EVERY tensor of the CUDA path is compared with the oracle's OWN value of it:
+routing and permutation bit-exact, the gather exact, and G, U, H, Ye, Y, dYe, dtopk_w, dXp, dX, the six adapter
+gradients (and dW_r / the router term of dX for cfg 4) within north_star's tolerance — both over the whole tensor and
+PER EXPERT (every expert's rows / gradient slices on their own, so that a tile-scheduler or TMA-coordinate bug that
+bites at one (expert, tile) position cannot hide in a global norm).
+
+With TQP_PARITY_REPORT=<path> in the environment every config appends its per-tensor error rows (markdown) to that
+file; profiles/r2_parity_errors.md is such a file.
+"""
+import os
+
 import numpy as np
 import pytest
 
 import oracle
 import tqp_inputs as ti
-from parity_util import assert_close, assert_routing_exact, run_gpu
+from parity_util import MAXABS_TOL, RELF_TOL, assert_routing_exact, run_gpu
 
 pytestmark = pytest.mark.gpu
 
-
-def sample_experts(counts, seed, n_random=3):
-    nz = np.nonzero(counts)[0]
-    S = {int(nz[np.argmax(counts[nz])]), int(nz[np.argmin(counts[nz])])}
-    empty = np.nonzero(counts == 0)[0]
-    if len(empty):
-        S.add(int(empty[0]))
-    rng = np.random.default_rng(seed)
-    S.update(int(e) for e in rng.choice(len(counts), size=n_random, replace=False))
-    return sorted(S)
+GRADS = ("dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down")
+# per-expert bounds: the same relative-Frobenius bound as the whole tensor; max-abs relative to the expert's own max
+PER_EXPERT_RELF = RELF_TOL
+PER_EXPERT_MAXABS = MAXABS_TOL
 
 
-def sub_problem(inp, S, offsets, perm):
-    """The layer restricted to the experts in S (weights sliced, rows re-based); X stays whole."""
-    sub = dict(inp)
-    for key in ("idx_gate", "idx_up", "idx_down", "scale_gate", "scale_up", "scale_down",
-                "A_gate", "B_gate", "A_up", "B_up", "A_down", "B_down"):
-        sub[key] = np.ascontiguousarray(inp[key][S])
-    sub["E"] = len(S)
-    segs = [np.arange(offsets[e], offsets[e + 1]) for e in S]
-    rows = np.concatenate(segs) if segs else np.zeros(0, np.int64)
-    offs = np.zeros(len(S) + 1, np.int32)
-    offs[1:] = np.cumsum([len(s) for s in segs])
-    return sub, rows, offs, np.ascontiguousarray(perm[rows])
+def row_stats(gpu, ref, chunk=16384):
+    """Per-row sum of squared error, sum of squared reference, max |error|, max |reference| (fp64 accumulation)."""
+    n = ref.shape[0]
+    se = np.empty(n); sr = np.empty(n); me = np.empty(n); mr = np.empty(n)
+    for i in range(0, n, chunk):
+        r = ref[i:i + chunk].astype(np.float64)
+        dlt = gpu[i:i + chunk].astype(np.float64) - r
+        se[i:i + chunk] = np.einsum("ij,ij->i", dlt, dlt)
+        sr[i:i + chunk] = np.einsum("ij,ij->i", r, r)
+        me[i:i + chunk] = np.abs(dlt).max(axis=1)
+        mr[i:i + chunk] = np.abs(r).max(axis=1)
+    return se, sr, me, mr
+
+
+def check_rows(name, gpu, ref, offsets, report):
+    """Whole tensor + every expert's row block of a [N][*] tensor."""
+    assert np.isfinite(gpu).all(), f"{name}: non-finite values on the GPU side"
+    se, sr, me, mr = row_stats(gpu, ref)
+    maxabs, relf = me.max() / mr.max(), np.sqrt(se.sum() / sr.sum())
+    nz = np.nonzero(np.diff(offsets))[0]
+    starts = offsets[nz].astype(np.int64)
+    e_relf = np.sqrt(np.add.reduceat(se, starts) / np.add.reduceat(sr, starts))
+    e_maxabs = np.maximum.reduceat(me, starts) / np.maximum.reduceat(mr, starts)
+    report.append((name, maxabs, relf, e_maxabs.max(), e_relf.max(), int(nz[np.argmax(e_relf)])))
+    assert maxabs <= MAXABS_TOL and relf <= RELF_TOL, f"{name}: maxabs/max|ref|={maxabs:.3e} relF={relf:.3e}"
+    assert e_relf.max() <= PER_EXPERT_RELF, f"{name}: expert {nz[np.argmax(e_relf)]} relF={e_relf.max():.3e}"
+    assert e_maxabs.max() <= PER_EXPERT_MAXABS, f"{name}: expert {nz[np.argmax(e_maxabs)]} maxabs={e_maxabs.max():.3e}"
+
+
+def check_grad(name, gpu, ref, counts, report):
+    """Whole tensor + every expert's slice of a [E][*][*] adapter gradient; empty experts exactly zero."""
+    assert np.isfinite(gpu).all(), f"{name}: non-finite values on the GPU side"
+    E = ref.shape[0]
+    g = gpu.reshape(E, -1).astype(np.float64); r = ref.reshape(E, -1).astype(np.float64)
+    dlt = g - r
+    se, sr = np.einsum("ij,ij->i", dlt, dlt), np.einsum("ij,ij->i", r, r)
+    me, mr = np.abs(dlt).max(axis=1), np.abs(r).max(axis=1)
+    maxabs, relf = me.max() / mr.max(), np.sqrt(se.sum() / sr.sum())
+    nz = counts > 0
+    assert (g[~nz] == 0).all() and (r[~nz] == 0).all(), f"{name}: an empty expert must have exactly zero gradient"
+    e_relf = np.sqrt(se[nz] / sr[nz]); e_maxabs = me[nz] / mr[nz]
+    ids = np.nonzero(nz)[0]
+    report.append((name, maxabs, relf, e_maxabs.max(), e_relf.max(), int(ids[np.argmax(e_relf)])))
+    assert maxabs <= MAXABS_TOL and relf <= RELF_TOL, f"{name}: maxabs/max|ref|={maxabs:.3e} relF={relf:.3e}"
+    # an expert with a handful of rows has a noisier gradient ratio; its bound is still north_star's
+    assert e_relf.max() <= PER_EXPERT_RELF, f"{name}: expert {ids[np.argmax(e_relf)]} relF={e_relf.max():.3e}"
+    assert e_maxabs.max() <= PER_EXPERT_MAXABS, f"{name}: expert {ids[np.argmax(e_maxabs)]} maxabs={e_maxabs.max():.3e}"
+
+
+def check_whole(name, gpu, ref, report, maxabs_tol=MAXABS_TOL, relf_tol=RELF_TOL):
+    assert np.isfinite(gpu).all(), f"{name}: non-finite values on the GPU side"
+    se, sr, me, mr = row_stats(gpu.reshape(gpu.shape[0], -1), ref.reshape(ref.shape[0], -1))
+    maxabs, relf = me.max() / mr.max(), np.sqrt(se.sum() / sr.sum())
+    report.append((name, maxabs, relf, None, None, None))
+    assert maxabs <= maxabs_tol and relf <= relf_tol, f"{name}: maxabs/max|ref|={maxabs:.3e} relF={relf:.3e}"
+
+
+def write_report(cfg, report, counts, seconds):
+    path = os.environ.get("TQP_PARITY_REPORT")
+    lines = [f"\n### {cfg.name}: T={cfg.T} d={cfg.d} F={cfg.F} E={cfg.E} k={cfg.k} r={cfg.r}"
+             f" ({'fwd+bwd' if cfg.backward else 'fwd'}{', router grad' if cfg.router_grad else ''}); "
+             f"{int((counts == 0).sum())} empty experts, largest {int(counts.max())} rows; "
+             f"oracle.layer {seconds:.0f} s on {oracle.num_threads()} threads\n",
+             "| tensor | maxabs / max\\|ref\\| (bound 2e-2) | relF (bound 1e-2) | worst expert: maxabs | worst expert: relF | (expert) |",
+             "|---|---|---|---|---|---|"]
+    for name, a, b, c, d_, e in report:
+        per = f"| {c:.2e} | {d_:.2e} | {e} |" if c is not None else "| — | — | — |"
+        lines.append(f"| {name} | {a:.2e} | {b:.2e} {per}")
+    text = "\n".join(lines) + "\n"
+    print(text)
+    if path:
+        with open(path, "a") as f:
+            f.write(text)
 
 
 @pytest.mark.parametrize("cfg_id", [1, 2, 3, 4, 5])
 def test_full_size_config(cfg_id):
+    import time
     cfg = ti.CONFIGS[cfg_id]
     inp = ti.make_inputs(cfg)
     T, k, E, d, F = cfg.T, cfg.k, cfg.E, cfg.d, cfg.F
     gpu = run_gpu(inp, backward=cfg.backward, router_grad=cfg.router_grad, gemm_impl=0)
+    t0 = time.time()
+    ref = oracle.layer(inp, dtype=np.float32, backward=cfg.backward, router_grad=cfg.router_grad)
+    seconds = time.time() - t0
 
     # ---- routing and permutation: whole tensors, bit-exact ----
-    lg = oracle.logits(inp["X"], inp["W_r"], inp["logit_bias"])
-    ref = {"logits": lg}
-    ref["topk_idx"], ref["topk_w"] = oracle.topk(lg, k)
-    ref["counts"], ref["offsets"], ref["perm"], ref["inv_perm"] = oracle.dispatch(ref["topk_idx"], E)
     assert_routing_exact(gpu, ref)
-    counts, offsets, perm, inv = ref["counts"], ref["offsets"], ref["perm"], ref["inv_perm"]
+    counts, offsets, perm = ref["counts"], ref["offsets"], ref["perm"]
     if cfg.skew:
         print(f"cfg{cfg_id}: zero-token experts {np.mean(counts == 0):.1%}, top expert share {counts.max() / counts.sum():.2%}")
         assert (counts == 0).sum() > 0
@@ -61,44 +125,22 @@ def test_full_size_config(cfg_id):
     Xf = ti.bf16_bits_to_f32(inp["X"])
     np.testing.assert_array_equal(gpu["Xp"], Xf[perm // k])
 
-    # ---- expert FFN forward on sampled experts ----
-    S = sample_experts(counts, seed=cfg.seed)
-    sub, rows, offs, perm_s = sub_problem(inp, S, offsets, perm)
-    nrows = int(offs[-1])
-    Ye_s, G_s, U_s, H_s = oracle.expert_fwd(sub, offs, perm_s, n_rows=nrows)
-    for name, r_ in (("G", G_s), ("U", U_s), ("H", H_s), ("Ye", Ye_s)):
-        assert_close(f"cfg{cfg_id} {name}[sampled experts {S}]", gpu[name][rows], r_)
-
-    # ---- combine: whole tensor, given the GPU's own Ye (isolates the step) ----
-    Y_ref = oracle.combine(gpu["Ye"], inv, ref["topk_w"])
-    assert_close(f"cfg{cfg_id} Y", gpu["Y"], Y_ref, maxabs_tol=4e-3, relf_tol=3e-3)    # one bf16 rounding of the output
-    if not cfg.backward:
-        return
-
-    # ---- combine backward: whole tensors ----
-    dYe_ref, dw_ref = oracle.combine_bwd(inp["dY"], gpu["Ye"], inv, ref["topk_w"])
-    assert_close(f"cfg{cfg_id} dYe", gpu["dYe"], dYe_ref, maxabs_tol=4e-3, relf_tol=3e-3)
-    assert_close(f"cfg{cfg_id} dtopk_w", gpu["dtopk_w"], dw_ref, maxabs_tol=1e-4, relf_tol=1e-5)
-
-    # ---- expert FFN backward on the sampled experts (oracle forward values, oracle dYe) ----
-    dYe_oracle_rows = dYe_ref[rows]
-    dXp_s, g_s = oracle.expert_bwd(sub, dYe_oracle_rows, G_s, U_s, H_s, offs, perm_s, n_rows=nrows)
-    assert_close(f"cfg{cfg_id} dXp[sampled]", gpu["dXp"][rows], dXp_s)
-    for key, val in g_s.items():
-        got = gpu[key][S]
-        nonempty = [i for i, e in enumerate(S) if counts[e] > 0]
-        assert_close(f"cfg{cfg_id} {key}[sampled]", got[nonempty], val[nonempty])
-        for i, e in enumerate(S):
-            if counts[e] == 0:
-                assert (got[i] == 0).all(), f"{key}: empty expert {e} must have exactly zero gradient"
-
-    # ---- dispatch backward: whole tensor, given the GPU's dXp ----
-    dX_ref = oracle.dispatch_bwd(gpu["dXp"], inv, T, k)
-    assert_close(f"cfg{cfg_id} dX_experts", gpu["dX_experts"], dX_ref, maxabs_tol=4e-3, relf_tol=3e-3)
-
-    # ---- router backward (configs 0 and 4): whole tensors, given the GPU's dtopk_w ----
-    if cfg.router_grad:
-        dX = dX_ref.copy()
-        dW_r, _ = oracle.route_bwd(inp["X"], inp["W_r"], ref["topk_idx"], ref["topk_w"], gpu["dtopk_w"], dX)
-        assert_close(f"cfg{cfg_id} dW_r", gpu["dW_r"], dW_r, maxabs_tol=1e-3, relf_tol=1e-4)
-        assert_close(f"cfg{cfg_id} dX", gpu["dX"], dX, maxabs_tol=8e-3, relf_tol=4e-3)
+    report = []
+    try:
+        # ---- expert FFN forward, every expert, against the oracle's own values ----
+        for name in ("G", "U", "H", "Ye"):
+            check_rows(name, gpu[name], ref[name], offsets, report)
+        # ---- combine, end to end (the oracle's own Y, not a recombination of the GPU's Ye) ----
+        check_whole("Y", gpu["Y"], ref["Y"], report)
+        if cfg.backward:
+            check_rows("dYe", gpu["dYe"], ref["dYe"], offsets, report)
+            check_whole("dtopk_w", gpu["dtopk_w"], ref["dtopk_w"], report)
+            check_rows("dXp", gpu["dXp"], ref["dXp"], offsets, report)
+            for name in GRADS:
+                check_grad(name, gpu[name], ref[name], counts, report)
+            check_whole("dX_experts", gpu["dX_experts"], ref["dX_experts"], report)
+            if cfg.router_grad:
+                check_whole("dW_r", gpu["dW_r"], ref["dW_r"], report)
+                check_whole("dX", gpu["dX"], ref["dX"], report)
+    finally:
+        write_report(cfg, report, counts, seconds)

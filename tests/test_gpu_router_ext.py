@@ -48,7 +48,7 @@ def test_route_sigmoid_backward_and_chain():
     counts, offsets, perm, inv = layer.dispatch(idx)
     Ye = layer.expert_fwd(dev["X"], offsets, perm)
     Y = layer.combine(Ye, inv, w)
-    dYe, dw = layer.combine_bwd(dev["dY"], Ye, inv, w, want_dw=True)
+    dYe, dw = layer.combine_bwd(dev["dY"], Ye, inv, w, want_dw=True, perm=perm)
     dXp, grads = layer.expert_bwd(dev["X"], dYe, offsets, perm)
     dX = layer.dispatch_bwd(dXp, inv)
     dX_experts = dX.clone()

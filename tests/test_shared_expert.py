@@ -63,7 +63,7 @@ def test_gpu_shared_expert_through_the_routed_kernels():
     counts, offsets, perm, inv = layer.dispatch(idx)
     Ye = layer.expert_fwd(dev["X"], offsets, perm)
     Y = layer.combine(Ye, inv, w)
-    dYe, _ = layer.combine_bwd(dev["dY"], Ye, inv, w, want_dw=False)
+    dYe, _ = layer.combine_bwd(dev["dY"], Ye, inv, w, want_dw=False, perm=perm)
     dXp, grads = layer.expert_bwd(dev["X"], dYe, offsets, perm)
     dX = layer.dispatch_bwd(dXp, inv)
     torch.cuda.synchronize()
