@@ -15,7 +15,8 @@
 //
 // Warp roles per CTA (480 threads, 1 CTA/SM, persistent over work items, cluster = 2 CTAs):
 //   warp 0  TMA producer of the activation / adapter-projection tiles (signals the LEADER's barrier)
-//   warp 1  MMA issuer (leader CTA only, one elected lane) + TMEM allocation
+//   warp 1  MMA issuer (leader CTA only, one elected lane) + TMEM allocation; in the PEER CTA the same warp is the item
+//           scheduler: it draws item ids from a global counter and publishes them to both CTAs through a 4-deep ring
 //   warp 2  TMA producer of the code-index tiles
 //   warps 3-10  dequant producers, two groups of four that alternate A stages
 //   warps 11-14 epilogue (TMEM -> registers -> bf16 -> staging tile -> 16-byte global stores)
@@ -38,6 +39,17 @@ constexpr int SMEM_BYTES = OFF_EPI + EPI_BYTES + 1024;
 constexpr int NTHREADS = 480;
 constexpr int W_DEQ0 = 3, W_EPI0 = 11;
 constexpr int TM_ACC = 0, TM_A = TN;                      // TMEM columns: accumulator [0, 256), A slots [256, 256 + 64 NASLOT)
+// Dynamic item schedule: every CTA pair draws its next item from a global counter (tile-list order = expert order) instead of
+// a fixed round-robin share, so no pair runs out of work early.  (Measured, cfg 2 / cfg 3 GEMM time per step on one box:
+// static 2.585 / 3.195 ms, dynamic 2.558 / 3.174 ms; with the tile list additionally sorted largest-first 2.565 / 3.275 ms
+// -- an item's cost hardly depends on its rows, a 16-row item is dequant-bound and costs ~0.7 of a 256-row one, so there
+// is nothing for a longest-first order to balance, and it was dropped.)  The five roles of both CTAs are decoupled (the index
+// loader runs about an item ahead of the MMAs, the epilogue an item behind), so ids travel through a ring: the scheduler
+// thread (peer CTA, warp 1) writes the id into BOTH CTAs' shared memory and arrives on both `sched_full` barriers; every
+// consumer warp of both CTAs arrives on the scheduler's `sched_empty` barrier after it has read the id.  Which pair runs
+// which item changes no result: items write disjoint outputs.
+constexpr int SQ = 4;                                     // ring depth
+constexpr int SCHED_CONSUMERS = 15 + 14;                  // warps that follow the ring: leader 0,1,2,3-10,11-14; peer 0,2,3-10,11-14
 
 struct Item {
     Tile t;
@@ -66,7 +78,8 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t *v) {
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
 gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__restrict__ lut_g, const Tile *__restrict__ tiles,
-                        const int32_t *__restrict__ num_tiles_p, int ablate, long long *__restrict__ trace) {
+                        const int32_t *__restrict__ num_tiles_p, int32_t *__restrict__ sched_counter, int ablate,
+                        long long *__restrict__ trace) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     const uint32_t sbase = smem_u32(smem);
@@ -80,10 +93,16 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
     const uint32_t tmem_full = bar0 + 8u * (2 * NSTAGE + 2 * NASLOT + 2 * IDXQ);       // local, multicast commit
     const uint32_t tmem_empty = bar0 + 8u * (2 * NSTAGE + 2 * NASLOT + 2 * IDXQ + 1);  // the leader's is used
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + OFF_BAR + 8 * (2 * NSTAGE + 2 * NASLOT + 2 * IDXQ + 4));
+    constexpr int NB0 = 2 * NSTAGE + 2 * NASLOT + 2 * IDXQ + 6;
+    auto sched_full = [&](int s) { return bar0 + 8u * (NB0 + s); };                  // local: one arrival by the scheduler
+    auto sched_empty = [&](int s) { return bar0 + 8u * (NB0 + SQ + s); };            // the PEER's (rank 1) is used
+    const uint32_t sched_item = bar0 + 8u * (NB0 + 2 * SQ);                          // SQ ints, a copy in each CTA
+    static_assert(8 * (NB0 + 2 * SQ) + 4 * SQ <= 512, "barrier area");
 
     const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
     const uint32_t rank = cluster_ctarank();
     const uint32_t fullB_remote = mapa(fullB(0), 0), fullA_remote = mapa(fullA(0), 0), tmem_empty_remote = mapa(tmem_empty, 0);
+    const uint32_t sched_empty_remote = mapa(sched_empty(0), 1);
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < NSTAGE; ++s) { mbar_init(fullB(s), 1); mbar_init(emptyB(s), 1); }
@@ -91,6 +110,7 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
         for (int s = 0; s < IDXQ; ++s) { mbar_init(idx_full(s), 1); mbar_init(idx_empty(s), 4); }
         mbar_init(tmem_full, 1);
         mbar_init(tmem_empty, 8);
+        for (int s = 0; s < SQ; ++s) { mbar_init(sched_full(s), 1); mbar_init(sched_empty(s), SCHED_CONSUMERS); }
         mbar_init_fence();
     }
     if (warp == 1) tmem_alloc<2>(smem_u32(tmem_slot), 512);
@@ -107,10 +127,27 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
     const int num_tiles = *num_tiles_p;
     const int nprob = args.nprob;
     const int MTP = args.p[0].M / (2 * BM);
-    const long long total = (long long)num_tiles * nprob * MTP;
+    const int total = num_tiles * nprob * MTP;
     const int cid = blockIdx.x >> 1, ncl = gridDim.x >> 1;
+    // next item id of this CTA pair (-1: none left); `sq` is the caller's ring position.  _thread: called by ONE thread of
+    // a warp (the single-thread roles); _warp: by all 32 lanes.
+    auto next_item_thread = [&](Pipe &sq) {
+        mbar_wait(sched_full(sq.s), sq.ph);
+        const uint32_t v = lds32(sched_item + 4u * sq.s);
+        mbar_arrive_cluster_after(sched_empty_remote + 8u * sq.s, v);
+        sq.next(SQ);
+        return (int)v;
+    };
+    auto next_item_warp = [&](Pipe &sq) {
+        mbar_wait(sched_full(sq.s), sq.ph);
+        const uint32_t v = lds32(sched_item + 4u * sq.s);
+        const uint32_t all = __reduce_or_sync(0xffffffffu, v);   // every lane's read has returned (all lanes read the same word)
+        if (lane == 0) mbar_arrive_cluster_after(sched_empty_remote + 8u * sq.s, all);
+        sq.next(SQ);
+        return (int)v;
+    };
 
-    auto get_item = [&](long long item, Item &it) {
+    auto get_item = [&](int item, Item &it) {
         const int tile_id = (int)(item / (nprob * MTP)), rem = (int)(item % (nprob * MTP));
         it.t = tiles[tile_id];
         it.prob = rem / MTP;
@@ -120,8 +157,8 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
     if (warp == 0) {
         // =========================== activation TMA producer ===========================
         if (lane == 0) {
-            Pipe st;
-            for (long long item = cid; item < total; item += ncl) {
+            Pipe st, sq;
+            for (int item; (item = next_item_thread(sq)) >= 0;) {
                 Item it;
                 get_item(item, it);
                 if (it.t.rows <= 0) continue;
@@ -154,8 +191,8 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
     } else if (warp == 2) {
         // =========================== code-index TMA producer ===========================
         if (lane == 0) {
-            Pipe iq;
-            for (long long item = cid; item < total; item += ncl) {
+            Pipe iq, sq;
+            for (int item; (item = next_item_thread(sq)) >= 0;) {
                 Item it;
                 get_item(item, it);
                 if (it.t.rows <= 0) continue;
@@ -194,12 +231,36 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
         }
     } else if (warp == 1) {
         // =========================== MMA issuer (leader CTA) ===========================
-        if (rank == 0 && elect_one()) {
-            Pipe st, sa;
+        if (rank == 1) {
+            // =========================== item scheduler (peer CTA) ===========================
+            if (elect_one()) {
+                Pipe sq;
+                const uint32_t item_r0 = mapa(sched_item, 0), full_r0 = mapa(sched_full(0), 0);
+                const uint32_t item_r1 = mapa(sched_item, 1), full_r1 = mapa(sched_full(0), 1);
+                for (;;) {
+                    mbar_wait(sched_empty(sq.s), sq.ph ^ 1);   // every consumer warp of both CTAs has read the entry's previous id
+                    const int f = atomicAdd(sched_counter, 1);
+                    const int v = f < total ? f : -1;
+                    // the id travels as an async store that completes the entry's `full` barrier in each CTA (no fences)
+                    mbar_expect_tx_cluster(full_r1 + 8u * sq.s, 4);
+                    st_async_u32(item_r1 + 4u * sq.s, (uint32_t)v, full_r1 + 8u * sq.s);
+                    mbar_expect_tx_cluster(full_r0 + 8u * sq.s, 4);
+                    st_async_u32(item_r0 + 4u * sq.s, (uint32_t)v, full_r0 + 8u * sq.s);
+                    if (v < 0) break;
+                    sq.next(SQ);
+                }
+                // the last pair to run dry re-arms the counters for the next launch (stream order: nobody fetches any more)
+                if (atomicAdd(sched_counter + 1, 1) == ncl - 1) {
+                    sched_counter[0] = 0;
+                    sched_counter[1] = 0;
+                }
+            }
+        } else if (elect_one()) {
+            Pipe st, sa, sq;
             int cnt = 0;
             const uint32_t hi_k = desc_hi(1024), lo_k = desc_lo_const(16);          // K-major SW128: SBO = 8 rows x 128 B
             const uint32_t x16 = (sbase + OFF_X) >> 4;
-            for (long long item = cid; item < total; item += ncl) {
+            for (int item; (item = next_item_thread(sq)) >= 0;) {
                 Item it;
                 get_item(item, it);
                 if (it.t.rows <= 0) continue;
@@ -273,7 +334,7 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
         const int rk = lane >> 2, jj = lane & 3;                       // MN-major: source row / channel pair of a movmatrix block
         const int kofs = 4 * (rk >> 1) + (rk & 1);
         const uint32_t lut_b = sbase + OFF_LUT + rk * 16 + jj * 4;   // replica rk: all 32 lanes hit distinct banks
-        Pipe sa, iq;
+        Pipe sa, iq, sq;
         int ja = 0;
         auto wait_slot_free = [&]() {   // MMAs of the previous use of this A slot have completed
             mbar_wait(emptyA(sa.s), sa.ph ^ 1);
@@ -285,7 +346,7 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(fullA_remote + 8u * sa.s);
         };
-        for (long long item = cid; item < total; item += ncl) {
+        for (int item; (item = next_item_warp(sq)) >= 0;) {
             Item it;
             get_item(item, it);
             if (it.t.rows <= 0) continue;
@@ -437,7 +498,8 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
         const int et = threadIdx.x - W_EPI0 * 32;
         const uint32_t ebuf = sbase + OFF_EPI;
         int cnt = 0;
-        for (long long item = cid; item < total; item += ncl) {
+        Pipe sq;
+        for (int item; (item = next_item_warp(sq)) >= 0;) {
             Item it;
             get_item(item, it);
             if (it.t.rows <= 0) continue;
@@ -508,8 +570,8 @@ tqp_status launch_gemm_tcgen05_ts2(tqp_ctx *c, const GemmProblem *probs, int npr
     const int grid = (c->num_sms / 2) * 2;
     const bool tr = c->trace > 0 && ++c->trace_seq == c->trace;   // debug timeline of cluster 0 (tqp_set_option "trace")
     gt2::gemm_tcgen05_ts2_kernel<<<grid, gt2::NTHREADS, gt2::SMEM_BYTES, st>>>(
-        args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), c->ablate,
-        tr ? c->p<long long>(c->ws.trace) : nullptr);
+        args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), c->p<int32_t>(c->ws.sched) + 4,
+        c->ablate, tr ? c->p<long long>(c->ws.trace) : nullptr);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }

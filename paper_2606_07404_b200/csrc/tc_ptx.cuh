@@ -42,6 +42,23 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
     asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
 }
+// arrive that cannot issue before `dep` (a value just loaded from shared memory) has arrived in its register: orders the
+// read before the arrive without a memory fence (release.cluster compiles to MEMBAR.ALL.GPU, which would wait for every
+// outstanding global store of the warp)
+__device__ __forceinline__ void mbar_arrive_cluster_after(uint32_t cluster_bar, uint32_t dep) {
+    asm volatile("{\n\t.reg .b32 t;\n\tand.b32 t, %1, 0;\n\tadd.u32 t, t, %0;\n\tmbarrier.arrive.shared::cluster.b64 _, [t];\n\t}" ::"r"(cluster_bar), "r"(dep)
+                 : "memory");
+}
+// expect-tx arrive on a barrier given by its shared::cluster address (possibly the peer CTA's)
+__device__ __forceinline__ void mbar_expect_tx_cluster(uint32_t cluster_bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cluster.b64 _, [%0], %1;" ::"r"(cluster_bar), "r"(bytes) : "memory");
+}
+// asynchronous 4-byte store into (possibly the peer CTA's) shared memory that completes `bytes` on the mbarrier next to it:
+// a waiter that observes the phase sees the value, as with a TMA load -- no fence on either side
+__device__ __forceinline__ void st_async_u32(uint32_t cluster_addr, uint32_t v, uint32_t cluster_bar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];" ::"r"(cluster_addr), "r"(v), "r"(cluster_bar)
+                 : "memory");
+}
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
