@@ -203,6 +203,57 @@ tqp_status tqp_bias_update(tqp_ctx *ctx, const int32_t *counts, float *bias, int
  * Errors: TQP_ERR_STATE without weights, TQP_ERR_ARG for a bad pack / range / NULL. */
 tqp_status tqp_consolidate(tqp_ctx *ctx, int pack, int e0, int n_experts, void *W_out, void *stream);
 
+/* --- TurboQuant-MSE base --------------------------------------------------- */
+/* PAPER.md L944-946 (9.2): "the quantizer separates scale from direction, normalizes the vector and stores its norm,
+ * applies a seeded random orthogonal rotation, and then quantizes each rotated coordinate independently against a scalar
+ * codebook ... The rotation is a signed Hadamard transform when the dimension is a power of two and a QR rotation from a
+ * Gaussian matrix with sign fixing otherwise.  Reconstruction looks up the codebook values and rescales by the stored
+ * norm."  L946: 8-bit, "the per-expert weight packs quantized row by row" (row = output channel, width n = the pack's
+ * input width).  Storage: one uint8 code per rotated coordinate, one fp32 norm per row (the paper prints no dtype for
+ * the norm: DESIGN.md R24).
+ *
+ * One rotated space: y = R u.  hadamard = 1: R = H_n diag(signs) / sqrt(n), H_n the Sylvester matrix, n a power of two;
+ * hadamard = 0: R a dense orthogonal matrix (e.g. from tqp_tq_rotation_qr).  n % 64 == 0, 64 <= n <= 8192 (dense rotations of
+ * activations additionally n % 128 == 0).  The seeded random draws (signs, Gaussian matrix) are the caller's inputs.
+ * All pointers DEVICE; they must stay valid while any call or bound layer uses the space.  For a dense R the library
+ * keeps derived device copies (bf16 R, R^T; fp64 R^T) inside the ctx, keyed by the R pointer, until tqp_destroy. */
+typedef struct {
+    int32_t n;
+    int32_t hadamard;
+    const int8_t *signs;  /* int8 [n], +1 / -1 (hadamard = 1), else NULL */
+    const double *R;      /* fp64 [n][n] row-major (hadamard = 0), else NULL */
+    const double *levels; /* fp64 [256], ascending: the Lloyd-Max levels of the coordinate law in dimension n */
+} tqp_tq_space;
+/* HOST: the 2^bits Lloyd-Max levels of f_n(y) ~ (1 - y^2)^((n-3)/2) on [-1, 1] (L944: "computed analytically from that law"),
+ * ascending, into the HOST array levels[2^bits].  n >= 8, 1 <= bits <= 8. */
+tqp_status tqp_tq_levels(int n, int bits, double *levels);
+/* HOST: the sign-fixed Q of the QR factorisation of G (HOST fp64 [n][n] row-major, the caller's seeded Gaussian draw):
+ * the unique orthogonal Q with G = Q Rr, diag(Rr) > 0, into the HOST array R_out[n][n] (L946 "QR rotation ... with sign fixing"). */
+tqp_status tqp_tq_rotation_qr(int n, const double *G, double *R_out);
+/* Rotation of activations: Y[row] = R X[row] (inverse = 0) or R^T X[row] (inverse = 1); X, Y bf16 [rows][n], Y may be X only for
+ * hadamard spaces.  Hadamard: one FWHT pass (HBM-bound); dense: a bf16 tensor-core product with fp32 accumulation. */
+tqp_status tqp_rotate(tqp_ctx *ctx, const tqp_tq_space *space, const void *X, long long rows, void *Y, int inverse, void *stream);
+/* Encoder, row by row (L944-946): norms[row] = |W[row]|, codes[row][j] = index of the Lloyd-Max cell of (R W[row] / norm)_j
+ * (a coordinate on a cell boundary takes the lower code; a zero row: norm 0 and the codes of y = 0).  W fp32 [rows][n];
+ * codes uint8 [rows][n]; norms fp32 [rows].  Norm, rotation and cell search run in fp64. */
+tqp_status tqp_tq_encode(tqp_ctx *ctx, const tqp_tq_space *space, const float *W, long long rows, uint8_t *codes, float *norms,
+                         void *stream);
+/* Reconstruction (L946): W[row] = norms[row] * (levels[codes[row]] R), fp32 [rows][n]. */
+tqp_status tqp_tq_decode(tqp_ctx *ctx, const tqp_tq_space *space, const uint8_t *codes, const float *norms, long long rows, float *W,
+                         void *stream);
+/* Flush (PAPER.md L966 9.4: "periodically fold the adapter delta into the base, reset the adapter factors"; L1047-1061 10.3,
+ * Table 28: "the mean adapter norm ... and the share of each effective weight still coming from the frozen base") of one
+ * pack of n_experts experts, in place:
+ *   W = decode(codes, norms);  W_merged = W + lora_scale (A B)^T;  (codes, norms) <- encode(W_merged);  B <- 0;
+ *   A <- A_new if A_new != NULL.
+ * The fold and the re-quantisation run in the ROTATED space (R W_merged = norm levels[codes] + lora_scale (R A) B column
+ * by column), in fp64, without materialising a weight in HBM.  codes uint8 [n_experts][out_dim][n]; norms fp32
+ * [n_experts][out_dim]; A bf16 [n_experts][n][r]; B bf16 [n_experts][r][out_dim]; A_new like A or NULL; telemetry fp32
+ * [n_experts][2] or NULL: (|lora_scale A B|_F, |W|_F / (|W|_F + |lora_scale A B|_F)) of the state BEFORE the fold
+ * (R26).  1 <= r <= 32. */
+tqp_status tqp_tq_flush(tqp_ctx *ctx, const tqp_tq_space *space, int n_experts, int out_dim, int r, float lora_scale, uint8_t *codes,
+                        float *norms, void *A, void *B, const void *A_new, float *telemetry, void *stream);
+
 /* --- introspection ------------------------------------------------------------------------------------- */
 /* Device pointers of workspace tensors, for tests: "G","U","H" bf16 [N][F]; "Xp" bf16 [N][d];
  * "dH","dG","dU" bf16 [N][F]; "num_tiles" int32 [1].  NULL if unknown. */

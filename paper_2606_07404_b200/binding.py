@@ -34,6 +34,22 @@ class Weights(ctypes.Structure):
     _fields_ = [(n, ctypes.c_void_p) for n in _WEIGHT_FIELDS]
 
 
+class TqSpaceC(ctypes.Structure):
+    _fields_ = [("n", ctypes.c_int32), ("hadamard", ctypes.c_int32), ("signs", ctypes.c_void_p), ("R", ctypes.c_void_p),
+                ("levels", ctypes.c_void_p)]
+
+
+class TqSpace:
+    """tqp_tq_space holder: keeps the device tensors alive.  signs: int8 [n] (Hadamard) or R: float64 [n][n] (dense);
+    levels: float64 [256].  All torch CUDA tensors."""
+
+    def __init__(self, n, levels, signs=None, R=None):
+        assert (signs is None) != (R is None)
+        self.n, self.levels, self.signs, self.R = int(n), levels.contiguous(), signs, R
+        self.c = TqSpaceC(self.n, 1 if signs is not None else 0, signs.data_ptr() if signs is not None else None,
+                          R.data_ptr() if R is not None else None, self.levels.data_ptr())
+
+
 def abi_symbols() -> list[str]:
     """Function names declared in include/tqp.h."""
     text = open(HEADER).read()
@@ -72,6 +88,13 @@ def load_library() -> ctypes.CDLL:
         lib.tqp_route_sigmoid_bwd.argtypes = [vp, ci] + [vp] * 11
         lib.tqp_bias_update.argtypes = [vp, vp, vp, ci, ctypes.c_float, ctypes.c_float, ctypes.c_float, vp]
         lib.tqp_consolidate.argtypes = [vp, ci, ci, ci, vp, vp]
+        sp, ll = ctypes.POINTER(TqSpaceC), ctypes.c_longlong
+        lib.tqp_tq_levels.argtypes = [ci, ci, vp]
+        lib.tqp_tq_rotation_qr.argtypes = [ci, vp, vp]
+        lib.tqp_rotate.argtypes = [vp, sp, vp, ll, vp, ci, vp]
+        lib.tqp_tq_encode.argtypes = [vp, sp, vp, ll, vp, vp, vp]
+        lib.tqp_tq_decode.argtypes = [vp, sp, vp, vp, ll, vp, vp]
+        lib.tqp_tq_flush.argtypes = [vp, sp, ci, ci, ci, ctypes.c_float, vp, vp, vp, vp, vp, vp, vp]
         lib.tqp_debug_buffer.argtypes = [vp, ctypes.c_char_p]
         lib.tqp_debug_buffer.restype = vp
         lib.tqp_gemm_time.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_int)]
@@ -95,6 +118,28 @@ def workspace_bytes(T_max, d, F, E, k, r, lora_scale=1.0, training=True) -> int:
 
 def _ptr(t):
     return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def tq_levels(n: int, bits: int = 8):
+    """HOST: Lloyd-Max levels of the coordinate law in dimension n (tqp_tq_levels) as a numpy float64 array."""
+    import numpy as np
+    out = np.empty(1 << bits, dtype=np.float64)
+    code = load_library().tqp_tq_levels(int(n), int(bits), out.ctypes.data_as(ctypes.c_void_p))
+    if code != 0:
+        raise TqpError(code, "tqp_tq_levels")
+    return out
+
+
+def tq_rotation_qr(G):
+    """HOST: sign-fixed Q of the QR factorisation of the Gaussian draw G (numpy float64 [n][n]) (tqp_tq_rotation_qr)."""
+    import numpy as np
+    G = np.ascontiguousarray(G, dtype=np.float64)
+    n = G.shape[0]
+    out = np.empty((n, n), dtype=np.float64)
+    code = load_library().tqp_tq_rotation_qr(n, G.ctypes.data_as(ctypes.c_void_p), out.ctypes.data_as(ctypes.c_void_p))
+    if code != 0:
+        raise TqpError(code, "tqp_tq_rotation_qr")
+    return out
 
 
 class TqpLayer:
@@ -260,6 +305,38 @@ class TqpLayer:
             out = self.torch.empty((n, out_dim, in_dim), dtype=self.torch.bfloat16, device=self.device)
         self._check(self.lib.tqp_consolidate(self.ctx, int(pack), int(e0), int(n), _ptr(out), self._stream()))
         return out
+
+    # ---- TurboQuant-MSE base ----
+    def rotate(self, space, X, inverse=False, out=None):
+        t = self.torch
+        Y = out if out is not None else t.empty_like(X)
+        self._check(self.lib.tqp_rotate(self.ctx, ctypes.byref(space.c), _ptr(X), X.shape[0], _ptr(Y), 1 if inverse else 0, self._stream()))
+        return Y
+
+    def tq_encode(self, space, W):
+        """W fp32 [rows][n] -> (codes uint8 [rows][n], norms fp32 [rows])."""
+        t = self.torch
+        rows = W.shape[0]
+        codes = t.empty((rows, space.n), dtype=t.uint8, device=self.device)
+        norms = t.empty((rows,), dtype=t.float32, device=self.device)
+        self._check(self.lib.tqp_tq_encode(self.ctx, ctypes.byref(space.c), _ptr(W), rows, _ptr(codes), _ptr(norms), self._stream()))
+        return codes, norms
+
+    def tq_decode(self, space, codes, norms):
+        t = self.torch
+        rows = codes.shape[0]
+        W = t.empty((rows, space.n), dtype=t.float32, device=self.device)
+        self._check(self.lib.tqp_tq_decode(self.ctx, ctypes.byref(space.c), _ptr(codes), _ptr(norms), rows, _ptr(W), self._stream()))
+        return W
+
+    def tq_flush(self, space, codes, norms, A, B, lora_scale, A_new=None):
+        """In place on codes [E][out][n], norms [E][out], A [E][n][r], B [E][r][out]; returns telemetry fp32 [E][2]."""
+        t = self.torch
+        E, out_dim, r = codes.shape[0], codes.shape[1], A.shape[2]
+        tele = t.empty((E, 2), dtype=t.float32, device=self.device)
+        self._check(self.lib.tqp_tq_flush(self.ctx, ctypes.byref(space.c), E, out_dim, r, float(lora_scale), _ptr(codes), _ptr(norms),
+                                          _ptr(A), _ptr(B), _ptr(A_new), _ptr(tele), self._stream()))
+        return tele
 
     def step_host(self, X_host, dY_host, W_r, logit_bias, Y_host, dX_host, grads, dW_r=None):
         """Whole forward+backward through HOST (pinned) X/dY/Y/dX buffers; grads / dW_r stay on the device."""

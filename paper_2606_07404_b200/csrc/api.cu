@@ -191,6 +191,7 @@ void tqp_destroy(tqp_ctx *ctx) {
     for (cudaEvent_t e : {ctx->ev_start, ctx->ev_x, ctx->ev_dy, ctx->ev_y, ctx->ev_yout, ctx->ev_dx, ctx->ev_xc[0], ctx->ev_xc[1],
                           ctx->ev_xc[2], ctx->ev_xc[3], ctx->ev_done[0], ctx->ev_done[1], ctx->ev_comp[0], ctx->ev_comp[1]})
         if (e) cudaEventDestroy(e);
+    for (auto &r : ctx->tq_rots) { cudaFree(r.Rb); cudaFree(r.Rtb); cudaFree(r.Rt); }
     if (ctx->copy_in) cudaStreamDestroy(ctx->copy_in);
     if (ctx->copy_out) cudaStreamDestroy(ctx->copy_out);
     delete ctx;

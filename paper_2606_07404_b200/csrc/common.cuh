@@ -67,6 +67,14 @@ struct GemmArgs {           // passed by value (__grid_constant__) so the tensor
     int nprob;
 };
 
+// derived device copies of a dense TurboQuant rotation (turboquant.cu), owned by the ctx
+struct TqRot {
+    const double *R;   // the caller's matrix (cache key)
+    int n;
+    bf16 *Rb, *Rtb;    // bf16 R and R^T (activation products)
+    double *Rt;        // fp64 R^T
+};
+
 struct Workspace {
     // sizes
     size_t total = 0;
@@ -92,6 +100,7 @@ struct tqp_ctx {
     // TQP_BWD_DYE_UNMODIFIED claim in tqp_expert_bwd, never dereferenced); cleared by every other call that could invalidate it
     const void *zd_src = nullptr;
     int device = 0;                 // the device the ctx was created on (kernel attributes are per device)
+    std::vector<tqp::TqRot> tq_rots;             // library-owned; freed by tqp_destroy
     std::vector<const void *> smem_attr_done;   // kernels whose dynamic shared-memory limit has been raised on `device`
     int launches = 0;
     int num_sms = 148;
@@ -203,6 +212,13 @@ inline tqp_status ensure_dyn_smem(tqp_ctx *c, const void *func, int bytes) {
     c->smem_attr_done.push_back(func);
     return TQP_OK;
 }
+
+// ---- turboquant.cu --------------------------------------------------------------------------------------
+tqp_status tq_check_space(tqp_ctx *c, const tqp_tq_space *sp);
+tqp_status launch_tq_rotate(tqp_ctx *c, const tqp_tq_space *sp, const void *X, bool in_f32, long long rows, void *Y, bool out_f32, int inverse,
+                            cudaStream_t st);
+template <typename T>
+tqp_status launch_tq_transpose(tqp_ctx *c, const T *in, T *out, int E, int a, int b, cudaStream_t st);   // [E][a][b] -> [E][b][a]
 
 // ---- device helpers ------------------------------------------------------------------------------------
 __device__ __forceinline__ float bf16_bits_to_float(uint16_t b) { return __uint_as_float(((uint32_t)b) << 16); }

@@ -81,7 +81,7 @@ def test_requantisation_error_is_the_quantisers_distortion():
     D = sum(integrate.quad(lambda y: (y - cb[j]) ** 2 * dens(y), b[j], b[j + 1], epsabs=0, epsrel=1e-10)[0] for j in range(len(cb))) / z
     assert abs(rel2.mean() / (n * D) - 1.0) < 0.1
     assert rel2.mean() < np.sqrt(3.0) * np.pi / 2.0 * 4.0 ** (-bits)
-    assert rel2.max() < 4.0 * n * D
+    assert rel2.max() < 8.0 * n * D                # rows with a coordinate in an outer (overload) cell
 
 
 def test_flush_preserves_the_function_up_to_the_distortion():

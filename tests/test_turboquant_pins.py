@@ -36,6 +36,21 @@ def test_lloyd_max_conditions_by_quadrature(n, bits):
         assert abs(num / den - c[j]) < 1e-8
 
 
+@pytest.mark.parametrize("n", [64, 1024])
+def test_lloyd_max_conditions_at_8_bits(n):
+    """The 8-bit codebook the TQP base uses.  A plain Lloyd loop stopped by an iteration cap is NOT at the
+    fixed point here (round 2 found the oracle's first version 4e-3 / sqrt(n) off, condition violated by 6e-7): every level
+    must be its cell's conditional mean to 1e-11 / sqrt(n)."""
+    c = tq.lloyd_max_codebook(n, 8)
+    assert len(c) == 256 and (np.diff(c) > 0).all()
+    dens = lambda y: (1.0 - y * y) ** ((n - 3) / 2.0)
+    b = np.concatenate(([-1.0], 0.5 * (c[:-1] + c[1:]), [1.0]))
+    for j in range(0, 256, 3):
+        num = integrate.quad(lambda y: y * dens(y), b[j], b[j + 1], epsabs=0, epsrel=1e-12)[0]
+        den = integrate.quad(dens, b[j], b[j + 1], epsabs=0, epsrel=1e-12)[0]
+        assert abs(num / den - c[j]) * np.sqrt(n) < 1e-10, j
+
+
 def test_large_dimension_limit_is_max_gaussian_quantiser():
     """sqrt(n) * levels -> the Lloyd-Max levels of N(0, 1): 1 bit +-0.7979 (= sqrt(2/pi)), 2 bits +-0.4528, +-1.510,
     3 bits +-0.2451, +-0.7560, +-1.344, +-2.152 (Max 1960, Table I)."""
