@@ -254,6 +254,32 @@ tqp_status tqp_tq_decode(tqp_ctx *ctx, const tqp_tq_space *space, const uint8_t 
 tqp_status tqp_tq_flush(tqp_ctx *ctx, const tqp_tq_space *space, int n_experts, int out_dim, int r, float lora_scale, uint8_t *codes,
                         float *norms, void *A, void *B, const void *A_new, float *telemetry, void *stream);
 
+/* The routed-expert layer over a TurboQuant base.  Frozen base: one code per rotated coordinate and one norm per row;
+ * W_eff[in][out] = norm[out] * (levels[codes[out]] R)[in] + lora_scale * (A . B)[in][out]  with R, levels of the pack's
+ * input space (space_d for gate / up, space_F for down).  Adapters as in tqp_weights (unrotated).  All DEVICE pointers. */
+typedef struct {
+    const uint8_t *codes_gate, *codes_up; /* [E][F][d] */
+    const uint8_t *codes_down;            /* [E][d][F] */
+    const float *norm_gate, *norm_up;     /* fp32 [E][F] */
+    const float *norm_down;               /* fp32 [E][d] */
+    tqp_tq_space space_d, space_F;
+    const void *A_gate, *A_up;            /* bf16 [E][d][r] */
+    const void *B_gate, *B_up;            /* bf16 [E][r][F] */
+    const void *A_down;                   /* bf16 [E][F][r] */
+    const void *B_down;                   /* bf16 [E][r][d] */
+} tqp_tq_weights;
+/* Binds a TurboQuant base in place of tqp_bind_weights; afterwards tqp_expert_fwd / tqp_expert_bwd / tqp_dispatch_bwd (and the
+ * tqp_step_host calls) run the same layer over it.  How: the rotation is applied ONCE to the activations (x' = R_d x on the
+ * T token rows before the gather; h' = R_F h after the SwiGLU), the grouped GEMM's mainloop then looks each code up in a
+ * 256-entry scalar table and scales by the row norm -- no weight is materialised -- and the adapters' input side is
+ * carried into the rotated space (A' = R A, so that x . A = x' . A'); gradients come back through R^T.  Two things differ
+ * for the caller: (1) with a TurboQuant base bound, the dXp tensor tqp_expert_bwd returns holds the gradient in the
+ * ROTATED input space, and tqp_dispatch_bwd undoes the rotation after the token sum (the rotation is linear);
+ * (2) needs r in {16, 32}, d % 256 == 0, F % 256 == 0, training ctx or not.  The library allocates its own device
+ * buffers for the rotated activations / adapters (freed by tqp_destroy or the next bind).  TQP_ERR_SHAPE for unsupported
+ * shapes or spaces whose n is not d / F. */
+tqp_status tqp_bind_weights_tq(tqp_ctx *ctx, const tqp_tq_weights *w, void *stream);
+
 /* --- introspection ------------------------------------------------------------------------------------- */
 /* Device pointers of workspace tensors, for tests: "G","U","H" bf16 [N][F]; "Xp" bf16 [N][d];
  * "dH","dG","dU" bf16 [N][F]; "num_tiles" int32 [1].  NULL if unknown. */

@@ -39,6 +39,15 @@ class TqSpaceC(ctypes.Structure):
                 ("levels", ctypes.c_void_p)]
 
 
+_TQ_FIELDS_A = ["codes_gate", "codes_up", "codes_down", "norm_gate", "norm_up", "norm_down"]
+_TQ_FIELDS_B = ["A_gate", "A_up", "B_gate", "B_up", "A_down", "B_down"]
+
+
+class TqWeightsC(ctypes.Structure):
+    _fields_ = ([(n, ctypes.c_void_p) for n in _TQ_FIELDS_A] + [("space_d", TqSpaceC), ("space_F", TqSpaceC)] +
+                [(n, ctypes.c_void_p) for n in _TQ_FIELDS_B])
+
+
 class TqSpace:
     """tqp_tq_space holder: keeps the device tensors alive.  signs: int8 [n] (Hadamard) or R: float64 [n][n] (dense);
     levels: float64 [256].  All torch CUDA tensors."""
@@ -89,6 +98,7 @@ def load_library() -> ctypes.CDLL:
         lib.tqp_bias_update.argtypes = [vp, vp, vp, ci, ctypes.c_float, ctypes.c_float, ctypes.c_float, vp]
         lib.tqp_consolidate.argtypes = [vp, ci, ci, ci, vp, vp]
         sp, ll = ctypes.POINTER(TqSpaceC), ctypes.c_longlong
+        lib.tqp_bind_weights_tq.argtypes = [vp, ctypes.POINTER(TqWeightsC), vp]
         lib.tqp_tq_levels.argtypes = [ci, ci, vp]
         lib.tqp_tq_rotation_qr.argtypes = [ci, vp, vp]
         lib.tqp_rotate.argtypes = [vp, sp, vp, ll, vp, ci, vp]
@@ -187,6 +197,14 @@ class TqpLayer:
         self.weights = {n: w[n].contiguous() for n in _WEIGHT_FIELDS}
         ws = Weights(*[self.weights[n].data_ptr() for n in _WEIGHT_FIELDS])
         self._check(self.lib.tqp_bind_weights(self.ctx, ctypes.byref(ws), self._stream()))
+
+    def bind_weights_tq(self, space_d, space_F, **w):
+        """TurboQuant base: codes_* uint8, norm_* fp32, bf16 adapters (tqp_tq_weights' fields); spaces are TqSpace objects."""
+        self.weights = {n: w[n].contiguous() for n in _TQ_FIELDS_A + _TQ_FIELDS_B}
+        self.spaces = (space_d, space_F)
+        ws = TqWeightsC(*([self.weights[n].data_ptr() for n in _TQ_FIELDS_A] + [space_d.c, space_F.c] +
+                          [self.weights[n].data_ptr() for n in _TQ_FIELDS_B]))
+        self._check(self.lib.tqp_bind_weights_tq(self.ctx, ctypes.byref(ws), self._stream()))
 
     # ---- forward ----
     def route(self, X, W_r, logit_bias=None, want_logits=False):

@@ -119,6 +119,8 @@ tqp_status set_lora(tqp_ctx *c, GemmLora *l, const bf16 *lact, uint64_t rows, co
     return act_map(c, &l->lact_map, lact, rows, kLoraPad);
 }
 
+void tq_free_state(tqp_ctx *c);   // defined with the TurboQuant binding below
+
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
 #define REQ(ctx, cond, code, msg)              \
@@ -192,6 +194,7 @@ void tqp_destroy(tqp_ctx *ctx) {
                           ctx->ev_xc[2], ctx->ev_xc[3], ctx->ev_done[0], ctx->ev_done[1], ctx->ev_comp[0], ctx->ev_comp[1]})
         if (e) cudaEventDestroy(e);
     for (auto &r : ctx->tq_rots) { cudaFree(r.Rb); cudaFree(r.Rtb); cudaFree(r.Rt); }
+    tq_free_state(ctx);
     if (ctx->copy_in) cudaStreamDestroy(ctx->copy_in);
     if (ctx->copy_out) cudaStreamDestroy(ctx->copy_out);
     delete ctx;
@@ -250,6 +253,7 @@ tqp_status tqp_bind_weights(tqp_ctx *c, const tqp_weights *w, void *stream) {
     for (const void *p : ptrs) PTR_OK(c, p);
     c->w = *w;
     c->launches = 0;
+    if (c->tq.on) tq_free_state(c);
     const tqp_layer_desc &D = c->desc;
     const uint64_t Np = (uint64_t)D.T_max * D.k + kRowPad;
     tqp_status st = launch_make_lut(c, (const __half *)w->codebook, c->p<bf16>(c->ws.lut), (cudaStream_t)stream);
@@ -284,6 +288,121 @@ tqp_status tqp_bind_weights(tqp_ctx *c, const tqp_weights *w, void *stream) {
     c->have_weights = true;
     return TQP_OK;
 }
+
+}  // extern "C"
+
+namespace {
+
+void tq_free_state(tqp_ctx *c) {
+    tqp::TqLayer &t = c->tq;
+    for (void *p : {(void *)t.Xr, (void *)t.Ar_gate, (void *)t.Ar_up, (void *)t.Ar_down, (void *)t.tmp_a, (void *)t.tmp_b, (void *)t.dAr_gate,
+                    (void *)t.dAr_up, (void *)t.dAr_down, (void *)t.tmp_f, (void *)t.lut_d, (void *)t.lut_F})
+        if (p) cudaFree(p);
+    t = tqp::TqLayer();
+}
+
+// scalar-format segment: codes [E][M][K] (kmajor) or used transposed [E][K][M]; box 128 bytes x 128 rows, 128-byte swizzle
+tqp_status set_seg_tq(tqp_ctx *c, GemmSeg *s, const bf16 *act, uint64_t act_rows, const uint8_t *codes, const float *norm, const bf16 *lut,
+                      int K, int M, int kmajor) {
+    s->act = act; s->idx = codes; s->scale = nullptr; s->norm = norm; s->lut = lut; s->scalar = 1; s->K = K; s->kmajor = kmajor;
+    tqp_status st = act_map(c, &s->act_map, act, act_rows, K);
+    if (st != TQP_OK) return st;
+    st = act_map(c, &s->act_map2, act, act_rows, K, kTileRows / 2);
+    if (st != TQP_OK) return st;
+    const uint64_t E = c->desc.E;
+    const uint64_t rows = kmajor ? E * M : E * K, bytes = kmajor ? K : M;
+    return make_map(c, &s->idx_map, codes, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, rows, bytes, 128, 128, CU_TENSOR_MAP_SWIZZLE_128B);
+}
+
+// A' = R A per expert:  A [E][n][r] -> transpose -> rows [E r][n] -> rotate -> transpose back
+tqp_status tq_rotate_adapter(tqp_ctx *c, const tqp_tq_space *sp, const bf16 *A, bf16 *Ar, cudaStream_t s) {
+    const int E = c->desc.E, r = c->desc.r, n = sp->n;
+    tqp_status st = launch_tq_transpose<bf16>(c, A, c->tq.tmp_a, E, n, r, s);
+    if (st == TQP_OK) st = launch_tq_rotate(c, sp, c->tq.tmp_a, false, (long long)E * r, c->tq.tmp_b, false, 0, s);
+    if (st == TQP_OK) st = launch_tq_transpose<bf16>(c, c->tq.tmp_b, Ar, E, r, n, s);
+    return st;
+}
+// dA = R^T dA' per expert (fp32): the same way back
+tqp_status tq_unrotate_grad(tqp_ctx *c, const tqp_tq_space *sp, float *dAr, float *dA, cudaStream_t s) {
+    const int E = c->desc.E, r = c->desc.r, n = sp->n;
+    tqp_status st = launch_tq_transpose<float>(c, dAr, c->tq.tmp_f, E, n, r, s);
+    if (st == TQP_OK) st = launch_tq_rotate(c, sp, c->tq.tmp_f, true, (long long)E * r, dAr, true, 1, s);
+    if (st == TQP_OK) st = launch_tq_transpose<float>(c, dAr, dA, E, r, n, s);
+    return st;
+}
+
+}  // namespace
+
+extern "C" tqp_status tqp_bind_weights_tq(tqp_ctx *c, const tqp_tq_weights *w, void *stream) {
+    if (!c || !w) return TQP_ERR_ARG;
+    REQ(c, c->base != nullptr, TQP_ERR_WORKSPACE, "bind a workspace first");
+    const void *ptrs[] = {w->codes_gate, w->codes_up, w->codes_down, w->norm_gate, w->norm_up, w->norm_down,
+                          w->A_gate, w->A_up, w->B_gate, w->B_up, w->A_down, w->B_down};
+    for (const void *p : ptrs) PTR_OK(c, p);
+    const tqp_layer_desc &D = c->desc;
+    tqp_status st = tq_check_space(c, &w->space_d);
+    if (st == TQP_OK) st = tq_check_space(c, &w->space_F);
+    if (st != TQP_OK) return st;
+    REQ(c, w->space_d.n == D.d && w->space_F.n == D.F, TQP_ERR_SHAPE, "space_d.n must be d and space_F.n must be F");
+    REQ(c, (D.r == 16 || D.r == 32) && D.d % 256 == 0 && D.F % 256 == 0, TQP_ERR_SHAPE,
+        "the TurboQuant-format layer needs r in {16, 32}, d % 256 == 0, F % 256 == 0");
+    cudaStream_t s = (cudaStream_t)stream;
+    c->launches = 0;
+    c->have_weights = false;
+    tq_free_state(c);
+    tqp::TqLayer &t = c->tq;
+    t.w = *w;
+    const size_t E = D.E, r = D.r, dm = D.d, F = D.F, mx = dm > F ? dm : F;
+    TQP_CUDA_OK(c, cudaMalloc(&t.Xr, (size_t)D.T_max * dm * 2));
+    TQP_CUDA_OK(c, cudaMalloc(&t.Ar_gate, E * dm * r * 2)); TQP_CUDA_OK(c, cudaMalloc(&t.Ar_up, E * dm * r * 2));
+    TQP_CUDA_OK(c, cudaMalloc(&t.Ar_down, E * F * r * 2));
+    TQP_CUDA_OK(c, cudaMalloc(&t.tmp_a, E * mx * r * 2)); TQP_CUDA_OK(c, cudaMalloc(&t.tmp_b, E * mx * r * 2));
+    if (D.training) {
+        TQP_CUDA_OK(c, cudaMalloc(&t.dAr_gate, E * dm * r * 4)); TQP_CUDA_OK(c, cudaMalloc(&t.dAr_up, E * dm * r * 4));
+        TQP_CUDA_OK(c, cudaMalloc(&t.dAr_down, E * F * r * 4)); TQP_CUDA_OK(c, cudaMalloc(&t.tmp_f, E * mx * r * 4));
+    }
+    TQP_CUDA_OK(c, cudaMalloc(&t.lut_d, 512)); TQP_CUDA_OK(c, cudaMalloc(&t.lut_F, 512));
+    st = launch_tq_make_lut(c, w->space_d.levels, t.lut_d, s);
+    if (st == TQP_OK) st = launch_tq_make_lut(c, w->space_F.levels, t.lut_F, s);
+    if (st != TQP_OK) return st;
+    // the adapter pointers of the common code path: B sides as given, A sides replaced by their rotated copies
+    memset(&c->w, 0, sizeof(c->w));
+    c->w.A_gate = t.Ar_gate; c->w.A_up = t.Ar_up; c->w.A_down = t.Ar_down;
+    c->w.B_gate = w->B_gate; c->w.B_up = w->B_up; c->w.B_down = w->B_down;
+    const uint64_t Np = (uint64_t)D.T_max * D.k + kRowPad;
+    bf16 *Xp = c->p<bf16>(c->ws.Xp), *G = c->p<bf16>(c->ws.G), *U = c->p<bf16>(c->ws.U), *H = c->p<bf16>(c->ws.H);
+    bf16 *dH = c->p<bf16>(c->ws.dH), *dG = c->p<bf16>(c->ws.dG), *dU = c->p<bf16>(c->ws.dU);
+    GemmProblem *P;
+#define CK(x) do { st = (x); if (st != TQP_OK) return st; } while (0)
+    P = &c->prob_gate; memset(P, 0, sizeof(*P));
+    P->nseg = 1; P->nlora = 1; P->M = D.F; P->r = D.r; P->out = G;
+    CK(set_seg_tq(c, &P->seg[0], Xp, Np, w->codes_gate, w->norm_gate, t.lut_d, D.d, D.F, 1));
+    CK(set_lora(c, &P->lora[0], c->p<bf16>(c->ws.XAg), Np, w->B_gate, 0));
+    P = &c->prob_up; memset(P, 0, sizeof(*P));
+    P->nseg = 1; P->nlora = 1; P->M = D.F; P->r = D.r; P->out = U;
+    CK(set_seg_tq(c, &P->seg[0], Xp, Np, w->codes_up, w->norm_up, t.lut_d, D.d, D.F, 1));
+    CK(set_lora(c, &P->lora[0], c->p<bf16>(c->ws.XAu), Np, w->B_up, 0));
+    P = &c->prob_down; memset(P, 0, sizeof(*P));
+    P->nseg = 1; P->nlora = 1; P->M = D.d; P->r = D.r; P->out = nullptr;
+    CK(set_seg_tq(c, &P->seg[0], H, Np, w->codes_down, w->norm_down, t.lut_F, D.F, D.d, 1));
+    CK(set_lora(c, &P->lora[0], c->p<bf16>(c->ws.HAd), Np, w->B_down, 0));
+    P = &c->prob_dh; memset(P, 0, sizeof(*P));
+    P->nseg = 1; P->nlora = 1; P->M = D.F; P->r = D.r; P->out = dH;
+    CK(set_seg_tq(c, &P->seg[0], dH /*placeholder*/, Np, w->codes_down, w->norm_down, t.lut_F, D.d, D.F, 0));
+    CK(set_lora(c, &P->lora[0], c->p<bf16>(c->ws.Zd), Np, t.Ar_down, 1));
+    P = &c->prob_dx; memset(P, 0, sizeof(*P));
+    P->nseg = 2; P->nlora = 2; P->M = D.d; P->r = D.r; P->out = nullptr;
+    CK(set_seg_tq(c, &P->seg[0], dG, Np, w->codes_gate, w->norm_gate, t.lut_d, D.F, D.d, 0));
+    CK(set_seg_tq(c, &P->seg[1], dU, Np, w->codes_up, w->norm_up, t.lut_d, D.F, D.d, 0));
+    CK(set_lora(c, &P->lora[0], c->p<bf16>(c->ws.Zg), Np, t.Ar_gate, 1));
+    CK(set_lora(c, &P->lora[1], c->p<bf16>(c->ws.Zu), Np, t.Ar_up, 1));
+#undef CK
+    t.on = true;
+    c->have_weights = true;
+    return TQP_OK;
+}
+
+extern "C" {
 
 tqp_status tqp_set_option(tqp_ctx *c, const char *name, int value) {
     if (!c || !name) return TQP_ERR_ARG;
@@ -354,6 +473,16 @@ tqp_status tqp_expert_fwd(tqp_ctx *c, int T, const void *X, const int32_t *offse
     bf16 *Xp = c->p<bf16>(c->ws.Xp), *G = c->p<bf16>(c->ws.G), *U = c->p<bf16>(c->ws.U), *H = c->p<bf16>(c->ws.H);
 #define CK(x) do { st = (x); if (st != TQP_OK) return st; } while (0)
     const bool fused = D.r == 16 || D.r == 32;   // rank 8 (config 0) keeps the separate CUDA-core kernels
+    const bool tq = c->tq.on;
+    if (tq) {
+        // TurboQuant base: carry the adapters' input sides and the token rows into the rotated spaces once;
+        // everything below then runs on x' = R_d x and A' = R A  (x . A = x' . A', x . W_row = norm level[codes] . x')
+        CK(tq_rotate_adapter(c, &c->tq.w.space_d, (const bf16 *)c->tq.w.A_gate, c->tq.Ar_gate, s));
+        CK(tq_rotate_adapter(c, &c->tq.w.space_d, (const bf16 *)c->tq.w.A_up, c->tq.Ar_up, s));
+        CK(tq_rotate_adapter(c, &c->tq.w.space_F, (const bf16 *)c->tq.w.A_down, c->tq.Ar_down, s));
+        CK(launch_tq_rotate(c, &c->tq.w.space_d, X, false, T, c->tq.Xr, false, 0, s));
+        X = c->tq.Xr;
+    }
     if (fused) {   // Xp = gather(X) and both adapter projections x.A_g | x.A_u in one pass over the rows
         if (D.d % 256 == 0) {   // rows by TMA gather4 (X is the caller's: its maps are encoded per call)
             CUtensorMap gm[3];
@@ -372,6 +501,14 @@ tqp_status tqp_expert_fwd(tqp_ctx *c, int T, const void *X, const int32_t *offse
     GemmProblem pr[2] = {c->prob_gate, c->prob_up};
     CK(run_gemm(c, pr, 2, s));
     CK(launch_swiglu_fwd(c, N, G, U, H, s));
+    if (tq) {   // h' = R_F h, in place for the Hadamard case (a dense R_F goes through the idle dG buffer)
+        if (c->tq.w.space_F.hadamard) {
+            CK(launch_tq_rotate(c, &c->tq.w.space_F, H, false, N, H, false, 0, s));
+        } else {
+            CK(launch_tq_rotate(c, &c->tq.w.space_F, H, false, N, c->p<bf16>(c->ws.dG), false, 0, s));
+            TQP_CUDA_OK(c, cudaMemcpyAsync(H, c->p<bf16>(c->ws.dG), (size_t)N * D.F * 2, cudaMemcpyDeviceToDevice, s));
+        }
+    }
     if (fused) CK(launch_rows_proj_tma(c, &c->prob_down.seg[0].act_map2, D.F, (const bf16 *)c->w.A_down, 1, ls, c->p<bf16>(c->ws.HAd), s));
     else CK(launch_rows_proj(c, H, D.F, nullptr, nullptr, nullptr, (const bf16 *)c->w.A_down, nullptr, 1, ls,
                              c->p<bf16>(c->ws.HAd), nullptr, s));
@@ -454,10 +591,24 @@ tqp_status tqp_expert_bwd(tqp_ctx *c, int T, const void *X, const void *dYe, con
     CK(act_map(c, &ph.seg[0].act_map, dye, (uint64_t)N, D.d));
     CK(act_map(c, &ph.seg[0].act_map2, dye, (uint64_t)N, D.d, kTileRows / 2));
     CK(run_gemm(c, &ph, 1, s));
+    const bool tq = c->tq.on;
+    if (tq) {   // the GEMM produced dh' = R_F dh (rotated F space): dh = R_F^T dh'
+        if (c->tq.w.space_F.hadamard) {
+            CK(launch_tq_rotate(c, &c->tq.w.space_F, dH, false, N, dH, false, 1, s));
+        } else {
+            CK(launch_tq_rotate(c, &c->tq.w.space_F, dH, false, N, dG, false, 1, s));
+            TQP_CUDA_OK(c, cudaMemcpyAsync(dH, dG, (size_t)N * D.F * 2, cudaMemcpyDeviceToDevice, s));
+        }
+    }
     CK(launch_swiglu_bwd(c, N, dH, G, U, dG, dU, s));
-    if (!c->defer_tail) {
+    // With a TurboQuant base the dA gradients are first formed w.r.t. A' = R A (the rows that multiply them are rotated) and
+    // then carried back, dA = R^T dA'; the deferred tail of tqp_step_host is not used in that mode.
+    const bool defer = c->defer_tail && !tq;
+    float *dAd = tq ? c->tq.dAr_down : dA_down, *dAg = tq ? c->tq.dAr_gate : dA_gate, *dAu = tq ? c->tq.dAr_up : dA_up;
+    if (!defer) {
         CK(launch_rows_wgrad(c, dye, D.d, c->p<bf16>(c->ws.HAd), nullptr, offsets, 0, dB_down, nullptr, s));
-        CK(launch_rows_wgrad(c, H, D.F, Zd, nullptr, offsets, 1, dA_down, nullptr, s));
+        CK(launch_rows_wgrad(c, H, D.F, Zd, nullptr, offsets, 1, dAd, nullptr, s));
+        if (tq) CK(tq_unrotate_grad(c, &c->tq.w.space_F, dAd, dA_down, s));
     }
     // gate / up projections: dXp = dG . Wg_eff^T + dU . Wu_eff^T and their adapter gradients
     if (D.r == 16 || D.r == 32) {   // dG, dU are workspace tensors the dXp GEMM already has tensor maps for
@@ -470,13 +621,17 @@ tqp_status tqp_expert_bwd(tqp_ctx *c, int T, const void *X, const void *dYe, con
     GemmProblem px = c->prob_dx;
     px.out = (bf16 *)dXp;
     CK(run_gemm(c, &px, 1, s));
-    if (c->defer_tail) {   // tqp_step_host: dX leaves for the host first (nothing below feeds it)
+    if (defer) {   // tqp_step_host: dX leaves for the host first (nothing below feeds it)
         c->tail = {dA_gate, dB_gate, dA_up, dB_up, dA_down, dB_down, dye, offsets, true};
         return TQP_OK;
     }
     CK(launch_rows_wgrad(c, dG, D.F, c->p<bf16>(c->ws.XAg), nullptr, offsets, 0, dB_gate, nullptr, s));
     CK(launch_rows_wgrad(c, dU, D.F, c->p<bf16>(c->ws.XAu), nullptr, offsets, 0, dB_up, nullptr, s));
-    CK(launch_rows_wgrad(c, Xp, D.d, Zg, Zu, offsets, 1, dA_gate, dA_up, s));   // one pass over Xp for both
+    CK(launch_rows_wgrad(c, Xp, D.d, Zg, Zu, offsets, 1, dAg, dAu, s));   // one pass over Xp for both
+    if (tq) {
+        CK(tq_unrotate_grad(c, &c->tq.w.space_d, dAg, dA_gate, s));
+        CK(tq_unrotate_grad(c, &c->tq.w.space_d, dAu, dA_up, s));
+    }
 #undef CK
     return TQP_OK;
 }
@@ -503,6 +658,13 @@ tqp_status tqp_dispatch_bwd(tqp_ctx *c, int T, const void *dXp, const int32_t *i
     tqp_status st = common_checks(c, T, false);
     if (st != TQP_OK) return st;
     PTR_OK(c, dXp); PTR_OK(c, inv_perm); PTR_OK(c, dX);
+    if (c->tq.on) {   // dXp is in the rotated input space: sum the tokens' rows there, then dX = R_d^T (sum)
+        st = launch_combine(c, T, (const bf16 *)dXp, inv_perm, nullptr, c->tq.Xr, (cudaStream_t)stream);
+        const int n1 = c->launches;
+        if (st == TQP_OK) st = launch_tq_rotate(c, &c->tq.w.space_d, c->tq.Xr, false, T, dX, false, 1, (cudaStream_t)stream);
+        (void)n1;
+        return st;
+    }
     return launch_combine(c, T, (const bf16 *)dXp, inv_perm, nullptr, (bf16 *)dX, (cudaStream_t)stream);
 }
 
@@ -550,7 +712,7 @@ tqp_status tqp_bias_update(tqp_ctx *c, const int32_t *counts, float *bias, int m
 tqp_status tqp_consolidate(tqp_ctx *c, int pack, int e0, int n_experts, void *W_out, void *stream) {
     if (!c) return TQP_ERR_ARG;
     c->launches = 0;
-    REQ(c, c->have_weights, TQP_ERR_STATE, "tqp_consolidate needs tqp_bind_weights first");
+    REQ(c, c->have_weights && !c->tq.on, TQP_ERR_STATE, "tqp_consolidate needs tqp_bind_weights (vector-quantised base) first");
     REQ(c, pack >= 0 && pack <= 2, TQP_ERR_ARG, "pack must be 0 (gate), 1 (up) or 2 (down)");
     REQ(c, e0 >= 0 && n_experts >= 0 && e0 + n_experts <= c->desc.E, TQP_ERR_ARG, "expert range outside [0, E)");
     if (n_experts == 0) return TQP_OK;

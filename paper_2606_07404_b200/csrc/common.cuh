@@ -40,6 +40,9 @@ struct GemmSeg {
     const bf16 *act;        // [N][K] bf16 activations (B operand)
     const uint8_t *idx;     // codes of all experts
     const __half *scale;    // per-output-channel scales of all experts
+    const float *norm;      // scalar (TurboQuant) format: fp32 row norms of all experts, in place of `scale`
+    const void *lut;        // scalar format: the 256 bf16 Lloyd-Max levels of this pack's input space (device)
+    int scalar;             // 1: TurboQuant codes, idx[e][M][K] / idx[e][K][M] one byte per weight; 0: vector-quantised
     int K;                  // contraction length of this segment
     int kmajor;             // 1: idx[e][M][K/8] (forward), 0: idx[e][K][M/8] (backward, transposed use)
     CUtensorMap act_map;    // box {64, kTileRows} over act, SWIZZLE_128B (1-CTA kernel)
@@ -75,6 +78,17 @@ struct TqRot {
     double *Rt;        // fp64 R^T
 };
 
+// TurboQuant-format layer state (tqp_bind_weights_tq): library-owned device buffers for the rotated activations / adapters
+struct TqLayer {
+    bool on = false;
+    tqp_tq_weights w;
+    bf16 *Xr = nullptr;                                    // [T_max][d] rotated X; reused for the rotated dX before it is turned back
+    bf16 *Ar_gate = nullptr, *Ar_up = nullptr, *Ar_down = nullptr;   // R A: the adapters' input side in the rotated space
+    bf16 *tmp_a = nullptr, *tmp_b = nullptr;               // [E][r][max(d,F)] transposition scratch
+    float *dAr_gate = nullptr, *dAr_up = nullptr, *dAr_down = nullptr, *tmp_f = nullptr;   // gradients w.r.t. R A, fp32
+    bf16 *lut_d = nullptr, *lut_F = nullptr;               // the 256 Lloyd-Max levels of either space as bf16
+};
+
 struct Workspace {
     // sizes
     size_t total = 0;
@@ -101,6 +115,7 @@ struct tqp_ctx {
     const void *zd_src = nullptr;
     int device = 0;                 // the device the ctx was created on (kernel attributes are per device)
     std::vector<tqp::TqRot> tq_rots;             // library-owned; freed by tqp_destroy
+    tqp::TqLayer tq;                             // TurboQuant-format weights bound (tqp_bind_weights_tq)
     std::vector<const void *> smem_attr_done;   // kernels whose dynamic shared-memory limit has been raised on `device`
     int launches = 0;
     int num_sms = 148;
@@ -217,6 +232,7 @@ inline tqp_status ensure_dyn_smem(tqp_ctx *c, const void *func, int bytes) {
 tqp_status tq_check_space(tqp_ctx *c, const tqp_tq_space *sp);
 tqp_status launch_tq_rotate(tqp_ctx *c, const tqp_tq_space *sp, const void *X, bool in_f32, long long rows, void *Y, bool out_f32, int inverse,
                             cudaStream_t st);
+tqp_status launch_tq_make_lut(tqp_ctx *c, const double *levels, bf16 *lut, cudaStream_t st);
 template <typename T>
 tqp_status launch_tq_transpose(tqp_ctx *c, const T *in, T *out, int E, int a, int b, cudaStream_t st);   // [E][a][b] -> [E][b][a]
 

@@ -29,13 +29,25 @@ using namespace ptx;
 
 constexpr int BM = 128, BK = 64, TN = kTileRows, HN = kTileRows / 2;
 constexpr int AK = 128;                                   // K of one A stage (one index tile, one producer hand-shake) = two B stages
-constexpr int NSTAGE = 6, NASLOT = 3, IDXQ = 8;           // B (activation) ring, A (weight) slots of 64 TMEM columns, index ring
-constexpr int X_BYTES = HN * 128, IDX_TILE = 128 * 16, SCL_BYTES = 128 * 2, LUT_BYTES = 256 * 8 * 16;
-constexpr int IDX_BYTES = IDX_TILE + SCL_BYTES;          // an index ring entry: the code tile + the 128 fp16 scales of its A stage
-constexpr int OFF_X = 0, OFF_LUT = OFF_X + NSTAGE * X_BYTES, OFF_IDX = OFF_LUT + LUT_BYTES,
-              OFF_BAR = OFF_IDX + IDXQ * IDX_BYTES, OFF_EPI = OFF_BAR + 512;
+constexpr int NASLOT = 3;                                 // A (weight) slots of 64 TMEM columns
+constexpr int X_BYTES = HN * 128;
 constexpr int EPI_ROWS = 32, EPI_BYTES = TN * BM * 2;      // staging: the whole [256 rows][128 channels] bf16 output tile
-constexpr int SMEM_BYTES = OFF_EPI + EPI_BYTES + 1024;
+// Shared-memory plan.  SC = false: the vector-quantised format of BASELINE.json (one uint8 code per 8 weights, shared 256 x 8
+// codebook, fp16 channel scales).  SC = true: the TurboQuant-MSE format of PAPER.md L944-946 (one uint8 code per rotated
+// coordinate, a 256-entry scalar Lloyd-Max table, fp32 row norms): an A stage then needs a 128 x 128-byte code tile instead
+// of 128 x 16, so the index ring is 3 deep instead of 8 and the activation ring 4 instead of 6.
+template <bool SC>
+struct Cfg {
+    static constexpr int NSTAGE = SC ? 4 : 6;                 // B (activation) ring
+    static constexpr int IDXQ = SC ? 3 : 8;                   // index ring
+    static constexpr int IDX_TILE = SC ? 128 * 128 : 128 * 16;
+    static constexpr int SCL_BYTES = SC ? 128 * 4 : 128 * 2;  // the stage's 128 fp32 norms / fp16 scales ride with the code tile
+    static constexpr int IDX_BYTES = SC ? IDX_TILE + 1024 : IDX_TILE + SCL_BYTES;   // SC: 128-byte-swizzled TMA tiles need 1024-byte alignment
+    static constexpr int LUT_BYTES = 256 * 8 * 16;            // VQ: 8 replicas of the 16-byte entries; SC: 32 lane-private copies of 4-byte entries
+    static constexpr int OFF_X = 0, OFF_LUT = OFF_X + NSTAGE * X_BYTES, OFF_IDX = OFF_LUT + LUT_BYTES,
+                         OFF_BAR = OFF_IDX + IDXQ * IDX_BYTES, OFF_EPI = OFF_BAR + 512;
+    static constexpr int SMEM_BYTES = OFF_EPI + EPI_BYTES + 1024;
+};
 constexpr int NTHREADS = 480;
 constexpr int W_DEQ0 = 3, W_EPI0 = 11;
 constexpr int TM_ACC = 0, TM_A = TN;                      // TMEM columns: accumulator [0, 256), A slots [256, 256 + 64 NASLOT)
@@ -76,10 +88,14 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t *v) {
 }
 
 
+template <bool SC>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
 gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__restrict__ lut_g, const Tile *__restrict__ tiles,
                         const int32_t *__restrict__ num_tiles_p, int32_t *__restrict__ sched_counter, int ablate,
                         long long *__restrict__ trace) {
+    using C = Cfg<SC>;
+    constexpr int NSTAGE = C::NSTAGE, IDXQ = C::IDXQ, IDX_TILE = C::IDX_TILE, SCL_BYTES = C::SCL_BYTES, IDX_BYTES = C::IDX_BYTES;
+    constexpr int OFF_X = C::OFF_X, OFF_LUT = C::OFF_LUT, OFF_IDX = C::OFF_IDX, OFF_BAR = C::OFF_BAR, OFF_EPI = C::OFF_EPI;
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     const uint32_t sbase = smem_u32(smem);
@@ -114,9 +130,13 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
         mbar_init_fence();
     }
     if (warp == 1) tmem_alloc<2>(smem_u32(tmem_slot), 512);
-    {   // replicated LUT: entry e, copy c at (e*8 + c) * 16 B  ->  lane c of every quarter-warp hits bank group c
+    if (!SC) {   // replicated LUT: entry e, copy c at (e*8 + c) * 16 B  ->  lane c of every quarter-warp hits bank group c
         uint4 *lut_s = reinterpret_cast<uint4 *>(smem + OFF_LUT);
         for (int i = threadIdx.x; i < 256 * 8; i += NTHREADS) lut_s[i] = lut_g[i >> 3];
+    } else {     // scalar table: level e (bf16, low half of a word), one copy per lane at (e * 32 + lane) * 4 B: bank = lane, never a conflict
+        uint32_t *lut_s = reinterpret_cast<uint32_t *>(smem + OFF_LUT);
+        const uint16_t *lv = reinterpret_cast<const uint16_t *>(lut_g);
+        for (int i = threadIdx.x; i < 256 * 32; i += NTHREADS) lut_s[i] = lv[i >> 5];
     }
     tc_fence_before();
     __syncthreads();
@@ -217,13 +237,15 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                     const int nka = S.K / AK;
                     for (int ka = 0; ka < nka; ++ka) {   // K-major: [128 channels][16 codes]; MN-major: [128 k][16 channel groups]
                         mbar_wait(idx_empty(iq.s), iq.ph ^ 1);
-                        mbar_expect_tx(idx_full(iq.s), IDX_BYTES);
-                        const int c0 = S.kmajor ? ka * 16 : it.m0 / 8;
+                        mbar_expect_tx(idx_full(iq.s), IDX_TILE + SCL_BYTES);
+                        // VQ: a code covers 8 weights along the pack's input dim; SC: one code per weight
+                        const int c0 = S.kmajor ? ka * (SC ? AK : AK / 8) : (SC ? it.m0 : it.m0 / 8);
                         const int c1 = S.kmajor ? it.t.expert * pb.M + it.m0 : it.t.expert * S.K + ka * AK;
                         tma_load_2d(sbase + OFF_IDX + iq.s * IDX_BYTES, &S.idx_map, c0, c1, idx_full(iq.s));
                         // the stage's scales ride along (K-major: of this CTA's 128 channels; MN-major: of the stage's 128 k), so
                         // that no producer waits on a global load when an item starts
-                        bulk_g2s(sbase + OFF_IDX + iq.s * IDX_BYTES + IDX_TILE, S.scale + c1, SCL_BYTES, idx_full(iq.s));
+                        if (SC) bulk_g2s(sbase + OFF_IDX + iq.s * IDX_BYTES + IDX_TILE, S.norm + c1, SCL_BYTES, idx_full(iq.s));
+                        else bulk_g2s(sbase + OFF_IDX + iq.s * IDX_BYTES + IDX_TILE, S.scale + c1, SCL_BYTES, idx_full(iq.s));
                         iq.next(IDXQ);
                     }
                 }
@@ -388,7 +410,105 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
             for (int sg = 0; sg < pb.nseg; ++sg) {
                 const GemmSeg &S = pb.seg[sg];
                 const int nka = S.K / AK;
-                if (S.kmajor) {
+                if (SC && S.kmajor) {
+                    // ---- TurboQuant forward: one code per coordinate.  This thread owns channel `row` (its TMEM lane) and
+                    // looks its 128 codes of the stage up one by one in its lane-private copy of the scalar table; the tile
+                    // row is 128 bytes, its 16-byte chunks XOR-swizzled by row (TMA SWIZZLE_128B), so the LDS.128 of the 32
+                    // lanes spread over all banks.  W'[m][k] = bf16( bf16(level[code]) * bf16(norm[m]) ).
+                    const uint32_t lut_l = sbase + OFF_LUT + lane * 4;
+                    for (int ka = 0; ka < nka; ++ka) {
+                        const bool own = (ja & 1) == g;
+                        if (own) {
+                            mbar_wait(idx_full(iq.s), iq.ph);
+                            const uint32_t tb = sbase + OFF_IDX + iq.s * IDX_BYTES;
+                            const __nv_bfloat162 s2 = __float2bfloat162_rn(__uint_as_float(lds32(tb + IDX_TILE + row * 4)));
+#pragma unroll
+                            for (int h = 0; h < 2; ++h) {
+                                uint32_t a[32];   // 64 bf16 of this channel's row = 32 TMEM columns
+#pragma unroll
+                                for (int j = 0; j < 4; ++j) {
+                                    const uint4 cq = lds128(tb + row * 128 + (((4 * h + j) ^ (row & 7)) << 4));
+                                    const uint32_t cw4[4] = {cq.x, cq.y, cq.z, cq.w};
+#pragma unroll
+                                    for (int w = 0; w < 4; ++w) {
+                                        uint32_t lv[4];
+#pragma unroll
+                                        for (int b = 0; b < 4; ++b) lv[b] = lds32(lut_l + (__byte_perm(cw4[w], 0, 0x4440 | b) << 7));
+#pragma unroll
+                                        for (int pr = 0; pr < 2; ++pr) {
+                                            uint32_t pk = __byte_perm(lv[2 * pr], lv[2 * pr + 1], 0x5410);
+                                            __nv_bfloat162 w2 = __hmul2(*reinterpret_cast<__nv_bfloat162 *>(&pk), s2);
+                                            a[8 * j + 2 * w + pr] = *reinterpret_cast<uint32_t *>(&w2);
+                                        }
+                                    }
+                                }
+                                if (h == 1) {   // all codes of the stage are in registers: hand the ring entry back
+                                    __syncwarp();
+                                    if (lane == 0) mbar_arrive(idx_empty(iq.s));
+                                }
+                                if (h == 0) wait_slot_free();
+                                tmem_st32(a_lane + sa.s * 64 + h * 32, a);
+                            }
+                            publish();
+                        }
+                        iq.next(IDXQ);
+                        sa.next(NASLOT);
+                        ++ja;
+                    }
+                } else if (SC) {
+                    // ---- TurboQuant backward: the contraction runs across the code rows (k = the pack's output channel, whose
+                    // norm scales the row); thread (rk, jj) of quadrant q fetches, for each of its 16 k, the code PAIRS of
+                    // channels 32 q + 8 cg + 2 jj (+1), cg = 0..3, looks both up and hands the bf16 pair to movmatrix exactly
+                    // like the vector-quantised path below.  Tile: 128 k rows of 128 bytes, chunks swizzled by k.
+                    const uint32_t lut_l = sbase + OFF_LUT + lane * 4;
+                    const int q4 = warp & 3;
+                    __nv_bfloat162 sc[16];
+                    for (int ka = 0; ka < nka; ++ka) {
+                        const bool own = (ja & 1) == g;
+                        if (own) {
+                            mbar_wait(idx_full(iq.s), iq.ph);
+                            const uint32_t tb = sbase + OFF_IDX + iq.s * IDX_BYTES;
+#pragma unroll
+                            for (int z = 0; z < 16; ++z) {
+                                const int kz = (z >> 3) * 64 + ((z >> 1) & 3) * 16 + (z & 1) * 2;
+                                sc[z] = __float2bfloat162_rn(__uint_as_float(lds32(tb + IDX_TILE + (kz + kofs) * 4)));
+                            }
+#pragma unroll
+                            for (int h = 0; h < 2; ++h) {
+#pragma unroll
+                                for (int hs = 0; hs < 2; ++hs) {
+                                    uint32_t rg[16];
+#pragma unroll
+                                    for (int x = 0; x < 4; ++x)
+#pragma unroll
+                                        for (int i = 0; i < 2; ++i)
+#pragma unroll
+                                            for (int mbi = 0; mbi < 2; ++mbi) {
+                                                const int z = 8 * h + 2 * x + i, cg = 2 * hs + mbi;
+                                                const int k = (z >> 3) * 64 + ((z >> 1) & 3) * 16 + (z & 1) * 2 + kofs;
+                                                // byte column m = 32 q + 8 cg + 2 jj: chunk 2 q + cg / 2, offset 8 (cg % 2) + 2 jj
+                                                const uint32_t cp = lds16(tb + k * 128 + (((2 * q4 + (cg >> 1)) ^ (k & 7)) << 4) + 8 * (cg & 1) + 2 * jj);
+                                                const uint32_t l0 = lds32(lut_l + ((cp & 0xffu) << 7));
+                                                const uint32_t l1 = lds32(lut_l + ((cp >> 8) << 7));
+                                                uint32_t pk = __byte_perm(l0, l1, 0x5410);
+                                                __nv_bfloat162 w2 = __hmul2(*reinterpret_cast<__nv_bfloat162 *>(&pk), sc[z]);
+                                                rg[4 * x + 2 * mbi + i] = movmatrix_t(*reinterpret_cast<uint32_t *>(&w2));
+                                            }
+                                    if (h == 1 && hs == 1) {
+                                        __syncwarp();
+                                        if (lane == 0) mbar_arrive(idx_empty(iq.s));
+                                    }
+                                    if (h == 0 && hs == 0) wait_slot_free();
+                                    tmem_st_16x256b_x4(a_lane + ((uint32_t)(16 * hs) << 16) + sa.s * 64 + h * 32, rg);
+                                }
+                            }
+                            publish();
+                        }
+                        iq.next(IDXQ);
+                        sa.next(NASLOT);
+                        ++ja;
+                    }
+                } else if (S.kmajor) {
                     // ---- forward: codes run along k; this thread owns TMEM lane `row` and writes its 128 k-values itself
                     for (int ka = 0; ka < nka; ++ka) {
                         const bool own = (ja & 1) == g;
@@ -557,21 +677,32 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
 }  // namespace gt2
 
 tqp_status launch_gemm_tcgen05_ts2(tqp_ctx *c, const GemmProblem *probs, int nprob, cudaStream_t st) {
+    const bool sc = probs[0].seg[0].scalar != 0;   // TurboQuant codes (one launch never mixes the two formats)
     for (int i = 0; i < nprob; ++i) {   // an even number of 128-channel tiles and whole 128-wide A stages per segment
         const GemmProblem &p = probs[i];
         bool ok = p.M % (2 * gt2::BM) == 0 && p.nlora <= 2;
-        for (int sg = 0; sg < p.nseg; ++sg) ok = ok && p.seg[sg].K % gt2::AK == 0;
-        if (!ok) return launch_gemm_tcgen05_2cta(c, probs, nprob, st);
+        for (int sg = 0; sg < p.nseg; ++sg) ok = ok && p.seg[sg].K % gt2::AK == 0 && (p.seg[sg].scalar != 0) == sc;
+        if (!ok) {
+            if (sc) { c->err = "TurboQuant-format GEMM needs M % 256 == 0 and K % 128 == 0"; return TQP_ERR_SHAPE; }
+            return launch_gemm_tcgen05_2cta(c, probs, nprob, st);
+        }
     }
-    if (tqp_status st_attr = ensure_dyn_smem(c, reinterpret_cast<const void *>(&gt2::gemm_tcgen05_ts2_kernel), gt2::SMEM_BYTES)) return st_attr;
     GemmArgs args;
     for (int i = 0; i < nprob; ++i) args.p[i] = probs[i];
     args.nprob = nprob;
     const int grid = (c->num_sms / 2) * 2;
-    const bool tr = c->trace > 0 && ++c->trace_seq == c->trace;   // debug timeline of cluster 0 (tqp_set_option "trace")
-    gt2::gemm_tcgen05_ts2_kernel<<<grid, gt2::NTHREADS, gt2::SMEM_BYTES, st>>>(
-        args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), c->p<int32_t>(c->ws.sched) + 4,
-        c->ablate, tr ? c->p<long long>(c->ws.trace) : nullptr);
+    const bool tr = c->trace > 0 && ++c->trace_seq == c->trace;   // debug timeline of cluster 0 (-DTQP_TRACE builds)
+    int32_t *counter = c->p<int32_t>(c->ws.sched) + 4;
+    long long *trace = tr ? c->p<long long>(c->ws.trace) : nullptr;
+    if (sc) {
+        if (tqp_status st_attr = ensure_dyn_smem(c, reinterpret_cast<const void *>(&gt2::gemm_tcgen05_ts2_kernel<true>), gt2::Cfg<true>::SMEM_BYTES)) return st_attr;
+        gt2::gemm_tcgen05_ts2_kernel<true><<<grid, gt2::NTHREADS, gt2::Cfg<true>::SMEM_BYTES, st>>>(
+            args, reinterpret_cast<const uint4 *>(probs[0].seg[0].lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), counter, c->ablate, trace);
+    } else {
+        if (tqp_status st_attr = ensure_dyn_smem(c, reinterpret_cast<const void *>(&gt2::gemm_tcgen05_ts2_kernel<false>), gt2::Cfg<false>::SMEM_BYTES)) return st_attr;
+        gt2::gemm_tcgen05_ts2_kernel<false><<<grid, gt2::NTHREADS, gt2::Cfg<false>::SMEM_BYTES, st>>>(
+            args, c->p<uint4>(c->ws.lut), c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), counter, c->ablate, trace);
+    }
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }

@@ -632,6 +632,15 @@ tqp_status launch_tq_rotate(tqp_ctx *c, const tqp_tq_space *sp, const void *X, b
     return TQP_OK;
 }
 
+__global__ void tq_make_lut_kernel(const double *__restrict__ levels, bf16 *__restrict__ lut) {
+    lut[threadIdx.x] = __float2bfloat16_rn((float)levels[threadIdx.x]);
+}
+tqp_status launch_tq_make_lut(tqp_ctx *c, const double *levels, bf16 *lut, cudaStream_t st) {
+    tq_make_lut_kernel<<<1, 256, 0, st>>>(levels, lut);
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
+
 template <typename T>
 tqp_status launch_tq_transpose(tqp_ctx *c, const T *in, T *out, int E, int a, int b, cudaStream_t st) {
     dim3 grid((unsigned)(((size_t)a * b + 255) / 256), E);
