@@ -179,6 +179,39 @@ def run_reference(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+def bind_tq_synthetic(tq, torch, layer, cfg, inp, up, dev):
+    """--format tq: a TurboQuant base of the same shape.  Input recipe: rotation = signed
+    Hadamard with seeded signs for power-of-two widths, else the library's sign-fixed QR of a seeded Gaussian draw; levels
+    = the library's Lloyd-Max solver; codes drawn i.i.d. from the coordinate law (a N(0, 1/n) draw put into its Lloyd-Max
+    cell -- what encoding Gaussian weight rows gives, without holding fp32 weights of 100B-scale packs); norms =
+    0.02 sqrt(n) U(0.5, 1.5); adapters as in the vector-quantised recipe."""
+    rng = np.random.default_rng(20_000 + cfg.seed)
+    gen = torch.Generator(device=dev); gen.manual_seed(30_000 + cfg.seed)
+    spaces = {}
+    for n in {cfg.d, cfg.F}:
+        lv = tq.tq_levels(n, 8)
+        lvd = torch.from_numpy(lv).to(dev)
+        if n & (n - 1) == 0:
+            signs = torch.from_numpy((rng.integers(0, 2, n) * 2 - 1).astype(np.int8)).to(dev)
+            spaces[n] = tq.TqSpace(n, lvd, signs=signs)
+        else:
+            R = tq.tq_rotation_qr(rng.standard_normal((n, n)))
+            spaces[n] = tq.TqSpace(n, lvd, R=torch.from_numpy(R).to(dev))
+        spaces[n].bounds = torch.from_numpy((0.5 * (lv[:-1] + lv[1:])).astype(np.float32)).to(dev)
+    w = {}
+    for pack, (out_dim, n) in dict(gate=(cfg.F, cfg.d), up=(cfg.F, cfg.d), down=(cfg.d, cfg.F)).items():
+        codes = torch.empty((cfg.E, out_dim, n), dtype=torch.uint8, device=dev)
+        for e0 in range(0, cfg.E, 16):
+            y = torch.randn((min(16, cfg.E - e0), out_dim, n), generator=gen, device=dev) * (1.0 / np.sqrt(n))
+            codes[e0:e0 + y.shape[0]] = torch.bucketize(y, spaces[n].bounds).to(torch.uint8)
+        w[f"codes_{pack}"] = codes
+        w[f"norm_{pack}"] = (torch.rand((cfg.E, out_dim), generator=gen, device=dev) + 0.5) * (0.02 * np.sqrt(n))
+    for key in ("A_gate", "A_up", "B_gate", "B_up", "A_down", "B_down"):
+        w[key] = up(inp[key])
+    layer.bind_weights_tq(spaces[cfg.d], spaces[cfg.F], **w)
+    return w, spaces
+
+
 def run_ours(args, cfg):
     import torch
     import paper_2606_07404_b200 as tq
@@ -206,7 +239,10 @@ def run_ours(args, cfg):
 
     wnames = ("idx_gate", "idx_up", "idx_down", "scale_gate", "scale_up", "scale_down", "codebook",
               "A_gate", "A_up", "B_gate", "B_up", "A_down", "B_down")
-    layer.bind_weights(**{n: up(inp[n]) for n in wnames})
+    if args.format == "tq":
+        tq_keep = bind_tq_synthetic(tq, torch, layer, cfg, inp, up, dev)   # noqa: F841  (keeps the device tensors alive)
+    else:
+        layer.bind_weights(**{n: up(inp[n]) for n in wnames})
     X, dY, W_r = up(inp["X"]), up(inp["dY"]), up(inp["W_r"])
     bias = up(inp["logit_bias"]) if inp["logit_bias"] is not None else None
     N = T * k
@@ -314,15 +350,17 @@ def run_ours(args, cfg):
     gemm_ms_step = gemm_ms / args.steps
     gemm_tflops = fl["gemm"] / (gemm_ms_step / 1e3) / 1e12 if gemm_ms_step > 0 else 0.0
     nl = 4 if cfg.backward else 2
-    traffic = NCU_GEMM_TRAFFIC.get(cfg.name, (None, None))
+    traffic = NCU_GEMM_TRAFFIC.get(cfg.name, (None, None)) if args.format == "vq" else (None, None)
     line = {
         "metric": METRIC, "value": value, "unit": "tokens/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
         "data": "synthetic",
-        "config": {"workload": cfg.name, "T": T, "d": cfg.d, "F": cfg.F, "E": cfg.E, "k": cfg.k, "r": cfg.r,
+        "config": {"workload": cfg.name + ("_tq" if args.format == "tq" else ""), "T": T, "d": cfg.d, "F": cfg.F, "E": cfg.E, "k": cfg.k, "r": cfg.r,
                    "passes": ("fwd+bwd" if cfg.backward else "fwd") + ("+router_grad" if cfg.router_grad else ""), "routing": "zipf1.1" if cfg.skew else "near-uniform",
                    "l2": f"inputs larger than L2 ({3 * cfg.E * cfg.d * cfg.F / 8 / 1e6:.0f} MB code indices + "
                          f"{T * cfg.k * cfg.d * 2 / 1e6:.0f} MB permuted rows per step), no flush",
+                   "base_format": "TurboQuant-MSE 8-bit scalar codes + row norms, rotated space (PAPER.md L944-948)" if args.format == "tq"
+                   else "vector-quantised, 8-vectors / 256-entry codebook / fp16 channel scales (BASELINE.json)",
                    "gemm_impl": GEMM_IMPL_NAMES.get(args.gemm_impl, str(args.gemm_impl)), "parallelism": f"replicas x{world}, no collective"},
         "tflops": world * fl["total"] / (ms_per_step / 1e3) / 1e12,
         "frac_of_bf16_peak": {"measured_burst": fl["total"] / (ms_per_step / 1e3) / 1e12 / pk["tensor_burst"],
@@ -360,6 +398,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (2 = 120B shape, fwd+bwd)")
     ap.add_argument("--gemm-impl", type=int, default=0)
+    ap.add_argument("--format", default="vq", choices=["vq", "tq"], help="frozen-base format: BASELINE.json's VQ (default) or TurboQuant-MSE")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-tokens", type=int, default=0, help="tokens of the cpu_baseline oracle pass (0: the whole batch, at most 8192)")

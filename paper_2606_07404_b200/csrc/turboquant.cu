@@ -185,26 +185,150 @@ __device__ __forceinline__ void fwht_smem(REAL *v, int n, int tid, int nthr) {
     __syncthreads();
 }
 
+// Activation kernel: radix-8 passes.  A row is handled by n / 8 threads; each thread takes its 16-byte chunk of the row
+// straight from global memory into registers, does three butterfly stages there, and the later passes (strides 8, 64, 512)
+// go registers <-> shared memory with one barrier per pass (4 barriers at n = 1024 instead of 10, two shared-memory
+// accesses per element and pass instead of per stage).  Shared rows are padded by one word per 32 (index i -> i + i / 32) so
+// that the stride-8 accesses of a pass spread over the banks.  A CTA holds max(1, 1024 / n) rows.  Bound: HBM.
+__device__ __forceinline__ int fw_pad(int i) { return i + (i >> 5); }
+
+template <typename T>
+__device__ __forceinline__ void fw_load8(const T *p, float (&v)[8]);
+template <>
+__device__ __forceinline__ void fw_load8<bf16>(const bf16 *p, float (&v)[8]) {
+    const uint4 q = *reinterpret_cast<const uint4 *>(p);
+    const uint32_t w[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { const float2 f = bf16x2_to_float2(w[j]); v[2 * j] = f.x; v[2 * j + 1] = f.y; }
+}
+template <>
+__device__ __forceinline__ void fw_load8<float>(const float *p, float (&v)[8]) {
+    const float4 a = *reinterpret_cast<const float4 *>(p), b = *reinterpret_cast<const float4 *>(p + 4);
+    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+}
+template <typename T>
+__device__ __forceinline__ void fw_store8(T *p, const float (&v)[8]);
+template <>
+__device__ __forceinline__ void fw_store8<bf16>(bf16 *p, const float (&v)[8]) {
+    uint4 q;
+    q.x = float2_to_bf16x2(v[0], v[1]); q.y = float2_to_bf16x2(v[2], v[3]); q.z = float2_to_bf16x2(v[4], v[5]); q.w = float2_to_bf16x2(v[6], v[7]);
+    *reinterpret_cast<uint4 *>(p) = q;
+}
+template <>
+__device__ __forceinline__ void fw_store8<float>(float *p, const float (&v)[8]) {
+    *reinterpret_cast<float4 *>(p) = make_float4(v[0], v[1], v[2], v[3]);
+    *reinterpret_cast<float4 *>(p + 4) = make_float4(v[4], v[5], v[6], v[7]);
+}
+// butterflies over the low `nb` bits of the register index
+__device__ __forceinline__ void fw_bfly8(float (&v)[8], int nb) {
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        if (b < nb) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+                if (!(k & (1 << b))) { const float x = v[k], y = v[k | (1 << b)]; v[k] = x + y; v[k | (1 << b)] = x - y; }
+        }
+    }
+}
+
 template <typename TIN, typename TOUT>
-__global__ void __launch_bounds__(256) tq_fwht_rows_kernel(const TIN *__restrict__ X, TOUT *__restrict__ Y, long long rows, int n,
-                                                            const int8_t *__restrict__ signs, int inverse) {
+__global__ void __launch_bounds__(1024) tq_fwht_rows_kernel(const TIN *__restrict__ X, TOUT *__restrict__ Y, long long rows, int n, int logn,
+                                                             const int8_t *__restrict__ signs, int inverse) {
     extern __shared__ float fw_s[];
+    const int tpr = n / 8, rpc = blockDim.x / tpr;             // threads per row, rows per CTA
+    const int lr = threadIdx.x / tpr, t = threadIdx.x % tpr, lane = threadIdx.x % 32;
+    float *sm = fw_s + lr * fw_pad(n);
     const float rs = rsqrtf((float)n);
-    for (long long row = blockIdx.x; row < rows; row += gridDim.x) {
-        const TIN *x = X + row * n;
-        for (int i = threadIdx.x; i < n; i += blockDim.x) {
-            float v = (float)x[i];
-            if (!inverse) v *= (float)signs[i];
-            fw_s[i] = v;
+    float sg[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) sg[k] = (float)signs[8 * t + k];
+    // bits 3 .. 7 of the element index are lane bits (a row's threads are consecutive lanes): butterflies by shuffle
+    const int nsh = min(logn, 8) - 3;
+    float fl[5];
+#pragma unroll
+    for (int b = 0; b < 5; ++b) fl[b] = (lane >> b) & 1 ? -1.f : 1.f;
+    // shared-memory passes for bits 8 and up (n > 256): element slots of this thread per pass, fixed for the whole kernel
+    int idx[2][8];
+#pragma unroll
+    for (int p = 0; p < 2; ++p) {
+        const int ls = 8 + 3 * p, nb = max(0, min(3, logn - ls)), s = 1 << ls;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int kb = k & ((1 << nb) - 1), rem = t * (8 >> nb) + (k >> nb);
+            idx[p][k] = fw_pad(((rem >> ls) << (ls + nb)) | (kb << ls) | (rem & (s - 1)));
         }
-        fwht_smem(fw_s, n, threadIdx.x, blockDim.x);
-        TOUT *y = Y + row * n;
-        for (int i = threadIdx.x; i < n; i += blockDim.x) {
-            float v = fw_s[i] * rs;
-            if (inverse) v *= (float)signs[i];
-            y[i] = (TOUT)v;
+    }
+    for (long long row0 = (long long)blockIdx.x * rpc; row0 < rows; row0 += (long long)gridDim.x * rpc) {
+        const long long row = row0 + lr;
+        const bool act = row < rows;
+        float v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[k] = 0.f;
+        if (act) {
+            fw_load8<TIN>(X + row * n + 8 * t, v);
+            if (!inverse) {
+#pragma unroll
+                for (int k = 0; k < 8; ++k) v[k] *= sg[k];
+            }
         }
+        fw_bfly8(v, 3);                                          // bits 0..2
+#pragma unroll
+        for (int b = 0; b < 5; ++b) {                            // bits 3..7: v = partner + (upper lane ? -v : v)
+            if (b < nsh) {
+#pragma unroll
+                for (int k = 0; k < 8; ++k) v[k] = fmaf(v[k], fl[b], __shfl_xor_sync(0xffffffffu, v[k], 1 << b));
+            }
+        }
+        if (logn > 8) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) sm[fw_pad(8 * t + k)] = v[k];
+#pragma unroll
+            for (int p = 0; p < 2; ++p) {
+                const int ls = 8 + 3 * p;
+                if (ls < logn) {
+                    __syncthreads();
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) v[k] = sm[idx[p][k]];
+                    fw_bfly8(v, min(3, logn - ls));
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) sm[idx[p][k]] = v[k];
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] = sm[fw_pad(8 * t + k)];
+            __syncthreads();
+        }
+        if (act) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                v[k] *= rs;
+                if (inverse) v[k] *= sg[k];
+            }
+            fw_store8<TOUT>(Y + row * n + 8 * t, v);
+        }
+    }
+}
+
+// Adapter tensors between [E][L][r] (dir 0 in) and [E][r][L] (dir 1 in), r <= 32 the adapter rank, L the layer width: a CTA takes
+// 256 positions of L, reads its 256 r elements as one contiguous run and writes r runs of 256 (or the reverse).
+template <typename T>
+__global__ void __launch_bounds__(256) tq_transpose_kernel(const T *__restrict__ in, T *__restrict__ out, int L, int r, int dir) {
+    __shared__ T tile[32][257];
+    const size_t e = blockIdx.y;
+    const int l0 = blockIdx.x * 256, nl = min(256, L - l0);
+    const T *src = in + e * (size_t)L * r;
+    T *dst = out + e * (size_t)L * r;
+    if (dir == 0) {
+        for (int v = threadIdx.x; v < nl * r; v += 256) tile[v % r][v / r] = src[(size_t)l0 * r + v];
         __syncthreads();
+        for (int q = 0; q < r; ++q)
+            for (int l = threadIdx.x; l < nl; l += 256) dst[(size_t)q * L + l0 + l] = tile[q][l];
+    } else {
+        for (int q = 0; q < r; ++q)
+            for (int l = threadIdx.x; l < nl; l += 256) tile[q][l] = src[(size_t)q * L + l0 + l];
+        __syncthreads();
+        for (int v = threadIdx.x; v < nl * r; v += 256) dst[(size_t)l0 * r + v] = tile[v % r][v / r];
     }
 }
 
@@ -532,16 +656,6 @@ __global__ void tq_flush_telemetry_kernel(const double *__restrict__ tele, int o
     out[2 * e + 1] = (float)(nb + na > 0.0 ? nb / (nb + na) : 1.0);
 }
 
-// [E][a][b] -> [E][b][a]
-template <typename T>
-__global__ void tq_transpose_kernel(const T *__restrict__ in, T *__restrict__ out, int a, int b) {
-    const size_t e = blockIdx.y;
-    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= (size_t)a * b) return;
-    const int i = (int)(idx / b), j = (int)(idx % b);
-    out[e * a * b + (size_t)j * a + i] = in[e * a * b + idx];
-}
-
 }  // namespace tqp
 
 // ======================================================================================================================
@@ -600,13 +714,16 @@ tqp_status launch_tq_rotate(tqp_ctx *c, const tqp_tq_space *sp, const void *X, b
     if (rows <= 0) return TQP_OK;
     const int n = sp->n;
     if (sp->hadamard) {
-        const int grid = (int)std::min<long long>(rows, (long long)c->num_sms * 8);
-        const int thr = n >= 512 ? 256 : 128;
-        const size_t sm = (size_t)n * 4;
-        if (in_f32 && out_f32) tq_fwht_rows_kernel<float, float><<<grid, thr, sm, st>>>((const float *)X, (float *)Y, rows, n, sp->signs, inverse);
-        else if (in_f32) tq_fwht_rows_kernel<float, bf16><<<grid, thr, sm, st>>>((const float *)X, (bf16 *)Y, rows, n, sp->signs, inverse);
-        else if (out_f32) tq_fwht_rows_kernel<bf16, float><<<grid, thr, sm, st>>>((const bf16 *)X, (float *)Y, rows, n, sp->signs, inverse);
-        else tq_fwht_rows_kernel<bf16, bf16><<<grid, thr, sm, st>>>((const bf16 *)X, (bf16 *)Y, rows, n, sp->signs, inverse);
+        const int tpr = n / 8, rpc = std::max(1, 128 / tpr), thr = tpr * rpc;   // >= 128 threads per CTA, whole rows
+        int logn = 0;
+        while ((1 << logn) < n) ++logn;
+        const long long ctas = (rows + rpc - 1) / rpc;
+        const int grid = (int)std::min<long long>(ctas, (long long)c->num_sms * std::max(1, 2048 / thr));
+        const size_t sm = (size_t)rpc * (n + n / 32) * 4;
+        if (in_f32 && out_f32) tq_fwht_rows_kernel<float, float><<<grid, thr, sm, st>>>((const float *)X, (float *)Y, rows, n, logn, sp->signs, inverse);
+        else if (in_f32) tq_fwht_rows_kernel<float, bf16><<<grid, thr, sm, st>>>((const float *)X, (bf16 *)Y, rows, n, logn, sp->signs, inverse);
+        else if (out_f32) tq_fwht_rows_kernel<bf16, float><<<grid, thr, sm, st>>>((const bf16 *)X, (float *)Y, rows, n, logn, sp->signs, inverse);
+        else tq_fwht_rows_kernel<bf16, bf16><<<grid, thr, sm, st>>>((const bf16 *)X, (bf16 *)Y, rows, n, logn, sp->signs, inverse);
         TQP_LAUNCH_OK(c);
         return TQP_OK;
     }
@@ -643,8 +760,11 @@ tqp_status launch_tq_make_lut(tqp_ctx *c, const double *levels, bf16 *lut, cudaS
 
 template <typename T>
 tqp_status launch_tq_transpose(tqp_ctx *c, const T *in, T *out, int E, int a, int b, cudaStream_t st) {
-    dim3 grid((unsigned)(((size_t)a * b + 255) / 256), E);
-    tq_transpose_kernel<T><<<grid, 256, 0, st>>>(in, out, a, b);
+    // [E][a][b] -> [E][b][a]; one of a, b is the rank
+    const int dir = b <= 32 ? 0 : 1, L = dir == 0 ? a : b, r = dir == 0 ? b : a;
+    if (r > 32) { c->err = "transpose: neither side is an adapter rank"; return TQP_ERR_ARG; }
+    dim3 grid((L + 255) / 256, E);
+    tq_transpose_kernel<T><<<grid, 256, 0, st>>>(in, out, L, r, dir);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }
