@@ -45,7 +45,8 @@ def flops(cfg, T):
 # roofline.traffic is NOT measured by this run (ncu cannot run inside a timed bench): it is dram__bytes_read.sum +
 # dram__bytes_write.sum per grouped-GEMM launch (average over the launches of one step) copied from the committed
 # `ncu --set full` capture named beside it; None for workloads without a capture.
-NCU_GEMM_TRAFFIC = {"cfg2_120b": (1.069e9, "profiles/r1g_gemm_ncu_cfg2.md")}
+NCU_GEMM_TRAFFIC = {"cfg2_120b": (1.063e9, "profiles/r2_gemm_ncu.md"), "cfg3_120b_skew": (0.970e9, "profiles/r2_gemm_ncu.md"),
+                    "cfg4_120b_mb": (1.925e9, "profiles/r2_gemm_ncu.md")}
 GEMM_IMPL_NAMES = {0: "tcgen05 CTA pairs, weight operand in TMEM (gemm_tcgen05_ts2)", 1: "CUDA-core scaffold",
                    2: "tcgen05 one CTA per tile, smem weight operand", 3: "tcgen05 CTA pairs, smem weight operand"}
 
