@@ -115,7 +115,7 @@ def write_report(cfg, report, counts, seconds):
             f.write(text)
 
 
-@pytest.mark.parametrize("cfg_id", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("cfg_id", [0, 1, 2, 3, 4, 5])
 def test_full_size_config(cfg_id):
     import time
     cfg = ti.CONFIGS[cfg_id]
