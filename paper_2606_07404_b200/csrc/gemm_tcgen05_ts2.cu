@@ -405,6 +405,20 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
 #pragma unroll
                         for (int q = 0; q < 16; ++q) ch[q] = lo[q] | (hi[q] << 16);
                     }
+                    if (pb.seg[0].kmajor) {
+                        // Forward items keep the channel scale OUT of the mainloop: the accumulator holds sum_k x[k] bf16(cb)[m][k]
+                        // and the epilogue multiplies lane m by the exact fp32 scale (one rounding of the weight instead of
+                        // three).  The adapter K-step shares that accumulator, so its row goes in divided by the scale.
+                        // (A channel whose scale is 0 -- a zero weight row -- has no base term: its producer writes zeros, the
+                        // epilogue multiplies by 1 and the adapter row goes in as it is.)
+                        const float scl = SC ? pb.seg[0].norm[(size_t)e * M + m0 + row] : __half2float(pb.seg[0].scale[(size_t)e * M + m0 + row]);
+                        const float inv = scl != 0.f ? 1.f / scl : 1.f;
+#pragma unroll
+                        for (int q = 0; q < 16; ++q) {
+                            const float2 f = bf16x2_to_float2(ch[q]);
+                            ch[q] = float2_to_bf16x2(f.x * inv, f.y * inv);
+                        }
+                    }
                 }
             }
             for (int sg = 0; sg < pb.nseg; ++sg) {
@@ -414,14 +428,14 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                     // ---- TurboQuant forward: one code per coordinate.  This thread owns channel `row` (its TMEM lane) and
                     // looks its 128 codes of the stage up one by one in its lane-private copy of the scalar table; the tile
                     // row is 128 bytes, its 16-byte chunks XOR-swizzled by row (TMA SWIZZLE_128B), so the LDS.128 of the 32
-                    // lanes spread over all banks.  W'[m][k] = bf16( bf16(level[code]) * bf16(norm[m]) ).
+                    // lanes spread over all banks.  The operand is bf16(level[code]); the row norm multiplies the accumulator lane in the epilogue.
                     const uint32_t lut_l = sbase + OFF_LUT + lane * 4;
                     for (int ka = 0; ka < nka; ++ka) {
                         const bool own = (ja & 1) == g;
                         if (own) {
                             mbar_wait(idx_full(iq.s), iq.ph);
                             const uint32_t tb = sbase + OFF_IDX + iq.s * IDX_BYTES;
-                            const __nv_bfloat162 s2 = __float2bfloat162_rn(__uint_as_float(lds32(tb + IDX_TILE + row * 4)));
+                            const bool zero_row = lds32(tb + IDX_TILE + row * 4) << 1 == 0;   // norm 0: no base term for this channel
 #pragma unroll
                             for (int h = 0; h < 2; ++h) {
                                 uint32_t a[32];   // 64 bf16 of this channel's row = 32 TMEM columns
@@ -435,12 +449,13 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
 #pragma unroll
                                         for (int b = 0; b < 4; ++b) lv[b] = lds32(lut_l + (__byte_perm(cw4[w], 0, 0x4440 | b) << 7));
 #pragma unroll
-                                        for (int pr = 0; pr < 2; ++pr) {
-                                            uint32_t pk = __byte_perm(lv[2 * pr], lv[2 * pr + 1], 0x5410);
-                                            __nv_bfloat162 w2 = __hmul2(*reinterpret_cast<__nv_bfloat162 *>(&pk), s2);
-                                            a[8 * j + 2 * w + pr] = *reinterpret_cast<uint32_t *>(&w2);
-                                        }
+                                        for (int pr = 0; pr < 2; ++pr)   // the row norm is applied by the epilogue (fp32)
+                                            a[8 * j + 2 * w + pr] = __byte_perm(lv[2 * pr], lv[2 * pr + 1], 0x5410);
                                     }
+                                }
+                                if (zero_row) {
+#pragma unroll
+                                    for (int j = 0; j < 32; ++j) a[j] = 0;
                                 }
                                 if (h == 1) {   // all codes of the stage are in registers: hand the ring entry back
                                     __syncwarp();
@@ -523,7 +538,7 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                         }
                         iq.next(IDXQ);
                         if (own) {
-                            const __nv_bfloat162 s2 = __float2bfloat162_rn(__half2float(__ushort_as_half((unsigned short)sraw)));
+                            // the channel scale is applied by the epilogue (fp32, exact); here it only matters whether it is zero
                             const uint32_t cwd[4] = {codes.x, codes.y, codes.z, codes.w};
 #pragma unroll
                             for (int h = 0; h < 2; ++h) {
@@ -531,11 +546,12 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
 #pragma unroll
                                 for (int j = 0; j < 8; ++j) {
                                     const uint32_t code = __byte_perm(cwd[2 * h + (j >> 2)], 0, 0x4440 | (j & 3));   // one PRMT
-                                    uint4 v = lds128(lut_a + code * 128);
-                                    __nv_bfloat162 *pv = reinterpret_cast<__nv_bfloat162 *>(&v);
-#pragma unroll
-                                    for (int q = 0; q < 4; ++q) pv[q] = __hmul2(pv[q], s2);
+                                    const uint4 v = lds128(lut_a + code * 128);
                                     a[4 * j] = v.x; a[4 * j + 1] = v.y; a[4 * j + 2] = v.z; a[4 * j + 3] = v.w;
+                                }
+                                if ((sraw & 0x7fffu) == 0) {   // zero scale: no base term for this channel
+#pragma unroll
+                                    for (int j = 0; j < 32; ++j) a[j] = 0;
                                 }
                                 if (h == 0) wait_slot_free();
                                 tmem_st32(a_lane + sa.s * 64 + h * 32, a);
@@ -627,10 +643,23 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
             const int M = pb.M;
             const uint32_t aph = cnt & 1;
             ++cnt;
-            mbar_wait(tmem_full, aph);
-            tc_fence_after();
             const bool tre = TQP_DBG(trace != nullptr) && cid == 0 && rank == 0 && et == 0 && cnt <= 400;
             if (tre) trace[4000 + (cnt - 1) * 4] = clock64();
+            // forward items: the exact fp32 channel scale (VQ) / row norm (TurboQuant) of this thread's four TMEM lanes
+            float esc[2][2] = {{1.f, 1.f}, {1.f, 1.f}};
+            if (pb.seg[0].kmajor) {
+                const size_t c0 = (size_t)it.t.expert * M + it.m0 + q * 32 + (lane >> 2);
+#pragma unroll
+                for (int hh = 0; hh < 2; ++hh)
+#pragma unroll
+                    for (int u = 0; u < 2; ++u)
+                    {
+                        const float v = SC ? pb.seg[0].norm[c0 + 16 * hh + 8 * u] : __half2float(pb.seg[0].scale[c0 + 16 * hh + 8 * u]);
+                        esc[hh][u] = v != 0.f ? v : 1.f;
+                    }
+            }
+            mbar_wait(tmem_full, aph);
+            tc_fence_after();
             named_bar_sync(1, 128);   // every epilogue warp has finished storing the previous item out of the staging tile
             const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + TM_ACC;
             for (int c0 = 0; c0 < it.t.rows; c0 += EPI_ROWS) {
@@ -642,10 +671,10 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                 for (int g8 = 0; g8 < 4; ++g8) {   // 8 routed rows per stmatrix.x4: channels 8j..8j+7 of this warp, j = lane/8
                     const int tok = c0 + g8 * 8 + (lane & 7);
                     const uint32_t addr = ebuf + tok * (BM * 2) + (((q * 4 + (lane >> 3)) ^ (tok & 7)) << 4);
-                    stsm_x4_t(addr, float2_to_bf16x2(__uint_as_float(v[0][4 * g8]), __uint_as_float(v[0][4 * g8 + 1])),
-                              float2_to_bf16x2(__uint_as_float(v[0][4 * g8 + 2]), __uint_as_float(v[0][4 * g8 + 3])),
-                              float2_to_bf16x2(__uint_as_float(v[1][4 * g8]), __uint_as_float(v[1][4 * g8 + 1])),
-                              float2_to_bf16x2(__uint_as_float(v[1][4 * g8 + 2]), __uint_as_float(v[1][4 * g8 + 3])));
+                    stsm_x4_t(addr, float2_to_bf16x2(__uint_as_float(v[0][4 * g8]) * esc[0][0], __uint_as_float(v[0][4 * g8 + 1]) * esc[0][0]),
+                              float2_to_bf16x2(__uint_as_float(v[0][4 * g8 + 2]) * esc[0][1], __uint_as_float(v[0][4 * g8 + 3]) * esc[0][1]),
+                              float2_to_bf16x2(__uint_as_float(v[1][4 * g8]) * esc[1][0], __uint_as_float(v[1][4 * g8 + 1]) * esc[1][0]),
+                              float2_to_bf16x2(__uint_as_float(v[1][4 * g8 + 2]) * esc[1][1], __uint_as_float(v[1][4 * g8 + 3]) * esc[1][1]));
                 }
             }
             tc_fence_before();

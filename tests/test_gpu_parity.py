@@ -178,6 +178,21 @@ def test_no_write_outside_the_buffers_guard_regions():
         assert_close(key, to_np(g), ref[key])
 
 
+def test_zero_scale_channels():
+    """The forward GEMMs apply the channel scale in the fp32 epilogue and feed the adapter row divided by it; a channel
+    whose scale is exactly 0 (a zero weight row) must still get its adapter term and produce no NaN / Inf."""
+    inp = _skewed(MID)
+    for key in ("scale_gate", "scale_up", "scale_down"):
+        sc = inp[key].copy()
+        sc[:, 3] = 0; sc[1, 100:140] = 0; sc[2, -1] = 0
+        inp[key] = sc
+    rng = np.random.default_rng(9)
+    for key in ("A_gate", "B_gate", "A_up", "B_up", "A_down", "B_down"):
+        inp[key] = ti.f32_to_bf16_bits(rng.standard_normal(inp[key].shape).astype(np.float32) * 0.05)
+    gpu, ref = check_all(inp, backward=True, router_grad=True, gemm_impl=0)
+    assert np.abs(ref["G"][:, 3]).max() > 0        # the adapter alone drives these channels
+
+
 def test_routing_ties_lower_id_wins():
     cfg = ti.CONFIGS[0]
     inp = ti.make_inputs(cfg)

@@ -146,3 +146,29 @@ def test_tq_layer_full_chain(cfg):
         print(f"{cfg.name} {key:10s} maxabs {ma:.2e} relF {rf:.2e}")
     for key in ("dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down"):
         assert (gpu[key][cfg.E - 1] == 0).all()
+
+
+def test_tq_step_host_matches_the_stepwise_calls():
+    """tqp_step_host_async over a TurboQuant base (pinned host X / dY in, Y / dX out, two steps in flight): bit-identical to
+    the stepwise API (same kernels, same order), including the gradients that come back through R^T."""
+    import torch
+    cfg = ti.Config("tq_host", T=1100, d=256, F=256, E=6, k=2, r=16, seed=64, router_grad=True)
+    inp, tqw, spaces = make_tq_inputs(cfg, adapter_std=0.03)
+    step, layer = run_gpu_tq(inp, tqw, spaces, router_grad=True)
+    T, d = cfg.T, cfg.d
+    pin = lambda a: torch.from_numpy(a.view(np.int16)).view(torch.bfloat16).pin_memory()
+    Xh, dYh = pin(inp["X"]), pin(inp["dY"])
+    outs = [(torch.zeros((T, d), dtype=torch.bfloat16).pin_memory(), torch.zeros((T, d), dtype=torch.bfloat16).pin_memory()) for _ in range(2)]
+    grads = layer.alloc_grads()
+    W_r = torch.from_numpy(inp["W_r"]).cuda()
+    dW_r = torch.zeros((d, cfg.E), dtype=torch.float32, device="cuda")
+    for i in range(2):
+        layer.step_host_async(Xh, dYh, W_r, None, outs[i][0], outs[i][1], grads, dW_r)
+    layer.step_host_wait(0)
+    torch.cuda.synchronize()
+    for i in range(2):
+        np.testing.assert_array_equal(to_np(outs[i][0]), step["Y"])
+        np.testing.assert_array_equal(to_np(outs[i][1]), step["dX"])
+    np.testing.assert_array_equal(to_np(dW_r), step["dW_r"])
+    for key in ("dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down"):
+        np.testing.assert_array_equal(to_np(grads[key]), step[key], err_msg=key)
