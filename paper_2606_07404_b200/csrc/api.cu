@@ -43,6 +43,7 @@ Workspace layout(const tqp_layer_desc &d) {
     // widest use: two rank-r gradients over d columns in one pass (dA_gate + dA_up)
     w.wg_scratch = d.training ? take((E + N / kWgradSeg + 2) * (size_t)2 * d.r * (dm > F ? dm : F) * 4) : take(16);
     w.lut = take(256 * 8 * 2);
+    w.sc2 = take(E * (dm + 2 * F) * 4);   // bf16-pair copies of scale_down | scale_gate | scale_up for the backward GEMMs
     w.WrT = take(E * dm * 4);
     w.dl = take(N * 4);
     w.trace = take(16384 * 8);
@@ -274,14 +275,20 @@ tqp_status tqp_bind_weights(tqp_ctx *c, const tqp_weights *w, void *stream) {
     P->nseg = 1; P->nlora = 1; P->M = D.d; P->r = D.r; P->out = nullptr;   // out = Ye, per call
     CK(set_seg(c, &P->seg[0], H, Np, w->idx_down, w->scale_down, D.F, D.d, 1));
     CK(set_lora(c, &P->lora[0], c->p<bf16>(c->ws.HAd), Np, w->B_down, 0));
+    uint32_t *sc2_down = c->p<uint32_t>(c->ws.sc2), *sc2_gate = sc2_down + (size_t)D.E * D.d, *sc2_up = sc2_gate + (size_t)D.E * D.F;
+    CK(launch_scale_pairs(c, (const __half *)w->scale_down, sc2_down, (size_t)D.E * D.d, (cudaStream_t)stream));
+    CK(launch_scale_pairs(c, (const __half *)w->scale_gate, sc2_gate, (size_t)D.E * D.F, (cudaStream_t)stream));
+    CK(launch_scale_pairs(c, (const __half *)w->scale_up, sc2_up, (size_t)D.E * D.F, (cudaStream_t)stream));
     P = &c->prob_dh; memset(P, 0, sizeof(*P));
     P->nseg = 1; P->nlora = 1; P->M = D.F; P->r = D.r; P->out = dH;       // seg[0].act = dYe, per call
     CK(set_seg(c, &P->seg[0], dH /*placeholder*/, Np, w->idx_down, w->scale_down, D.d, D.F, 0));
+    P->seg[0].scale2 = sc2_down;
     CK(set_lora(c, &P->lora[0], c->p<bf16>(c->ws.Zd), Np, w->A_down, 1));
     P = &c->prob_dx; memset(P, 0, sizeof(*P));
     P->nseg = 2; P->nlora = 2; P->M = D.d; P->r = D.r; P->out = nullptr;   // out = dXp, per call
     CK(set_seg(c, &P->seg[0], dG, Np, w->idx_gate, w->scale_gate, D.F, D.d, 0));
     CK(set_seg(c, &P->seg[1], dU, Np, w->idx_up, w->scale_up, D.F, D.d, 0));
+    P->seg[0].scale2 = sc2_gate; P->seg[1].scale2 = sc2_up;
     CK(set_lora(c, &P->lora[0], c->p<bf16>(c->ws.Zg), Np, w->A_gate, 1));
     CK(set_lora(c, &P->lora[1], c->p<bf16>(c->ws.Zu), Np, w->A_up, 1));
 #undef CK

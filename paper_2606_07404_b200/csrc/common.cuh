@@ -40,6 +40,7 @@ struct GemmSeg {
     const bf16 *act;        // [N][K] bf16 activations (B operand)
     const uint8_t *idx;     // codes of all experts
     const __half *scale;    // per-output-channel scales of all experts
+    const uint32_t *scale2; // MN-major (backward) VQ segments: the scales as bf16 pairs (s, s), converted at bind time
     const float *norm;      // scalar (TurboQuant) format: fp32 row norms of all experts, in place of `scale`
     const void *lut;        // scalar format: the 256 bf16 Lloyd-Max levels of this pack's input space (device)
     int scalar;             // 1: TurboQuant codes, idx[e][M][K] / idx[e][K][M] one byte per weight; 0: vector-quantised
@@ -93,7 +94,7 @@ struct Workspace {
     // sizes
     size_t total = 0;
     // offsets (bytes) into the bound buffer
-    size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, xsegs, xfirst, wg_scratch, sched, lut, WrT, dl,
+    size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, xsegs, xfirst, wg_scratch, sched, lut, sc2, WrT, dl,
         // tqp_step_host staging
         trace, hX, hdY, hX2, hdY2, hY, hdX, topk_idx, topk_w, counts, offsets, perm, inv_perm, Ye, dYe, dXp, dtopk_w;
 };
@@ -190,6 +191,7 @@ tqp_status launch_bias_update(tqp_ctx *c, const int32_t *counts, float *bias, in
 tqp_status launch_combine_dw(tqp_ctx *c, int T, const bf16 *dY, const bf16 *Ye, const int32_t *inv_perm, float *dtopk_w,
                              cudaStream_t s);
 tqp_status launch_make_lut(tqp_ctx *c, const __half *codebook, bf16 *lut, cudaStream_t s);
+tqp_status launch_scale_pairs(tqp_ctx *c, const __half *scale, uint32_t *out, size_t n, cudaStream_t s);
 
 // ---- lora.cu -------------------------------------------------------------------------------------------
 // out_w[p][0..r) = s * row(p) . W_w[e]  for w < (W1 ? 2 : 1); W_e is [K][r] if w_kr else [r][K]; out is [N][kLoraPad] bf16.

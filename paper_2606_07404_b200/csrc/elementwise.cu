@@ -207,6 +207,18 @@ tqp_status launch_combine_dw(tqp_ctx *c, int T, const bf16 *dY, const bf16 *Ye, 
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }
+// fp16 scale -> the bf16 pair (s, s) the backward dequant producers multiply with: frozen weights, so done once at bind time
+__global__ void scale_pairs_kernel(const __half *__restrict__ scale, uint32_t *__restrict__ out, size_t n) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const __nv_bfloat162 v = __float2bfloat162_rn(__half2float(scale[i]));
+    out[i] = *reinterpret_cast<const uint32_t *>(&v);
+}
+tqp_status launch_scale_pairs(tqp_ctx *c, const __half *scale, uint32_t *out, size_t n, cudaStream_t s) {
+    scale_pairs_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(scale, out, n);
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
 tqp_status launch_make_lut(tqp_ctx *c, const __half *codebook, bf16 *lut, cudaStream_t s) {
     make_lut_kernel<<<8, 256, 0, s>>>(codebook, lut);
     TQP_LAUNCH_OK(c);

@@ -41,7 +41,7 @@ struct Cfg {
     static constexpr int NSTAGE = SC ? 4 : 6;                 // B (activation) ring
     static constexpr int IDXQ = SC ? 3 : 8;                   // index ring
     static constexpr int IDX_TILE = SC ? 128 * 128 : 128 * 16;
-    static constexpr int SCL_BYTES = SC ? 128 * 4 : 128 * 2;  // the stage's 128 fp32 norms / fp16 scales ride with the code tile
+    static constexpr int SCL_BYTES = 128 * 4;                 // 128 values ride with the code tile: fp32 norms (SC), bf16-pair scales (VQ backward), fp16 scales (VQ forward: 256 B)
     static constexpr int IDX_BYTES = SC ? IDX_TILE + 1024 : IDX_TILE + SCL_BYTES;   // SC: 128-byte-swizzled TMA tiles need 1024-byte alignment
     static constexpr int LUT_BYTES = 256 * 8 * 16;            // VQ: 8 replicas of the 16-byte entries; SC: 32 lane-private copies of 4-byte entries
     static constexpr int OFF_X = 0, OFF_LUT = OFF_X + NSTAGE * X_BYTES, OFF_IDX = OFF_LUT + LUT_BYTES,
@@ -237,7 +237,8 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                     const int nka = S.K / AK;
                     for (int ka = 0; ka < nka; ++ka) {   // K-major: [128 channels][16 codes]; MN-major: [128 k][16 channel groups]
                         mbar_wait(idx_empty(iq.s), iq.ph ^ 1);
-                        mbar_expect_tx(idx_full(iq.s), IDX_TILE + SCL_BYTES);
+                        const uint32_t scl_bytes = (SC || !S.kmajor) ? SCL_BYTES : 256u;
+                        mbar_expect_tx(idx_full(iq.s), IDX_TILE + scl_bytes);
                         // VQ: a code covers 8 weights along the pack's input dim; SC: one code per weight
                         const int c0 = S.kmajor ? ka * (SC ? AK : AK / 8) : (SC ? it.m0 : it.m0 / 8);
                         const int c1 = S.kmajor ? it.t.expert * pb.M + it.m0 : it.t.expert * S.K + ka * AK;
@@ -245,7 +246,8 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                         // the stage's scales ride along (K-major: of this CTA's 128 channels; MN-major: of the stage's 128 k), so
                         // that no producer waits on a global load when an item starts
                         if (SC) bulk_g2s(sbase + OFF_IDX + iq.s * IDX_BYTES + IDX_TILE, S.norm + c1, SCL_BYTES, idx_full(iq.s));
-                        else bulk_g2s(sbase + OFF_IDX + iq.s * IDX_BYTES + IDX_TILE, S.scale + c1, SCL_BYTES, idx_full(iq.s));
+                        else if (S.kmajor) bulk_g2s(sbase + OFF_IDX + iq.s * IDX_BYTES + IDX_TILE, S.scale + c1, 256u, idx_full(iq.s));
+                        else bulk_g2s(sbase + OFF_IDX + iq.s * IDX_BYTES + IDX_TILE, S.scale2 + c1, SCL_BYTES, idx_full(iq.s));   // bf16 pairs, ready to multiply
                         iq.next(IDXQ);
                     }
                 }
@@ -574,12 +576,13 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
                         if (own) {   // one index tile = 128 k x 16 channel groups = this A stage
                             mbar_wait(idx_full(iq.s), iq.ph);
                             const uint32_t is = sbase + OFF_IDX + iq.s * IDX_BYTES + kofs * 16 + (warp & 3) * 4;
-                            const uint32_t ss = sbase + OFF_IDX + iq.s * IDX_BYTES + IDX_TILE + kofs * 2;   // the stage's per-k scales
+                            const uint32_t ss = sbase + OFF_IDX + iq.s * IDX_BYTES + IDX_TILE + kofs * 4;   // the stage's per-k scales as bf16 pairs
 #pragma unroll
                             for (int z = 0; z < 16; ++z) {   // z = 8 h + 2 x + i  ->  k = 64 h + 16 x + kofs + 2 i
                                 const int kz = (z >> 3) * 64 + ((z >> 1) & 3) * 16 + (z & 1) * 2;
                                 cw[z] = lds32(is + kz * 16);
-                                sc[z] = __float2bfloat162_rn(__half2float(__ushort_as_half((unsigned short)lds16(ss + kz * 2))));
+                                const uint32_t sv = lds32(ss + kz * 4);
+                                sc[z] = *reinterpret_cast<const __nv_bfloat162 *>(&sv);
                             }
                             __syncwarp();
                             if (lane == 0) mbar_arrive(idx_empty(iq.s));
