@@ -148,7 +148,9 @@ tqp_status tqp_route_bwd(tqp_ctx *ctx, int T, const void *X, const float *W_r, c
 /* Copies X and dY (bf16 [T][d], pinned HOST memory) to the device, runs the whole forward+backward chain
  * above on `stream` and copies Y and dX (bf16 [T][d]) back to the HOST buffers.  W_r / logit_bias and the
  * adapter-gradient outputs are DEVICE pointers as above (dW_r may be NULL to skip tqp_route_bwd).
- * Synchronises `stream` before returning. */
+ * Synchronises `stream` before returning.  The device-side staging of these calls (two upload sets, the routing arrays,
+ * Ye / dYe / dXp: 1.7 GB at configs[2]) is NOT part of the caller's workspace: the library allocates it on the first call
+ * and frees it in tqp_destroy, so a caller of the stepwise API never pays for it. */
 tqp_status tqp_step_host(tqp_ctx *ctx, int T, const void *X_host, const void *dY_host, const float *W_r,
                          const float *logit_bias, void *Y_host, void *dX_host, float *dA_gate,
                          float *dB_gate, float *dA_up, float *dB_up, float *dA_down, float *dB_down,

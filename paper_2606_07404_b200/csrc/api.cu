@@ -47,12 +47,16 @@ Workspace layout(const tqp_layer_desc &d) {
     w.WrT = take(E * dm * 4);
     w.dl = take(N * 4);
     w.trace = take(16384 * 8);
+    w.total = off;
+    // Staging of tqp_step_host (X / dY twice, Y, dX, the routing arrays, Ye / dYe / dXp): NOT part of the caller's workspace;
+    // the library allocates it on the first tqp_step_host call (a stepwise caller never pays for it: 1.7 GB at cfg 2).
+    off = 0;
     w.hX = take(T * dm * 2); w.hdY = take(T * dm * 2); w.hY = take(T * dm * 2); w.hdX = take(T * dm * 2);
     w.hX2 = take(T * dm * 2); w.hdY2 = take(T * dm * 2);   // second upload set (tqp_step_host_async)
     w.topk_idx = take(N * 4); w.topk_w = take(N * 4); w.counts = take(E * 4); w.offsets = take((E + 1) * 4);
     w.perm = take(N * 4); w.inv_perm = take(N * 4);
     w.Ye = take(N * dm * 2); w.dYe = take(N * dm * 2); w.dXp = take(N * dm * 2); w.dtopk_w = take(N * 4);
-    w.total = off;
+    w.host_total = off;
     return w;
 }
 
@@ -196,6 +200,7 @@ void tqp_destroy(tqp_ctx *ctx) {
         if (e) cudaEventDestroy(e);
     for (auto &r : ctx->tq_rots) { cudaFree(r.Rb); cudaFree(r.Rtb); cudaFree(r.Rt); }
     tq_free_state(ctx);
+    if (ctx->host_base) cudaFree(ctx->host_base);
     if (ctx->copy_in) cudaStreamDestroy(ctx->copy_in);
     if (ctx->copy_out) cudaStreamDestroy(ctx->copy_out);
     delete ctx;
@@ -761,12 +766,17 @@ tqp_status tqp_step_host_async(tqp_ctx *c, int T, const void *X_host, const void
     const tqp_layer_desc &D = c->desc;
     const size_t row_bytes = (size_t)T * D.d * 2;
     const int par = (int)(c->host_seq & 1);   // upload staging set of this step
-    bf16 *X = c->p<bf16>(par ? c->ws.hX2 : c->ws.hX), *dY = c->p<bf16>(par ? c->ws.hdY2 : c->ws.hdY);
-    bf16 *Y = c->p<bf16>(c->ws.hY), *dX = c->p<bf16>(c->ws.hdX);
-    int32_t *ti = c->p<int32_t>(c->ws.topk_idx), *counts = c->p<int32_t>(c->ws.counts), *offs = c->p<int32_t>(c->ws.offsets);
-    int32_t *perm = c->p<int32_t>(c->ws.perm), *inv = c->p<int32_t>(c->ws.inv_perm);
-    float *tw = c->p<float>(c->ws.topk_w), *dtw = c->p<float>(c->ws.dtopk_w);
-    bf16 *Ye = c->p<bf16>(c->ws.Ye), *dYe = c->p<bf16>(c->ws.dYe), *dXp = c->p<bf16>(c->ws.dXp);
+    if (!c->host_base) {   // first use: the library's own staging (freed by tqp_destroy)
+        TQP_CUDA_OK(c, cudaMalloc(&c->host_base, c->ws.host_total));
+        TQP_CUDA_OK(c, cudaMemsetAsync(c->host_base, 0, c->ws.host_total, s));
+    }
+    auto hp = [&](size_t off) { return c->host_base + off; };
+    bf16 *X = (bf16 *)hp(par ? c->ws.hX2 : c->ws.hX), *dY = (bf16 *)hp(par ? c->ws.hdY2 : c->ws.hdY);
+    bf16 *Y = (bf16 *)hp(c->ws.hY), *dX = (bf16 *)hp(c->ws.hdX);
+    int32_t *ti = (int32_t *)hp(c->ws.topk_idx), *counts = (int32_t *)hp(c->ws.counts), *offs = (int32_t *)hp(c->ws.offsets);
+    int32_t *perm = (int32_t *)hp(c->ws.perm), *inv = (int32_t *)hp(c->ws.inv_perm);
+    float *tw = (float *)hp(c->ws.topk_w), *dtw = (float *)hp(c->ws.dtopk_w);
+    bf16 *Ye = (bf16 *)hp(c->ws.Ye), *dYe = (bf16 *)hp(c->ws.dYe), *dXp = (bf16 *)hp(c->ws.dXp);
     int total = 0;
 #define CK(x) do { st = (x); total += c->launches; if (st != TQP_OK) return st; } while (0)
     if (!c->copy_in) {

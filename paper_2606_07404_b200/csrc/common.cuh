@@ -92,7 +92,8 @@ struct TqLayer {
 
 struct Workspace {
     // sizes
-    size_t total = 0;
+    size_t total = 0;        // the caller's workspace
+    size_t host_total = 0;   // tqp_step_host staging (library-owned, allocated on first use)
     // offsets (bytes) into the bound buffer
     size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, xsegs, xfirst, wg_scratch, sched, lut, sc2, WrT, dl,
         // tqp_step_host staging
@@ -105,6 +106,7 @@ struct tqp_ctx {
     tqp_layer_desc desc;
     tqp::Workspace ws;
     char *base = nullptr;       // bound workspace
+    char *host_base = nullptr;  // tqp_step_host staging (cudaMalloc on first use)
     size_t bound_bytes = 0;
     tqp_weights w;
     bool have_weights = false;
