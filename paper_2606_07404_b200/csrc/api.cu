@@ -512,11 +512,13 @@ tqp_status tqp_expert_fwd(tqp_ctx *c, int T, const void *X, const int32_t *offse
     }
     GemmProblem pr[2] = {c->prob_gate, c->prob_up};
     CK(run_gemm(c, pr, 2, s));
-    CK(launch_swiglu_fwd(c, N, G, U, H, s));
-    if (tq) {   // h' = R_F h, in place for the Hadamard case (a dense R_F goes through the idle dG buffer)
-        if (c->tq.w.space_F.hadamard) {
-            CK(launch_tq_rotate(c, &c->tq.w.space_F, H, false, N, H, false, 0, s));
-        } else {
+    if (tq && c->tq.w.space_F.hadamard) {   // h' = R_F (silu(g) u) in one pass: h itself is never stored
+        CK(launch_tq_swiglu_fwd_rot(c, &c->tq.w.space_F, G, U, H, N, s));
+    } else {
+        CK(launch_swiglu_fwd(c, N, G, U, H, s));
+    }
+    if (tq) {   // a dense R_F goes through the idle dG buffer
+        if (!c->tq.w.space_F.hadamard) {
             CK(launch_tq_rotate(c, &c->tq.w.space_F, H, false, N, c->p<bf16>(c->ws.dG), false, 0, s));
             TQP_CUDA_OK(c, cudaMemcpyAsync(H, c->p<bf16>(c->ws.dG), (size_t)N * D.F * 2, cudaMemcpyDeviceToDevice, s));
         }
@@ -604,15 +606,15 @@ tqp_status tqp_expert_bwd(tqp_ctx *c, int T, const void *X, const void *dYe, con
     CK(act_map(c, &ph.seg[0].act_map2, dye, (uint64_t)N, D.d, kTileRows / 2));
     CK(run_gemm(c, &ph, 1, s));
     const bool tq = c->tq.on;
-    if (tq) {   // the GEMM produced dh' = R_F dh (rotated F space): dh = R_F^T dh'
-        if (c->tq.w.space_F.hadamard) {
-            CK(launch_tq_rotate(c, &c->tq.w.space_F, dH, false, N, dH, false, 1, s));
-        } else {
+    if (tq && c->tq.w.space_F.hadamard) {   // the GEMM produced dh' = R_F dh: un-rotate and apply the SwiGLU backward in one pass
+        CK(launch_tq_swiglu_bwd_rot(c, &c->tq.w.space_F, dH, G, U, dG, dU, N, s));
+    } else {
+        if (tq) {
             CK(launch_tq_rotate(c, &c->tq.w.space_F, dH, false, N, dG, false, 1, s));
             TQP_CUDA_OK(c, cudaMemcpyAsync(dH, dG, (size_t)N * D.F * 2, cudaMemcpyDeviceToDevice, s));
         }
+        CK(launch_swiglu_bwd(c, N, dH, G, U, dG, dU, s));
     }
-    CK(launch_swiglu_bwd(c, N, dH, G, U, dG, dU, s));
     // With a TurboQuant base the dA gradients are first formed w.r.t. A' = R A (the rows that multiply them are rotated) and
     // then carried back, dA = R^T dA'; the deferred tail of tqp_step_host is not used in that mode.
     const bool defer = c->defer_tail && !tq;

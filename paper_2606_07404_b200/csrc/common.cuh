@@ -236,6 +236,9 @@ inline tqp_status ensure_dyn_smem(tqp_ctx *c, const void *func, int bytes) {
 tqp_status tq_check_space(tqp_ctx *c, const tqp_tq_space *sp);
 tqp_status launch_tq_rotate(tqp_ctx *c, const tqp_tq_space *sp, const void *X, bool in_f32, long long rows, void *Y, bool out_f32, int inverse,
                             cudaStream_t st);
+tqp_status launch_tq_swiglu_fwd_rot(tqp_ctx *c, const tqp_tq_space *sp, const bf16 *G, const bf16 *U, bf16 *Hr, long long rows, cudaStream_t st);
+tqp_status launch_tq_swiglu_bwd_rot(tqp_ctx *c, const tqp_tq_space *sp, const bf16 *dHr, const bf16 *G, const bf16 *U, bf16 *dG, bf16 *dU,
+                                    long long rows, cudaStream_t st);
 tqp_status launch_tq_make_lut(tqp_ctx *c, const double *levels, bf16 *lut, cudaStream_t st);
 template <typename T>
 tqp_status launch_tq_transpose(tqp_ctx *c, const T *in, T *out, int E, int a, int b, cudaStream_t st);   // [E][a][b] -> [E][b][a]

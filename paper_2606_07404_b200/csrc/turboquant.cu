@@ -231,9 +231,13 @@ __device__ __forceinline__ void fw_bfly8(float (&v)[8], int nb) {
     }
 }
 
-template <typename TIN, typename TOUT>
+// MODE 0: Y = rotation of X.  MODE 1 (bf16): Y = R (silu(X) * X2) -- the SwiGLU of the TurboQuant layer with the rotation of its
+// result in the same pass (h is never rounded or stored unrotated).  MODE 2 (bf16, inverse): dh = R^T X, then the SwiGLU
+// backward against the saved g = X2, u = X3:  Y = dg, Y2 = du  (dh stays in registers).
+template <typename TIN, typename TOUT, int MODE>
 __global__ void __launch_bounds__(1024) tq_fwht_rows_kernel(const TIN *__restrict__ X, TOUT *__restrict__ Y, long long rows, int n, int logn,
-                                                             const int8_t *__restrict__ signs, int inverse) {
+                                                             const int8_t *__restrict__ signs, int inverse, const TIN *__restrict__ X2,
+                                                             const TIN *__restrict__ X3, TOUT *__restrict__ Y2) {
     extern __shared__ float fw_s[];
     const int tpr = n / 8, rpc = blockDim.x / tpr;             // threads per row, rows per CTA
     const int lr = threadIdx.x / tpr, t = threadIdx.x % tpr, lane = threadIdx.x % 32;
@@ -266,6 +270,12 @@ __global__ void __launch_bounds__(1024) tq_fwht_rows_kernel(const TIN *__restric
         for (int k = 0; k < 8; ++k) v[k] = 0.f;
         if (act) {
             fw_load8<TIN>(X + row * n + 8 * t, v);
+            if (MODE == 1) {
+                float u[8];
+                fw_load8<TIN>(X2 + row * n + 8 * t, u);
+#pragma unroll
+                for (int k = 0; k < 8; ++k) v[k] = v[k] / (1.f + __expf(-v[k])) * u[k];
+            }
             if (!inverse) {
 #pragma unroll
                 for (int k = 0; k < 8; ++k) v[k] *= sg[k];
@@ -305,7 +315,21 @@ __global__ void __launch_bounds__(1024) tq_fwht_rows_kernel(const TIN *__restric
                 v[k] *= rs;
                 if (inverse) v[k] *= sg[k];
             }
-            fw_store8<TOUT>(Y + row * n + 8 * t, v);
+            if (MODE == 2) {   // v = dh: sig = sigmoid(g); du = dh g sig; dg = dh u sig (1 + g (1 - sig))
+                float g[8], u[8], dg[8];
+                fw_load8<TIN>(X2 + row * n + 8 * t, g);
+                fw_load8<TIN>(X3 + row * n + 8 * t, u);
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const float sig = 1.f / (1.f + __expf(-g[k]));
+                    dg[k] = v[k] * u[k] * sig * (1.f + g[k] * (1.f - sig));
+                    v[k] = v[k] * g[k] * sig;
+                }
+                fw_store8<TOUT>(Y + row * n + 8 * t, dg);
+                fw_store8<TOUT>(Y2 + row * n + 8 * t, v);
+            } else {
+                fw_store8<TOUT>(Y + row * n + 8 * t, v);
+            }
         }
     }
 }
@@ -720,10 +744,10 @@ tqp_status launch_tq_rotate(tqp_ctx *c, const tqp_tq_space *sp, const void *X, b
         const long long ctas = (rows + rpc - 1) / rpc;
         const int grid = (int)std::min<long long>(ctas, (long long)c->num_sms * std::max(1, 2048 / thr));
         const size_t sm = (size_t)rpc * (n + n / 32) * 4;
-        if (in_f32 && out_f32) tq_fwht_rows_kernel<float, float><<<grid, thr, sm, st>>>((const float *)X, (float *)Y, rows, n, logn, sp->signs, inverse);
-        else if (in_f32) tq_fwht_rows_kernel<float, bf16><<<grid, thr, sm, st>>>((const float *)X, (bf16 *)Y, rows, n, logn, sp->signs, inverse);
-        else if (out_f32) tq_fwht_rows_kernel<bf16, float><<<grid, thr, sm, st>>>((const bf16 *)X, (float *)Y, rows, n, logn, sp->signs, inverse);
-        else tq_fwht_rows_kernel<bf16, bf16><<<grid, thr, sm, st>>>((const bf16 *)X, (bf16 *)Y, rows, n, logn, sp->signs, inverse);
+        if (in_f32 && out_f32) tq_fwht_rows_kernel<float, float, 0><<<grid, thr, sm, st>>>((const float *)X, (float *)Y, rows, n, logn, sp->signs, inverse, nullptr, nullptr, nullptr);
+        else if (in_f32) tq_fwht_rows_kernel<float, bf16, 0><<<grid, thr, sm, st>>>((const float *)X, (bf16 *)Y, rows, n, logn, sp->signs, inverse, nullptr, nullptr, nullptr);
+        else if (out_f32) tq_fwht_rows_kernel<bf16, float, 0><<<grid, thr, sm, st>>>((const bf16 *)X, (float *)Y, rows, n, logn, sp->signs, inverse, nullptr, nullptr, nullptr);
+        else tq_fwht_rows_kernel<bf16, bf16, 0><<<grid, thr, sm, st>>>((const bf16 *)X, (bf16 *)Y, rows, n, logn, sp->signs, inverse, nullptr, nullptr, nullptr);
         TQP_LAUNCH_OK(c);
         return TQP_OK;
     }
@@ -754,6 +778,27 @@ __global__ void tq_make_lut_kernel(const double *__restrict__ levels, bf16 *__re
 }
 tqp_status launch_tq_make_lut(tqp_ctx *c, const double *levels, bf16 *lut, cudaStream_t st) {
     tq_make_lut_kernel<<<1, 256, 0, st>>>(levels, lut);
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
+
+// Hadamard spaces only: H' = R (silu(G) * U)   /   dG, dU from dH' = R dh and the saved G, U   (one pass each)
+tqp_status launch_tq_swiglu_fwd_rot(tqp_ctx *c, const tqp_tq_space *sp, const bf16 *G, const bf16 *U, bf16 *Hr, long long rows, cudaStream_t st) {
+    const int n = sp->n, tpr = n / 8, rpc = std::max(1, 128 / tpr), thr = tpr * rpc;
+    int logn = 0;
+    while ((1 << logn) < n) ++logn;
+    const int grid = (int)std::min<long long>((rows + rpc - 1) / rpc, (long long)c->num_sms * std::max(1, 2048 / thr));
+    tq_fwht_rows_kernel<bf16, bf16, 1><<<grid, thr, (size_t)rpc * (n + n / 32) * 4, st>>>(G, Hr, rows, n, logn, sp->signs, 0, U, nullptr, nullptr);
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
+tqp_status launch_tq_swiglu_bwd_rot(tqp_ctx *c, const tqp_tq_space *sp, const bf16 *dHr, const bf16 *G, const bf16 *U, bf16 *dG, bf16 *dU,
+                                    long long rows, cudaStream_t st) {
+    const int n = sp->n, tpr = n / 8, rpc = std::max(1, 128 / tpr), thr = tpr * rpc;
+    int logn = 0;
+    while ((1 << logn) < n) ++logn;
+    const int grid = (int)std::min<long long>((rows + rpc - 1) / rpc, (long long)c->num_sms * std::max(1, 2048 / thr));
+    tq_fwht_rows_kernel<bf16, bf16, 2><<<grid, thr, (size_t)rpc * (n + n / 32) * 4, st>>>(dHr, dG, rows, n, logn, sp->signs, 1, G, U, dU);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }

@@ -128,6 +128,7 @@ CASES = [
     ti.Config("tq_hadamard", T=640, d=256, F=512, E=6, k=3, r=16, seed=61, router_grad=True),
     ti.Config("tq_r32", T=300, d=512, F=256, E=5, k=2, r=32, seed=62, router_grad=True, lora_scale=0.5),
     ti.Config("tq_dense_d", T=500, d=768, F=256, E=4, k=2, r=16, seed=63, router_grad=True),     # d = 768: sign-fixed QR rotation
+    ti.Config("tq_dense_F", T=400, d=256, F=768, E=4, k=2, r=16, seed=65, router_grad=True),     # F = 768: QR rotation of the hidden space
 ]
 
 
