@@ -8,6 +8,7 @@
 #include <stdint.h>
 
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/tqp.h"
@@ -119,7 +120,7 @@ struct tqp_ctx {
     int device = 0;                 // the device the ctx was created on (kernel attributes are per device)
     std::vector<tqp::TqRot> tq_rots;             // library-owned; freed by tqp_destroy
     tqp::TqLayer tq;                             // TurboQuant-format weights bound (tqp_bind_weights_tq)
-    std::vector<const void *> smem_attr_done;   // kernels whose dynamic shared-memory limit has been raised on `device`
+    std::vector<std::pair<const void *, int>> smem_attr_done;   // kernels whose dynamic shared-memory limit has been raised on `device`, and to what
     int launches = 0;
     int num_sms = 148;
     int max_tiles = 0;
@@ -221,14 +222,20 @@ tqp_status launch_gemm_tcgen05_ts2(tqp_ctx *c, const GemmProblem *probs, int npr
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: raised once per ctx (a ctx lives on one device)
 inline tqp_status ensure_dyn_smem(tqp_ctx *c, const void *func, int bytes) {
-    for (const void *f : c->smem_attr_done)
-        if (f == func) return TQP_OK;
+    for (auto &f : c->smem_attr_done)
+        if (f.first == func) {
+            if (f.second >= bytes) return TQP_OK;
+            cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);   // a larger request than before
+            if (e != cudaSuccess) { c->err = std::string("cudaFuncSetAttribute(MaxDynamicSharedMemorySize): ") + cudaGetErrorString(e); return TQP_ERR_CUDA; }
+            f.second = bytes;
+            return TQP_OK;
+        }
     cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e != cudaSuccess) {
         c->err = std::string("cudaFuncSetAttribute(MaxDynamicSharedMemorySize): ") + cudaGetErrorString(e);
         return TQP_ERR_CUDA;
     }
-    c->smem_attr_done.push_back(func);
+    c->smem_attr_done.push_back({func, bytes});
     return TQP_OK;
 }
 
