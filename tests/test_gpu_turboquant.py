@@ -126,3 +126,32 @@ def test_flush_against_the_oracle(n, out_dim, r, s):
     assert (Bd.float() == 0).all()                                           # reset: B <- 0, A <- the fresh draw
     np.testing.assert_array_equal(Ad.view(torch.int16).cpu().numpy().view(np.uint16), A_new)
     print(f"flush n={n}: {ndiff} codes differ at cell boundaries")
+
+
+def test_error_codes():
+    import torch
+    import paper_2606_07404_b200 as tq
+    layer = _layer()
+    lv = torch.zeros(256, dtype=torch.float64, device="cuda")
+    sg = torch.ones(192, dtype=torch.int8, device="cuda")
+    X = torch.zeros((4, 192), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(tq.TqpError) as e:                       # signed Hadamard needs a power-of-two width
+        layer.rotate(tq.TqSpace(192, lv, signs=sg), X)
+    assert e.value.code == 2
+    with pytest.raises(tq.TqpError) as e:                       # width not a multiple of 64
+        layer.rotate(tq.TqSpace(100, lv, signs=sg), X)
+    assert e.value.code == 2
+    sp, _, _ = _space(128, 3)
+    big = tq.TqpLayer(64, 128, 128, 4, 2, 8)                    # r = 8: the TurboQuant-format layer needs r in {16, 32}
+    z8 = lambda *s: torch.zeros(s, dtype=torch.uint8, device="cuda")
+    zf = lambda *s: torch.zeros(s, dtype=torch.float32, device="cuda")
+    zb = lambda *s: torch.zeros(s, dtype=torch.bfloat16, device="cuda")
+    w = dict(codes_gate=z8(4, 128, 128), codes_up=z8(4, 128, 128), codes_down=z8(4, 128, 128), norm_gate=zf(4, 128), norm_up=zf(4, 128),
+             norm_down=zf(4, 128), A_gate=zb(4, 128, 8), A_up=zb(4, 128, 8), B_gate=zb(4, 8, 128), B_up=zb(4, 8, 128), A_down=zb(4, 128, 8),
+             B_down=zb(4, 8, 128))
+    with pytest.raises(tq.TqpError) as e:
+        big.bind_weights_tq(sp, sp, **w)
+    assert e.value.code == 2
+    with pytest.raises(tq.TqpError) as e:                       # flush: rank out of range
+        layer.tq_flush(sp, z8(1, 8, 128), zf(1, 8), zb(1, 128, 64), zb(1, 64, 8), 1.0)
+    assert e.value.code == 1
