@@ -173,3 +173,40 @@ def test_tq_step_host_matches_the_stepwise_calls():
     np.testing.assert_array_equal(to_np(dW_r), step["dW_r"])
     for key in ("dA_gate", "dB_gate", "dA_up", "dB_up", "dA_down", "dB_down"):
         np.testing.assert_array_equal(to_np(grads[key]), step[key], err_msg=key)
+
+
+def test_rebinding_between_the_two_base_formats():
+    """One ctx: TurboQuant base bound, then the vector-quantised base of the same shape, then TurboQuant again.  Each bind
+    must fully replace the other's state (GEMM problems, look-up tables, rotated-adapter buffers): results equal those of
+    a fresh ctx bit for bit."""
+    import torch
+    from parity_util import make_layer, run_gpu, to_dev
+    cfg = ti.Config("tq_rebind", T=300, d=256, F=256, E=4, k=2, r=16, seed=66, router_grad=False)
+    inp, tqw, spaces = make_tq_inputs(cfg, adapter_std=0.03)
+    fresh_tq, layer = run_gpu_tq(inp, tqw, spaces, router_grad=False)
+    fresh_vq = run_gpu(inp, backward=True, router_grad=False)
+    dev = to_dev(inp)
+    layer.bind_weights(**{n: dev[n] for n in ("idx_gate", "idx_up", "idx_down", "scale_gate", "scale_up", "scale_down", "codebook",
+                                              "A_gate", "A_up", "B_gate", "B_up", "A_down", "B_down")})
+
+    def chain():
+        idx, w = layer.route(dev["X"], dev["W_r"], None)
+        counts, offsets, perm, inv = layer.dispatch(idx)
+        Ye = layer.expert_fwd(dev["X"], offsets, perm)
+        Y = layer.combine(Ye, inv, w)
+        dYe, _ = layer.combine_bwd(dev["dY"], Ye, inv, w, want_dw=False, perm=perm)
+        dXp, grads = layer.expert_bwd(dev["X"], dYe, offsets, perm, dYe_unmodified=True)
+        dX = layer.dispatch_bwd(dXp, inv)
+        torch.cuda.synchronize()
+        return dict(Y=to_np(Y), dX_experts=to_np(dX), **{k_: to_np(v) for k_, v in grads.items()})
+
+    got_vq = chain()
+    for key in got_vq:
+        np.testing.assert_array_equal(got_vq[key], fresh_vq[key], err_msg=f"VQ after TQ: {key}")
+    sp = layer.spaces
+    wt = {key: torch.from_numpy(v).cuda() for key, v in tqw.items()}
+    wt.update({key: dev[key] for key in ("A_gate", "A_up", "B_gate", "B_up", "A_down", "B_down")})
+    layer.bind_weights_tq(sp[0], sp[1], **wt)
+    got_tq = chain()
+    for key in got_tq:
+        np.testing.assert_array_equal(got_tq[key], fresh_tq[key], err_msg=f"TQ after VQ: {key}")
