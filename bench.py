@@ -233,6 +233,8 @@ def run_ours(args, cfg):
     layer = tq.TqpLayer(T, cfg.d, cfg.F, cfg.E, cfg.k, cfg.r, lora_scale=cfg.lora_scale, training=True, device=str(dev))
     if args.gemm_impl:
         layer.set_option("gemm_impl", args.gemm_impl)
+    if args.route_impl:
+        layer.set_option("route_impl", args.route_impl)
 
     def up(a):
         t = torch.from_numpy(a.view(np.int16)).view(torch.bfloat16) if a.dtype == np.uint16 else torch.from_numpy(a)
@@ -286,6 +288,9 @@ def run_ours(args, cfg):
     e1.record()
     barrier()
     ms = e0.elapsed_time(e1)
+    screened, fallback = layer.route_info()   # of the last timed step (outside the timed region: it synchronises)
+    router_desc = ("screened: tcgen05 approximate logits + canonical fp32 chain for the candidates (bit-identical top-k)"
+                   + (", FALLBACK to the dense chain taken" if fallback else "")) if screened else "dense canonical fp32 chain"
     # second pass of the same K steps with every grouped-GEMM launch bracketed by CUDA events on its own stream
     # (tqp_gemm_time); the headline time above carries no such events.  The clock sampler covers both passes.
     layer.set_option("time_gemm", 1)
@@ -362,7 +367,7 @@ def run_ours(args, cfg):
                          f"{T * cfg.k * cfg.d * 2 / 1e6:.0f} MB permuted rows per step), no flush",
                    "base_format": "TurboQuant-MSE 8-bit scalar codes + row norms, rotated space (PAPER.md L944-948)" if args.format == "tq"
                    else "vector-quantised, 8-vectors / 256-entry codebook / fp16 channel scales (BASELINE.json)",
-                   "gemm_impl": GEMM_IMPL_NAMES.get(args.gemm_impl, str(args.gemm_impl)), "parallelism": f"replicas x{world}, no collective"},
+                   "gemm_impl": GEMM_IMPL_NAMES.get(args.gemm_impl, str(args.gemm_impl)), "router": router_desc, "parallelism": f"replicas x{world}, no collective"},
         "tflops": world * fl["total"] / (ms_per_step / 1e3) / 1e12,
         "frac_of_bf16_peak": {"measured_burst": fl["total"] / (ms_per_step / 1e3) / 1e12 / pk["tensor_burst"],
                               "measured_sustained": fl["total"] / (ms_per_step / 1e3) / 1e12 / pk["tensor_sustained"],
@@ -399,6 +404,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (2 = 120B shape, fwd+bwd)")
     ap.add_argument("--gemm-impl", type=int, default=0)
+    ap.add_argument("--route-impl", type=int, default=0, help="0 library's choice, 1 dense fp32 chain, 2 screened router (see tqp_route_info)")
     ap.add_argument("--format", default="vq", choices=["vq", "tq"], help="frozen-base format: BASELINE.json's VQ (default) or TurboQuant-MSE")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

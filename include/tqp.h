@@ -87,7 +87,7 @@ tqp_status tqp_bind_weights(tqp_ctx *ctx, const tqp_weights *w, void *stream);
  * (default), 1 = CUDA-core scaffold (test reference), 2 = tcgen05 grouped GEMM, one CTA per tile, weight operand
  * through shared memory (fallback for M % 256 != 0), 3 = CTA pairs, weight operand through shared memory (fallback for
  * K % 128 != 0).
- * "time_gemm": 0/1, see tqp_gemm_time.  "host_chunks": 0 (default) lets tqp_step_host_async choose at run time
+ * "route_impl": 0..3, see tqp_route_info.  "time_gemm": 0/1, see tqp_gemm_time.  "host_chunks": 0 (default) lets tqp_step_host_async choose at run time
  * whether X goes up and is routed in one piece or in four token chunks; 1 / 4 pin the choice (same results).  Unknown names return TQP_ERR_ARG.  (Kernel instrumentation -- "trace",
  * "ablate" -- exists only in builds compiled with -DTQP_TRACE and is not part of this interface.) */
 tqp_status tqp_set_option(tqp_ctx *ctx, const char *name, int value);
@@ -99,6 +99,15 @@ tqp_status tqp_set_option(tqp_ctx *ctx, const char *name, int value);
  * NULL; topk_idx int32 [T][k]; topk_w fp32 [T][k]; logits_out fp32 [T][E] or NULL. */
 tqp_status tqp_route(tqp_ctx *ctx, int T, const void *X, const float *W_r, const float *logit_bias,
                      int32_t *topk_idx, float *topk_w, float *logits_out, void *stream);
+/* How the last tqp_route of this ctx ran (synchronises `stream`).  *screened = 1: the screened router (needs
+ * logits_out == NULL, d % 128 == 0, E <= 1024, k <= 32 and X 16-byte aligned; option "route_impl" 0, the default, takes it
+ * where it is the faster one -- E > 6 (k + 4) and T E d >= 3e9 --, 2 wherever it can run):
+ * approximate logits on the tensor cores with a proven error bound, the canonical fmaf chain only for the experts within
+ * that bound of a token's k-th largest, top-k and softmax on those exact values -- topk_idx and topk_w are bit-identical
+ * to the dense chain (R1, section 6).  *fallback = 1: the screen's self-check tripped (or a token had more than
+ * 64 candidates, e.g. an all-zero row) and the dense chain recomputed the call behind it; the results are the same.
+ * "route_impl" 1 = always the dense chain; 3 = as 2 with the self-check forced to fail (exercises the fallback). */
+tqp_status tqp_route_info(tqp_ctx *ctx, int *screened, int *fallback, void *stream);
 /* Stable counting sort of a = t*k+j by expert id ("expert dispatch").  counts int32 [E];
  * offsets int32 [E+1] (exclusive scan, offsets[E] = N); perm int32 [N]; inv_perm int32 [N].  Also builds
  * the grouped-GEMM tile list inside the workspace. */

@@ -83,6 +83,7 @@ def load_library() -> ctypes.CDLL:
         lib.tqp_bind_weights.argtypes = [vp, ctypes.POINTER(Weights), vp]
         lib.tqp_set_option.argtypes = [vp, ctypes.c_char_p, ci]
         lib.tqp_route.argtypes = [vp, ci] + [vp] * 7
+        lib.tqp_route_info.argtypes = [vp, ctypes.POINTER(ci), ctypes.POINTER(ci), vp]
         lib.tqp_dispatch.argtypes = [vp, ci] + [vp] * 6
         lib.tqp_expert_fwd.argtypes = [vp, ci] + [vp] * 5
         lib.tqp_combine.argtypes = [vp, ci] + [vp] * 5
@@ -216,6 +217,12 @@ class TqpLayer:
         self._check(self.lib.tqp_route(self.ctx, T, _ptr(X), _ptr(W_r), _ptr(logit_bias), _ptr(idx), _ptr(w), _ptr(lg),
                                        self._stream()))
         return (idx, w, lg) if want_logits else (idx, w)
+
+    def route_info(self):
+        """(screened, fallback) of the last route() on this layer: see tqp_route_info in include/tqp.h."""
+        a, b = ctypes.c_int(0), ctypes.c_int(0)
+        self._check(self.lib.tqp_route_info(self.ctx, ctypes.byref(a), ctypes.byref(b), self._stream()))
+        return a.value, b.value
 
     def dispatch(self, topk_idx):
         t = self.torch

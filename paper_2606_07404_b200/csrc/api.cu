@@ -45,6 +45,9 @@ Workspace layout(const tqp_layer_desc &d) {
     w.lut = take(256 * 8 * 2);
     w.sc2 = take(E * (dm + 2 * F) * 4);   // bf16-pair copies of scale_down | scale_gate | scale_up for the backward GEMMs
     w.WrT = take(E * dm * 4);
+    w.WrHL = take(E * dm * 4);   // bf16 hi | lo split of W_r^T, [E][2d] (screened router)
+    w.wnorm = take(E * 4);
+    w.rflag = take(16);
     w.dl = take(N * 4);
     w.trace = take(16384 * 8);
     w.total = off;
@@ -418,6 +421,11 @@ extern "C" {
 
 tqp_status tqp_set_option(tqp_ctx *c, const char *name, int value) {
     if (!c || !name) return TQP_ERR_ARG;
+    if (!strcmp(name, "route_impl")) {
+        REQ(c, value >= 0 && value <= 3, TQP_ERR_ARG, "route_impl must be 0..3");
+        c->route_impl = value;
+        return TQP_OK;
+    }
     if (!strcmp(name, "gemm_impl")) {
         REQ(c, value >= 0 && value <= 3, TQP_ERR_ARG, "gemm_impl must be 0..3");
         c->gemm_impl = value;
@@ -457,8 +465,31 @@ tqp_status tqp_route(tqp_ctx *c, int T, const void *X, const float *W_r, const f
     tqp_status st = common_checks(c, T, false);
     if (st != TQP_OK) return st;
     PTR_OK(c, X); PTR_OK(c, W_r); PTR_OK(c, topk_idx); PTR_OK(c, topk_w);
+    if (!logits_out && c->route_impl != 1 && route_screen_applicable(c, T, c->route_impl >= 2) && ((uintptr_t)X & 15) == 0) {
+        CUtensorMap mx, mw;
+        st = act_map(c, &mx, X, (uint64_t)T, c->desc.d, 128);
+        if (st == TQP_OK) st = act_map(c, &mw, c->p<bf16>(c->ws.WrHL), (uint64_t)c->desc.E, 2 * (uint64_t)c->desc.d, 256);
+        if (st != TQP_OK) return st;
+        c->last_route_screened = 1;
+        return launch_route_screened(c, T, (const bf16 *)X, W_r, logit_bias, topk_idx, topk_w, &mx, &mw, (cudaStream_t)stream);
+    }
+    c->last_route_screened = 0;
     float *lg = logits_out ? logits_out : c->p<float>(c->ws.logits);
     return launch_route(c, T, (const bf16 *)X, W_r, logit_bias, topk_idx, topk_w, lg, (cudaStream_t)stream);
+}
+
+tqp_status tqp_route_info(tqp_ctx *c, int *screened, int *fallback, void *stream) {
+    if (!c) return TQP_ERR_ARG;
+    REQ(c, c->base != nullptr, TQP_ERR_WORKSPACE, "no workspace bound");
+    if (screened) *screened = c->last_route_screened;
+    if (fallback) {
+        *fallback = 0;
+        if (c->last_route_screened) {
+            TQP_CUDA_OK(c, cudaMemcpyAsync(fallback, c->p<int>(c->ws.rflag), sizeof(int), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+            TQP_CUDA_OK(c, cudaStreamSynchronize((cudaStream_t)stream));
+        }
+    }
+    return TQP_OK;
 }
 
 tqp_status tqp_dispatch(tqp_ctx *c, int T, const int32_t *topk_idx, int32_t *counts, int32_t *offsets, int32_t *perm,
@@ -807,7 +838,6 @@ tqp_status tqp_step_host_async(tqp_ctx *c, int T, const void *X_host, const void
         // "host_chunks" = 1 / 4 pins the choice for tests.)
         const bool behind = c->host_seq >= 1 && cudaEventQuery(c->ev_comp[par ^ 1]) == cudaErrorNotReady;
         const int nch = c->host_chunks ? c->host_chunks : (T >= 1024 && !behind) ? 4 : 1, per = ((T + nch - 1) / nch + 3) & ~3;   // chunk starts stay 16-byte aligned in every array
-        float *lg = c->p<float>(c->ws.logits);
         for (int ch = 0; ch < nch; ++ch) {
             const int t0 = ch * per, tc = std::min(per, T - t0);
             if (tc <= 0) break;
@@ -815,7 +845,7 @@ tqp_status tqp_step_host_async(tqp_ctx *c, int T, const void *X_host, const void
             TQP_CUDA_OK(c, cudaMemcpyAsync(X + eo, (const bf16 *)X_host + eo, (size_t)tc * D.d * 2, cudaMemcpyHostToDevice, c->copy_in));
             TQP_CUDA_OK(c, cudaEventRecord(c->ev_xc[ch], c->copy_in));
             TQP_CUDA_OK(c, cudaStreamWaitEvent(s, c->ev_xc[ch], 0));
-            CK(tqp_route(c, tc, X + eo, W_r, logit_bias, ti + (size_t)t0 * D.k, tw + (size_t)t0 * D.k, lg + (size_t)t0 * D.E, s));
+            CK(tqp_route(c, tc, X + eo, W_r, logit_bias, ti + (size_t)t0 * D.k, tw + (size_t)t0 * D.k, nullptr, s));
         }
     }
     TQP_CUDA_OK(c, cudaMemcpyAsync(dY, dY_host, row_bytes, cudaMemcpyHostToDevice, c->copy_in));

@@ -96,7 +96,7 @@ struct Workspace {
     size_t total = 0;        // the caller's workspace
     size_t host_total = 0;   // tqp_step_host staging (library-owned, allocated on first use)
     // offsets (bytes) into the bound buffer
-    size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, xsegs, xfirst, wg_scratch, sched, lut, sc2, WrT, dl,
+    size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, xsegs, xfirst, wg_scratch, sched, lut, sc2, WrT, WrHL, wnorm, rflag, dl,
         // tqp_step_host staging
         trace, hX, hdY, hX2, hdY2, hY, hdX, topk_idx, topk_w, counts, offsets, perm, inv_perm, Ye, dYe, dXp, dtopk_w;
 };
@@ -111,6 +111,8 @@ struct tqp_ctx {
     size_t bound_bytes = 0;
     tqp_weights w;
     bool have_weights = false;
+    int last_route_screened = 0;
+    int route_impl = 0;         // 0 screened router where it pays, 1 dense exact chain, 2 screened wherever applicable, 3 = 2 with the self-check forced to fail
     int gemm_impl = 0;          // 0 tcgen05 CTA-pair kernel, 1 scaffold, 2 tcgen05 single-CTA kernel
     int fwd_T = -1;             // T of the last training-mode expert_fwd (TQP_ERR_STATE check)
     int disp_T = -1;
@@ -172,8 +174,14 @@ namespace tqp {
     } while (0)
 
 // ---- kernels.cu ----------------------------------------------------------------------------------------
+// gate (device int, or NULL): when given, both kernels return at once unless *gate != 0
 tqp_status launch_route(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const float *bias, int32_t *topk_idx,
-                        float *topk_w, float *logits, cudaStream_t s);
+                        float *topk_w, float *logits, cudaStream_t s, const int *gate = nullptr);
+// Screened router (route.cu): same results as launch_route, bit for bit; mapX = X as bf16 [T][d], box {64, 128}, mapW = the
+// bf16 hi|lo split of W_r^T in the workspace [E][2d], box {64, 256}, both SWIZZLE_128B.
+bool route_screen_applicable(const tqp_ctx *c, int T, bool forced);
+tqp_status launch_route_screened(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const float *bias, int32_t *topk_idx,
+                                 float *topk_w, const CUtensorMap *mapX, const CUtensorMap *mapW, cudaStream_t s);
 tqp_status launch_dispatch(tqp_ctx *c, int T, const int32_t *topk_idx, int32_t *counts, int32_t *offsets,
                            int32_t *perm, int32_t *inv_perm, cudaStream_t s);
 tqp_status launch_gather_rows(tqp_ctx *c, int N, const bf16 *X, const int32_t *perm, bf16 *Xp, cudaStream_t s);

@@ -42,7 +42,7 @@ def make_layer(inp, T_max=None, training=True, gemm_impl=0):
     return layer, dev
 
 
-def run_gpu(inp, backward=True, router_grad=False, gemm_impl=0, keep_dev=False, fused_bwd=True):
+def run_gpu(inp, backward=True, router_grad=False, gemm_impl=0, keep_dev=False, fused_bwd=True, route_impl=0):
     """The whole chain through the C ABI; returns fp32/int numpy arrays keyed like oracle.layer().  fused_bwd: the call
     sequence bench.py times (tqp_combine_bwd with perm, tqp_expert_bwd with TQP_BWD_DYE_UNMODIFIED); False: the plain
     combine_bwd kernel and an expert_bwd that trusts nothing from earlier calls."""
@@ -52,7 +52,15 @@ def run_gpu(inp, backward=True, router_grad=False, gemm_impl=0, keep_dev=False, 
     N = T * k
     out = {}
     bias = dev.get("logit_bias")
-    idx, w, lg = layer.route(dev["X"], dev["W_r"], bias, want_logits=True)
+    # the dense canonical chain (logits requested) and the call bench.py makes (no logits: the screened router where the
+    # library picks it) must agree bit for bit; the rest of the chain runs on the second call's outputs
+    idx_d, w_d, lg = layer.route(dev["X"], dev["W_r"], bias, want_logits=True)
+    assert layer.route_info() == (0, 0)
+    layer.set_option("route_impl", route_impl)
+    idx, w = layer.route(dev["X"], dev["W_r"], bias)
+    out_info = layer.route_info()
+    assert torch.equal(idx, idx_d), "topk_idx: screened router differs from the dense chain"
+    assert torch.equal(w.view(torch.int32), w_d.view(torch.int32)), "topk_w: screened router differs from the dense chain (bitwise)"
     counts, offsets, perm, inv = layer.dispatch(idx)
     Ye = layer.expert_fwd(dev["X"], offsets, perm)
     Y = layer.combine(Ye, inv, w)
@@ -73,6 +81,7 @@ def run_gpu(inp, backward=True, router_grad=False, gemm_impl=0, keep_dev=False, 
             res["dX"] = dX
     torch.cuda.synchronize()
     out = {key: to_np(v) for key, v in res.items()}
+    out["route_info"] = out_info   # (screened, fallback) of the second route call
     if keep_dev:
         out["_layer"], out["_dev"], out["_res"] = layer, dev, res
     return out
