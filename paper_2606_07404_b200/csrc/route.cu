@@ -351,7 +351,7 @@ constexpr int RS_A_BYTES = RS_BM * RS_BK * 2, RS_B_BYTES = RS_BN * RS_BK * 2, RS
 constexpr int RS_TC_SMEM = RS_STAGES * RS_STAGE_BYTES + 1024 + 256;
 constexpr int RS_CMAX = 64;   // candidates per token held by the screen (two per lane)
 constexpr int RS_ROWS = 24, RS_KC = 64, RS_LD = RS_KC + 4;   // candidate rows per chain batch, columns per chunk, floats per tile row
-constexpr int RS_WARP_SMEM = 2 * RS_ROWS * RS_LD * 4 + 2 * RS_KC * 2 + RS_KC * 4 + 2 * RS_CMAX * 4;   // per warp of route_screen_kernel
+constexpr int RS_WARP_SMEM = 2 * RS_ROWS * RS_LD * 4 + 2 * RS_KC * 2 + 2 * RS_CMAX * 4;   // per warp of route_screen_kernel
 
 // W_r [d][E] fp32 -> WrT [E][d] fp32 (rows of the candidate chains) and WrHL [E][2d] bf16 (hi | lo, K-major MMA operand)
 __global__ void __launch_bounds__(256) route_prep_kernel(const float *__restrict__ W_r, float *__restrict__ WrT, bf16 *__restrict__ WrHL,
@@ -484,9 +484,8 @@ __global__ void __launch_bounds__(128) route_screen_kernel(const float *__restri
     if (t >= T) return;   // warp-uniform; nothing below synchronises the block
     uint8_t *wsm = rs_sm + (size_t)wib * RS_WARP_SMEM;
     const uint32_t tile_s = ptx::smem_u32(wsm);                       // [2][RS_ROWS][RS_LD] fp32 (rows padded by 16 bytes: conflict-free)
-    const uint32_t xb_s = tile_s + 2 * RS_ROWS * RS_LD * 4;          // [2][64] bf16: the token's chunk as it comes from X
-    float *xf = reinterpret_cast<float *>(wsm + 2 * RS_ROWS * RS_LD * 4 + 2 * RS_KC * 2);   // [64] fp32: the same, widened
-    int *cl_e = reinterpret_cast<int *>(xf + RS_KC);
+    const uint32_t xb_s = tile_s + 2 * RS_ROWS * RS_LD * 4;          // [2][RS_KC] bf16: the token's chunk as it comes from X
+    int *cl_e = reinterpret_cast<int *>(wsm + 2 * RS_ROWS * RS_LD * 4 + 2 * RS_KC * 2);
     float *cl_v = reinterpret_cast<float *>(cl_e + RS_CMAX);         // approximate value, replaced by the exact one
 
     // |x_t|^2
@@ -553,47 +552,49 @@ __global__ void __launch_bounds__(128) route_screen_kernel(const float *__restri
     // canonical chains (R1): acc = fmaf(x_i, W_r[i][e], acc), i ascending, then + bias.  Lane = candidate; the
     // candidates' rows of W_r^T come in 64-column chunks, two rows per warp-wide cp.async (a half-warp covers 256 contiguous
     // bytes; a lane streaming its own row with 16-byte loads costs one L1 tag cycle per lane and load: 376 us at cfg 2),
-    // double-buffered in shared memory.
-    const int half = lane >> 4, q = lane & 15;
+    // double-buffered in shared memory; the token's bf16 chunk rides along and is widened in the lane (a shift / a mask).
+    constexpr int LPR = RS_KC / 4, RPI = 32 / LPR;   // lanes per row chunk (16 bytes each), rows per warp-wide cp.async
+    const int sub = lane / LPR, q = lane % LPR;
     for (int b = 0; b < count; b += RS_ROWS) {
         const int nb = min(RS_ROWS, count - b);
-        // row 2 r + half: its chunk column in W_r^T (advanced by two chunks per trip) and its place in buffer 0
-        const float *gp[RS_ROWS / 2];
-        bool on[RS_ROWS / 2];
+        // row RPI r + sub: its chunk column in W_r^T (advanced by two chunks per trip) and its place in buffer 0
+        const float *gp[RS_ROWS / RPI];
+        bool on[RS_ROWS / RPI];
 #pragma unroll
-        for (int r = 0; r < RS_ROWS / 2; ++r) {
-            const int row = 2 * r + half;
-            on[r] = 2 * r < nb;   // warp-uniform: with an odd nb the last pair fetches the last candidate's row twice
+        for (int r = 0; r < RS_ROWS / RPI; ++r) {
+            const int row = RPI * r + sub;
+            on[r] = RPI * r < nb;   // warp-uniform: past nb the last group fetches the last candidate's row again
             gp[r] = WrT + (size_t)(on[r] ? cl_e[b + min(row, nb - 1)] : 0) * d + q * 4;
         }
-        const uint32_t dst0 = tile_s + (uint32_t)(half * RS_LD * 4 + q * 16);
+        const uint32_t dst0 = tile_s + (uint32_t)(sub * RS_LD * 4 + q * 16);
         const bf16 *xp = X + (size_t)t * d + lane * 8;
         const uint32_t rowa = tile_s + (uint32_t)(lane * RS_LD * 4);
         float acc = 0.f;
 #define RS_ISSUE(BUF, OFF)                                                                                                         \
     do {                                                                                                                           \
-        _Pragma("unroll") for (int r = 0; r < RS_ROWS / 2; ++r) if (on[r])                                                         \
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst0 + (uint32_t)(((BUF) * RS_ROWS + 2 * r) * RS_LD * 4)), \
+        _Pragma("unroll") for (int r = 0; r < RS_ROWS / RPI; ++r) if (on[r])                                                       \
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst0 + (uint32_t)(((BUF) * RS_ROWS + RPI * r) * RS_LD * 4)), \
                          "l"(gp[r] + (OFF)) : "memory");                                                                           \
-        if (lane < 8)                                                                                                              \
+        if (lane < RS_KC / 8)                                                                                                      \
             asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(xb_s + (BUF) * RS_KC * 2 + lane * 16), "l"(xp + (OFF)) : "memory"); \
         asm volatile("cp.async.commit_group;" ::: "memory");                                                                       \
     } while (0)
 #define RS_CHUNK(BUF)                                                                                                              \
     do {                                                                                                                           \
         __syncwarp();                                                                                                              \
-        if (lane < 16) {                                                                                                           \
-            const uint2 u = ptx::lds64(xb_s + (BUF) * RS_KC * 2 + lane * 8);                                                       \
-            const float2 f0 = bf16x2_to_float2(u.x), f1 = bf16x2_to_float2(u.y);                                                   \
-            *reinterpret_cast<float4 *>(xf + 4 * lane) = make_float4(f0.x, f0.y, f1.x, f1.y);                                      \
-        }                                                                                                                          \
-        __syncwarp();                                                                                                              \
         if (lane < nb) {                                                                                                           \
-            _Pragma("unroll") for (int j = 0; j < 16; ++j) {                                                                       \
-                const uint4 wu = ptx::lds128(rowa + (uint32_t)((BUF) * RS_ROWS * RS_LD * 4 + j * 16));                              \
-                const float4 xv = *reinterpret_cast<const float4 *>(xf + 4 * j);                                                   \
-                acc = fmaf(xv.x, __uint_as_float(wu.x), acc); acc = fmaf(xv.y, __uint_as_float(wu.y), acc);                        \
-                acc = fmaf(xv.z, __uint_as_float(wu.z), acc); acc = fmaf(xv.w, __uint_as_float(wu.w), acc);                        \
+            _Pragma("unroll") for (int j = 0; j < RS_KC / 8; ++j) {   /* 8 bf16 of x (widened in the lane: a shift / a mask) x 8 of the row */ \
+                const uint4 xu = ptx::lds128(xb_s + (uint32_t)((BUF) * RS_KC * 2 + j * 16));                                       \
+                const uint4 w0 = ptx::lds128(rowa + (uint32_t)((BUF) * RS_ROWS * RS_LD * 4 + j * 32));                              \
+                const uint4 w1 = ptx::lds128(rowa + (uint32_t)((BUF) * RS_ROWS * RS_LD * 4 + j * 32 + 16));                         \
+                acc = fmaf(__uint_as_float(xu.x << 16), __uint_as_float(w0.x), acc);                                               \
+                acc = fmaf(__uint_as_float(xu.x & 0xffff0000u), __uint_as_float(w0.y), acc);                                       \
+                acc = fmaf(__uint_as_float(xu.y << 16), __uint_as_float(w0.z), acc);                                               \
+                acc = fmaf(__uint_as_float(xu.y & 0xffff0000u), __uint_as_float(w0.w), acc);                                       \
+                acc = fmaf(__uint_as_float(xu.z << 16), __uint_as_float(w1.x), acc);                                               \
+                acc = fmaf(__uint_as_float(xu.z & 0xffff0000u), __uint_as_float(w1.y), acc);                                       \
+                acc = fmaf(__uint_as_float(xu.w << 16), __uint_as_float(w1.z), acc);                                               \
+                acc = fmaf(__uint_as_float(xu.w & 0xffff0000u), __uint_as_float(w1.w), acc);                                       \
             }                                                                                                                      \
         }                                                                                                                          \
         __syncwarp();                                                                                                              \
