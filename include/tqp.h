@@ -184,7 +184,8 @@ tqp_status tqp_step_host_wait(tqp_ctx *ctx, int age);
  * logit bias".  logits as in tqp_route (canonical fmaf chain, NO bias added); selection = the k largest keys
  * logits[t][e] + select_bias[e] (fp32 add; ties -> lower id; select_bias fp32 [E] or NULL); topk_s[t][j] =
  * sigmoid(logit) of the UNBIASED selected logit; topk_w = topk_s / sum_j topk_s (summed in ascending j) -- DESIGN.md
- * R21, R22.  topk_idx int32 [T][k]; topk_w, topk_s fp32 [T][k]; logits_out fp32 [T][E] or NULL.  All DEVICE pointers. */
+ * R21, R22.  topk_idx int32 [T][k]; topk_w, topk_s fp32 [T][k]; logits_out fp32 [T][E] or NULL.  All DEVICE pointers.
+ * With logits_out == NULL the screened router runs under the same rule as in tqp_route (tqp_route_info reports it). */
 tqp_status tqp_route_sigmoid(tqp_ctx *ctx, int T, const void *X, const float *W_r, const float *select_bias,
                              int32_t *topk_idx, float *topk_w, float *topk_s, float *logits_out, void *stream);
 /* Router backward for tqp_route_sigmoid (selection held constant, the bias has no gradient):

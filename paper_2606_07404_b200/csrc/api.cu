@@ -471,7 +471,7 @@ tqp_status tqp_route(tqp_ctx *c, int T, const void *X, const float *W_r, const f
         if (st == TQP_OK) st = act_map(c, &mw, c->p<bf16>(c->ws.WrHL), (uint64_t)c->desc.E, 2 * (uint64_t)c->desc.d, 256);
         if (st != TQP_OK) return st;
         c->last_route_screened = 1;
-        return launch_route_screened(c, T, (const bf16 *)X, W_r, logit_bias, topk_idx, topk_w, &mx, &mw, (cudaStream_t)stream);
+        return launch_route_screened(c, T, (const bf16 *)X, W_r, logit_bias, topk_idx, topk_w, nullptr, &mx, &mw, (cudaStream_t)stream);
     }
     c->last_route_screened = 0;
     float *lg = logits_out ? logits_out : c->p<float>(c->ws.logits);
@@ -729,6 +729,15 @@ tqp_status tqp_route_sigmoid(tqp_ctx *c, int T, const void *X, const float *W_r,
     tqp_status st = common_checks(c, T, false);
     if (st != TQP_OK) return st;
     PTR_OK(c, X); PTR_OK(c, W_r); PTR_OK(c, topk_idx); PTR_OK(c, topk_w); PTR_OK(c, topk_s);
+    if (!logits_out && c->route_impl != 1 && route_screen_applicable(c, T, c->route_impl >= 2) && ((uintptr_t)X & 15) == 0) {
+        CUtensorMap mx, mw;
+        st = act_map(c, &mx, X, (uint64_t)T, c->desc.d, 128);
+        if (st == TQP_OK) st = act_map(c, &mw, c->p<bf16>(c->ws.WrHL), (uint64_t)c->desc.E, 2 * (uint64_t)c->desc.d, 256);
+        if (st != TQP_OK) return st;
+        c->last_route_screened = 1;
+        return launch_route_screened(c, T, (const bf16 *)X, W_r, select_bias, topk_idx, topk_w, topk_s, &mx, &mw, (cudaStream_t)stream);
+    }
+    c->last_route_screened = 0;
     float *lg = logits_out ? logits_out : c->p<float>(c->ws.logits);
     return launch_route_sigmoid(c, T, (const bf16 *)X, W_r, select_bias, topk_idx, topk_w, topk_s, lg, (cudaStream_t)stream);
 }

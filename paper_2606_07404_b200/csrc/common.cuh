@@ -181,7 +181,8 @@ tqp_status launch_route(tqp_ctx *c, int T, const bf16 *X, const float *W_r, cons
 // bf16 hi|lo split of W_r^T in the workspace [E][2d], box {64, 256}, both SWIZZLE_128B.
 bool route_screen_applicable(const tqp_ctx *c, int T, bool forced);
 tqp_status launch_route_screened(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const float *bias, int32_t *topk_idx,
-                                 float *topk_w, const CUtensorMap *mapX, const CUtensorMap *mapW, cudaStream_t s);
+                                 float *topk_w, float *topk_s /* non-NULL: sigmoid variant */, const CUtensorMap *mapX,
+                                 const CUtensorMap *mapW, cudaStream_t s);
 tqp_status launch_dispatch(tqp_ctx *c, int T, const int32_t *topk_idx, int32_t *counts, int32_t *offsets,
                            int32_t *perm, int32_t *inv_perm, cudaStream_t s);
 tqp_status launch_gather_rows(tqp_ctx *c, int N, const bf16 *X, const int32_t *perm, bf16 *Xp, cudaStream_t s);
@@ -196,7 +197,7 @@ tqp_status launch_route_bwd(tqp_ctx *c, int T, const bf16 *X, const float *W_r, 
                             const float *topk_w, const float *topk_s, const float *dtopk_w, const int32_t *offsets,
                             const int32_t *perm, bf16 *dX, float *dW_r, cudaStream_t s);
 tqp_status launch_route_sigmoid(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const float *select_bias, int32_t *topk_idx,
-                                float *topk_w, float *topk_s, float *logits, cudaStream_t s);
+                                float *topk_w, float *topk_s, float *logits, cudaStream_t s, const int *gate = nullptr);
 tqp_status launch_bias_update(tqp_ctx *c, const int32_t *counts, float *bias, int mode, float gamma, float cap_hi, float cap_lo,
                               cudaStream_t s);
 tqp_status launch_combine_dw(tqp_ctx *c, int T, const bf16 *dY, const bf16 *Ye, const int32_t *inv_perm, float *dtopk_w,

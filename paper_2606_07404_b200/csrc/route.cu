@@ -231,7 +231,8 @@ __global__ void __launch_bounds__(128) route_topk_kernel(const float *__restrict
 template <int PER>
 __global__ void __launch_bounds__(128) route_topk_sigmoid_kernel(const float *__restrict__ logits, const float *__restrict__ bias,
                                                                  int32_t *__restrict__ topk_idx, float *__restrict__ topk_w,
-                                                                 float *__restrict__ topk_s, int T, int E, int k) {
+                                                                 float *__restrict__ topk_s, int T, int E, int k, const int *__restrict__ gate) {
+    if (gate && *gate == 0) return;
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) / 32, lane = threadIdx.x % 32;
     if (warp >= T) return;
     const float *l = logits + (size_t)warp * E;
@@ -295,11 +296,11 @@ static void launch_logits(const bf16 *X, const float *W_r, const float *bias, fl
 }
 
 tqp_status launch_route_sigmoid(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const float *select_bias, int32_t *topk_idx,
-                                float *topk_w, float *topk_s, float *logits, cudaStream_t s) {
+                                float *topk_w, float *topk_s, float *logits, cudaStream_t s, const int *gate) {
     const int d = c->desc.d, E = c->desc.E, k = c->desc.k;
-    launch_logits(X, W_r, nullptr, logits, T, d, E, c->num_sms, s);
+    launch_logits(X, W_r, nullptr, logits, T, d, E, c->num_sms, s, gate);
     TQP_LAUNCH_OK(c);
-#define TQP_TOPK(P) route_topk_sigmoid_kernel<P><<<(T + 3) / 4, 128, 0, s>>>(logits, select_bias, topk_idx, topk_w, topk_s, T, E, k)
+#define TQP_TOPK(P) route_topk_sigmoid_kernel<P><<<(T + 3) / 4, 128, 0, s>>>(logits, select_bias, topk_idx, topk_w, topk_s, T, E, k, gate)
     if (E <= 64) TQP_TOPK(2); else if (E <= 128) TQP_TOPK(4); else if (E <= 256) TQP_TOPK(8); else if (E <= 512) TQP_TOPK(16); else TQP_TOPK(32);
 #undef TQP_TOPK
     TQP_LAUNCH_OK(c);
@@ -351,7 +352,7 @@ constexpr int RS_A_BYTES = RS_BM * RS_BK * 2, RS_B_BYTES = RS_BN * RS_BK * 2, RS
 constexpr int RS_TC_SMEM = RS_STAGES * RS_STAGE_BYTES + 1024 + 256;
 constexpr int RS_CMAX = 64;   // candidates per token held by the screen (two per lane)
 constexpr int RS_ROWS = 24, RS_KC = 64, RS_LD = RS_KC + 4;   // candidate rows per chain batch, columns per chunk, floats per tile row
-constexpr int RS_WARP_SMEM = 2 * RS_ROWS * RS_LD * 4 + 2 * RS_KC * 2 + 2 * RS_CMAX * 4;   // per warp of route_screen_kernel
+constexpr int RS_WARP_SMEM = 2 * RS_ROWS * RS_LD * 4 + 2 * RS_KC * 2 + 2 * RS_CMAX * 4;   // + RS_CMAX * 4 in the sigmoid variant   // per warp of route_screen_kernel
 
 // W_r [d][E] fp32 -> WrT [E][d] fp32 (rows of the candidate chains) and WrHL [E][2d] bf16 (hi | lo, K-major MMA operand)
 __global__ void __launch_bounds__(256) route_prep_kernel(const float *__restrict__ W_r, float *__restrict__ WrT, bf16 *__restrict__ WrHL,
@@ -473,20 +474,23 @@ __global__ void __launch_bounds__(192) route_tc_logits_kernel(const __grid_const
 }
 
 // One warp per token: candidates from the approximate logits, canonical chains for them, exact top-k + softmax.
-template <int PER>
+// SIG: the paper-faithful variant (route_topk_sigmoid_kernel): selection by logit + bias, gate = sigmoid of the UNBIASED logit
+// normalised over the selected set, topk_s = the sigmoid values.
+template <int PER, bool SIG>
 __global__ void __launch_bounds__(128) route_screen_kernel(const float *__restrict__ A, const bf16 *__restrict__ X, const float *__restrict__ WrT,
                                                            const float *__restrict__ wn, const float *__restrict__ bias,
-                                                           int32_t *__restrict__ topk_idx, float *__restrict__ topk_w, int *__restrict__ flag,
-                                                           int T, int d, int E, int k, float cK, float chk) {
+                                                           int32_t *__restrict__ topk_idx, float *__restrict__ topk_w, float *__restrict__ topk_s,
+                                                           int *__restrict__ flag, int T, int d, int E, int k, float cK, float chk) {
     extern __shared__ __align__(16) uint8_t rs_sm[];
     const int wib = threadIdx.x / 32, lane = threadIdx.x % 32;
     const int t = blockIdx.x * 4 + wib;
     if (t >= T) return;   // warp-uniform; nothing below synchronises the block
-    uint8_t *wsm = rs_sm + (size_t)wib * RS_WARP_SMEM;
+    uint8_t *wsm = rs_sm + (size_t)wib * (RS_WARP_SMEM + (SIG ? RS_CMAX * 4 : 0));
     const uint32_t tile_s = ptx::smem_u32(wsm);                       // [2][RS_ROWS][RS_LD] fp32 (rows padded by 16 bytes: conflict-free)
     const uint32_t xb_s = tile_s + 2 * RS_ROWS * RS_LD * 4;          // [2][RS_KC] bf16: the token's chunk as it comes from X
     int *cl_e = reinterpret_cast<int *>(wsm + 2 * RS_ROWS * RS_LD * 4 + 2 * RS_KC * 2);
     float *cl_v = reinterpret_cast<float *>(cl_e + RS_CMAX);         // approximate value, replaced by the exact one
+    float *cl_u = cl_v + RS_CMAX;                                    // SIG: the exact logit without the bias
 
     // |x_t|^2
     float ss = 0.f;
@@ -620,6 +624,7 @@ __global__ void __launch_bounds__(128) route_screen_kernel(const float *__restri
 #undef RS_CHUNK
         if (lane < nb) {
             const int e = cl_e[b + lane];
+            if (SIG) cl_u[b + lane] = acc;
             if (bias) acc = acc + bias[e];
             if (!(fabsf(acc - cl_v[b + lane]) <= chk * delta)) bad = true;   // cl_v held the approximate value until here
             cl_v[b + lane] = acc;
@@ -644,9 +649,26 @@ __global__ void __launch_bounds__(128) route_screen_kernel(const float *__restri
         if (ck[1] == m) cand = ce[1];
         if (ck[0] == m) cand = min(cand, ce[0]);
         const int e = __reduce_min_sync(0xffffffffu, cand);   // ties -> lower expert id
+        float u = 0.f;   // SIG: the winner's unbiased logit, from the lane that holds it
+        if (SIG) {
+            const float mine = ce[0] == e ? cl_u[lane] : ce[1] == e ? cl_u[32 + lane] : 0.f;
+            const uint32_t own = __ballot_sync(0xffffffffu, ce[0] == e || ce[1] == e);
+            u = __shfl_sync(0xffffffffu, mine, __ffs(own) - 1);
+        }
         if (ce[0] == e) ck[0] = 0u;
         if (ce[1] == e) ck[1] = 0u;
-        if (lane == j) { sel_l = key_value(m); sel_e = e; }
+        if (lane == j) { sel_l = SIG ? u : key_value(m); sel_e = e; }
+    }
+    if (SIG) {
+        const float sc = (lane < k) ? 1.f / (1.f + expf(-sel_l)) : 0.f;
+        float ssum = 0.f;
+        for (int j = 0; j < k; ++j) ssum = ssum + __shfl_sync(0xffffffffu, sc, j);
+        if (lane < k) {
+            topk_idx[(size_t)t * k + lane] = sel_e;
+            topk_s[(size_t)t * k + lane] = sc;
+            topk_w[(size_t)t * k + lane] = sc / ssum;
+        }
+        return;
     }
     const float m0 = __shfl_sync(0xffffffffu, sel_l, 0);
     const float ex = (lane < k) ? expf(sel_l - m0) : 0.f;
@@ -669,7 +691,8 @@ bool route_screen_applicable(const tqp_ctx *c, int T, bool forced) {
 }
 
 tqp_status launch_route_screened(tqp_ctx *c, int T, const bf16 *X, const float *W_r, const float *bias, int32_t *topk_idx,
-                                 float *topk_w, const CUtensorMap *mapX, const CUtensorMap *mapW, cudaStream_t s) {
+                                 float *topk_w, float *topk_s, const CUtensorMap *mapX, const CUtensorMap *mapW, cudaStream_t s) {
+    const bool sig = topk_s != nullptr;
     const int d = c->desc.d, E = c->desc.E, k = c->desc.k;
     float *WrT = c->p<float>(c->ws.WrT), *wn = c->p<float>(c->ws.wnorm), *A = c->p<float>(c->ws.logits);
     bf16 *WrHL = c->p<bf16>(c->ws.WrHL);
@@ -683,16 +706,22 @@ tqp_status launch_route_screened(tqp_ctx *c, int T, const bf16 *X, const float *
     TQP_LAUNCH_OK(c);
     const float cK = ((float)d * 4.76837158e-7f + 1.52587891e-5f) * 1.01f;   // d 2^-21 + 2^-16
     const float chk = c->route_impl == 3 ? -1.f : 0.5f;
-    const int smem = 4 * RS_WARP_SMEM;
+    const int smem = 4 * (RS_WARP_SMEM + (sig ? RS_CMAX * 4 : 0));
 #define TQP_SCREEN(P)                                                                                                     \
     do {                                                                                                                  \
-        if (tqp_status st = ensure_dyn_smem(c, reinterpret_cast<const void *>(&route_screen_kernel<P>), smem)) return st; \
-        route_screen_kernel<P><<<(T + 3) / 4, 128, smem, s>>>(A, X, WrT, wn, bias, topk_idx, topk_w, flag, T, d, E, k, cK, chk); \
+        if (sig) {                                                                                                        \
+            if (tqp_status st = ensure_dyn_smem(c, reinterpret_cast<const void *>(&route_screen_kernel<P, true>), smem)) return st; \
+            route_screen_kernel<P, true><<<(T + 3) / 4, 128, smem, s>>>(A, X, WrT, wn, bias, topk_idx, topk_w, topk_s, flag, T, d, E, k, cK, chk); \
+        } else {                                                                                                          \
+            if (tqp_status st = ensure_dyn_smem(c, reinterpret_cast<const void *>(&route_screen_kernel<P, false>), smem)) return st; \
+            route_screen_kernel<P, false><<<(T + 3) / 4, 128, smem, s>>>(A, X, WrT, wn, bias, topk_idx, topk_w, nullptr, flag, T, d, E, k, cK, chk); \
+        }                                                                                                                 \
     } while (0)
     if (E <= 64) TQP_SCREEN(2); else if (E <= 128) TQP_SCREEN(4); else if (E <= 256) TQP_SCREEN(8); else if (E <= 512) TQP_SCREEN(16); else TQP_SCREEN(32);
 #undef TQP_SCREEN
     TQP_LAUNCH_OK(c);
     // the dense exact kernels behind the flag: two empty launches unless the self-check tripped
+    if (sig) return launch_route_sigmoid(c, T, X, W_r, bias, topk_idx, topk_w, topk_s, A, s, flag);
     return launch_route(c, T, X, W_r, bias, topk_idx, topk_w, A, s, flag);
 }
 

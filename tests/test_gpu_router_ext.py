@@ -36,6 +36,34 @@ def test_route_sigmoid_bit_exact_selection(cfg_id, with_bias):
     np.testing.assert_allclose(to_np(w).sum(1), 1.0, atol=2e-6)
 
 
+@pytest.mark.parametrize("cfg_id,with_bias,impl", [(0, True, 2), (2, True, 0), (2, False, 2), (3, True, 2), (2, True, 3)])
+def test_route_sigmoid_screened_matches_dense_and_oracle(cfg_id, with_bias, impl):
+    """The screened router (csrc/route.cu) in its sigmoid variant: no logits requested -> tensor-core screen + canonical
+    chains for the candidates; idx / w / s bitwise equal to the dense chain's and idx equal to the oracle's.  impl 3 forces
+    the self-check to fail (the gated dense sigmoid kernels must then produce the result)."""
+    import torch
+    cfg = ti.CONFIGS[cfg_id]
+    inp = ti.make_inputs(cfg)
+    if cfg_id == 0:
+        inp["W_r"][:, 5] = inp["W_r"][:, 1]          # exact ties
+    layer, dev = make_layer(inp, training=False)
+    bias = _bias(cfg.E, 33) if with_bias else None
+    bdev = torch.from_numpy(bias).cuda() if with_bias else None
+    Wd = torch.from_numpy(inp["W_r"]).cuda()
+    layer.set_option("route_impl", 1)
+    i1, w1, s1 = layer.route_sigmoid(dev["X"], Wd, bdev)
+    assert layer.route_info() == (0, 0)
+    layer.set_option("route_impl", impl)
+    i2, w2, s2 = layer.route_sigmoid(dev["X"], Wd, bdev)
+    assert layer.route_info() == (1, 1 if impl == 3 else 0)
+    assert torch.equal(i1, i2)
+    assert torch.equal(w1.view(torch.int32), w2.view(torch.int32)) and torch.equal(s1.view(torch.int32), s2.view(torch.int32))
+    lg_ref = oracle.logits(inp["X"], inp["W_r"], None)
+    i_ref, w_ref, s_ref = rx.route_sigmoid(lg_ref, bias, cfg.k)
+    np.testing.assert_array_equal(to_np(i2), i_ref)
+    assert np.abs(to_np(w2) - w_ref).max() <= 1e-6 and np.abs(to_np(s2) - s_ref).max() <= 1e-6
+
+
 def test_route_sigmoid_backward_and_chain():
     """cfg 0 with sigmoid routing through the whole chain: Y against the oracle's expert path fed the oracle's routing,
     then dtopk_w -> dl -> dX, dW_r."""
