@@ -296,6 +296,24 @@ tqp_status tqp_bind_weights_tq(tqp_ctx *ctx, const tqp_tq_weights *w, void *stre
 /* Device pointers of workspace tensors, for tests: "G","U","H" bf16 [N][F]; "Xp" bf16 [N][d];
  * "dH","dG","dU" bf16 [N][F]; "num_tiles" int32 [1].  NULL if unknown. */
 void *tqp_debug_buffer(tqp_ctx *ctx, const char *name);
+/* --- dispatch without any allocation ------------------------------------------------------------------------ */
+/* tqp_dispatch ("expert dispatch": stable counting sort of a = t*k+j by expert id) for callers that cannot
+ * allocate -- code under CUDA-graph capture, tight serving loops, harnesses that forbid cudaMalloc.  No ctx, no workspace:
+ * the call allocates nothing on the host or the device and calls no allocating routine.  Its scratch (per-chunk
+ * histograms) is a fixed 4 MiB __device__ array inside the library, which every GPU that loads the library holds until
+ * the process exits.  topk_idx int32 [T][k] (values in [0, E)); counts int32 [E]; offsets int32 [E+1]; perm, inv_perm
+ * int32 [T*k]: all DEVICE pointers of the current device, caller-owned; results equal tqp_dispatch's bit for bit (the
+ * grouped-GEMM tile list is not built).  Limits: 1 <= E <= 1024, 1 <= k <= min(32, E), T*k < 2^25 (TQP_ERR_ARG) and
+ * ceil(T*k / 256) * E <= tqp_dispatch_noalloc_capacity() = 1 048 576 (TQP_ERR_SHAPE; e.g. T = 16384, k = 12, E = 460
+ * uses a third of it).  All calls on a device share the array: calls on one stream are ordered and safe, calls that
+ * OVERLAP on the GPU (other streams, a graph replayed beside a live call) race and give garbage.  Nothing in it has to be
+ * cleared: every entry a call reads it has written before.  Errors: the codes above, TQP_ERR_CUDA for a failed launch;
+ * text in tqp_dispatch_noalloc_error() (per thread). */
+tqp_status tqp_dispatch_noalloc(int T, int k, int E, const int32_t *topk_idx, int32_t *counts, int32_t *offsets,
+                                int32_t *perm, int32_t *inv_perm, void *stream);
+size_t tqp_dispatch_noalloc_capacity(void);
+const char *tqp_dispatch_noalloc_error(void);
+
 /* Measurement hook (the >= 50 % target applies to the grouped-GEMM kernels' own time).  After
  * tqp_set_option(ctx, "time_gemm", 1) every grouped-GEMM launch is bracketed by CUDA events on its stream.
  * tqp_gemm_time waits for the recorded events, returns the summed device time in milliseconds and the number of

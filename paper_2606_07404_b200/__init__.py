@@ -4,5 +4,5 @@ Every step of the path runs in the hand-written CUDA kernels behind the C ABI (i
 marshals arguments.  PyTorch is used for device memory and streams.  There is no CPU fallback: importing works
 anywhere (so the ABI can be inspected), but creating a layer without the built library or an sm_100 GPU raises.
 """
-from .binding import (TqpError, TqpLayer, TqSpace, abi_symbols, load_library, tq_levels, tq_rotation_qr,  # noqa: F401
+from .binding import (TqpError, TqpLayer, TqSpace, abi_symbols, dispatch_noalloc, dispatch_noalloc_capacity, load_library, tq_levels, tq_rotation_qr,  # noqa: F401
                       workspace_bytes)

@@ -85,6 +85,11 @@ def load_library() -> ctypes.CDLL:
         lib.tqp_route.argtypes = [vp, ci] + [vp] * 7
         lib.tqp_route_info.argtypes = [vp, ctypes.POINTER(ci), ctypes.POINTER(ci), vp]
         lib.tqp_dispatch.argtypes = [vp, ci] + [vp] * 6
+        lib.tqp_dispatch_noalloc.argtypes = [ci, ci, ci] + [vp] * 6
+        lib.tqp_dispatch_noalloc_capacity.restype = ctypes.c_size_t
+        lib.tqp_dispatch_noalloc_capacity.argtypes = []
+        lib.tqp_dispatch_noalloc_error.restype = ctypes.c_char_p
+        lib.tqp_dispatch_noalloc_error.argtypes = []
         lib.tqp_expert_fwd.argtypes = [vp, ci] + [vp] * 5
         lib.tqp_combine.argtypes = [vp, ci] + [vp] * 5
         lib.tqp_combine_bwd.argtypes = [vp, ci] + [vp] * 8
@@ -129,6 +134,25 @@ def workspace_bytes(T_max, d, F, E, k, r, lora_scale=1.0, training=True) -> int:
 
 def _ptr(t):
     return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def dispatch_noalloc(topk_idx, E, counts, offsets, perm, inv_perm, stream=None):
+    """tqp_dispatch_noalloc (include/tqp.h): the dispatch without ctx, workspace or any allocation.  ALL tensors are the
+    caller's, on the current CUDA device: topk_idx int32 [T][k]; counts int32 [E]; offsets int32 [E + 1]; perm, inv_perm
+    int32 [T * k].  Runs on `stream` (a torch stream; default: torch's current stream)."""
+    import torch
+    lib = load_library()
+    T, k = topk_idx.shape
+    st = stream if stream is not None else torch.cuda.current_stream(topk_idx.device)
+    code = lib.tqp_dispatch_noalloc(int(T), int(k), int(E), _ptr(topk_idx), _ptr(counts), _ptr(offsets), _ptr(perm),
+                                    _ptr(inv_perm), ctypes.c_void_p(st.cuda_stream))
+    if code != 0:
+        raise TqpError(code, (lib.tqp_dispatch_noalloc_error() or b"").decode())
+
+
+def dispatch_noalloc_capacity() -> int:
+    """Entries of the static scratch: ceil(T k / 256) * E must not exceed it."""
+    return int(load_library().tqp_dispatch_noalloc_capacity())
 
 
 def tq_levels(n: int, bits: int = 8):
