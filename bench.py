@@ -235,6 +235,9 @@ def run_ours(args, cfg):
         layer.set_option("gemm_impl", args.gemm_impl)
     if args.route_impl:
         layer.set_option("route_impl", args.route_impl)
+    for kv in args.opt:   # any other library option (tqp_set_option), e.g. --opt fuse_dgu=0
+        name, _, val = kv.partition("=")
+        layer.set_option(name, int(val))
 
     def up(a):
         t = torch.from_numpy(a.view(np.int16)).view(torch.bfloat16) if a.dtype == np.uint16 else torch.from_numpy(a)
@@ -404,6 +407,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (2 = 120B shape, fwd+bwd)")
     ap.add_argument("--gemm-impl", type=int, default=0)
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=INT", help="library option passed to tqp_set_option (repeatable)")
     ap.add_argument("--route-impl", type=int, default=0, help="0 library's choice, 1 dense fp32 chain, 2 screened router (see tqp_route_info)")
     ap.add_argument("--format", default="vq", choices=["vq", "tq"], help="frozen-base format: BASELINE.json's VQ (default) or TurboQuant-MSE")
     ap.add_argument("--no-e2e", action="store_true")

@@ -38,10 +38,13 @@ Workspace layout(const tqp_layer_desc &d) {
     w.num_tiles = take(16);
     w.xsegs = take((N / kWgradSeg + 2) * sizeof(Tile));
     w.xfirst = take((E + 1) * 4);
+    w.tfirst = take((E + 1) * 4);
     w.sched = take(64);   // work counters of the persistent kernels (zeroed before each launch)
     // partial weight gradients of split experts: first segments indexed by expert, extra segments by list position;
     // widest use: two rank-r gradients over d columns in one pass (dA_gate + dA_up)
-    w.wg_scratch = d.training ? take((E + N / kWgradSeg + 2) * (size_t)2 * d.r * (dm > F ? dm : F) * 4) : take(16);
+    // ... and the per-tile partials of rows_proj_wgrad_kernel: [2][max_tiles][r][F]
+    w.wg_scratch = d.training ? take(std::max((E + N / kWgradSeg + 2) * (size_t)2 * d.r * (dm > F ? dm : F) * 4,
+                                              (size_t)2 * (E + N / kTileRows + 1) * d.r * F * 4)) : take(16);
     w.lut = take(256 * 8 * 2);
     w.sc2 = take(E * (dm + 2 * F) * 4);   // bf16-pair copies of scale_down | scale_gate | scale_up for the backward GEMMs
     w.WrT = take(E * dm * 4);
@@ -421,6 +424,11 @@ extern "C" {
 
 tqp_status tqp_set_option(tqp_ctx *c, const char *name, int value) {
     if (!c || !name) return TQP_ERR_ARG;
+    if (!strcmp(name, "fuse_dgu")) {
+        REQ(c, value >= 0 && value <= 2, TQP_ERR_ARG, "fuse_dgu must be 0..2");
+        c->fuse_dgu = value;
+        return TQP_OK;
+    }
     if (!strcmp(name, "route_impl")) {
         REQ(c, value >= 0 && value <= 3, TQP_ERR_ARG, "route_impl must be 0..3");
         c->route_impl = value;
@@ -656,7 +664,13 @@ tqp_status tqp_expert_bwd(tqp_ctx *c, int T, const void *X, const void *dYe, con
         if (tq) CK(tq_unrotate_grad(c, &c->tq.w.space_F, dAd, dA_down, s));
     }
     // gate / up projections: dXp = dG . Wg_eff^T + dU . Wu_eff^T and their adapter gradients
-    if (D.r == 16 || D.r == 32) {   // dG, dU are workspace tensors the dXp GEMM already has tensor maps for
+    // one pass over dG / dU for projection + dB pays while most experts fit one tile (cfg 2: 189 -> 121 us); with two or more
+    // tiles per expert every gradient goes through per-tile partials and the gain is gone (cfg 4: 380 -> 387 us)
+    const bool dgu = (D.r == 16 || D.r == 32) && (c->fuse_dgu == 2 || (c->fuse_dgu == 1 && (long long)N <= (long long)D.E * kTileRows));
+    if (dgu) {   // projections and dB_gate / dB_up from one pass over dG and dU
+        CK(launch_rows_proj_wgrad(c, &c->prob_dx.seg[0].act_map, &c->prob_dx.seg[1].act_map, D.F, (const bf16 *)c->w.B_gate, (const bf16 *)c->w.B_up,
+                                  c->p<bf16>(c->ws.XAg), c->p<bf16>(c->ws.XAu), ls, Zg, Zu, dB_gate, dB_up, s));
+    } else if (D.r == 16 || D.r == 32) {   // dG, dU are workspace tensors the dXp GEMM already has tensor maps for
         CK(launch_rows_proj_tma(c, &c->prob_dx.seg[0].act_map2, D.F, (const bf16 *)c->w.B_gate, 0, ls, Zg, s));
         CK(launch_rows_proj_tma(c, &c->prob_dx.seg[1].act_map2, D.F, (const bf16 *)c->w.B_up, 0, ls, Zu, s));
     } else {
@@ -667,11 +681,13 @@ tqp_status tqp_expert_bwd(tqp_ctx *c, int T, const void *X, const void *dYe, con
     px.out = (bf16 *)dXp;
     CK(run_gemm(c, &px, 1, s));
     if (defer) {   // tqp_step_host: dX leaves for the host first (nothing below feeds it)
-        c->tail = {dA_gate, dB_gate, dA_up, dB_up, dA_down, dB_down, dye, offsets, true};
+        c->tail = {dA_gate, dB_gate, dA_up, dB_up, dA_down, dB_down, dye, offsets, true, dgu};
         return TQP_OK;
     }
-    CK(launch_rows_wgrad(c, dG, D.F, c->p<bf16>(c->ws.XAg), nullptr, offsets, 0, dB_gate, nullptr, s));
-    CK(launch_rows_wgrad(c, dU, D.F, c->p<bf16>(c->ws.XAu), nullptr, offsets, 0, dB_up, nullptr, s));
+    if (!dgu) {
+        CK(launch_rows_wgrad(c, dG, D.F, c->p<bf16>(c->ws.XAg), nullptr, offsets, 0, dB_gate, nullptr, s));
+        CK(launch_rows_wgrad(c, dU, D.F, c->p<bf16>(c->ws.XAu), nullptr, offsets, 0, dB_up, nullptr, s));
+    }
     CK(launch_rows_wgrad(c, Xp, D.d, Zg, Zu, offsets, 1, dAg, dAu, s));   // one pass over Xp for both
     if (tq) {
         CK(tq_unrotate_grad(c, &c->tq.w.space_d, dAg, dA_gate, s));
@@ -691,8 +707,10 @@ static tqp_status expert_bwd_tail(tqp_ctx *c, cudaStream_t s) {
 #define CK(x) do { st = (x); if (st != TQP_OK) return st; } while (0)
     CK(launch_rows_wgrad(c, c->tail.dYe, D.d, c->p<bf16>(c->ws.HAd), nullptr, c->tail.offsets, 0, c->tail.dB_down, nullptr, s));
     CK(launch_rows_wgrad(c, c->p<bf16>(c->ws.H), D.F, c->p<bf16>(c->ws.Zd), nullptr, c->tail.offsets, 1, c->tail.dA_down, nullptr, s));
-    CK(launch_rows_wgrad(c, c->p<bf16>(c->ws.dG), D.F, c->p<bf16>(c->ws.XAg), nullptr, c->tail.offsets, 0, c->tail.dB_gate, nullptr, s));
-    CK(launch_rows_wgrad(c, c->p<bf16>(c->ws.dU), D.F, c->p<bf16>(c->ws.XAu), nullptr, c->tail.offsets, 0, c->tail.dB_up, nullptr, s));
+    if (!c->tail.dgu_done) {
+        CK(launch_rows_wgrad(c, c->p<bf16>(c->ws.dG), D.F, c->p<bf16>(c->ws.XAg), nullptr, c->tail.offsets, 0, c->tail.dB_gate, nullptr, s));
+        CK(launch_rows_wgrad(c, c->p<bf16>(c->ws.dU), D.F, c->p<bf16>(c->ws.XAu), nullptr, c->tail.offsets, 0, c->tail.dB_up, nullptr, s));
+    }
     CK(launch_rows_wgrad(c, c->p<bf16>(c->ws.Xp), D.d, c->p<bf16>(c->ws.Zg), c->p<bf16>(c->ws.Zu), c->tail.offsets, 1, c->tail.dA_gate,
                          c->tail.dA_up, s));
 #undef CK

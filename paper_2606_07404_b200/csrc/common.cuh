@@ -96,7 +96,7 @@ struct Workspace {
     size_t total = 0;        // the caller's workspace
     size_t host_total = 0;   // tqp_step_host staging (library-owned, allocated on first use)
     // offsets (bytes) into the bound buffer
-    size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, xsegs, xfirst, wg_scratch, sched, lut, sc2, WrT, WrHL, wnorm, rflag, dl,
+    size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, xsegs, xfirst, tfirst, wg_scratch, sched, lut, sc2, WrT, WrHL, wnorm, rflag, dl,
         // tqp_step_host staging
         trace, hX, hdY, hX2, hdY2, hY, hdX, topk_idx, topk_w, counts, offsets, perm, inv_perm, Ye, dYe, dXp, dtopk_w;
 };
@@ -143,7 +143,8 @@ struct tqp_ctx {
     int host_chunks = 0;        // tqp_step_host_async: X upload / router in 1 or 4 token chunks (0: chosen at run time)
     // tqp_step_host defers all adapter weight gradients (nothing else depends on them) until dX is on its way to the host
     int defer_tail = 0;
-    struct { float *dA_gate, *dB_gate, *dA_up, *dB_up, *dA_down, *dB_down; const tqp::bf16 *dYe; const int32_t *offsets; bool pending; } tail = {};
+    int fuse_dgu = 1;           // dG / dU: adapter projection and dB in one pass (rows_proj_wgrad_kernel): 1 where it pays, 2 always, 0 never
+    struct { float *dA_gate, *dB_gate, *dA_up, *dB_up, *dA_down, *dB_down; const tqp::bf16 *dYe; const int32_t *offsets; bool pending; bool dgu_done; } tail = {};
     std::vector<cudaEvent_t> ev; // pairs (start, stop)
     int ev_used = 0;
     // tensor maps over weights / workspace (built in bind_weights)
@@ -220,6 +221,8 @@ tqp_status launch_rows_gather_proj(tqp_ctx *c, const CUtensorMap *in_map, int in
 // W[e - e0][out][in] = bf16(deq + s A B) for experts e0 .. e0 + n_experts of pack 0 (gate) / 1 (up) / 2 (down) (consolidate.cu)
 tqp_status launch_consolidate(tqp_ctx *c, int pack, int e0, int n_experts, bf16 *W, cudaStream_t st);
 // grad_w[e] = sum_{p in e} small_w[p][q] * big[p][a]; stored [a][q] (out_ar=1: dA) or [q][a] (out_ar=0: dB), fp32
+tqp_status launch_rows_proj_wgrad(tqp_ctx *c, const CUtensorMap *map_g, const CUtensorMap *map_u, int F, const bf16 *B_gate, const bf16 *B_up,
+                                  const bf16 *XAg, const bf16 *XAu, float s, bf16 *Zg, bf16 *Zu, float *dB_gate, float *dB_up, cudaStream_t st);
 tqp_status launch_rows_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 *small0, const bf16 *small1,
                              const int32_t *offsets, int out_ar, float *grad0, float *grad1, cudaStream_t st);
 

@@ -49,7 +49,8 @@ __global__ void __launch_bounds__(256) dispatch_scan_chunks_kernel(int32_t *__re
 __global__ void __launch_bounds__(1024) dispatch_scan_experts_kernel(const int32_t *__restrict__ counts, int E,
                                                                      int32_t *__restrict__ offsets, Tile *__restrict__ tiles,
                                                                      int32_t *__restrict__ num_tiles, int tile_rows,
-                                                                     Tile *__restrict__ xsegs, int32_t *__restrict__ xfirst) {
+                                                                     Tile *__restrict__ xsegs, int32_t *__restrict__ xfirst,
+                                                                     int32_t *__restrict__ tfirst) {
     __shared__ int32_t w_off[32], w_til[32], w_xs[32];
     const int e = threadIdx.x, lane = e % 32, warp = e / 32;
     const int cnt = (e < E) ? counts[e] : 0;
@@ -91,7 +92,8 @@ __global__ void __launch_bounds__(1024) dispatch_scan_experts_kernel(const int32
             xsegs[xs_e + i] = t;
         }
         offsets[e] = off_e;
-        if (e == E - 1) { offsets[E] = off_e + cnt; *num_tiles = til_e + nt; }
+        tfirst[e] = til_e;   // the expert's tiles are [tfirst[e], tfirst[e + 1])
+        if (e == E - 1) { offsets[E] = off_e + cnt; *num_tiles = til_e + nt; tfirst[E] = til_e + nt; }
         if (nt > 0) {
             int per = (cnt + nt - 1) / nt;
             per = (per + 15) & ~15;   // balanced tiles, multiples of 16 rows (UMMA N granularity)
@@ -151,7 +153,7 @@ tqp_status launch_dispatch(tqp_ctx *c, int T, const int32_t *topk_idx, int32_t *
     dispatch_scan_chunks_kernel<<<(E + 7) / 8, 256, 0, s>>>(blk, nchunks, E, counts);
     TQP_LAUNCH_OK(c);
     dispatch_scan_experts_kernel<<<1, 1024, 0, s>>>(counts, E, offsets, c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), kTileRows,
-                                                    c->p<Tile>(c->ws.xsegs), c->p<int32_t>(c->ws.xfirst));
+                                                    c->p<Tile>(c->ws.xsegs), c->p<int32_t>(c->ws.xfirst), c->p<int32_t>(c->ws.tfirst));
     TQP_LAUNCH_OK(c);
     dispatch_scatter_kernel<<<nblk, 128, smem, s>>>(topk_idx, N, E, blk, offsets, perm, inv_perm);
     TQP_LAUNCH_OK(c);

@@ -975,4 +975,231 @@ tqp_status launch_rows_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 
     return launch_wgrad_t<32, 2>(c, a, offsets, st);
 }
 
+// ---- dG . B_g^T | dU . B_u^T together with (x.A_g)^T dG | (x.A_u)^T dU: one pass over dG and dU -----------------------------
+// The backward of the gate / up adapters needs dG (and dU) twice: the projection Z = s dG . B^T (the adapter K-step of the dXp
+// GEMM and the row operand of dA) and the weight gradient dB = (s x.A)^T dG.  As separate passes (rows_proj_tma + rows_wgrad)
+// each streams the [N][F] tensor from HBM; here one CTA owns one grouped-GEMM tile (<= 256 rows of one expert), streams its
+// rows once in 64-column TMA stages (the GEMM's own tensor map: box {64, 256}, 128-byte swizzle) and feeds both
+// contractions from the stage: warp w multiplies rows [32 w, 32 w + 32) by the adapter chunk (projection, accumulated over
+// the whole width) and columns [8 w, 8 w + 8) of the stage by the tile's x.A rows (weight gradient: complete for this tile
+// after every stage, written out and reset).  An expert with one tile writes its gradient directly; an expert with several
+// writes per-tile partials to the scratch and projwg_reduce_kernel sums them in tile order (deterministic, no atomics);
+// experts without rows are zeroed there.  grid = (max_tiles, 2): y = 0 gate, 1 up.
+template <int R>
+struct ProjWgCfg {
+    static constexpr int NST = R == 16 ? 3 : 5;                       // r = 16: 112 KB, two CTAs per SM (one CTA with six stages: 129 against 106 us at cfg 2)
+    static constexpr int WLD = PJ_LD;                                 // adapter chunk Ws[R][64 + 8]
+    static constexpr int ROWS_BYTES = kTileRows * PJ_KC * 2;          // 32 KB (swizzled, unpadded)
+    static constexpr int W_BYTES = (R * WLD * 2 + 127) / 128 * 128;
+    static constexpr int CPR = R / 8;                                 // 16-byte chunks per x.A row
+    static constexpr int S_BYTES = kTileRows * R * 2;                 // x.A rows of the tile, dense [256][R], chunks XOR-swizzled
+    static constexpr int OFF_W = NST * ROWS_BYTES;
+    static constexpr int OFF_S = OFF_W + NST * W_BYTES;
+    static constexpr int SMEM = OFF_S + S_BYTES + 1024;
+};
+
+struct ProjWgArgs {
+    CUtensorMap map[2];      // dG, dU: [N][F], box {64, 256}, SWIZZLE_128B
+    const bf16 *W[2];        // B_gate, B_up: [E][R][F]
+    const bf16 *small_[2];   // s x.A_g, s x.A_u: [N][kLoraPad]
+    bf16 *out[2];            // Z_g, Z_u: [N][kLoraPad]
+    float *grad[2];          // dB_gate, dB_up: [E][R][F]
+    float *scratch;          // [2][max_tiles][R][F] partials of experts with more than one tile
+    const int32_t *tfirst;   // [E + 1]: expert e owns tiles [tfirst[e], tfirst[e + 1])
+    int K, E, max_tiles;
+    float s;
+};
+
+template <int R>
+__global__ void __launch_bounds__(PJ_THREADS, R == 16 ? 2 : 1) rows_proj_wgrad_kernel(const __grid_constant__ ProjWgArgs a,
+                                                                                      const Tile *__restrict__ tiles,
+                                                                                      const int32_t *__restrict__ num_tiles) {
+    using C = ProjWgCfg<R>;
+    using namespace ptx;
+    constexpr int NST = C::NST, MT = R / 16;
+    extern __shared__ uint8_t pw_smem_raw[];
+    __shared__ __align__(8) uint64_t s_full[NST];
+    const int nt_all = *num_tiles, j = blockIdx.x, y = blockIdx.y;
+    if (j >= nt_all) return;
+    const Tile t = tiles[j];
+    const int valid = t.rows, row0 = t.row0, e = t.expert;
+    if (valid <= 0) return;
+    const bool single = (j == 0 || tiles[j - 1].expert != e) && (j + 1 >= nt_all || tiles[j + 1].expert != e);
+    const int K = a.K, nk = K / PJ_KC;
+    float *dst = single ? a.grad[y] + (size_t)e * R * K : a.scratch + ((size_t)y * a.max_tiles + j) * R * K;
+    const int tid = threadIdx.x, warp = tid / 32, lane = tid % 32;
+    const uint32_t sbase = (smem_u32(pw_smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar0 = smem_u32(s_full), s_s = sbase + C::OFF_S;
+    if (tid == 0) {
+        for (int s = 0; s < NST; ++s) mbar_init(bar0 + 8 * s, 1);
+        mbar_init_fence();
+    }
+    __syncthreads();
+    const CUtensorMap *map = &a.map[y];
+    const bf16 *W = a.W[y] + (size_t)e * R * K;
+    auto issue = [&](int kc) {   // rows by TMA (one thread), adapter chunk by cp.async (everyone)
+        const int st = kc % NST;
+        if (tid == 0) {
+            mbar_expect_tx(bar0 + 8 * st, C::ROWS_BYTES);
+            tma_load_2d(sbase + st * C::ROWS_BYTES, map, kc * PJ_KC, row0, bar0 + 8 * st);
+        }
+        const uint32_t w_s = sbase + C::OFF_W + st * C::W_BYTES;
+        for (int v = tid; v < R * PJ_KC / 8; v += PJ_THREADS) {
+            const int q = v / (PJ_KC / 8), cc = v % (PJ_KC / 8);
+            cp_async16(w_s + (q * C::WLD + cc * 8) * 2, W + (size_t)q * K + kc * PJ_KC + cc * 8, 16);
+        }
+    };
+    // the tile's x.A rows (zero past `valid`: those stage rows belong to the next tile); part of the first commit group
+    for (int v = tid; v < kTileRows * C::CPR; v += PJ_THREADS) {
+        const int pr = v / C::CPR, cc = v % C::CPR;
+        const bool ok = pr < valid;
+        cp_async16(s_s + pr * (R * 2) + ((cc ^ ((pr * C::CPR / 8) % C::CPR)) << 4), a.small_[y] + (size_t)(row0 + (ok ? pr : 0)) * kLoraPad + cc * 8,
+                   ok ? 16 : 0);
+    }
+    for (int s = 0; s < NST - 1; ++s) {
+        if (s < nk) issue(s);
+        cp_async_commit();
+    }
+    float acc[2][R / 8][4], wacc[MT][4];
+#pragma unroll
+    for (int m = 0; m < 2; ++m)
+#pragma unroll
+        for (int n = 0; n < R / 8; ++n)
+#pragma unroll
+            for (int q = 0; q < 4; ++q) acc[m][n][q] = 0.f;
+#pragma unroll
+    for (int m = 0; m < MT; ++m)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) wacc[m][q] = 0.f;
+    const int prow = warp * 32 + lane % 16;   // this lane's row of the projection's A fragments (ldmatrix x4), first 16-row group
+    for (int kc = 0; kc < nk; ++kc) {
+        const int st = kc % NST;
+        mbar_wait(bar0 + 8 * st, (kc / NST) & 1);
+        cp_async_wait<NST - 2>();
+        __syncthreads();   // chunk kc visible to everyone; everyone is past chunk kc - 1 (its stage is refilled below)
+        if (kc + NST - 1 < nk) issue(kc + NST - 1);
+        cp_async_commit();
+        const uint32_t rows_s = sbase + st * C::ROWS_BYTES, w_s = sbase + C::OFF_W + st * C::W_BYTES;
+        // projection: rows [32 warp, 32 warp + 32) x this 64-column chunk of the adapter
+        if (warp * 32 < valid) {
+            const uint32_t b_addr = w_s + (((lane / 16) * 8 + lane % 8) * C::WLD + ((lane / 8) % 2) * 8) * 2;
+#pragma unroll
+            for (int kk = 0; kk < PJ_KC; kk += 16) {
+                uint32_t bq[MT][4];
+#pragma unroll
+                for (int np = 0; np < MT; ++np) ldsm_x4(b_addr + (np * 16 * C::WLD + kk) * 2, bq[np]);
+#pragma unroll
+                for (int m = 0; m < 2; ++m) {
+                    if (warp * 32 + 16 * m >= valid) continue;
+                    const int ar = prow + 16 * m;
+                    uint32_t af[4];
+                    ldsm_x4(rows_s + ar * 128 + ((((kk >> 3) + (lane >> 4)) ^ (ar & 7)) << 4), af);
+#pragma unroll
+                    for (int np = 0; np < MT; ++np) {
+                        mma16816(acc[m][2 * np], af, bq[np][0], bq[np][1]);
+                        mma16816(acc[m][2 * np + 1], af, bq[np][2], bq[np][3]);
+                    }
+                }
+            }
+        }
+        // weight gradient: (x.A)^T [R x rows] . stage [rows x 8 columns of this warp], two 16-row k-steps per load
+        for (int pb = 0; pb < valid; pb += 32) {
+            uint32_t bq[4];
+            const int pr = pb + lane;
+            ldsm_x4_t(rows_s + pr * 128 + ((warp ^ (pr & 7)) << 4), bq);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int pa = pb + 16 * h + (lane / 16) * 8 + lane % 8;
+#pragma unroll
+                for (int m = 0; m < MT; ++m) {
+                    uint32_t af[4];
+                    const int cq = 2 * m + (lane / 8) % 2;
+                    ldsm_x4_t(s_s + pa * (R * 2) + ((cq ^ ((pa * C::CPR / 8) % C::CPR)) << 4), af);
+                    mma16816(wacc[m], af, bq[2 * h], bq[2 * h + 1]);
+                }
+            }
+        }
+        {
+            const int col = kc * PJ_KC + warp * 8 + (lane % 4) * 2;
+#pragma unroll
+            for (int m = 0; m < MT; ++m) {
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    *reinterpret_cast<float2 *>(dst + (size_t)(m * 16 + lane / 4 + 8 * h) * K + col) = make_float2(wacc[m][2 * h], wacc[m][2 * h + 1]);
+                    wacc[m][2 * h] = 0.f;
+                    wacc[m][2 * h + 1] = 0.f;
+                }
+            }
+        }
+    }
+    cp_async_wait<0>();
+#pragma unroll
+    for (int m = 0; m < 2; ++m) {
+#pragma unroll
+        for (int n = 0; n < R / 8; ++n) {
+            const int q = n * 8 + (lane % 4) * 2;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int r = warp * 32 + 16 * m + lane / 4 + 8 * h;
+                if (r < valid)
+                    *reinterpret_cast<uint32_t *>(a.out[y] + (size_t)(row0 + r) * kLoraPad + q) =
+                        float2_to_bf16x2(a.s * acc[m][n][2 * h], a.s * acc[m][n][2 * h + 1]);
+            }
+        }
+    }
+}
+
+// grid = (E, 2, PWR_SPLIT), block = 256: expert e, gate / up, one slice of the [R][F] gradient.  No tile: the slice is zeroed; one tile: nothing to do (the kernel wrote the
+// gradient itself); several: their partials are summed in tile order.  (One CTA per expert was 200 us at cfg 3, where one
+// expert owns dozens of tiles.)
+constexpr int PWR_SPLIT = 8;
+__global__ void __launch_bounds__(256) projwg_reduce_kernel(const __grid_constant__ ProjWgArgs a, const Tile *__restrict__ tiles, int R) {
+    const int e = blockIdx.x, y = blockIdx.y;
+    const size_t per = (size_t)R * a.K, slice = per / 4 / PWR_SPLIT;   // float4 elements; R F / 4 is a multiple of 8 (F % 64 == 0)
+    const int j = a.tfirst[e], n = a.tfirst[e + 1] - j;   // the expert's tiles (dispatch)
+    if (n == 1) return;
+    float4 *out = reinterpret_cast<float4 *>(a.grad[y] + (size_t)e * per) + blockIdx.z * slice;
+    if (n == 0) {
+        for (size_t i = threadIdx.x; i < slice; i += blockDim.x) out[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        return;
+    }
+    const float4 *base = reinterpret_cast<const float4 *>(a.scratch + ((size_t)y * a.max_tiles + j) * per) + blockIdx.z * slice;
+    for (size_t i = threadIdx.x; i < slice; i += blockDim.x) {
+        float4 s = base[i];
+        for (int q = 1; q < n; ++q) {
+            if (tiles[j + q].rows <= 0) continue;    // balanced tiles: trailing tiles of an expert can be empty
+            const float4 v = base[(size_t)q * (per / 4) + i];
+            s.x += v.x; s.y += v.y; s.z += v.z; s.w += v.w;
+        }
+        out[i] = s;
+    }
+}
+
+template <int R>
+static tqp_status launch_projwg_t(tqp_ctx *c, const ProjWgArgs &a, cudaStream_t st) {
+    using C = ProjWgCfg<R>;
+    if (tqp_status st_attr = ensure_dyn_smem(c, reinterpret_cast<const void *>(&rows_proj_wgrad_kernel<R>), C::SMEM)) return st_attr;
+    const Tile *tiles = c->p<Tile>(c->ws.tiles);
+    const int32_t *nt = c->p<int32_t>(c->ws.num_tiles);
+    rows_proj_wgrad_kernel<R><<<dim3(c->max_tiles, 2), PJ_THREADS, C::SMEM, st>>>(a, tiles, nt);
+    TQP_LAUNCH_OK(c);
+    projwg_reduce_kernel<<<dim3(c->desc.E, 2, PWR_SPLIT), 256, 0, st>>>(a, tiles, R);
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
+
+// Z_g = s dG . B_g^T, Z_u = s dU . B_u^T, dB_gate = (s x.A_g)^T dG, dB_up = (s x.A_u)^T dU  (r = 16 / 32; F % 64 == 0).
+// map_g / map_u: the tensor maps of dG / dU with box {64, kTileRows}, 128-byte swizzle.
+tqp_status launch_rows_proj_wgrad(tqp_ctx *c, const CUtensorMap *map_g, const CUtensorMap *map_u, int F, const bf16 *B_gate, const bf16 *B_up,
+                                  const bf16 *XAg, const bf16 *XAu, float s, bf16 *Zg, bf16 *Zu, float *dB_gate, float *dB_up, cudaStream_t st) {
+    const int r = c->desc.r;
+    ProjWgArgs a;
+    a.map[0] = *map_g; a.map[1] = *map_u; a.W[0] = B_gate; a.W[1] = B_up; a.small_[0] = XAg; a.small_[1] = XAu;
+    a.out[0] = Zg; a.out[1] = Zu; a.grad[0] = dB_gate; a.grad[1] = dB_up; a.scratch = c->p<float>(c->ws.wg_scratch);
+    a.tfirst = c->p<int32_t>(c->ws.tfirst); a.K = F; a.E = c->desc.E; a.max_tiles = c->max_tiles; a.s = s;
+    if (r == 16) return launch_projwg_t<16>(c, a, st);
+    if (r == 32) return launch_projwg_t<32>(c, a, st);
+    return TQP_ERR_ARG;
+}
+
 }  // namespace tqp
