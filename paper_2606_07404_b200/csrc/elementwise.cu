@@ -24,12 +24,9 @@ __global__ void __launch_bounds__(256) gather_rows_kernel(const bf16 *__restrict
     for (int v = lane; v < d / 8; v += 32) dst[v] = src[v];
 }
 
-// H = silu(G) * U
-__global__ void __launch_bounds__(256) swiglu_fwd_kernel(const uint4 *__restrict__ G, const uint4 *__restrict__ U,
-                                                         uint4 *__restrict__ H, size_t nvec) {
-    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= nvec) return;
-    uint4 g = ld_nc(G + i), u = ld_nc(U + i), h;
+// H = silu(G) * U.  Two 16-byte vectors per thread (half a grid apart), all four loads issued before the arithmetic.
+__device__ __forceinline__ uint4 swiglu_fwd_vec(const uint4 &g, const uint4 &u) {
+    uint4 h;
     const uint32_t *gp = reinterpret_cast<const uint32_t *>(&g), *up = reinterpret_cast<const uint32_t *>(&u);
     uint32_t *hp = reinterpret_cast<uint32_t *>(&h);
 #pragma unroll
@@ -39,7 +36,17 @@ __global__ void __launch_bounds__(256) swiglu_fwd_kernel(const uint4 *__restrict
         float h1 = gf.y / (1.f + __expf(-gf.y)) * uf.y;
         hp[q] = float2_to_bf16x2(h0, h1);
     }
-    H[i] = h;
+    return h;
+}
+__global__ void __launch_bounds__(256) swiglu_fwd_kernel(const uint4 *__restrict__ G, const uint4 *__restrict__ U,
+                                                         uint4 *__restrict__ H, size_t nvec, size_t half) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x, i2 = i + half;
+    if (i >= half) return;
+    const bool two = i2 < nvec;
+    const uint4 z = make_uint4(0, 0, 0, 0);
+    const uint4 g = ld_nc(G + i), u = ld_nc(U + i), g2 = two ? ld_nc(G + i2) : z, u2 = two ? ld_nc(U + i2) : z;
+    H[i] = swiglu_fwd_vec(g, u);
+    if (two) H[i2] = swiglu_fwd_vec(g2, u2);
 }
 
 // sig = sigmoid(G); dU = dH*G*sig; dG = dH*U*sig*(1+G*(1-sig))
@@ -72,27 +79,39 @@ __global__ void __launch_bounds__(256) combine_kernel(const bf16 *__restrict__ Y
     const int t = gw / slabs, slab = gw % slabs;
     if (t >= T) return;
     const int col = slab * 256 + lane * 8;
-    if (col >= d) return;
+    const bool on = col < d;   // d % 256 == 128: the upper half-warp of the last slab only takes part in the shuffles
     float acc[8];
 #pragma unroll
     for (int q = 0; q < 8; ++q) acc[q] = 0.f;
-    for (int j = 0; j < k; ++j) {
-        const int p = inv_perm[(size_t)t * k + j];
-        const float wj = w ? w[(size_t)t * k + j] : 1.f;
-        uint4 v = ld_nc(reinterpret_cast<const uint4 *>(Ye + (size_t)p * d + col));
-        const uint32_t *vp = reinterpret_cast<const uint32_t *>(&v);
+    // lane j holds the j-th source row and weight (k <= 32); the rows are fetched four at a time (independent loads in flight)
+    // and accumulated in ascending j
+    const int my_p = lane < k ? inv_perm[(size_t)t * k + lane] : 0;
+    const float my_w = (w && lane < k) ? w[(size_t)t * k + lane] : 1.f;
+    for (int j0 = 0; j0 < k; j0 += 4) {
+        uint4 v[4];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            float2 f = bf16x2_to_float2(vp[q]);
-            acc[2 * q] = fmaf(wj, f.x, acc[2 * q]);
-            acc[2 * q + 1] = fmaf(wj, f.y, acc[2 * q + 1]);
+        for (int u = 0; u < 4; ++u) {
+            const int p = __shfl_sync(0xffffffffu, my_p, (j0 + u) & 31);
+            v[u] = (on && j0 + u < k) ? ld_nc(reinterpret_cast<const uint4 *>(Ye + (size_t)p * d + col)) : make_uint4(0, 0, 0, 0);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const float wj = __shfl_sync(0xffffffffu, my_w, (j0 + u) & 31);
+            if (j0 + u >= k) continue;
+            const uint32_t *vp = reinterpret_cast<const uint32_t *>(&v[u]);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                float2 f = bf16x2_to_float2(vp[q]);
+                acc[2 * q] = fmaf(wj, f.x, acc[2 * q]);
+                acc[2 * q + 1] = fmaf(wj, f.y, acc[2 * q + 1]);
+            }
         }
     }
     uint4 o;
     uint32_t *op = reinterpret_cast<uint32_t *>(&o);
 #pragma unroll
     for (int q = 0; q < 4; ++q) op[q] = float2_to_bf16x2(acc[2 * q], acc[2 * q + 1]);
-    *reinterpret_cast<uint4 *>(Y + (size_t)t * d + col) = o;
+    if (on) *reinterpret_cast<uint4 *>(Y + (size_t)t * d + col) = o;
 }
 
 // dYe[p] = w[a] * dY[t];  dw[a] = <dY[t], Ye[p]>.  One warp per assignment a.
@@ -172,8 +191,8 @@ tqp_status launch_gather_rows(tqp_ctx *c, int N, const bf16 *X, const int32_t *p
     return TQP_OK;
 }
 tqp_status launch_swiglu_fwd(tqp_ctx *c, int N, const bf16 *G, const bf16 *U, bf16 *H, cudaStream_t s) {
-    size_t nvec = (size_t)N * c->desc.F / 8;
-    swiglu_fwd_kernel<<<(unsigned)((nvec + 255) / 256), 256, 0, s>>>((const uint4 *)G, (const uint4 *)U, (uint4 *)H, nvec);
+    const size_t nvec = (size_t)N * c->desc.F / 8, half = (nvec + 1) / 2;
+    swiglu_fwd_kernel<<<(unsigned)((half + 255) / 256), 256, 0, s>>>((const uint4 *)G, (const uint4 *)U, (uint4 *)H, nvec, half);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
 }
