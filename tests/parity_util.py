@@ -42,12 +42,14 @@ def make_layer(inp, T_max=None, training=True, gemm_impl=0):
     return layer, dev
 
 
-def run_gpu(inp, backward=True, router_grad=False, gemm_impl=0, keep_dev=False, fused_bwd=True, route_impl=0):
+def run_gpu(inp, backward=True, router_grad=False, gemm_impl=0, keep_dev=False, fused_bwd=True, route_impl=0, options=None):
     """The whole chain through the C ABI; returns fp32/int numpy arrays keyed like oracle.layer().  fused_bwd: the call
     sequence bench.py times (tqp_combine_bwd with perm, tqp_expert_bwd with TQP_BWD_DYE_UNMODIFIED); False: the plain
     combine_bwd kernel and an expert_bwd that trusts nothing from earlier calls."""
     import torch
     layer, dev = make_layer(inp, training=backward, gemm_impl=gemm_impl)
+    for name, value in (options or {}).items():   # any other library option (tqp_set_option)
+        layer.set_option(name, value)
     T, k, F, d = inp["T"], inp["k"], inp["F"], inp["d"]
     N = T * k
     out = {}
