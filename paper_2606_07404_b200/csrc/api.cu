@@ -425,7 +425,7 @@ extern "C" {
 tqp_status tqp_set_option(tqp_ctx *c, const char *name, int value) {
     if (!c || !name) return TQP_ERR_ARG;
     if (!strcmp(name, "fuse_dgu")) {
-        REQ(c, value >= 0 && value <= 2, TQP_ERR_ARG, "fuse_dgu must be 0..2");
+        REQ(c, value == 0 || value == 1, TQP_ERR_ARG, "fuse_dgu must be 0 or 1");
         c->fuse_dgu = value;
         return TQP_OK;
     }
@@ -664,9 +664,8 @@ tqp_status tqp_expert_bwd(tqp_ctx *c, int T, const void *X, const void *dYe, con
         if (tq) CK(tq_unrotate_grad(c, &c->tq.w.space_F, dAd, dA_down, s));
     }
     // gate / up projections: dXp = dG . Wg_eff^T + dU . Wu_eff^T and their adapter gradients
-    // one pass over dG / dU for projection + dB pays while most experts fit one tile (cfg 2: 189 -> 121 us); with two or more
-    // tiles per expert every gradient goes through per-tile partials and the gain is gone (cfg 4: 380 -> 387 us)
-    const bool dgu = (D.r == 16 || D.r == 32) && (c->fuse_dgu == 2 || (c->fuse_dgu == 1 && (long long)N <= (long long)D.E * kTileRows));
+    // one pass over dG / dU for projection + dB (cfg 2: 189 -> 116 us; cfg 4, two tiles per expert and r = 32: 380 -> 335 us)
+    const bool dgu = (D.r == 16 || D.r == 32) && c->fuse_dgu != 0;
     if (dgu) {   // projections and dB_gate / dB_up from one pass over dG and dU
         CK(launch_rows_proj_wgrad(c, &c->prob_dx.seg[0].act_map, &c->prob_dx.seg[1].act_map, D.F, (const bf16 *)c->w.B_gate, (const bf16 *)c->w.B_up,
                                   c->p<bf16>(c->ws.XAg), c->p<bf16>(c->ws.XAu), ls, Zg, Zu, dB_gate, dB_up, s));

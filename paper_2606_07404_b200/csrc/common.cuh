@@ -143,7 +143,7 @@ struct tqp_ctx {
     int host_chunks = 0;        // tqp_step_host_async: X upload / router in 1 or 4 token chunks (0: chosen at run time)
     // tqp_step_host defers all adapter weight gradients (nothing else depends on them) until dX is on its way to the host
     int defer_tail = 0;
-    int fuse_dgu = 1;           // dG / dU: adapter projection and dB in one pass (rows_proj_wgrad_kernel): 1 where it pays, 2 always, 0 never
+    int fuse_dgu = 1;           // dG / dU: adapter projection and dB in one pass (rows_proj_wgrad_kernel) for r = 16 / 32; 0 = separate passes
     struct { float *dA_gate, *dB_gate, *dA_up, *dB_up, *dA_down, *dB_down; const tqp::bf16 *dYe; const int32_t *offsets; bool pending; bool dgu_done; } tail = {};
     std::vector<cudaEvent_t> ev; // pairs (start, stop)
     int ev_used = 0;

@@ -989,7 +989,7 @@ tqp_status launch_rows_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 
 // instructions per stage from one thread.)
 template <int R>
 struct ProjWgCfg {
-    static constexpr int NST = R == 16 ? 3 : 5;                       // r = 16: 112 KB, two CTAs per SM (one CTA with six stages: 129 against 106 us at cfg 2)
+    static constexpr int NST = R == 16 ? 3 : 2;                       // 112 KB (r = 16) / 90 KB (r = 32): two CTAs per SM                       // r = 16: 112 KB, two CTAs per SM (one CTA with six stages: 129 against 106 us at cfg 2)
     static constexpr int WLD = PJ_LD;                                 // adapter chunk Ws[R][64 + 8]
     static constexpr int ROWS_BYTES = kTileRows * PJ_KC * 2;          // 32 KB (swizzled, unpadded)
     static constexpr int W_BYTES = (R * WLD * 2 + 127) / 128 * 128;
@@ -1013,7 +1013,7 @@ struct ProjWgArgs {
 };
 
 template <int R>
-__global__ void __launch_bounds__(PJ_THREADS, R == 16 ? 2 : 1) rows_proj_wgrad_kernel(const __grid_constant__ ProjWgArgs a,
+__global__ void __launch_bounds__(PJ_THREADS, 2) rows_proj_wgrad_kernel(const __grid_constant__ ProjWgArgs a,
                                                                                       const Tile *__restrict__ tiles,
                                                                                       const int32_t *__restrict__ num_tiles) {
     using C = ProjWgCfg<R>;

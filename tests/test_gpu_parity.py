@@ -90,12 +90,12 @@ def test_two_runs_are_bitwise_identical(cfg):
 def test_dgu_projection_and_dB_in_one_pass_forced_and_off(cfg):
     """rows_proj_wgrad_kernel (dG . B^T with (x.A)^T dG from one pass over dG, same for dU) against the separate passes it
     replaces, on a skewed batch where one expert owns several tiles (per-tile partials + ordered reduction), several own one
-    tile (direct write) and one owns none (zeroed): option fuse_dgu = 2 forces it, 0 switches it off.  Both must match the
+    tile (direct write) and one owns none (zeroed): option fuse_dgu = 1 (the default), 0 switches it off.  Both must match the
     oracle; between the two only the fp32 summation order of dB differs."""
     inp = _skewed(cfg)
     ref = oracle_ref(inp, True, False)
     res = {}
-    for mode in (0, 2):
+    for mode in (0, 1):
         gpu = run_gpu(inp, backward=True, options={"fuse_dgu": mode})
         for key in BWD_KEYS:
             assert_close(f"{key} (fuse_dgu={mode})", gpu[key], ref[key])
@@ -104,7 +104,7 @@ def test_dgu_projection_and_dB_in_one_pass_forced_and_off(cfg):
         res[mode] = gpu
     assert ref["counts"].max() > 256 and ref["counts"].min() == 0
     for key in ("dB_gate", "dB_up", "dA_gate", "dA_up", "dXp"):
-        _, relf = errors(res[2][key], res[0][key])
+        _, relf = errors(res[1][key], res[0][key])
         assert relf <= 1e-5, f"{key}: the two paths differ by relF {relf:.2e}"
 
 
