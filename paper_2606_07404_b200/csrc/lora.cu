@@ -791,7 +791,7 @@ struct WgradCfg {
     static constexpr int SMEM = WG_NST * STAGE + 128;
 };
 
-// grid = (E + max extra segments, width / 128), block = 128.  Warp w owns columns [32 w, 32 w + 32) of the slab and all RT
+// grid = (E + max extra segments) x (width / 128) CTAs, block = 128.  Warp w owns columns [32 w, 32 w + 32) of the slab and all RT
 // adapter columns.  Blocks [0, E): the first kWgradSeg rows of expert blockIdx.x; blocks >= E: one extra segment each.
 template <int R, int NS>
 __global__ void __launch_bounds__(128) rows_wgrad_kernel(const __grid_constant__ WgradArgs a, const int32_t *__restrict__ offsets) {
@@ -799,13 +799,16 @@ __global__ void __launch_bounds__(128) rows_wgrad_kernel(const __grid_constant__
     extern __shared__ __align__(128) uint8_t wg_smem[];
     uint8_t *smem = wg_smem;
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem);
-    const int a0 = blockIdx.y * WG_COLS;
+    // 1-D grid, slab index fastest: the column slabs of one expert run side by side, so that the 256-byte pieces they take
+    // from the same rows arrive at the DRAM pages together
+    const int nslab = a.width / WG_COLS, bx = blockIdx.x / nslab;
+    const int a0 = (blockIdx.x % nslab) * WG_COLS;
     const int tid = threadIdx.x, warp = tid / 32;
     const int width = a.width;
     int e, p0, p1;
     float *dst[2];
-    if ((int)blockIdx.x < a.E) {
-        e = blockIdx.x;
+    if (bx < a.E) {
+        e = bx;
         p0 = offsets[e];
         const int cnt = offsets[e + 1] - p0;
         p1 = p0 + min(cnt, kWgradSeg);
@@ -813,7 +816,7 @@ __global__ void __launch_bounds__(128) rows_wgrad_kernel(const __grid_constant__
         for (int w = 0; w < NS; ++w)
             dst[w] = cnt > kWgradSeg ? a.scratch + (size_t)e * a.entry + (size_t)w * R * width : a.grad[w] + (size_t)e * R * width;
     } else {
-        const int j = blockIdx.x - a.E;
+        const int j = bx - a.E;
         if (j >= a.xfirst[a.E]) return;
         const Tile t = a.xsegs[j];
         e = t.expert;
@@ -943,7 +946,7 @@ template <int R, int NS>
 static tqp_status launch_wgrad_t(tqp_ctx *c, const WgradArgs &a, const int32_t *offsets, cudaStream_t st) {
     using C = WgradCfg<R, NS>;
     if (tqp_status st_attr = ensure_dyn_smem(c, reinterpret_cast<const void *>(&rows_wgrad_kernel<R, NS>), C::SMEM)) return st_attr;
-    rows_wgrad_kernel<R, NS><<<dim3(c->desc.E + c->max_xsegs, a.width / WG_COLS), 128, C::SMEM, st>>>(a, offsets);
+    rows_wgrad_kernel<R, NS><<<(unsigned)((c->desc.E + c->max_xsegs) * (a.width / WG_COLS)), 128, C::SMEM, st>>>(a, offsets);
     TQP_LAUNCH_OK(c);
     wgrad_reduce_kernel<<<dim3(c->desc.E, 4), 512, 0, st>>>(a, NS, R);
     TQP_LAUNCH_OK(c);
