@@ -498,19 +498,30 @@ gemm_tcgen05_ts2_kernel(const __grid_constant__ GemmArgs args, const uint4 *__re
 #pragma unroll
                                     for (int x = 0; x < 4; ++x)
 #pragma unroll
-                                        for (int i = 0; i < 2; ++i)
+                                        for (int mbi = 0; mbi < 2; ++mbi) {
+                                            // The eight source rows of a movmatrix block are k0 + {0,1,4,5,8,9,12,13}: rows rk and rk + 4 share
+                                            // k & 7, hence the chunk the 128-byte swizzle puts their codes in, hence their banks.  The upper
+                                            // half-warp therefore fetches its i = 1 codes while the lower one fetches i = 0 (k & 7 then
+                                            // takes all eight values) and the two results are swapped back before the transposition.
+                                            const int cg = 2 * hs + mbi;
+                                            uint32_t pk[2];
 #pragma unroll
-                                            for (int mbi = 0; mbi < 2; ++mbi) {
-                                                const int z = 8 * h + 2 * x + i, cg = 2 * hs + mbi;
-                                                const int k = (z >> 3) * 64 + ((z >> 1) & 3) * 16 + (z & 1) * 2 + kofs;
+                                            for (int pass = 0; pass < 2; ++pass) {
+                                                const int k = 64 * h + 16 * x + 2 * (pass ^ (rk >> 2)) + kofs;
                                                 // byte column m = 32 q + 8 cg + 2 jj: chunk 2 q + cg / 2, offset 8 (cg % 2) + 2 jj
                                                 const uint32_t cp = lds16(tb + k * 128 + (((2 * q4 + (cg >> 1)) ^ (k & 7)) << 4) + 8 * (cg & 1) + 2 * jj);
                                                 const uint32_t l0 = lds32(lut_l + ((cp & 0xffu) << 7));
                                                 const uint32_t l1 = lds32(lut_l + ((cp >> 8) << 7));
-                                                uint32_t pk = __byte_perm(l0, l1, 0x5410);
-                                                __nv_bfloat162 w2 = __hmul2(*reinterpret_cast<__nv_bfloat162 *>(&pk), sc[z]);
+                                                pk[pass] = __byte_perm(l0, l1, 0x5410);
+                                            }
+#pragma unroll
+                                            for (int i = 0; i < 2; ++i) {
+                                                const int z = 8 * h + 2 * x + i;
+                                                uint32_t p = (rk >> 2) ? pk[i ^ 1] : pk[i];
+                                                __nv_bfloat162 w2 = __hmul2(*reinterpret_cast<__nv_bfloat162 *>(&p), sc[z]);
                                                 rg[4 * x + 2 * mbi + i] = movmatrix_t(*reinterpret_cast<uint32_t *>(&w2));
                                             }
+                                        }
                                     if (h == 1 && hs == 1) {
                                         __syncwarp();
                                         if (lane == 0) mbar_arrive(idx_empty(iq.s));
