@@ -335,6 +335,7 @@ tqp_status set_seg_tq(tqp_ctx *c, GemmSeg *s, const bf16 *act, uint64_t act_rows
 // A' = R A per expert:  A [E][n][r] -> transpose -> rows [E r][n] -> rotate -> transpose back
 tqp_status tq_rotate_adapter(tqp_ctx *c, const tqp_tq_space *sp, const bf16 *A, bf16 *Ar, cudaStream_t s) {
     const int E = c->desc.E, r = c->desc.r, n = sp->n;
+    if (sp->hadamard && n <= 8192) return launch_tq_fwht_strided<bf16>(c, sp, A, Ar, E, r, 0, s);   // one pass, no transposes
     tqp_status st = launch_tq_transpose<bf16>(c, A, c->tq.tmp_a, E, n, r, s);
     if (st == TQP_OK) st = launch_tq_rotate(c, sp, c->tq.tmp_a, false, (long long)E * r, c->tq.tmp_b, false, 0, s);
     if (st == TQP_OK) st = launch_tq_transpose<bf16>(c, c->tq.tmp_b, Ar, E, r, n, s);
@@ -343,6 +344,7 @@ tqp_status tq_rotate_adapter(tqp_ctx *c, const tqp_tq_space *sp, const bf16 *A, 
 // dA = R^T dA' per expert (fp32): the same way back
 tqp_status tq_unrotate_grad(tqp_ctx *c, const tqp_tq_space *sp, float *dAr, float *dA, cudaStream_t s) {
     const int E = c->desc.E, r = c->desc.r, n = sp->n;
+    if (sp->hadamard && n <= 8192) return launch_tq_fwht_strided<float>(c, sp, dAr, dA, E, r, 1, s);
     tqp_status st = launch_tq_transpose<float>(c, dAr, c->tq.tmp_f, E, n, r, s);
     if (st == TQP_OK) st = launch_tq_rotate(c, sp, c->tq.tmp_f, true, (long long)E * r, dAr, true, 1, s);
     if (st == TQP_OK) st = launch_tq_transpose<float>(c, dAr, dA, E, r, n, s);

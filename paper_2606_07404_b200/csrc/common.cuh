@@ -260,6 +260,8 @@ tqp_status launch_tq_swiglu_bwd_rot(tqp_ctx *c, const tqp_tq_space *sp, const bf
                                     long long rows, cudaStream_t st);
 tqp_status launch_tq_make_lut(tqp_ctx *c, const double *levels, bf16 *lut, cudaStream_t st);
 template <typename T>
+tqp_status launch_tq_fwht_strided(tqp_ctx *c, const tqp_tq_space *sp, const T *X, T *Y, int E, int r, int inverse, cudaStream_t st);   // [E][n][r], FWHT over n
+template <typename T>
 tqp_status launch_tq_transpose(tqp_ctx *c, const T *in, T *out, int E, int a, int b, cudaStream_t st);   // [E][a][b] -> [E][b][a]
 
 // ---- device helpers ------------------------------------------------------------------------------------

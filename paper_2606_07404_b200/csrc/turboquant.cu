@@ -803,6 +803,142 @@ tqp_status launch_tq_swiglu_bwd_rot(tqp_ctx *c, const tqp_tq_space *sp, const bf
     return TQP_OK;
 }
 
+// ---- rotation of the adapters along their STRIDED dimension: A[e][i][q] (i < n, q < r): FWHT over i for every (e, q) --------
+// (replaces transpose -> row FWHT -> transpose for Hadamard spaces: three passes over the tensor and two temporaries become
+// one pass.)  CTA = (expert, group of 8 columns).  The rows come in coalesced (8 values = 16 / 32 bytes of every row), are
+// spread into 8 column vectors in shared memory (fp32, padded like the row kernel's), every column goes through the row
+// kernel's passes (registers for bits 0-2 of the index, shuffles for bits 3-7, shared memory above), and the rows go out
+// coalesced again.  Forward: y = H (signs * x) / sqrt(n); inverse: x = signs * (H y) / sqrt(n).
+// CG values of one row: 8 / 16 bytes (bf16) or 16 / 32 bytes (fp32)
+template <typename T, int CG>
+__device__ __forceinline__ void fs_load(const T *p, float (&v)[CG]) {
+    if constexpr (sizeof(T) == 2) {
+        uint32_t w[CG / 2];
+        if constexpr (CG == 8) { const uint4 q = *reinterpret_cast<const uint4 *>(p); w[0] = q.x; w[1] = q.y; w[2] = q.z; w[3] = q.w; }
+        else { const uint2 q = *reinterpret_cast<const uint2 *>(p); w[0] = q.x; w[1] = q.y; }
+#pragma unroll
+        for (int j = 0; j < CG / 2; ++j) { const float2 f = bf16x2_to_float2(w[j]); v[2 * j] = f.x; v[2 * j + 1] = f.y; }
+    } else {
+#pragma unroll
+        for (int j = 0; j < CG / 4; ++j) {
+            const float4 q = *reinterpret_cast<const float4 *>(p + 4 * j);
+            v[4 * j] = q.x; v[4 * j + 1] = q.y; v[4 * j + 2] = q.z; v[4 * j + 3] = q.w;
+        }
+    }
+}
+template <typename T, int CG>
+__device__ __forceinline__ void fs_store(T *p, const float (&v)[CG]) {
+    if constexpr (sizeof(T) == 2) {
+        uint32_t w[CG / 2];
+#pragma unroll
+        for (int j = 0; j < CG / 2; ++j) w[j] = float2_to_bf16x2(v[2 * j], v[2 * j + 1]);
+        if constexpr (CG == 8) *reinterpret_cast<uint4 *>(p) = make_uint4(w[0], w[1], w[2], w[3]);
+        else *reinterpret_cast<uint2 *>(p) = make_uint2(w[0], w[1]);
+    } else {
+#pragma unroll
+        for (int j = 0; j < CG / 4; ++j) *reinterpret_cast<float4 *>(p + 4 * j) = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+    }
+}
+
+template <typename T, int CG>
+__global__ void __launch_bounds__(1024) tq_fwht_strided_kernel(const T *__restrict__ X, T *__restrict__ Y, int n, int logn, int r,
+                                                                const int8_t *__restrict__ signs, int inverse) {
+    extern __shared__ float fs_s[];
+    const int np = n + n / 32;   // floats per column
+    const T *src = X + (size_t)blockIdx.y * n * r + blockIdx.x * CG;
+    T *dst = Y + (size_t)blockIdx.y * n * r + blockIdx.x * CG;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        float v[CG];
+        fs_load<T, CG>(src + (size_t)i * r, v);
+        const float sg = inverse ? 1.f : (float)signs[i];
+#pragma unroll
+        for (int c = 0; c < CG; ++c) fs_s[c * np + fw_pad(i)] = v[c] * sg;
+    }
+    __syncthreads();
+    const int tpr = n / 8, cpi = blockDim.x / tpr;             // threads per column, columns per round (blockDim = tpr * cpi, cpi | CG)
+    const int lr = threadIdx.x / tpr, t = threadIdx.x % tpr, lane = threadIdx.x % 32;
+    const float rs = rsqrtf((float)n);
+    const int nsh = min(logn, 8) - 3;
+    float fl[5];
+#pragma unroll
+    for (int b = 0; b < 5; ++b) fl[b] = (lane >> b) & 1 ? -1.f : 1.f;
+    int idx[2][8];
+#pragma unroll
+    for (int p = 0; p < 2; ++p) {
+        const int ls = 8 + 3 * p, nb = max(0, min(3, logn - ls)), s = 1 << ls;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int kb = k & ((1 << nb) - 1), rem = t * (8 >> nb) + (k >> nb);
+            idx[p][k] = fw_pad(((rem >> ls) << (ls + nb)) | (kb << ls) | (rem & (s - 1)));
+        }
+    }
+    float sgo[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) sgo[k] = inverse ? (float)signs[8 * t + k] : 1.f;
+    for (int cb = 0; cb < CG; cb += cpi) {
+        float *sm = fs_s + (cb + lr) * np;
+        float v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[k] = sm[fw_pad(8 * t + k)];
+        fw_bfly8(v, 3);
+#pragma unroll
+        for (int b = 0; b < 5; ++b) {
+            if (b < nsh) {
+#pragma unroll
+                for (int k = 0; k < 8; ++k) v[k] = fmaf(v[k], fl[b], __shfl_xor_sync(0xffffffffu, v[k], 1 << b));
+            }
+        }
+        if (logn > 8) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) sm[fw_pad(8 * t + k)] = v[k];
+#pragma unroll
+            for (int p = 0; p < 2; ++p) {
+                const int ls = 8 + 3 * p;
+                if (ls < logn) {
+                    __syncthreads();
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) v[k] = sm[idx[p][k]];
+                    fw_bfly8(v, min(3, logn - ls));
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) sm[idx[p][k]] = v[k];
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] = sm[fw_pad(8 * t + k)];
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) sm[fw_pad(8 * t + k)] = v[k] * rs * sgo[k];
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        float v[CG];
+#pragma unroll
+        for (int c = 0; c < CG; ++c) v[c] = fs_s[c * np + fw_pad(i)];
+        fs_store<T, CG>(dst + (size_t)i * r, v);
+    }
+}
+
+// Y[e][i][q] = rotation along i of X[e][i][q]  (Hadamard spaces, 128 <= n <= 8192, r % 8 == 0); X may equal Y
+template <typename T>
+tqp_status launch_tq_fwht_strided(tqp_ctx *c, const tqp_tq_space *sp, const T *X, T *Y, int E, int r, int inverse, cudaStream_t st) {
+    const int n = sp->n;
+    TQ_REQ(c, sp->hadamard && n >= 128 && n <= 8192 && r % 8 == 0, TQP_ERR_ARG, "strided FWHT: Hadamard space, 128 <= n <= 8192, r % 8 == 0");
+    int logn = 0;
+    while ((1 << logn) < n) ++logn;
+    // eight columns per CTA (135 KB of shared memory at n = 4096, one CTA per SM): 78 / 96 us per bf16 / fp32 adapter pack at
+    // cfg 5; four columns and two CTAs per SM were slower (fp32: 106 us)
+    constexpr int CG = 8;
+    const int tpr = n / 8, cpi = std::max(1, std::min(CG, 1024 / tpr));
+    const int smem = CG * (n + n / 32) * 4;
+    if (tqp_status s = ensure_dyn_smem(c, reinterpret_cast<const void *>(&tq_fwht_strided_kernel<T, CG>), smem)) return s;
+    tq_fwht_strided_kernel<T, CG><<<dim3(r / CG, E), tpr * cpi, smem, st>>>(X, Y, n, logn, r, sp->signs, inverse);
+    TQP_LAUNCH_OK(c);
+    return TQP_OK;
+}
+template tqp_status launch_tq_fwht_strided<bf16>(tqp_ctx *, const tqp_tq_space *, const bf16 *, bf16 *, int, int, int, cudaStream_t);
+template tqp_status launch_tq_fwht_strided<float>(tqp_ctx *, const tqp_tq_space *, const float *, float *, int, int, int, cudaStream_t);
+
 template <typename T>
 tqp_status launch_tq_transpose(tqp_ctx *c, const T *in, T *out, int E, int a, int b, cudaStream_t st) {
     // [E][a][b] -> [E][b][a]; one of a, b is the rank
