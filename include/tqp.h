@@ -308,7 +308,9 @@ void *tqp_debug_buffer(tqp_ctx *ctx, const char *name);
  * ceil(T*k / 256) * E <= tqp_dispatch_noalloc_capacity() = 1 048 576 (TQP_ERR_SHAPE; e.g. T = 16384, k = 12, E = 460
  * uses a third of it).  All calls on a device share the array: calls on one stream are ordered and safe, calls that
  * OVERLAP on the GPU (other streams, a graph replayed beside a live call) race and give garbage.  Nothing in it has to be
- * cleared: every entry a call reads it has written before.  Errors: the codes above, TQP_ERR_CUDA for a failed launch;
+ * cleared: every entry a call reads it has written before.  The first call on a device also looks the array's device address
+ * up (cudaGetSymbolAddress, once per device): make that call before a stream capture begins.  Errors: the codes above,
+ * TQP_ERR_CUDA for a failed look-up or launch;
  * text in tqp_dispatch_noalloc_error() (per thread). */
 tqp_status tqp_dispatch_noalloc(int T, int k, int E, const int32_t *topk_idx, int32_t *counts, int32_t *offsets,
                                 int32_t *perm, int32_t *inv_perm, void *stream);
