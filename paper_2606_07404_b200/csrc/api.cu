@@ -45,6 +45,7 @@ Workspace layout(const tqp_layer_desc &d) {
     // ... and the per-tile partials of rows_proj_wgrad_kernel: [2][max_tiles][r][F]
     w.wg_scratch = d.training ? take(std::max((E + N / kWgradSeg + 2) * (size_t)2 * d.r * (dm > F ? dm : F) * 4,
                                               (size_t)2 * (E + N / kTileRows + 1) * d.r * F * 4)) : take(16);
+    w.wg_done = take(E * ((dm > F ? dm : F) / 128) * 4);   // arrival counters of split experts (rows_wgrad_kernel), zero between launches
     w.lut = take(256 * 8 * 2);
     w.sc2 = take(E * (dm + 2 * F) * 4);   // bf16-pair copies of scale_down | scale_gate | scale_up for the backward GEMMs
     w.WrT = take(E * dm * 4);

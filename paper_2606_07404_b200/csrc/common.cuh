@@ -96,7 +96,7 @@ struct Workspace {
     size_t total = 0;        // the caller's workspace
     size_t host_total = 0;   // tqp_step_host staging (library-owned, allocated on first use)
     // offsets (bytes) into the bound buffer
-    size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, xsegs, xfirst, tfirst, wg_scratch, sched, lut, sc2, WrT, WrHL, wnorm, rflag, dl,
+    size_t Xp, G, U, H, dH, dG, dU, XAg, XAu, HAd, Zd, Zg, Zu, logits, blk_counts, tiles, num_tiles, xsegs, xfirst, tfirst, wg_scratch, wg_done, sched, lut, sc2, WrT, WrHL, wnorm, rflag, dl,
         // tqp_step_host staging
         trace, hX, hdY, hX2, hdY2, hY, hdX, topk_idx, topk_w, counts, offsets, perm, inv_perm, Ye, dYe, dXp, dtopk_w;
 };

@@ -773,12 +773,13 @@ struct WgradArgs {
     int width, out_ar;
     // experts with more than kWgradSeg rows are split into row segments (one CTA each); their partial gradients go to
     // `scratch` (entry e: first segment of expert e; entry E + j: extra segment j of the device-built list) and are
-    // summed in segment order by wgrad_reduce_kernel -- deterministic, no atomics
+    // summed in segment order by the CTA that finishes last -- deterministic, no atomics on the data
     const Tile *xsegs;
     const int32_t *xfirst;   // [E + 1]: first extra segment of every expert; xfirst[E] = number of extra segments
     float *scratch;
     int E;
     size_t entry;            // floats per scratch entry = ns * R * width
+    int32_t *done;           // [E][width / 128] arrival counters of split experts (zero between launches: the last arriver resets its own)
 };
 
 template <int R, int NS>
@@ -807,14 +808,16 @@ __global__ void __launch_bounds__(128) rows_wgrad_kernel(const __grid_constant__
     const int width = a.width;
     int e, p0, p1;
     float *dst[2];
+    bool split;   // the expert has more than kWgradSeg rows: this CTA writes a partial, the last CTA of the expert's slab sums them
     if (bx < a.E) {
         e = bx;
         p0 = offsets[e];
         const int cnt = offsets[e + 1] - p0;
         p1 = p0 + min(cnt, kWgradSeg);
+        split = cnt > kWgradSeg;
 #pragma unroll
         for (int w = 0; w < NS; ++w)
-            dst[w] = cnt > kWgradSeg ? a.scratch + (size_t)e * a.entry + (size_t)w * R * width : a.grad[w] + (size_t)e * R * width;
+            dst[w] = split ? a.scratch + (size_t)e * a.entry + (size_t)w * R * width : a.grad[w] + (size_t)e * R * width;
     } else {
         const int j = bx - a.E;
         if (j >= a.xfirst[a.E]) return;
@@ -822,6 +825,7 @@ __global__ void __launch_bounds__(128) rows_wgrad_kernel(const __grid_constant__
         e = t.expert;
         p0 = t.row0;
         p1 = p0 + t.rows;
+        split = true;
 #pragma unroll
         for (int w = 0; w < NS; ++w) dst[w] = a.scratch + (size_t)(a.E + j) * a.entry + (size_t)w * R * width;
     }
@@ -904,24 +908,37 @@ __global__ void __launch_bounds__(128) rows_wgrad_kernel(const __grid_constant__
             }
         }
     }
-}
-
-// Sum of the partial gradients of split experts, in segment order.  grid = (E, 4), block = 512; float4 elements.
-__global__ void __launch_bounds__(512) wgrad_reduce_kernel(const __grid_constant__ WgradArgs a, int ns, int R) {
-    const int e = blockIdx.x;
+    if (!split) return;
+    // Split expert: the CTA that arrives last at the expert's slab counter sums the partials of this slab in SEGMENT order (first
+    // segment, then the extra segments of the device-built list) -- deterministic whoever arrives last, no atomics on the data --
+    // and resets the counter for the next launch.  (A separate reduction kernel per gradient cost 4 us + a launch gap even when no
+    // expert was split, 10-46 us under skew.)
+    __shared__ int s_last;
     const int x0 = a.xfirst[e], nx = a.xfirst[e + 1] - x0;
-    if (nx <= 0) return;
-    const size_t per = (size_t)R * a.width;   // floats per gradient of one expert
-    for (int w = 0; w < ns; ++w) {
-        const float4 *first = reinterpret_cast<const float4 *>(a.scratch + (size_t)e * a.entry + (size_t)w * per);
-        float4 *out = reinterpret_cast<float4 *>(a.grad[w] + (size_t)e * per);
-        for (size_t i = blockIdx.y * blockDim.x + threadIdx.x; i < per / 4; i += (size_t)gridDim.y * blockDim.x) {
-            float4 s = first[i];
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+        int32_t *cnt = a.done + (size_t)e * nslab + a0 / WG_COLS;
+        const int prev = atomicAdd(cnt, 1);
+        s_last = prev == nx;
+        if (prev == nx) *cnt = 0;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+#pragma unroll
+    for (int w = 0; w < NS; ++w) {
+        const float *first = a.scratch + (size_t)e * a.entry + (size_t)w * R * width;
+        float *out = a.grad[w] + (size_t)e * R * width;
+        // this slab's region: out_ar ? rows [a0, a0 + 128) of [width][R] (contiguous) : columns [a0, a0 + 128) of each of the R rows
+        for (int v = tid; v < R * WG_COLS / 4; v += 128) {
+            const size_t off = a.out_ar ? (size_t)a0 * R + (size_t)v * 4 : (size_t)(v / (WG_COLS / 4)) * width + a0 + (v % (WG_COLS / 4)) * 4;
+            float4 sum = __ldcg(reinterpret_cast<const float4 *>(first + off));
             for (int j = 0; j < nx; ++j) {
-                const float4 v = reinterpret_cast<const float4 *>(a.scratch + (size_t)(a.E + x0 + j) * a.entry + (size_t)w * per)[i];
-                s.x += v.x; s.y += v.y; s.z += v.z; s.w += v.w;
+                const float4 t4 = __ldcg(reinterpret_cast<const float4 *>(a.scratch + (size_t)(a.E + x0 + j) * a.entry + (size_t)w * R * width + off));
+                sum.x += t4.x; sum.y += t4.y; sum.z += t4.z; sum.w += t4.w;
             }
-            out[i] = s;
+            *reinterpret_cast<float4 *>(out + off) = sum;
         }
     }
 }
@@ -948,8 +965,6 @@ static tqp_status launch_wgrad_t(tqp_ctx *c, const WgradArgs &a, const int32_t *
     if (tqp_status st_attr = ensure_dyn_smem(c, reinterpret_cast<const void *>(&rows_wgrad_kernel<R, NS>), C::SMEM)) return st_attr;
     rows_wgrad_kernel<R, NS><<<(unsigned)((c->desc.E + c->max_xsegs) * (a.width / WG_COLS)), 128, C::SMEM, st>>>(a, offsets);
     TQP_LAUNCH_OK(c);
-    wgrad_reduce_kernel<<<dim3(c->desc.E, 4), 512, 0, st>>>(a, NS, R);
-    TQP_LAUNCH_OK(c);
     return TQP_OK;
 }
 
@@ -971,7 +986,7 @@ tqp_status launch_rows_wgrad(tqp_ctx *c, const bf16 *big, int width, const bf16 
     a.width = width; a.out_ar = out_ar;
     const int ns = small1 ? 2 : 1;
     a.xsegs = c->p<Tile>(c->ws.xsegs); a.xfirst = c->p<int32_t>(c->ws.xfirst); a.scratch = c->p<float>(c->ws.wg_scratch);
-    a.E = E; a.entry = (size_t)ns * r * width;
+    a.E = E; a.entry = (size_t)ns * r * width; a.done = c->p<int32_t>(c->ws.wg_done);
     if (r == 16 && ns == 1) return launch_wgrad_t<16, 1>(c, a, offsets, st);
     if (r == 16 && ns == 2) return launch_wgrad_t<16, 2>(c, a, offsets, st);
     if (r == 32 && ns == 1) return launch_wgrad_t<32, 1>(c, a, offsets, st);
