@@ -83,14 +83,18 @@ tqp_status tqp_bind_workspace(tqp_ctx *ctx, void *dev_ptr, size_t bytes, void *s
 /* Records the weight pointers, builds the TMA descriptors over the code indices and converts the codebook
  * to the bf16 lookup table the GEMM mainloop gathers from.  One-time, untimed; needs a bound workspace. */
 tqp_status tqp_bind_weights(tqp_ctx *ctx, const tqp_weights *w, void *stream);
-/* Options.  "gemm_impl": 0 = tcgen05 grouped GEMM on CTA pairs with the dequantised weight operand in tensor memory
- * (default), 1 = CUDA-core scaffold (test reference), 2 = tcgen05 grouped GEMM, one CTA per tile, weight operand
- * through shared memory (fallback for M % 256 != 0), 3 = CTA pairs, weight operand through shared memory (fallback for
- * K % 128 != 0).
+/* Options.
+ * "gemm_impl": 0 = tcgen05 grouped GEMM on CTA pairs with the dequantised weight operand in tensor memory (default),
+ *   1 = CUDA-core scaffold (test reference), 2 = tcgen05 grouped GEMM, one CTA per tile, weight operand through shared
+ *   memory (fallback for M % 256 != 0), 3 = CTA pairs, weight operand through shared memory (fallback for K % 128 != 0).
+ * "route_impl": 0..3, see tqp_route_info.
  * "fuse_dgu": 1 (default) lets tqp_expert_bwd form the gate / up adapter projections and dB_gate / dB_up in one pass over
- * dG / dU (r in {16, 32}), 0 keeps the separate passes; same results within fp32 summation order.  "route_impl": 0..3, see tqp_route_info.  "time_gemm": 0/1, see tqp_gemm_time.  "host_chunks": 0 (default) lets tqp_step_host_async choose at run time
- * whether X goes up and is routed in one piece or in four token chunks; 1 / 4 pin the choice (same results).  Unknown names return TQP_ERR_ARG.  (Kernel instrumentation -- "trace",
- * "ablate" -- exists only in builds compiled with -DTQP_TRACE and is not part of this interface.) */
+ *   dG / dU (r in {16, 32}), 0 keeps the separate passes; same results within fp32 summation order.
+ * "time_gemm": 0 / 1, see tqp_gemm_time.
+ * "host_chunks": 0 (default) lets tqp_step_host_async choose at run time whether X goes up and is routed in one piece or
+ *   in four token chunks; 1 / 4 pin the choice (same results).
+ * Unknown names return TQP_ERR_ARG.  (Kernel instrumentation -- "trace", "ablate" -- exists only in builds compiled with
+ * -DTQP_TRACE and is not part of this interface.) */
 tqp_status tqp_set_option(tqp_ctx *ctx, const char *name, int value);
 
 /* --- forward ------------------------------------------------------------------------------------------ */
