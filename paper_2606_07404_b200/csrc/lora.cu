@@ -503,7 +503,13 @@ __global__ void __launch_bounds__(GP_THREADS, 1) rows_gather_proj_kernel(const _
                 __threadfence_block();
                 *(volatile int *)&s_pub = seq + 1;
             }
-            if (it >= n_items) break;
+            if (it >= n_items) {   // no more work: the last CTA to get here re-arms the counters for the next launch (no memset node)
+                if (lane == 0 && atomicAdd(counter + 1, 1) == (int)gridDim.x - 1) {
+                    counter[0] = 0;
+                    counter[1] = 0;
+                }
+                break;
+            }
             const int nl = (g.valid + 3) / 4;
             int sr[4];     // rows past `valid`: an index past the tensor (zero fill, no traffic)
 #pragma unroll
@@ -682,8 +688,7 @@ static tqp_status launch_gather_t(tqp_ctx *c, const GatherArgs &a, cudaStream_t 
     using C = GatherCfg<R, NW, KR>;
     if (tqp_status st_attr = ensure_dyn_smem(c, reinterpret_cast<const void *>(&rows_gather_proj_kernel<R, NW, KR, SCALE>), C::SMEM)) return st_attr;
     const int grid = std::min(c->num_sms, c->max_tiles * (kTileRows / PJ_ROWS));
-    int32_t *counter = c->p<int32_t>(c->ws.sched);
-    TQP_CUDA_OK(c, cudaMemsetAsync(counter, 0, sizeof(int32_t), st));
+    int32_t *counter = c->p<int32_t>(c->ws.sched);   // [0] items drawn, [1] CTAs finished: zero at bind, re-armed by the kernel
     rows_gather_proj_kernel<R, NW, KR, SCALE><<<grid, GP_THREADS, C::SMEM, st>>>(a, c->p<Tile>(c->ws.tiles), c->p<int32_t>(c->ws.num_tiles), counter);
     TQP_LAUNCH_OK(c);
     return TQP_OK;
