@@ -40,3 +40,21 @@ SEEDS = sorted({(s, False) for s in (1000, 1001, 1002, 1003, 1004, 1017, 1020, 1
 def test_random_shape_matches_the_oracle(seed, big):
     cfg, inp = _case(seed, big)
     check_all(inp, backward=True, router_grad=cfg.router_grad, gemm_impl=0)
+
+
+# The screened router is the library's choice only for large E and T (tqp_route_info); here it is FORCED (route_impl = 2) on
+# random shapes -- few experts, k close to E, a flooded and an emptied expert, T far below one 128-token tile -- and
+# run_gpu asserts its topk_idx / topk_w bitwise against the dense chain before the rest of the layer runs on them.
+# Seeds 1100-1103 and 5100-5103: the first four of either range of a one-off sweep over 1100-1139 / 5100-5139 (80 shapes, all
+# green on the B200) that was run once when the router was written.
+@pytest.mark.parametrize("seed,big", [(s, False) for s in range(1100, 1104)] + [(s, True) for s in range(5100, 5104)])
+def test_random_shape_through_the_forced_screened_router(seed, big):
+    from parity_util import assert_close, assert_routing_exact, run_gpu
+    from test_gpu_parity import BWD_KEYS, FWD_KEYS, RG_KEYS, oracle_ref
+    cfg, inp = _case(seed, big)
+    ref = oracle_ref(inp, True, cfg.router_grad)
+    gpu = run_gpu(inp, backward=True, router_grad=cfg.router_grad, route_impl=2)
+    assert gpu["route_info"][0] == 1
+    assert_routing_exact(gpu, ref)
+    for key in FWD_KEYS + BWD_KEYS + (RG_KEYS if cfg.router_grad else ()):
+        assert_close(key, gpu[key], ref[key])
